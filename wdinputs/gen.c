@@ -1,0 +1,170 @@
+/* wdinputs/gen.c — seeded, counter-based generators of SYNTHETIC input fields.
+ *
+ * This module serves both the CPU oracle (oracle/) and the CUDA library (tests, bench) with
+ * the same input arrays.  It holds NONE of the method's arithmetic: no gamma matrices, no
+ * Dirac operator, no plaquettes, no clover construction.  It only draws random numbers and
+ * shapes them into the value distributions DESIGN.md §"Input recipe" lists (stand-ins for the
+ * paper's gauge configurations, which are not available):
+ *
+ *   - i.i.d. N(0,1) reals                      (spinor entries, BASELINE.json configs)
+ *   - Haar-random SU(3) 3x3 matrices           (Gram-Schmidt of a complex Gaussian matrix,
+ *                                               determinant phase divided out)
+ *   - U = exp(i*eps*H), H traceless Hermitian  (near-unit "smooth-like" links)
+ *   - random Hermitian block-diagonal self-coupling arrays in the 42-entry format
+ *
+ * Every value depends only on (seed, element index), so fields of any size are generated in
+ * parallel and reproducibly.  All arrays are host arrays of doubles, complex = (re, im).
+ */
+#include <complex.h>
+#include <math.h>
+#include <stddef.h>
+#include <stdint.h>
+
+typedef double complex cplx;
+
+static inline uint64_t mix64(uint64_t z) {
+    z += 0x9E3779B97F4A7C15ULL;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+    return z ^ (z >> 31);
+}
+
+/* uniform in (0,1), 53 bits, never 0 or 1 */
+static inline double u01(uint64_t seed, uint64_t ctr) {
+    uint64_t r = mix64(mix64(seed) ^ mix64(ctr * 0xD1B54A32D192ED03ULL + 0x2545F4914F6CDD1DULL));
+    return ((double)(r >> 11) + 0.5) * (1.0 / 9007199254740992.0);
+}
+
+/* n-th standard normal of stream `seed` (Box-Muller on the pair n/2) */
+static inline double gauss(uint64_t seed, uint64_t n) {
+    uint64_t pair = n >> 1;
+    double u1 = u01(seed, 2 * pair), u2 = u01(seed, 2 * pair + 1);
+    double r = sqrt(-2.0 * log(u1));
+    double a = 6.283185307179586476925286766559 * u2;
+    return (n & 1) ? r * sin(a) : r * cos(a);
+}
+
+void wdin_gaussian(double *out, uint64_t n, uint64_t seed) {
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < (int64_t)n; i++) out[i] = gauss(seed, (uint64_t)i);
+}
+
+static void gaussian_3x3(cplx g[3][3], uint64_t seed, uint64_t link) {
+    for (int k = 0; k < 9; k++)
+        g[k / 3][k % 3] = gauss(seed, 18 * link + 2 * k) + I * gauss(seed, 18 * link + 2 * k + 1);
+}
+
+static cplx det3(cplx m[3][3]) {
+    return m[0][0] * (m[1][1] * m[2][2] - m[1][2] * m[2][1]) -
+           m[0][1] * (m[1][0] * m[2][2] - m[1][2] * m[2][0]) +
+           m[0][2] * (m[1][0] * m[2][1] - m[1][1] * m[2][0]);
+}
+
+/* Haar SU(3): columns of a complex Gaussian matrix orthonormalised by modified Gram-Schmidt
+ * (= QR with positive R diagonal, Haar on U(3)), then multiplied by exp(-i arg(det)/3). */
+void wdin_su3_haar(double *U, uint64_t nlinks, uint64_t seed) {
+#pragma omp parallel for schedule(static)
+    for (int64_t l = 0; l < (int64_t)nlinks; l++) {
+        cplx g[3][3];
+        gaussian_3x3(g, seed, (uint64_t)l);
+        for (int c = 0; c < 3; c++) {
+            for (int p = 0; p < c; p++) {
+                cplx dot = 0;
+                for (int r = 0; r < 3; r++) dot += conj(g[r][p]) * g[r][c];
+                for (int r = 0; r < 3; r++) g[r][c] -= dot * g[r][p];
+            }
+            double nrm = 0;
+            for (int r = 0; r < 3; r++) nrm += creal(g[r][c]) * creal(g[r][c]) + cimag(g[r][c]) * cimag(g[r][c]);
+            nrm = 1.0 / sqrt(nrm);
+            for (int r = 0; r < 3; r++) g[r][c] *= nrm;
+        }
+        cplx d = det3(g);
+        double th = atan2(cimag(d), creal(d)) / 3.0;
+        cplx ph = cos(th) - I * sin(th);
+        double *o = U + 18 * l;
+        for (int k = 0; k < 9; k++) {
+            cplx v = g[k / 3][k % 3] * ph;
+            o[2 * k] = creal(v);
+            o[2 * k + 1] = cimag(v);
+        }
+    }
+}
+
+static void matmul3(cplx c[3][3], cplx a[3][3], cplx b[3][3]) {
+    cplx t[3][3];
+    for (int i = 0; i < 3; i++)
+        for (int j = 0; j < 3; j++) {
+            cplx s = 0;
+            for (int k = 0; k < 3; k++) s += a[i][k] * b[k][j];
+            t[i][j] = s;
+        }
+    for (int i = 0; i < 3; i++)
+        for (int j = 0; j < 3; j++) c[i][j] = t[i][j];
+}
+
+/* U = exp(i*eps*H), H = (G+G^H)/2 - tr/3 with G complex Gaussian: scaling and squaring around a
+ * degree-20 Taylor polynomial (argument norm scaled below 1/4). */
+void wdin_su3_exp(double *U, uint64_t nlinks, uint64_t seed, double eps) {
+#pragma omp parallel for schedule(static)
+    for (int64_t l = 0; l < (int64_t)nlinks; l++) {
+        cplx g[3][3], a[3][3];
+        gaussian_3x3(g, seed, (uint64_t)l);
+        cplx tr = 0;
+        for (int i = 0; i < 3; i++) tr += creal(g[i][i]);
+        double nrm = 0;
+        for (int i = 0; i < 3; i++)
+            for (int j = 0; j < 3; j++) {
+                cplx h = 0.5 * (g[i][j] + conj(g[j][i]));
+                if (i == j) h -= tr / 3.0;
+                a[i][j] = I * eps * h;
+                nrm += cabs(a[i][j]);
+            }
+        int s = 0;
+        while (nrm > 0.25) { nrm *= 0.5; s++; }
+        double sc = ldexp(1.0, -s);
+        for (int i = 0; i < 3; i++)
+            for (int j = 0; j < 3; j++) a[i][j] *= sc;
+        cplx e[3][3], term[3][3];
+        for (int i = 0; i < 3; i++)
+            for (int j = 0; j < 3; j++) e[i][j] = term[i][j] = (i == j) ? 1.0 : 0.0;
+        for (int k = 1; k <= 20; k++) {
+            matmul3(term, term, a);
+            for (int i = 0; i < 3; i++)
+                for (int j = 0; j < 3; j++) {
+                    term[i][j] /= (double)k;
+                    e[i][j] += term[i][j];
+                }
+        }
+        for (int q = 0; q < s; q++) matmul3(e, e, e);
+        double *o = U + 18 * l;
+        for (int k = 0; k < 9; k++) {
+            o[2 * k] = creal(e[k / 3][k % 3]);
+            o[2 * k + 1] = cimag(e[k / 3][k % 3]);
+        }
+    }
+}
+
+void wdin_su3_unit(double *U, uint64_t nlinks) {
+#pragma omp parallel for schedule(static)
+    for (int64_t l = 0; l < (int64_t)nlinks; l++) {
+        double *o = U + 18 * l;
+        for (int k = 0; k < 18; k++) o[k] = 0.0;
+        o[0] = o[8] = o[16] = 1.0;
+    }
+}
+
+/* Random self-coupling array in the 42-complex-per-site format (include/wd.h, R6):
+ * entries 0..11 real diagonal = shift + scale*N(0,1) (imaginary part 0), entries 12..41 complex
+ * off-diagonals scale*(N(0,1) + i N(0,1)).  An arbitrary Hermitian block-diagonal input, not a
+ * clover term built from links. */
+void wdin_selfcoupling_random(double *C, uint64_t nsites, uint64_t seed, double shift, double scale) {
+#pragma omp parallel for schedule(static)
+    for (int64_t x = 0; x < (int64_t)nsites; x++) {
+        double *o = C + 84 * x;
+        for (int k = 0; k < 42; k++) {
+            double a = gauss(seed, 84 * (uint64_t)x + 2 * k), b = gauss(seed, 84 * (uint64_t)x + 2 * k + 1);
+            if (k < 12) { o[2 * k] = shift + scale * a; o[2 * k + 1] = 0.0; }
+            else        { o[2 * k] = scale * a;         o[2 * k + 1] = scale * b; }
+        }
+    }
+}
