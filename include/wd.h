@@ -1,0 +1,152 @@
+/* include/wd.h — C-ABI of libwd: the finest-level Wilson(-clover) Dirac operator on one B200.
+ *
+ *   (D psi)(x) = S(x) psi(x)
+ *              - 1/2 sum_mu [ (I4 - gamma_mu) (x) U_mu(x)       ] psi(x + mu)
+ *              - 1/2 sum_mu [ (I4 + gamma_mu) (x) U_mu(x - mu)^H ] psi(x - mu)        (eq. 1.13,
+ *   S(x) = (m0+4) I12 - csw/32 sum_{mu,nu} (gamma_mu gamma_nu) (x) (Q_mu_nu(x) - Q_nu_mu(x))
+ *                                                      PAPER.md:227-230; eq. 2.5)
+ * with lattice spacing a = 1, periodic boundary conditions in all four directions
+ * (PAPER.md:187), FP64 complex arithmetic, and the gamma matrices of DESIGN.md R1.
+ *
+ * Plain C: opaque handle, plain pointers (each documented as HOST or DEVICE) and sizes, no torch
+ * or C++ types.  Every function returns 0 (WD_OK) or a negative error code; nothing throws or
+ * aborts across this boundary; wd_last_error() gives the text of the last failure on a handle.
+ *
+ * CANONICAL HOST LAYOUTS (what the paper's CPU code stores; complex = re,im):
+ *   site index      i = ((t*Z + z)*Y + y)*X + x, 0-based, X fastest; V = T*Z*Y*X
+ *   directions      mu = 0,1,2,3 = T,Z,Y,X
+ *   spinor          double [nrhs][V][12][2], component 3*spin + colour
+ *   gauge           double [V][4][3][3][2]: forward links U_mu(x) of the own site, row-major 3x3
+ *
+ *   self-coupling   double [V][42][2]: the 42 entries of S(x) = D_sc, INCLUDING the
+ *                   (m0+4) diagonal: entries 0..11 the real diagonal (imaginary part ignored),
+ *                   12..26 the strict upper triangle, row-major, of S[0:6,0:6] (spins 0,1),
+ *                   27..41 the same of S[6:12,6:12] (spins 2,3); lower triangles are the
+ *                   conjugates (R6).
+ *
+ * DEVICE LAYOUT: chosen by the library, opaque to the caller.
+ * A device spinor buffer holds wd_spinor_bytes(h, nrhs) bytes, is 256-byte aligned, and is
+ * filled / read with wd_pack_spinor / wd_unpack_spinor (or wd_apply_host).  Fields stay
+ * device-resident in device layout between applications: wd_apply never repacks (the lesson of
+ * PAPER.md:1015, where per-application reordering ate the gain).
+ *
+ * OWNERSHIP: the library owns gauge, self-coupling and staging storage on the device; the
+ * caller owns every pointer it passes in (host arrays are copied before the call returns;
+ * device spinor buffers are caller-allocated, e.g. by PyTorch).
+ *
+ * THREADING: a handle is used by one host thread at a time.  All device work of a handle is
+ * issued on the handle's stream (default: the legacy default stream; see wd_set_stream).
+ */
+#ifndef WD_H
+#define WD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct wd_handle wd_handle;
+
+enum {
+    WD_OK = 0,
+    WD_EINVAL = -1, /* bad dimensions, null pointer, nrhs < 1, unknown option or value         */
+    WD_ENOMEM = -2, /* host or device allocation failed                                          */
+    WD_ESTATE = -3, /* e.g. apply before the gauge field is loaded, clover missing with csw != 0 */
+    WD_ECUDA = -4   /* a CUDA runtime call or kernel launch failed (text in wd_last_error)       */
+};
+
+/* Options for wd_set_option / wd_get_option. */
+enum {
+    WD_OPT_VARIANT = 1,   /* 0 = fused single pass (default), 1 = unfused: hopping kernel + self-coupling kernel */
+    WD_OPT_KERNEL = 2,    /* hopping/fused kernel geometry id; -1 = automatic (default); see wd_kernel_name        */
+    WD_OPT_TCHUNK = 3,    /* T-extent marched by one CTA in tiled geometries; 0 = automatic                       */
+    WD_OPT_ZGROUP = 4,    /* number of Z-tiles per rasterisation group in tiled geometries; 0 = automatic         */
+    WD_OPT_DEVICE_PACK = 5/* 1 = wd_load_* / wd_pack_* transpose on the device instead of on the host (default 0) */
+};
+
+/* Create an operator for a T x Z x Y x X periodic lattice.  Every extent >= 1 (n = 2, where
+ * x+mu and x-mu are the same site, and n = 1 are handled: both hopping terms are applied,
+ * DESIGN.md R12).  csw == 0: pure Wilson, S = (m0+4) I, no self-coupling array is needed.
+ * csw != 0: S must be supplied with wd_load_clover or built with wd_build_clover.
+ * Uses the current CUDA device.  Errors: WD_EINVAL, WD_ENOMEM, WD_ECUDA. */
+int wd_create(wd_handle **h, int T, int Z, int Y, int X, double m0, double csw);
+
+/* Free all device and host storage of the handle.  Synchronises the handle's stream. */
+int wd_destroy(wd_handle *h);
+
+/* HOST pointer, canonical gauge layout.  Packed into the device layout and copied; the caller
+ * keeps ownership.  Links are treated as general 3x3 complex matrices (U and U^H are used,
+ * never U^-1; R11).  Synchronous w.r.t. the host array. */
+int wd_load_gauge(wd_handle *h, const double *host_U);
+
+/* HOST pointer, canonical self-coupling layout (the whole S(x), eq. 2.5).  Required iff csw != 0
+ * (allowed also with csw == 0: the loaded S then replaces (m0+4) I). */
+int wd_load_clover(wd_handle *h, const double *host_C);
+
+/* Build S(x) of eq. 2.5 on the device from the loaded gauge field (Q_mu_nu of eq. 1.12,
+ * PAPER.md:221, all 16 ordered pairs, R8) with the handle's m0 and csw.
+ * Errors: WD_ESTATE if no gauge field is loaded. */
+int wd_build_clover(wd_handle *h);
+
+/* Read S(x) back: HOST pointer, canonical self-coupling layout [V][42][2]. */
+int wd_get_clover(wd_handle *h, double *host_C);
+
+/* out = D in for nrhs right-hand sides (eq. 1.13).  DEVICE pointers in DEVICE layout, each
+ * wd_spinor_bytes(h, nrhs) bytes, 256-byte aligned; out must not overlap in.  Asynchronous:
+ * enqueued on the handle's stream, no host synchronisation, no host<->device copies, no
+ * repacking.  Errors: WD_EINVAL, WD_ESTATE (no gauge; csw != 0 and no self-coupling), WD_ECUDA. */
+int wd_apply(wd_handle *h, void *dev_out, const void *dev_in, int nrhs);
+
+/* Same operation on HOST arrays in canonical spinor layout: host->device copy, on-device
+ * repack, wd_apply, repack, device->host copy, all inside the call; returns after the result is
+ * in host_out.  (Pinned host memory makes the copies faster but is not required.) */
+int wd_apply_host(wd_handle *h, double *host_out, const double *host_in, int nrhs);
+
+/* Size in bytes of a device spinor buffer for nrhs right-hand sides (0 on error). */
+size_t wd_spinor_bytes(const wd_handle *h, int nrhs);
+
+/* HOST canonical [nrhs][V][12][2]  <->  DEVICE layout.  Synchronous. */
+int wd_pack_spinor(wd_handle *h, void *dev_dst, const double *host_src, int nrhs);
+int wd_unpack_spinor(wd_handle *h, double *host_dst, const void *dev_src, int nrhs);
+
+/* The host packer by itself (step a0; no GPU needed): writes the host-side IMAGE of the device
+ * layout of one field — exactly the bytes wd_load_gauge / wd_load_clover / wd_pack_spinor place
+ * in device memory — and its inverse.  field: WD_FIELD_SPINOR (one RHS, canonical 12 complex per
+ * site), WD_FIELD_GAUGE (36), WD_FIELD_CLOVER (canonical 42 complex -> 36 packed slots; unpacking
+ * returns zero imaginary parts on the diagonal).  HOST pointers; nsites = V.
+ * wd_layout_bytes: size of the packed image (0 on error). */
+enum { WD_FIELD_SPINOR = 0, WD_FIELD_GAUGE = 1, WD_FIELD_CLOVER = 2 };
+size_t wd_layout_bytes(int field, long long nsites);
+int wd_layout_pack_host(int field, long long nsites, const double *canonical, double *packed);
+int wd_layout_unpack_host(int field, long long nsites, const double *packed, double *canonical);
+
+/* cudaStream_t passed as void* (NULL = legacy default stream).  PyTorch supplies memory and
+ * streams only. */
+int wd_set_stream(wd_handle *h, void *cuda_stream);
+
+/* Block the host until all work enqueued on the handle's stream has finished. */
+int wd_synchronize(wd_handle *h);
+
+int wd_set_option(wd_handle *h, int option, long value);
+int wd_get_option(const wd_handle *h, int option, long *value);
+
+/* Number of compiled kernel geometries and their names ("linear256", "tile_1x4x4x16", ...);
+ * NULL if id is out of range.  wd_kernel_in_use: the id the next wd_apply will launch. */
+int wd_kernel_count(void);
+const char *wd_kernel_name(int id);
+int wd_kernel_in_use(const wd_handle *h);
+
+/* Number of kernel launches issued by this handle so far (all kernels of this library). */
+long wd_launch_count(const wd_handle *h);
+
+/* Text of the last error on this handle (h == NULL: of the last failed wd_create on this thread).
+ * Never NULL. */
+const char *wd_last_error(const wd_handle *h);
+
+const char *wd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WD_H */

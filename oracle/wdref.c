@@ -112,6 +112,50 @@ static void expand_selfcoupling(const cplx *c42, cplx S[12][12]) {
 }
 
 /* ---- eq. 1.13, a = 1 ------------------------------------------------- */
+/* One site: acc = S(x) psi(x) - 1/2 sum_mu [...]; S == NULL means S = (m0+4) I. */
+static void apply_site(const dims_t *d, double m0, const double *U, cplx (*S)[12], const cplx *psi,
+                       int64_t x, cplx gam[4][4][4], cplx acc[12]) {
+    /* first line of eq. 1.13: the self-coupling term S(x) psi(x) */
+    if (S) {
+        for (int i = 0; i < 12; i++) {
+            cplx s = 0;
+            for (int j = 0; j < 12; j++) s += S[i][j] * psi[x * 12 + j];
+            acc[i] = s;
+        }
+    } else {
+        for (int i = 0; i < 12; i++) acc[i] = (m0 + 4.0) * psi[x * 12 + i];
+    }
+    for (int mu = 0; mu < 4; mu++) {
+        const int64_t xp = shifted(d, x, mu, +1, -1, 0);
+        const int64_t xm = shifted(d, x, mu, -1, -1, 0);
+        const cplx *Uf = link(U, x, mu);  /* U_mu(x)     */
+        const cplx *Ub = link(U, xm, mu); /* U_mu(x-mu)  */
+        cplx fw[4][3], bw[4][3];
+        for (int s = 0; s < 4; s++)
+            for (int c = 0; c < 3; c++) {
+                cplx f = 0, b = 0;
+                for (int k = 0; k < 3; k++) {
+                    f += Uf[3 * c + k] * psi[xp * 12 + 3 * s + k];       /* U psi(x+mu)   */
+                    b += conj(Ub[3 * k + c]) * psi[xm * 12 + 3 * s + k]; /* U^H psi(x-mu) */
+                }
+                fw[s][c] = f;
+                bw[s][c] = b;
+            }
+        /* second and third line of eq. 1.13 */
+        for (int s = 0; s < 4; s++)
+            for (int c = 0; c < 3; c++) {
+                cplx f = 0, b = 0;
+                for (int sp = 0; sp < 4; sp++) {
+                    cplx delta = (s == sp) ? 1.0 : 0.0;
+                    f += (delta - gam[mu][s][sp]) * fw[sp][c];
+                    b += (delta + gam[mu][s][sp]) * bw[sp][c];
+                }
+                acc[3 * s + c] -= 0.5 * f;
+                acc[3 * s + c] -= 0.5 * b;
+            }
+    }
+}
+
 int wdref_apply(int T, int Z, int Y, int X, double m0, const double *U, const double *C,
                 double *out, const double *in, int nrhs) {
     if (T < 1 || Z < 1 || Y < 1 || X < 1 || !U || !out || !in || nrhs < 1) return -1;
@@ -125,48 +169,9 @@ int wdref_apply(int T, int Z, int Y, int X, double m0, const double *U, const do
         cplx *eta = (cplx *)out + (int64_t)r * V * 12;
 #pragma omp parallel for schedule(static)
         for (int64_t x = 0; x < V; x++) {
-            cplx acc[12];
-            /* first line of eq. 1.13: the self-coupling term S(x) psi(x) */
-            if (C) {
-                cplx S[12][12];
-                expand_selfcoupling((const cplx *)C + x * 42, S);
-                for (int i = 0; i < 12; i++) {
-                    cplx s = 0;
-                    for (int j = 0; j < 12; j++) s += S[i][j] * psi[x * 12 + j];
-                    acc[i] = s;
-                }
-            } else {
-                for (int i = 0; i < 12; i++) acc[i] = (m0 + 4.0) * psi[x * 12 + i];
-            }
-            for (int mu = 0; mu < 4; mu++) {
-                const int64_t xp = shifted(&d, x, mu, +1, -1, 0);
-                const int64_t xm = shifted(&d, x, mu, -1, -1, 0);
-                const cplx *Uf = link(U, x, mu);  /* U_mu(x)     */
-                const cplx *Ub = link(U, xm, mu); /* U_mu(x-mu)  */
-                cplx fw[4][3], bw[4][3];
-                for (int s = 0; s < 4; s++)
-                    for (int c = 0; c < 3; c++) {
-                        cplx f = 0, b = 0;
-                        for (int k = 0; k < 3; k++) {
-                            f += Uf[3 * c + k] * psi[xp * 12 + 3 * s + k];       /* U psi(x+mu)   */
-                            b += conj(Ub[3 * k + c]) * psi[xm * 12 + 3 * s + k]; /* U^H psi(x-mu) */
-                        }
-                        fw[s][c] = f;
-                        bw[s][c] = b;
-                    }
-                /* second and third line of eq. 1.13 */
-                for (int s = 0; s < 4; s++)
-                    for (int c = 0; c < 3; c++) {
-                        cplx f = 0, b = 0;
-                        for (int sp = 0; sp < 4; sp++) {
-                            cplx delta = (s == sp) ? 1.0 : 0.0;
-                            f += (delta - gam[mu][s][sp]) * fw[sp][c];
-                            b += (delta + gam[mu][s][sp]) * bw[sp][c];
-                        }
-                        acc[3 * s + c] -= 0.5 * f;
-                        acc[3 * s + c] -= 0.5 * b;
-                    }
-            }
+            cplx acc[12], S[12][12];
+            if (C) expand_selfcoupling((const cplx *)C + x * 42, S);
+            apply_site(&d, m0, U, C ? S : NULL, psi, x, gam, acc);
             for (int i = 0; i < 12; i++) eta[x * 12 + i] = acc[i];
         }
     }
@@ -268,6 +273,15 @@ int wdref_build_clover_full(int T, int Z, int Y, int X, double m0, double csw, c
     return 0;
 }
 
+static void pack_selfcoupling(cplx S[12][12], cplx *c) {
+    for (int k = 0; k < 12; k++) c[k] = creal(S[k][k]);
+    for (int b = 0; b < 2; b++) {
+        int k = 12 + 15 * b;
+        for (int r = 0; r < 6; r++)
+            for (int cc = r + 1; cc < 6; cc++, k++) c[k] = S[6 * b + r][6 * b + cc];
+    }
+}
+
 /* Stores the 42 entries of DESIGN.md R6.  Entries outside the two 6x6 blocks and the imaginary
  * parts of the diagonal are dropped (pin P6 checks on wdref_build_clover_full that they vanish);
  * the lower triangle is the conjugate of the upper one (S Hermitian, same pin). */
@@ -282,13 +296,35 @@ int wdref_build_clover(int T, int Z, int Y, int X, double m0, double csw, const 
     for (int64_t x = 0; x < V; x++) {
         cplx S[12][12];
         selfcoupling_full(&d, m0, csw, U, x, gam, S);
-        cplx *c = (cplx *)C + x * 42;
-        for (int k = 0; k < 12; k++) c[k] = creal(S[k][k]);
-        for (int b = 0; b < 2; b++) {
-            int k = 12 + 15 * b;
-            for (int r = 0; r < 6; r++)
-                for (int cc = r + 1; cc < 6; cc++, k++) c[k] = S[6 * b + r][6 * b + cc];
+        pack_selfcoupling(S, (cplx *)C + x * 42);
+    }
+    return 0;
+}
+
+/* (D psi)(x) at the listed sites only, from U, psi, m0, csw alone: S(x) is built from U by
+ * eq. 2.5 when csw != 0.  For parity checks at lattice sizes where a whole-lattice oracle pass
+ * would take too long; same per-site arithmetic as wdref_apply + wdref_build_clover. */
+int wdref_apply_sites(int T, int Z, int Y, int X, double m0, double csw, const double *U,
+                      const double *in, const int64_t *sites, int64_t nsites,
+                      double *out /* [nsites][12][2] */) {
+    if (T < 1 || Z < 1 || Y < 1 || X < 1 || !U || !out || !in || !sites || nsites < 0) return -1;
+    dims_t d = {{T, Z, Y, X}};
+    const int64_t V = (int64_t)T * Z * Y * X;
+    cplx gam[4][4][4];
+    for (int mu = 0; mu < 4; mu++) gamma_c(mu, gam[mu]);
+    for (int64_t k = 0; k < nsites; k++)
+        if (sites[k] < 0 || sites[k] >= V) return -2;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t k = 0; k < nsites; k++) {
+        cplx acc[12], S[12][12];
+        if (csw != 0.0) { /* same S as wdref_build_clover -> wdref_apply: through the 42 entries */
+            cplx c42[42];
+            selfcoupling_full(&d, m0, csw, U, sites[k], gam, S);
+            pack_selfcoupling(S, c42);
+            expand_selfcoupling(c42, S);
         }
+        apply_site(&d, m0, U, (csw != 0.0) ? S : NULL, (const cplx *)in, sites[k], gam, acc);
+        for (int i = 0; i < 12; i++) ((cplx *)out)[k * 12 + i] = acc[i];
     }
     return 0;
 }

@@ -1,0 +1,204 @@
+"""paper_2407_00041_b200 — B200-native Wilson(-clover) Dirac operator (arxiv 2407.00041 hot path).
+
+Thin ctypes binding of the C-ABI in include/wd.h: the functions below have the same names and
+argument order as the C entry points and do argument marshalling only — every step of the path
+(packing on request, neighbour indexing, projection, SU(3) multiply, reconstruction, clover,
+store) runs inside libwd.so's CUDA kernels.  PyTorch is used by callers for device memory and
+streams only.  There is NO CPU fallback: importing works without a GPU (so that the symbol table
+can be checked), but any compute call needs a CUDA device, and a missing libwd.so raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libwd.so")
+
+WD_OK, WD_EINVAL, WD_ENOMEM, WD_ESTATE, WD_ECUDA = 0, -1, -2, -3, -4
+WD_FIELD_SPINOR, WD_FIELD_GAUGE, WD_FIELD_CLOVER = 0, 1, 2
+WD_OPT_VARIANT, WD_OPT_KERNEL, WD_OPT_TCHUNK, WD_OPT_ZGROUP, WD_OPT_DEVICE_PACK = 1, 2, 3, 4, 5
+
+# name -> (restype, argtypes); mirrors include/wd.h declaration by declaration
+_vp, _i, _d, _l, _sz, _cp = (ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_long,
+                             ctypes.c_size_t, ctypes.c_char_p)
+SIGNATURES = {
+    "wd_create": (_i, [ctypes.POINTER(_vp), _i, _i, _i, _i, _d, _d]),
+    "wd_destroy": (_i, [_vp]),
+    "wd_load_gauge": (_i, [_vp, _vp]),
+    "wd_load_clover": (_i, [_vp, _vp]),
+    "wd_build_clover": (_i, [_vp]),
+    "wd_get_clover": (_i, [_vp, _vp]),
+    "wd_apply": (_i, [_vp, _vp, _vp, _i]),
+    "wd_apply_host": (_i, [_vp, _vp, _vp, _i]),
+    "wd_spinor_bytes": (_sz, [_vp, _i]),
+    "wd_pack_spinor": (_i, [_vp, _vp, _vp, _i]),
+    "wd_unpack_spinor": (_i, [_vp, _vp, _vp, _i]),
+    "wd_layout_bytes": (_sz, [_i, ctypes.c_longlong]),
+    "wd_layout_pack_host": (_i, [_i, ctypes.c_longlong, _vp, _vp]),
+    "wd_layout_unpack_host": (_i, [_i, ctypes.c_longlong, _vp, _vp]),
+    "wd_set_stream": (_i, [_vp, _vp]),
+    "wd_synchronize": (_i, [_vp]),
+    "wd_set_option": (_i, [_vp, _i, _l]),
+    "wd_get_option": (_i, [_vp, _i, ctypes.POINTER(_l)]),
+    "wd_kernel_count": (_i, []),
+    "wd_kernel_name": (_cp, [_i]),
+    "wd_kernel_in_use": (_i, [_vp]),
+    "wd_launch_count": (_l, [_vp]),
+    "wd_last_error": (_cp, [_vp]),
+    "wd_version": (_cp, []),
+}
+
+_lib = None
+
+
+class WDError(RuntimeError):
+    def __init__(self, code: int, text: str):
+        super().__init__(f"libwd error {code}: {text}")
+        self.code = code
+
+
+def lib() -> ctypes.CDLL:
+    """Load libwd.so (built in-tree by paper_2407_00041_b200.build).  Raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(
+                f"{LIB_PATH} not found: build it with `python -m paper_2407_00041_b200.build` "
+                "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _ptr(x) -> int | None:
+    """Marshal a pointer argument: int address, None, numpy array (host) or torch tensor."""
+    if x is None or isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    if hasattr(x, "ctypes"):
+        return x.ctypes.data
+    raise TypeError(type(x))
+
+
+def _check(h, rc: int) -> None:
+    if rc != WD_OK:
+        raise WDError(rc, lib().wd_last_error(h).decode())
+
+
+# ---- same names as the C entry points ------------------------------------------------------------
+def wd_create(T: int, Z: int, Y: int, X: int, m0: float, csw: float) -> int:
+    h = _vp()
+    rc = lib().wd_create(ctypes.byref(h), T, Z, Y, X, m0, csw)
+    _check(None, rc)
+    return h.value
+
+
+def wd_destroy(h) -> None:
+    _check(h, lib().wd_destroy(h))
+
+
+def wd_load_gauge(h, host_U) -> None:
+    _check(h, lib().wd_load_gauge(h, _ptr(host_U)))
+
+
+def wd_load_clover(h, host_C) -> None:
+    _check(h, lib().wd_load_clover(h, _ptr(host_C)))
+
+
+def wd_build_clover(h) -> None:
+    _check(h, lib().wd_build_clover(h))
+
+
+def wd_get_clover(h, host_C) -> None:
+    _check(h, lib().wd_get_clover(h, _ptr(host_C)))
+
+
+def wd_apply(h, dev_out, dev_in, nrhs: int = 1) -> None:
+    _check(h, lib().wd_apply(h, _ptr(dev_out), _ptr(dev_in), nrhs))
+
+
+def wd_apply_host(h, host_out, host_in, nrhs: int = 1) -> None:
+    _check(h, lib().wd_apply_host(h, _ptr(host_out), _ptr(host_in), nrhs))
+
+
+def wd_spinor_bytes(h, nrhs: int = 1) -> int:
+    return int(lib().wd_spinor_bytes(h, nrhs))
+
+
+def wd_pack_spinor(h, dev_dst, host_src, nrhs: int = 1) -> None:
+    _check(h, lib().wd_pack_spinor(h, _ptr(dev_dst), _ptr(host_src), nrhs))
+
+
+def wd_unpack_spinor(h, host_dst, dev_src, nrhs: int = 1) -> None:
+    _check(h, lib().wd_unpack_spinor(h, _ptr(host_dst), _ptr(dev_src), nrhs))
+
+
+def wd_layout_bytes(field: int, nsites: int) -> int:
+    return int(lib().wd_layout_bytes(field, nsites))
+
+
+def wd_layout_pack_host(field: int, nsites: int, canonical, packed) -> None:
+    rc = lib().wd_layout_pack_host(field, nsites, _ptr(canonical), _ptr(packed))
+    if rc != WD_OK:
+        raise WDError(rc, "wd_layout_pack_host: bad argument")
+
+
+def wd_layout_unpack_host(field: int, nsites: int, packed, canonical) -> None:
+    rc = lib().wd_layout_unpack_host(field, nsites, _ptr(packed), _ptr(canonical))
+    if rc != WD_OK:
+        raise WDError(rc, "wd_layout_unpack_host: bad argument")
+
+
+def wd_set_stream(h, cuda_stream) -> None:
+    _check(h, lib().wd_set_stream(h, _ptr(cuda_stream)))
+
+
+def wd_synchronize(h) -> None:
+    _check(h, lib().wd_synchronize(h))
+
+
+def wd_set_option(h, option: int, value: int) -> None:
+    _check(h, lib().wd_set_option(h, option, value))
+
+
+def wd_get_option(h, option: int) -> int:
+    v = _l()
+    _check(h, lib().wd_get_option(h, option, ctypes.byref(v)))
+    return v.value
+
+
+def wd_kernel_count() -> int:
+    return lib().wd_kernel_count()
+
+
+def wd_kernel_name(kid: int) -> str | None:
+    s = lib().wd_kernel_name(kid)
+    return s.decode() if s else None
+
+
+def wd_kernel_in_use(h) -> int:
+    return lib().wd_kernel_in_use(h)
+
+
+def wd_launch_count(h) -> int:
+    return int(lib().wd_launch_count(h))
+
+
+def wd_last_error(h) -> str:
+    return lib().wd_last_error(h).decode()
+
+
+def wd_version() -> str:
+    return lib().wd_version().decode()
+
+
+def kernel_id(name: str) -> int:
+    for k in range(wd_kernel_count()):
+        if wd_kernel_name(k) == name:
+            return k
+    raise KeyError(name)

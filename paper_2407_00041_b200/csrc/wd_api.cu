@@ -1,0 +1,514 @@
+// wd_api.cu — the C-ABI of include/wd.h: handle, storage, load/pack paths, kernel selection.
+// There is no CPU fallback anywhere in this library: every operator application is a kernel
+// launch; if CUDA is unavailable the calls fail with WD_ECUDA.
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/wd.h"
+#include "wd_internal.h"
+
+using namespace wd;
+
+struct wd_handle {
+    int n[4];
+    long long V;
+    double m0, csw;
+    int device;
+    cudaStream_t stream;
+    double2 *dU, *dS;
+    bool has_gauge, has_clover;
+    // options
+    long variant, kernel_opt, tchunk_opt, zgroup_opt, device_pack;
+    // staging
+    double2 *pinned[2];
+    size_t pinned_bytes;
+    cudaEvent_t pinned_ev[2];
+    double2 *dstage;
+    size_t dstage_bytes;
+    double2 *work_in, *work_out;  // wd_apply_host
+    long launches;
+    std::string err;
+};
+
+static thread_local std::string g_create_err = "";
+
+static int fail(wd_handle *h, int code, const std::string &msg) {
+    if (h) h->err = msg; else g_create_err = msg;
+    return code;
+}
+
+#define WD_CUDA(h, call)                                                                          \
+    do {                                                                                          \
+        cudaError_t e_ = (call);                                                                  \
+        if (e_ != cudaSuccess)                                                                    \
+            return fail(h, (e_ == cudaErrorMemoryAllocation) ? WD_ENOMEM : WD_ECUDA,              \
+                        std::string(#call) + ": " + cudaGetErrorString(e_));                     \
+    } while (0)
+
+static const size_t kStageSites = 1 << 16;  // sites per host staging chunk
+
+static int ensure_pinned(wd_handle *h, size_t bytes) {
+    if (h->pinned_bytes >= bytes) return WD_OK;
+    for (int b = 0; b < 2; b++) {
+        if (h->pinned[b]) cudaFreeHost(h->pinned[b]);
+        h->pinned[b] = nullptr;
+    }
+    h->pinned_bytes = 0;
+    for (int b = 0; b < 2; b++) WD_CUDA(h, cudaMallocHost((void **)&h->pinned[b], bytes));
+    h->pinned_bytes = bytes;
+    return WD_OK;
+}
+
+static int ensure_dstage(wd_handle *h, size_t bytes) {
+    if (h->dstage_bytes >= bytes) return WD_OK;
+    if (h->dstage) cudaFree(h->dstage);
+    h->dstage = nullptr;
+    h->dstage_bytes = 0;
+    WD_CUDA(h, cudaMalloc((void **)&h->dstage, bytes));
+    h->dstage_bytes = bytes;
+    return WD_OK;
+}
+
+static void release_dstage(wd_handle *h) {
+    if (h->dstage) cudaFree(h->dstage);
+    h->dstage = nullptr;
+    h->dstage_bytes = 0;
+}
+
+extern "C" {
+
+const char *wd_version(void) { return "wd-b200 0.1 (sm_100a, FP64)"; }
+
+const char *wd_last_error(const wd_handle *h) { return h ? h->err.c_str() : g_create_err.c_str(); }
+
+int wd_create(wd_handle **out, int T, int Z, int Y, int X, double m0, double csw) {
+    if (!out) return fail(nullptr, WD_EINVAL, "wd_create: null handle pointer");
+    *out = nullptr;
+    if (T < 1 || Z < 1 || Y < 1 || X < 1) return fail(nullptr, WD_EINVAL, "wd_create: every lattice extent must be >= 1");
+    const long long V = (long long)T * Z * Y * X;
+    if (V > (1LL << 31) / 42) return fail(nullptr, WD_EINVAL, "wd_create: lattice too large for 32-bit element indexing");
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(nullptr, WD_ECUDA, std::string("wd_create: no CUDA device: ") + cudaGetErrorString(e));
+    wd_handle *h = new (std::nothrow) wd_handle();
+    if (!h) return fail(nullptr, WD_ENOMEM, "wd_create: out of host memory");
+    h->n[0] = T; h->n[1] = Z; h->n[2] = Y; h->n[3] = X;
+    h->V = V;
+    h->m0 = m0;
+    h->csw = csw;
+    h->device = dev;
+    h->stream = nullptr;
+    h->dU = h->dS = nullptr;
+    h->has_gauge = h->has_clover = false;
+    h->variant = 0;
+    h->kernel_opt = -1;
+    h->tchunk_opt = 0;
+    h->zgroup_opt = 0;
+    h->device_pack = 0;
+    h->pinned[0] = h->pinned[1] = nullptr;
+    h->pinned_bytes = 0;
+    h->pinned_ev[0] = h->pinned_ev[1] = nullptr;
+    h->dstage = nullptr;
+    h->dstage_bytes = 0;
+    h->work_in = h->work_out = nullptr;
+    h->launches = 0;
+    e = cudaMalloc((void **)&h->dU, (size_t)V * kGaugeComps * sizeof(double2));
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->pinned_ev[0], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->pinned_ev[1], cudaEventDisableTiming);
+    if (e != cudaSuccess) {
+        const int code = (e == cudaErrorMemoryAllocation) ? WD_ENOMEM : WD_ECUDA;
+        fail(nullptr, code, std::string("wd_create: ") + cudaGetErrorString(e));
+        wd_destroy(h);
+        cudaGetLastError();
+        return code;
+    }
+    *out = h;
+    return WD_OK;
+}
+
+int wd_destroy(wd_handle *h) {
+    if (!h) return WD_EINVAL;
+    cudaStreamSynchronize(h->stream);
+    if (h->dU) cudaFree(h->dU);
+    if (h->dS) cudaFree(h->dS);
+    if (h->dstage) cudaFree(h->dstage);
+    if (h->work_in) cudaFree(h->work_in);
+    if (h->work_out) cudaFree(h->work_out);
+    for (int b = 0; b < 2; b++) {
+        if (h->pinned[b]) cudaFreeHost(h->pinned[b]);
+        if (h->pinned_ev[b]) cudaEventDestroy(h->pinned_ev[b]);
+    }
+    delete h;
+    return WD_OK;
+}
+
+int wd_set_stream(wd_handle *h, void *cuda_stream) {
+    if (!h) return WD_EINVAL;
+    h->stream = (cudaStream_t)cuda_stream;
+    return WD_OK;
+}
+
+int wd_synchronize(wd_handle *h) {
+    if (!h) return WD_EINVAL;
+    WD_CUDA(h, cudaStreamSynchronize(h->stream));
+    return WD_OK;
+}
+
+// ---- host -> device loads ---------------------------------------------------------------------
+// Generic chunked path: pack `cnt` sites into pinned staging [ncomp_dev][cnt], then one strided
+// 2-D copy into the SoA arrays (row pitch V elements).  Two staging buffers alternate so that
+// packing chunk k+1 overlaps the copy of chunk k.
+typedef void (*pack_fn)(double2 *, const double2 *, long long, long long);
+
+static void pack_gauge_chunk(double2 *dst, const double2 *src, long long i0, long long cnt) {
+    host_pack_aos_to_soa(dst, src, i0, cnt, kGaugeComps);
+}
+static void pack_spinor_chunk(double2 *dst, const double2 *src, long long i0, long long cnt) {
+    host_pack_aos_to_soa(dst, src, i0, cnt, kSpinorComps);
+}
+
+static int load_chunked(wd_handle *h, double2 *dev, const double2 *host, int ncomp_dev, pack_fn pack) {
+    const long long V = h->V;
+    const long long chunk = (V < (long long)kStageSites) ? V : (long long)kStageSites;
+    int rc = ensure_pinned(h, (size_t)chunk * 42 * sizeof(double2));
+    if (rc) return rc;
+    int b = 0;
+    for (long long i0 = 0; i0 < V; i0 += chunk, b ^= 1) {
+        const long long cnt = (V - i0 < chunk) ? V - i0 : chunk;
+        WD_CUDA(h, cudaEventSynchronize(h->pinned_ev[b]));
+        pack(h->pinned[b], host, i0, cnt);
+        WD_CUDA(h, cudaMemcpy2DAsync(dev + i0, (size_t)V * sizeof(double2), h->pinned[b], (size_t)cnt * sizeof(double2),
+                                     (size_t)cnt * sizeof(double2), ncomp_dev, cudaMemcpyHostToDevice, h->stream));
+        WD_CUDA(h, cudaEventRecord(h->pinned_ev[b], h->stream));
+    }
+    WD_CUDA(h, cudaStreamSynchronize(h->stream));
+    return WD_OK;
+}
+
+typedef void (*unpack_fn)(double2 *, const double2 *, long long, long long);
+static void unpack_spinor_chunk(double2 *dst, const double2 *src, long long i0, long long cnt) {
+    host_unpack_soa_to_aos(dst, src, i0, cnt, kSpinorComps);
+}
+
+static int store_chunked(wd_handle *h, double2 *host, const double2 *dev, int ncomp_dev, unpack_fn unpack) {
+    const long long V = h->V;
+    const long long chunk = (V < (long long)kStageSites) ? V : (long long)kStageSites;
+    int rc = ensure_pinned(h, (size_t)chunk * 42 * sizeof(double2));
+    if (rc) return rc;
+    for (long long i0 = 0; i0 < V; i0 += chunk) {
+        const long long cnt = (V - i0 < chunk) ? V - i0 : chunk;
+        WD_CUDA(h, cudaMemcpy2DAsync(h->pinned[0], (size_t)cnt * sizeof(double2), dev + i0, (size_t)V * sizeof(double2),
+                                     (size_t)cnt * sizeof(double2), ncomp_dev, cudaMemcpyDeviceToHost, h->stream));
+        WD_CUDA(h, cudaStreamSynchronize(h->stream));
+        unpack(host, h->pinned[0], i0, cnt);
+    }
+    return WD_OK;
+}
+
+int wd_load_gauge(wd_handle *h, const double *host_U) {
+    if (!h) return WD_EINVAL;
+    if (!host_U) return fail(h, WD_EINVAL, "wd_load_gauge: null pointer");
+    const size_t bytes = (size_t)h->V * kGaugeComps * sizeof(double2);
+    if (h->device_pack) {
+        int rc = ensure_dstage(h, bytes);
+        if (rc) return rc;
+        WD_CUDA(h, cudaMemcpyAsync(h->dstage, host_U, bytes, cudaMemcpyHostToDevice, h->stream));
+        WD_CUDA(h, launch_aos_to_soa(h->dU, h->dstage, h->V, kGaugeComps, h->stream));
+        h->launches++;
+        WD_CUDA(h, cudaStreamSynchronize(h->stream));
+        release_dstage(h);
+    } else {
+        int rc = load_chunked(h, h->dU, (const double2 *)host_U, kGaugeComps, pack_gauge_chunk);
+        if (rc) return rc;
+    }
+    h->has_gauge = true;
+    return WD_OK;
+}
+
+static int ensure_clover_storage(wd_handle *h) {
+    if (!h->dS) WD_CUDA(h, cudaMalloc((void **)&h->dS, (size_t)h->V * kCloverSlots * sizeof(double2)));
+    return WD_OK;
+}
+
+int wd_load_clover(wd_handle *h, const double *host_C) {
+    if (!h) return WD_EINVAL;
+    if (!host_C) return fail(h, WD_EINVAL, "wd_load_clover: null pointer");
+    int rc = ensure_clover_storage(h);
+    if (rc) return rc;
+    if (h->device_pack) {
+        const size_t bytes = (size_t)h->V * kCloverCanon * sizeof(double2);
+        rc = ensure_dstage(h, bytes);
+        if (rc) return rc;
+        WD_CUDA(h, cudaMemcpyAsync(h->dstage, host_C, bytes, cudaMemcpyHostToDevice, h->stream));
+        WD_CUDA(h, launch_clover_canon_to_dev(h->dS, h->dstage, h->V, h->stream));
+        h->launches++;
+        WD_CUDA(h, cudaStreamSynchronize(h->stream));
+        release_dstage(h);
+    } else {
+        rc = load_chunked(h, h->dS, (const double2 *)host_C, kCloverSlots, host_pack_clover);
+        if (rc) return rc;
+    }
+    h->has_clover = true;
+    return WD_OK;
+}
+
+int wd_build_clover(wd_handle *h) {
+    if (!h) return WD_EINVAL;
+    if (!h->has_gauge) return fail(h, WD_ESTATE, "wd_build_clover: no gauge field loaded");
+    int rc = ensure_clover_storage(h);
+    if (rc) return rc;
+    WD_CUDA(h, launch_build_clover(h->dS, h->dU, h->n, h->V, h->m0 + 4.0, h->csw, h->stream));
+    h->launches++;
+    h->has_clover = true;
+    return WD_OK;
+}
+
+int wd_get_clover(wd_handle *h, double *host_C) {
+    if (!h) return WD_EINVAL;
+    if (!host_C) return fail(h, WD_EINVAL, "wd_get_clover: null pointer");
+    if (!h->has_clover) return fail(h, WD_ESTATE, "wd_get_clover: no self-coupling field present");
+    return store_chunked(h, (double2 *)host_C, h->dS, kCloverSlots, host_unpack_clover);
+}
+
+// ---- spinors ------------------------------------------------------------------------------------
+size_t wd_spinor_bytes(const wd_handle *h, int nrhs) {
+    if (!h || nrhs < 1) return 0;
+    return (size_t)nrhs * (size_t)h->V * kSpinorComps * sizeof(double2);
+}
+
+static bool misaligned(const void *p) { return ((size_t)p & 15) != 0; }
+
+int wd_pack_spinor(wd_handle *h, void *dev_dst, const double *host_src, int nrhs) {
+    if (!h) return WD_EINVAL;
+    if (!dev_dst || !host_src || nrhs < 1 || misaligned(dev_dst)) return fail(h, WD_EINVAL, "wd_pack_spinor: bad argument");
+    const size_t per = (size_t)h->V * kSpinorComps;
+    for (int r = 0; r < nrhs; r++) {
+        double2 *dst = (double2 *)dev_dst + r * per;
+        const double2 *src = (const double2 *)host_src + r * per;
+        if (h->device_pack) {
+            int rc = ensure_dstage(h, per * sizeof(double2));
+            if (rc) return rc;
+            WD_CUDA(h, cudaMemcpyAsync(h->dstage, src, per * sizeof(double2), cudaMemcpyHostToDevice, h->stream));
+            WD_CUDA(h, launch_aos_to_soa(dst, h->dstage, h->V, kSpinorComps, h->stream));
+            h->launches++;
+            WD_CUDA(h, cudaStreamSynchronize(h->stream));
+        } else {
+            int rc = load_chunked(h, dst, src, kSpinorComps, pack_spinor_chunk);
+            if (rc) return rc;
+        }
+    }
+    return WD_OK;
+}
+
+int wd_unpack_spinor(wd_handle *h, double *host_dst, const void *dev_src, int nrhs) {
+    if (!h) return WD_EINVAL;
+    if (!host_dst || !dev_src || nrhs < 1 || misaligned(dev_src)) return fail(h, WD_EINVAL, "wd_unpack_spinor: bad argument");
+    const size_t per = (size_t)h->V * kSpinorComps;
+    for (int r = 0; r < nrhs; r++) {
+        double2 *dst = (double2 *)host_dst + r * per;
+        const double2 *src = (const double2 *)dev_src + r * per;
+        if (h->device_pack) {
+            int rc = ensure_dstage(h, per * sizeof(double2));
+            if (rc) return rc;
+            WD_CUDA(h, launch_soa_to_aos(h->dstage, src, h->V, kSpinorComps, h->stream));
+            h->launches++;
+            WD_CUDA(h, cudaMemcpyAsync(dst, h->dstage, per * sizeof(double2), cudaMemcpyDeviceToHost, h->stream));
+            WD_CUDA(h, cudaStreamSynchronize(h->stream));
+        } else {
+            int rc = store_chunked(h, dst, src, kSpinorComps, unpack_spinor_chunk);
+            if (rc) return rc;
+        }
+    }
+    return WD_OK;
+}
+
+// ---- the host packer alone (CPU-testable) -------------------------------------------------------
+size_t wd_layout_bytes(int field, long long nsites) {
+    if (nsites < 1) return 0;
+    switch (field) {
+    case WD_FIELD_SPINOR: return (size_t)nsites * kSpinorComps * sizeof(double2);
+    case WD_FIELD_GAUGE: return (size_t)nsites * kGaugeComps * sizeof(double2);
+    case WD_FIELD_CLOVER: return (size_t)nsites * kCloverSlots * sizeof(double2);
+    default: return 0;
+    }
+}
+
+int wd_layout_pack_host(int field, long long nsites, const double *canonical, double *packed) {
+    if (nsites < 1 || !canonical || !packed) return WD_EINVAL;
+    switch (field) {
+    case WD_FIELD_SPINOR: host_pack_aos_to_soa((double2 *)packed, (const double2 *)canonical, 0, nsites, kSpinorComps); return WD_OK;
+    case WD_FIELD_GAUGE: host_pack_aos_to_soa((double2 *)packed, (const double2 *)canonical, 0, nsites, kGaugeComps); return WD_OK;
+    case WD_FIELD_CLOVER: host_pack_clover((double2 *)packed, (const double2 *)canonical, 0, nsites); return WD_OK;
+    default: return WD_EINVAL;
+    }
+}
+
+int wd_layout_unpack_host(int field, long long nsites, const double *packed, double *canonical) {
+    if (nsites < 1 || !canonical || !packed) return WD_EINVAL;
+    switch (field) {
+    case WD_FIELD_SPINOR: host_unpack_soa_to_aos((double2 *)canonical, (const double2 *)packed, 0, nsites, kSpinorComps); return WD_OK;
+    case WD_FIELD_GAUGE: host_unpack_soa_to_aos((double2 *)canonical, (const double2 *)packed, 0, nsites, kGaugeComps); return WD_OK;
+    case WD_FIELD_CLOVER: host_unpack_clover((double2 *)canonical, (const double2 *)packed, 0, nsites); return WD_OK;
+    default: return WD_EINVAL;
+    }
+}
+
+// ---- kernel selection -----------------------------------------------------------------------------
+static bool geometry_fits(const wd_handle *h, const KernelInfo &k) {
+    if (k.bx == 0) return true;
+    return h->n[0] % k.bt == 0 && h->n[1] % k.bz == 0 && h->n[2] % k.by == 0 && h->n[3] % k.bx == 0;
+}
+
+static int auto_kernel(const wd_handle *h) {
+    // preference order among the tiled geometries; linear256 always fits
+    static const char *pref[] = {"tile_1x4x4x16", "tile_1x4x8x8", "tile_1x2x4x32", "tile_2x4x4x8", "tile_4x4x4x4",
+                                 "tile_1x4x4x8", "tile_1x4x4x4"};
+    for (const char *name : pref)
+        for (int id = 0; id < kernel_count(); id++)
+            if (!strcmp(kernel_info(id).name, name) && geometry_fits(h, kernel_info(id))) return id;
+    return 0;
+}
+
+int wd_kernel_count(void) { return kernel_count(); }
+const char *wd_kernel_name(int id) { return (id >= 0 && id < kernel_count()) ? kernel_info(id).name : nullptr; }
+
+int wd_kernel_in_use(const wd_handle *h) {
+    if (!h) return WD_EINVAL;
+    if (h->kernel_opt >= 0) return (int)h->kernel_opt;
+    return auto_kernel(h);
+}
+
+long wd_launch_count(const wd_handle *h) { return h ? h->launches : 0; }
+
+int wd_set_option(wd_handle *h, int option, long value) {
+    if (!h) return WD_EINVAL;
+    switch (option) {
+    case WD_OPT_VARIANT:
+        if (value != 0 && value != 1) return fail(h, WD_EINVAL, "WD_OPT_VARIANT: 0 (fused) or 1 (unfused)");
+        h->variant = value;
+        return WD_OK;
+    case WD_OPT_KERNEL:
+        if (value < -1 || value >= kernel_count()) return fail(h, WD_EINVAL, "WD_OPT_KERNEL: id out of range");
+        if (value >= 0 && !geometry_fits(h, kernel_info((int)value)))
+            return fail(h, WD_EINVAL, std::string("WD_OPT_KERNEL: tile of ") + kernel_info((int)value).name + " does not divide the lattice");
+        h->kernel_opt = value;
+        return WD_OK;
+    case WD_OPT_TCHUNK:
+        if (value < 0 || (value > 0 && h->n[0] % value != 0)) return fail(h, WD_EINVAL, "WD_OPT_TCHUNK: must divide T");
+        h->tchunk_opt = value;
+        return WD_OK;
+    case WD_OPT_ZGROUP:
+        if (value < 0) return fail(h, WD_EINVAL, "WD_OPT_ZGROUP: must be >= 0");
+        h->zgroup_opt = value;
+        return WD_OK;
+    case WD_OPT_DEVICE_PACK:
+        h->device_pack = value ? 1 : 0;
+        return WD_OK;
+    default:
+        return fail(h, WD_EINVAL, "wd_set_option: unknown option");
+    }
+}
+
+int wd_get_option(const wd_handle *h, int option, long *value) {
+    if (!h || !value) return WD_EINVAL;
+    switch (option) {
+    case WD_OPT_VARIANT: *value = h->variant; return WD_OK;
+    case WD_OPT_KERNEL: *value = h->kernel_opt; return WD_OK;
+    case WD_OPT_TCHUNK: *value = h->tchunk_opt; return WD_OK;
+    case WD_OPT_ZGROUP: *value = h->zgroup_opt; return WD_OK;
+    case WD_OPT_DEVICE_PACK: *value = h->device_pack; return WD_OK;
+    default: return WD_EINVAL;
+    }
+}
+
+// ---- apply ------------------------------------------------------------------------------------------
+static int fill_params(wd_handle *h, KParams &p, const KernelInfo &k) {
+    p.U = h->dU;
+    p.S = h->dS;
+    p.V = h->V;
+    for (int a = 0; a < 4; a++) p.n[a] = h->n[a];
+    p.stride[3] = 1;
+    p.stride[2] = h->n[3];
+    p.stride[1] = h->n[3] * h->n[2];
+    p.stride[0] = h->n[3] * h->n[2] * h->n[1];
+    p.mass = h->m0 + 4.0;
+    p.ntx = p.nty = p.ntz = p.ntc = p.gz = p.tchunk = 1;
+    if (k.bx) {
+        p.ntx = h->n[3] / k.bx;
+        p.nty = h->n[2] / k.by;
+        p.ntz = h->n[1] / k.bz;
+        long tchunk = h->tchunk_opt;
+        if (tchunk == 0) {  // automatic: the largest divisor of T that is <= 16 and a multiple of BT
+            tchunk = k.bt;
+            for (int c = k.bt; c <= 16 && c <= h->n[0]; c += k.bt)
+                if (h->n[0] % c == 0) tchunk = c;
+        }
+        if (tchunk % k.bt != 0 || h->n[0] % tchunk != 0) return fail(h, WD_EINVAL, "WD_OPT_TCHUNK incompatible with the kernel's T tile");
+        p.tchunk = (int)tchunk;
+        p.ntc = h->n[0] / p.tchunk;
+        long gz = h->zgroup_opt;
+        if (gz == 0) gz = p.ntz;  // automatic: one group (whole Z range)
+        if (gz > p.ntz || p.ntz % gz != 0) return fail(h, WD_EINVAL, "WD_OPT_ZGROUP must divide the number of Z tiles");
+        p.gz = (int)gz;
+    }
+    return WD_OK;
+}
+
+int wd_apply(wd_handle *h, void *dev_out, const void *dev_in, int nrhs) {
+    if (!h) return WD_EINVAL;
+    if (!dev_out || !dev_in || nrhs < 1) return fail(h, WD_EINVAL, "wd_apply: null pointer or nrhs < 1");
+    if (misaligned(dev_out) || misaligned(dev_in)) return fail(h, WD_EINVAL, "wd_apply: spinor buffers must be 16-byte aligned");
+    const size_t bytes = wd_spinor_bytes(h, nrhs);
+    const char *o = (const char *)dev_out, *i = (const char *)dev_in;
+    if (o < i + bytes && i < o + bytes) return fail(h, WD_EINVAL, "wd_apply: out overlaps in");
+    if (!h->has_gauge) return fail(h, WD_ESTATE, "wd_apply: no gauge field loaded");
+    if (h->csw != 0.0 && !h->has_clover)
+        return fail(h, WD_ESTATE, "wd_apply: csw != 0 but no self-coupling field (wd_load_clover / wd_build_clover)");
+    const int kid = wd_kernel_in_use(h);
+    const KernelInfo &k = kernel_info(kid);
+    KParams p;
+    int rc = fill_params(h, p, k);
+    if (rc) return rc;
+    const int self = h->has_clover ? SELF_CLOVER : SELF_MASS;
+    const size_t per = (size_t)h->V * kSpinorComps;
+    for (int r = 0; r < nrhs; r++) {
+        p.psi = (const double2 *)dev_in + r * per;
+        p.out = (double2 *)dev_out + r * per;
+        if (h->variant == 0) {
+            WD_CUDA(h, k.launch(p, self, h->stream));
+            h->launches++;
+        } else {
+            WD_CUDA(h, k.launch(p, SELF_NONE, h->stream));
+            WD_CUDA(h, launch_selfcoupling(p, self, h->stream));
+            h->launches += 2;
+        }
+    }
+    return WD_OK;
+}
+
+int wd_apply_host(wd_handle *h, double *host_out, const double *host_in, int nrhs) {
+    if (!h) return WD_EINVAL;
+    if (!host_out || !host_in || nrhs < 1) return fail(h, WD_EINVAL, "wd_apply_host: null pointer or nrhs < 1");
+    const size_t per = (size_t)h->V * kSpinorComps, bytes = per * sizeof(double2);
+    if (!h->work_in) WD_CUDA(h, cudaMalloc((void **)&h->work_in, bytes));
+    if (!h->work_out) WD_CUDA(h, cudaMalloc((void **)&h->work_out, bytes));
+    int rc = ensure_dstage(h, bytes);
+    if (rc) return rc;
+    for (int r = 0; r < nrhs; r++) {
+        WD_CUDA(h, cudaMemcpyAsync(h->dstage, (const double2 *)host_in + r * per, bytes, cudaMemcpyHostToDevice, h->stream));
+        WD_CUDA(h, launch_aos_to_soa(h->work_in, h->dstage, h->V, kSpinorComps, h->stream));
+        h->launches++;
+        rc = wd_apply(h, h->work_out, h->work_in, 1);
+        if (rc) return rc;
+        WD_CUDA(h, launch_soa_to_aos(h->dstage, h->work_out, h->V, kSpinorComps, h->stream));
+        h->launches++;
+        WD_CUDA(h, cudaMemcpyAsync((double2 *)host_out + r * per, h->dstage, bytes, cudaMemcpyDeviceToHost, h->stream));
+    }
+    WD_CUDA(h, cudaStreamSynchronize(h->stream));
+    return WD_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,72 @@
+// wd_internal.h — shared declarations of libwd's translation units (not part of the C-ABI).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <string>
+
+namespace wd {
+
+// ---------------------------------------------------------------------------------------------
+// Device layout ("SoA over sites").  Element = one complex
+// double = double2 = 16 B; the site index i (canonical order, X fastest) is the fastest index of
+// every array, so a warp that handles 32 consecutive sites reads 512 contiguous bytes per
+// component:
+//   spinor  double2 [nrhs][12][V]       component c = 3*spin + colour
+//   gauge   double2 [4][9][V]           mu = T,Z,Y,X; k = 3*row + col; forward links only, each
+//                                       link stored ONCE (U_mu(x-mu) is read from site x-mu)
+//   selfcpl double2 [36][V]             slot j<6: (S_{2j,2j}, S_{2j+1,2j+1}) real diagonal pairs;
+//                                       slot 6+k: k-th strict-upper entry of block A (k<15) then
+//                                       block B (72 reals = 576 B per site, R6/R7)
+// ---------------------------------------------------------------------------------------------
+constexpr int kSpinorComps = 12;
+constexpr int kGaugeComps = 36;
+constexpr int kCloverSlots = 36;
+constexpr int kCloverCanon = 42;
+
+enum SelfMode { SELF_NONE = 0, SELF_MASS = 1, SELF_CLOVER = 2 };
+
+struct KParams {
+    const double2 *psi;
+    const double2 *U;
+    const double2 *S;
+    double2 *out;
+    long long V;
+    int n[4];       // T, Z, Y, X
+    int stride[4];  // site-index strides of T, Z, Y, X
+    double mass;    // m0 + 4
+    // tiled geometries: rasterisation of CTAs (see wd_kernels.cu)
+    int ntx, nty, ntz, ntc;  // number of tiles in X, Y, Z and of T-chunks
+    int gz;                  // Z-tiles per rasterisation group
+    int tchunk;              // T-extent marched by one CTA
+};
+
+struct KernelInfo {
+    const char *name;
+    int bt, bz, by, bx;  // tile extents (all 0: linear geometry, any lattice)
+    int threads;
+    cudaError_t (*launch)(const KParams &p, int self, cudaStream_t st);
+};
+
+int kernel_count();
+const KernelInfo &kernel_info(int id);
+
+// self-coupling kernel of the unfused variant: out += S psi (clover) or out += mass * psi
+cudaError_t launch_selfcoupling(const KParams &p, int self, cudaStream_t st);
+
+// device-side layout transposes (wd_pack.cu): canonical AoS <-> device SoA, on device buffers
+cudaError_t launch_aos_to_soa(double2 *dst_soa, const double2 *src_aos, long long V, int ncomp, cudaStream_t st);
+cudaError_t launch_soa_to_aos(double2 *dst_aos, const double2 *src_soa, long long V, int ncomp, cudaStream_t st);
+cudaError_t launch_clover_canon_to_dev(double2 *dst_slots, const double2 *src42, long long V, cudaStream_t st);
+cudaError_t launch_clover_dev_to_canon(double2 *dst42, const double2 *src_slots, long long V, cudaStream_t st);
+
+// host packers (wd_pack.cu): canonical AoS chunk [i0, i0+cnt) -> SoA staging [ncomp][cnt]
+void host_pack_aos_to_soa(double2 *dst, const double2 *src_aos, long long i0, long long cnt, int ncomp);
+void host_unpack_soa_to_aos(double2 *dst_aos, const double2 *src, long long i0, long long cnt, int ncomp);
+void host_pack_clover(double2 *dst, const double2 *src42, long long i0, long long cnt);
+void host_unpack_clover(double2 *dst42, const double2 *src, long long i0, long long cnt);
+
+// device clover construction (wd_clover.cu): S slots from the device gauge field
+cudaError_t launch_build_clover(double2 *S_slots, const double2 *U, const int n[4], long long V, double mass,
+                                double csw, cudaStream_t st);
+
+}  // namespace wd

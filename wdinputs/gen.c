@@ -35,23 +35,38 @@ static inline double u01(uint64_t seed, uint64_t ctr) {
     return ((double)(r >> 11) + 0.5) * (1.0 / 9007199254740992.0);
 }
 
-/* n-th standard normal of stream `seed` (Box-Muller on the pair n/2) */
-static inline double gauss(uint64_t seed, uint64_t n) {
-    uint64_t pair = n >> 1;
+/* pair-th Box-Muller pair of stream `seed`: two independent standard normals */
+static inline void gauss_pair(uint64_t seed, uint64_t pair, double *g0, double *g1) {
     double u1 = u01(seed, 2 * pair), u2 = u01(seed, 2 * pair + 1);
     double r = sqrt(-2.0 * log(u1));
     double a = 6.283185307179586476925286766559 * u2;
-    return (n & 1) ? r * sin(a) : r * cos(a);
+    *g0 = r * cos(a);
+    *g1 = r * sin(a);
+}
+
+/* n-th standard normal of stream `seed` */
+static inline double gauss(uint64_t seed, uint64_t n) {
+    double g0, g1;
+    gauss_pair(seed, n >> 1, &g0, &g1);
+    return (n & 1) ? g1 : g0;
 }
 
 void wdin_gaussian(double *out, uint64_t n, uint64_t seed) {
 #pragma omp parallel for schedule(static)
-    for (int64_t i = 0; i < (int64_t)n; i++) out[i] = gauss(seed, (uint64_t)i);
+    for (int64_t p = 0; p < (int64_t)((n + 1) / 2); p++) {
+        double g0, g1;
+        gauss_pair(seed, (uint64_t)p, &g0, &g1);
+        out[2 * p] = g0;
+        if ((uint64_t)(2 * p + 1) < n) out[2 * p + 1] = g1;
+    }
 }
 
 static void gaussian_3x3(cplx g[3][3], uint64_t seed, uint64_t link) {
-    for (int k = 0; k < 9; k++)
-        g[k / 3][k % 3] = gauss(seed, 18 * link + 2 * k) + I * gauss(seed, 18 * link + 2 * k + 1);
+    for (int k = 0; k < 9; k++) {
+        double re, im;
+        gauss_pair(seed, 9 * link + k, &re, &im);
+        g[k / 3][k % 3] = re + I * im;
+    }
 }
 
 static cplx det3(cplx m[3][3]) {
