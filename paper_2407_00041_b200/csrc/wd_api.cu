@@ -436,6 +436,8 @@ static int fill_params(wd_handle *h, KParams &p, const KernelInfo &k) {
     p.stride[0] = h->n[3] * h->n[2] * h->n[1];
     p.mass = h->m0 + 4.0;
     p.ntx = p.nty = p.ntz = p.ntc = p.gz = p.tchunk = 1;
+    p.opt_tchunk = (int)h->tchunk_opt;
+    p.opt_zgroup = (int)h->zgroup_opt;
     if (k.bx) {
         p.ntx = h->n[3] / k.bx;
         p.nty = h->n[2] / k.by;

@@ -132,12 +132,12 @@ __global__ void __launch_bounds__(128) k_build_clover(const CloverParams p) {
     // store the 36 slots (wd_internal.h): real diagonal pairs, then the strict upper triangles
     for (int j = 0; j < 6; j++) {
         const int b = j / 3, r = 2 * (j % 3);
-        p.S[(long long)j * V + i] = make_double2(blk[b][r][r].x, blk[b][r + 1][r + 1].x);
+        p.S[(long long)slot_diag(b, j % 3) * V + i] = make_double2(blk[b][r][r].x, blk[b][r + 1][r + 1].x);
     }
     for (int b = 0; b < 2; b++) {
-        int k = 6 + 15 * b;
+        int k = 0;
         for (int r = 0; r < 6; r++)
-            for (int q2 = r + 1; q2 < 6; q2++, k++) p.S[(long long)k * V + i] = blk[b][r][q2];
+            for (int q2 = r + 1; q2 < 6; q2++, k++) p.S[(long long)slot_off(b, k) * V + i] = blk[b][r][q2];
     }
 }
 

@@ -14,14 +14,19 @@ namespace wd {
 //   spinor  double2 [nrhs][12][V]       component c = 3*spin + colour
 //   gauge   double2 [4][9][V]           mu = T,Z,Y,X; k = 3*row + col; forward links only, each
 //                                       link stored ONCE (U_mu(x-mu) is read from site x-mu)
-//   selfcpl double2 [36][V]             slot j<6: (S_{2j,2j}, S_{2j+1,2j+1}) real diagonal pairs;
-//                                       slot 6+k: k-th strict-upper entry of block A (k<15) then
-//                                       block B (72 reals = 576 B per site, R6/R7)
+//   selfcpl double2 [36][V]             18 slots per chirality block b (A = 0, B = 1), block-contiguous
+//                                       so that one block is one TMA box: slot 18b+j (j<3) holds the
+//                                       real diagonal pair (B_{2j,2j}, B_{2j+1,2j+1}); slot 18b+3+k the
+//                                       k-th strict-upper entry (row-major) of the 6x6 block
+//                                       (72 reals = 576 B per site, R6/R7)
 // ---------------------------------------------------------------------------------------------
 constexpr int kSpinorComps = 12;
 constexpr int kGaugeComps = 36;
 constexpr int kCloverSlots = 36;
 constexpr int kCloverCanon = 42;
+
+__host__ __device__ constexpr int slot_diag(int b, int j) { return 18 * b + j; }      // j = 0..2
+__host__ __device__ constexpr int slot_off(int b, int k) { return 18 * b + 3 + k; }   // k = 0..14
 
 enum SelfMode { SELF_NONE = 0, SELF_MASS = 1, SELF_CLOVER = 2 };
 
@@ -38,6 +43,7 @@ struct KParams {
     int ntx, nty, ntz, ntc;  // number of tiles in X, Y, Z and of T-chunks
     int gz;                  // Z-tiles per rasterisation group
     int tchunk;              // T-extent marched by one CTA
+    int opt_tchunk, opt_zgroup;  // the raw WD_OPT_TCHUNK / WD_OPT_ZGROUP values (0 = automatic)
 };
 
 struct KernelInfo {
@@ -49,6 +55,10 @@ struct KernelInfo {
 
 int kernel_count();
 const KernelInfo &kernel_info(int id);
+
+// TMA-staged T-marching kernels (wd_tma.cu)
+cudaError_t launch_tma_2x4x16(const KParams &p, int self, cudaStream_t st);
+cudaError_t launch_tma_4x4x8(const KParams &p, int self, cudaStream_t st);
 
 // self-coupling kernel of the unfused variant: out += S psi (clover) or out += mass * psi
 cudaError_t launch_selfcoupling(const KParams &p, int self, cudaStream_t st);

@@ -89,12 +89,12 @@ __device__ __forceinline__ void site_apply(const KParams &p, long long i, int t,
             double d[6];
 #pragma unroll
             for (int j = 0; j < 3; j++) {
-                const cd dd = ldg(S + (long long)(3 * b + j) * V + i);
+                const cd dd = ldg(S + (long long)slot_diag(b, j) * V + i);
                 d[2 * j] = dd.x;
                 d[2 * j + 1] = dd.y;
             }
 #pragma unroll
-            for (int k = 0; k < 15; k++) a[k] = ldg(S + (long long)(6 + 15 * b + k) * V + i);
+            for (int k = 0; k < 15; k++) a[k] = ldg(S + (long long)slot_off(b, k) * V + i);
 #pragma unroll
             for (int c = 0; c < 6; c++) q[c] = ldg(psi + (long long)(6 * b + c) * V + i);
             herm6_mul(r, d, a, q);
@@ -187,12 +187,12 @@ template <int SELF> __global__ void __launch_bounds__(256) k_selfcoupling(const 
             double d[6];
 #pragma unroll
             for (int j = 0; j < 3; j++) {
-                const cd dd = ldg(S + (long long)(3 * b + j) * V + i);
+                const cd dd = ldg(S + (long long)slot_diag(b, j) * V + i);
                 d[2 * j] = dd.x;
                 d[2 * j + 1] = dd.y;
             }
 #pragma unroll
-            for (int k = 0; k < 15; k++) a[k] = ldg(S + (long long)(6 + 15 * b + k) * V + i);
+            for (int k = 0; k < 15; k++) a[k] = ldg(S + (long long)slot_off(b, k) * V + i);
 #pragma unroll
             for (int c = 0; c < 6; c++) q[c] = ldg(psi + (long long)(6 * b + c) * V + i);
             herm6_mul(r, d, a, q);
@@ -228,6 +228,8 @@ static const KernelInfo kKernels[] = {
     {"tile_1x2x4x16", 1, 2, 4, 16, 128, launch_tiled<1, 2, 4, 16>},
     {"tile_1x2x2x32", 1, 2, 2, 32, 128, launch_tiled<1, 2, 2, 32>},
     {"tile_1x4x4x4", 1, 4, 4, 4, 64, launch_tiled<1, 4, 4, 4>},
+    {"tma_2x4x16", 1, 2, 4, 16, 160, launch_tma_2x4x16},
+    {"tma_4x4x8", 1, 4, 4, 8, 160, launch_tma_4x4x8},
 };
 
 int kernel_count() { return (int)(sizeof(kKernels) / sizeof(kKernels[0])); }

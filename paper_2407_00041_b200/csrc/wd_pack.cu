@@ -33,13 +33,16 @@ void host_unpack_soa_to_aos(double2 *dst_aos, const double2 *src, long long i0, 
     }
 }
 
-// canonical 42 complex -> 36 slots: slot j<6 = (Re c[2j], Re c[2j+1]); slot 6+k = c[12+k]
+// canonical 42 complex -> 36 slots (wd_internal.h): pair q of the real diagonal -> slot_diag(q/3, q%3),
+// strict-upper entry k of c[12..41] -> slot_off(k/15, k%15)
+__host__ __device__ static inline int slot_of_pair(int q) { return slot_diag(q / 3, q % 3); }
+__host__ __device__ static inline int slot_of_upper(int k) { return slot_off(k / 15, k % 15); }
 void host_pack_clover(double2 *dst, const double2 *src42, long long i0, long long cnt) {
 #pragma omp parallel for schedule(static)
     for (long long j = 0; j < cnt; j++) {
         const double2 *s = src42 + (i0 + j) * kCloverCanon;
-        for (int q = 0; q < 6; q++) dst[(long long)q * cnt + j] = make_double2(s[2 * q].x, s[2 * q + 1].x);
-        for (int k = 0; k < 30; k++) dst[(long long)(6 + k) * cnt + j] = s[12 + k];
+        for (int q = 0; q < 6; q++) dst[(long long)slot_of_pair(q) * cnt + j] = make_double2(s[2 * q].x, s[2 * q + 1].x);
+        for (int k = 0; k < 30; k++) dst[(long long)slot_of_upper(k) * cnt + j] = s[12 + k];
     }
 }
 
@@ -48,11 +51,11 @@ void host_unpack_clover(double2 *dst42, const double2 *src, long long i0, long l
     for (long long j = 0; j < cnt; j++) {
         double2 *d = dst42 + (i0 + j) * kCloverCanon;
         for (int q = 0; q < 6; q++) {
-            const double2 v = src[(long long)q * cnt + j];
+            const double2 v = src[(long long)slot_of_pair(q) * cnt + j];
             d[2 * q] = make_double2(v.x, 0.0);
             d[2 * q + 1] = make_double2(v.y, 0.0);
         }
-        for (int k = 0; k < 30; k++) d[12 + k] = src[(long long)(6 + k) * cnt + j];
+        for (int k = 0; k < 30; k++) d[12 + k] = src[(long long)slot_of_upper(k) * cnt + j];
     }
 }
 
@@ -109,18 +112,20 @@ __global__ void __launch_bounds__(256) k_clover_convert(double2 *__restrict__ ds
             tile[(e / kCloverCanon) * pitch + (e % kCloverCanon)] = src[i0 * kCloverCanon + e];
         __syncthreads();
         for (int e = threadIdx.x; e < kCloverSlots * TS; e += blockDim.x) {
-            const int q = e / TS, j = e % TS;
+            const int q = e / TS, j = e % TS;  // q = 0..5 diagonal pairs, 6..35 strict-upper entries
             if (j >= cnt) continue;
             double2 v;
             if (q < 6) v = make_double2(tile[j * pitch + 2 * q].x, tile[j * pitch + 2 * q + 1].x);
             else v = tile[j * pitch + 6 + q];
-            dst[(long long)q * V + i0 + j] = v;
+            const int slot = (q < 6) ? slot_of_pair(q) : slot_of_upper(q - 6);
+            dst[(long long)slot * V + i0 + j] = v;
         }
     } else {
         for (int e = threadIdx.x; e < kCloverSlots * TS; e += blockDim.x) {
             const int q = e / TS, j = e % TS;
             if (j >= cnt) continue;
-            const double2 v = src[(long long)q * V + i0 + j];
+            const int slot = (q < 6) ? slot_of_pair(q) : slot_of_upper(q - 6);
+            const double2 v = src[(long long)slot * V + i0 + j];
             if (q < 6) {
                 tile[j * pitch + 2 * q] = make_double2(v.x, 0.0);
                 tile[j * pitch + 2 * q + 1] = make_double2(v.y, 0.0);

@@ -1,0 +1,491 @@
+// wd_tma.cu — the Blackwell-native fused Wilson-clover kernel: TMA-staged, warp-specialised,
+// marching along T.
+//
+// out(x) = S(x) psi(x) - 1/2 sum_mu [ (1-gamma_mu) U_mu(x) psi(x+mu) + (1+gamma_mu) U_mu(x-mu)^H psi(x-mu) ]
+// (eq. 1.13), steps a1-a7 of SURVEY.md §8(a) in one pass.
+//
+// Why this shape (profiles/r1a_*.md): the one-thread-per-site LDG kernels are latency-bound — the
+// bytes in flight per SM are (resident warps) x (registers a thread can spare), and with 140-180
+// registers per thread only 8-11 warps fit.  Here the bytes in flight are decoupled from registers:
+//   * a persistent CTA (one per SM) owns a BZ x BY x BX tile of sites and marches it along T;
+//   * ONE producer thread streams everything the tile needs — own links, the x-mu face links, S,
+//     psi and its six spatial faces — into ~222 KB of shared memory with cp.async.bulk.tensor
+//     (5-D tensor maps over the SoA fields), each object guarded by a full/empty mbarrier pair;
+//   * N = BZ*BY*BX compute threads (one per site) read operands from shared memory only
+//     (conflict-free LDS.128 on the SoA boxes), so they never wait on DRAM directly;
+//   * each object's buffer is refilled for slice t+1 as soon as slice t has consumed it: at any
+//     time all of shared memory except the object being consumed is either landing or waiting,
+//     i.e. ~150-200 KB in flight per SM (Little: 6.5 TB/s x ~1 us / 148 SMs = 45 KB needed).
+// T direction: psi(t-1) and psi(t+1) are never fetched.  The backward hop of slice t uses the
+// half-spinor (1+gamma_T) psi(t-1) carried in registers from the previous step; the forward hop
+// of slice t-1 is added when psi(t) arrives, just before out(t-1) is stored (U_T(t-1) is the
+// "T object").  So per site and step HBM supplies psi 192 + U 576 + S 576 B and takes 192 B: the
+// algorithmic 1536 B, plus face re-reads that hit L2 (neighbouring tiles march concurrently).
+// Neighbour indexing and the periodic wrap (a1) are box coordinates computed by the producer.
+#include <cstdio>
+
+#include "wd_internal.h"
+#include "wd_math.cuh"
+#include "wd_tma.cuh"
+
+namespace wd {
+
+// ---------------------------------------------------------------- tensor-map encoder (host)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+cudaError_t encode_field_map(CUtensorMap *map, const void *base, const int n[4], int ncomp, int bx, int by, int bz,
+                             int bc) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return cudaErrorNotSupported;
+    const cuuint64_t T = n[0], Z = n[1], Y = n[2], X = n[3];
+    const cuuint64_t dims[5] = {2 * X, Y, Z, T, (cuuint64_t)ncomp};
+    const cuuint64_t strides[4] = {X * 16, X * Y * 16, X * Y * Z * 16, X * Y * Z * T * 16};  // bytes, dims 1..4
+    const cuuint32_t box[5] = {(cuuint32_t)(2 * bx), (cuuint32_t)by, (cuuint32_t)bz, 1u, (cuuint32_t)bc};
+    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    const CUtensorMapL2promotion promo = (bx * 16 >= 256)   ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B
+                                         : (bx * 16 >= 128) ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B
+                                                            : CU_TENSOR_MAP_L2_PROMOTION_NONE;
+    const CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, const_cast<void *>(base), dims, strides, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, promo,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return (r == CUDA_SUCCESS) ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+// ---------------------------------------------------------------- shared-memory plan
+// Objects (each with a full/empty mbarrier pair), refilled once per T step:
+//   C  psi(t) interior                                    [12][N]
+//   T  U_T(t-1) interior                                  [9][N]
+//   Z  U_Z(t) interior | U_Z face z0-1 | psi faces z0-1, z0+BZ      [9][N] [9][FZ] [12][FZ] [12][FZ]
+//   Y  same for Y;  X  same for X
+//   SA, SB  the two 6x6 blocks of S(t)                    [18][N] each
+enum { OB_C = 0, OB_T, OB_Z, OB_Y, OB_X, OB_SA, OB_SB, OB_COUNT };
+
+template <int BZ_, int BY_, int BX_, int SELF_> struct Plan {
+    static constexpr int BZ = BZ_, BY = BY_, BX = BX_, SELF = SELF_;
+    static constexpr int N = BZ * BY * BX;  // sites per tile = compute threads
+    static constexpr int NW = N / 32;       // compute warps
+    static constexpr int NTHREADS = N + 32; // + the producer warp
+    static constexpr int FZ = BY * BX, FY = BZ * BX, FX = BZ * BY;  // sites per face
+    static constexpr uint32_t E = 16;                               // bytes per element
+    static constexpr uint32_t SZ_C = 12 * N * E, SZ_U = 9 * N * E, SZ_S = 18 * N * E;
+    static constexpr uint32_t OFF_C = 0;
+    static constexpr uint32_t OFF_T = OFF_C + SZ_C;
+    static constexpr uint32_t OFF_Z = OFF_T + SZ_U;
+    static constexpr uint32_t OFF_ZUF = OFF_Z + SZ_U, OFF_ZLO = OFF_ZUF + 9 * FZ * E, OFF_ZHI = OFF_ZLO + 12 * FZ * E;
+    static constexpr uint32_t SZ_Z = SZ_U + (9 + 24) * FZ * E;
+    static constexpr uint32_t OFF_Y = OFF_Z + SZ_Z;
+    static constexpr uint32_t OFF_YUF = OFF_Y + SZ_U, OFF_YLO = OFF_YUF + 9 * FY * E, OFF_YHI = OFF_YLO + 12 * FY * E;
+    static constexpr uint32_t SZ_Y = SZ_U + (9 + 24) * FY * E;
+    static constexpr uint32_t OFF_X = OFF_Y + SZ_Y;
+    static constexpr uint32_t OFF_XUF = OFF_X + SZ_U, OFF_XLO = OFF_XUF + 9 * FX * E, OFF_XHI = OFF_XLO + 12 * FX * E;
+    static constexpr uint32_t SZ_X = SZ_U + (9 + 24) * FX * E;
+    static constexpr uint32_t OFF_SA = OFF_X + SZ_X;
+    static constexpr uint32_t OFF_SB = OFF_SA + SZ_S;
+    static constexpr uint32_t OFF_BAR = (SELF == SELF_CLOVER) ? OFF_SB + SZ_S : OFF_SA;
+    static constexpr uint32_t SMEM = OFF_BAR + 2 * OB_COUNT * 8;
+    static_assert(N % 32 == 0 && FZ % 8 == 0 && FY % 8 == 0 && FX % 8 == 0, "tile faces must keep 128-byte alignment");
+    static_assert(SMEM <= 232448, "shared-memory plan exceeds 227 KB");
+};
+
+struct TmaMaps {
+    CUtensorMap psi_c, psi_z, psi_y, psi_x;  // boxes: interior, z-face, y-face, x-face (12 components)
+    CUtensorMap u_c, u_z, u_y, u_x;          // same shapes, 9 components (one link)
+    CUtensorMap s_c;                         // interior box, 18 components (one 6x6 block)
+};
+
+struct TmaParams {
+    double2 *out;
+    long long V;
+    int n[4];
+    int ntx, nty, ntz;   // tiles per direction
+    int py, pz;          // rasterisation panel (in tiles); py | nty, pz | ntz
+    int tchunk, ntc;     // T steps per work item, items per tile
+    int nitems;          // ntx*nty*ntz*ntc
+    double mass;
+};
+
+// ---------------------------------------------------------------- shared-memory operand fetch
+__device__ __forceinline__ cd lds(const unsigned char *smem, uint32_t off) {
+    return *reinterpret_cast<const cd *>(smem + off);
+}
+
+// One direction MU != T of the stencil for the thread's site: both hops, operands from shared
+// memory.  (base, stride) pairs select interior or face storage per thread (no divergence: both
+// are shared-memory addresses).
+template <int MU>
+__device__ __forceinline__ void hop_pair_smem(cd acc[12], const unsigned char *smem, uint32_t u_own, uint32_t u_own_stride,
+                                              uint32_t pf, uint32_t pf_stride, uint32_t ub, uint32_t ub_stride,
+                                              uint32_t pb, uint32_t pb_stride) {
+    cd p[12], u[9];
+#pragma unroll
+    for (int k = 0; k < 9; k++) u[k] = lds(smem, u_own + k * u_own_stride);
+#pragma unroll
+    for (int c = 0; c < 12; c++) p[c] = lds(smem, pf + c * pf_stride);
+    hop_term<MU, -1>(acc, p, u);
+#pragma unroll
+    for (int k = 0; k < 9; k++) u[k] = lds(smem, ub + k * ub_stride);
+#pragma unroll
+    for (int c = 0; c < 12; c++) p[c] = lds(smem, pb + c * pb_stride);
+    hop_term<MU, +1>(acc, p, u);
+}
+
+}  // namespace wd
+
+namespace wd {
+
+struct Item {
+    int x0, y0, z0, t0;
+};
+
+template <class P> __device__ __forceinline__ Item decode_item(const TmaParams &prm, int item) {
+    const int ntiles = prm.ntx * prm.nty * prm.ntz;
+    const int chunk = item / ntiles;
+    const int tile = item - chunk * ntiles;
+    const int tpp = prm.ntx * prm.py * prm.pz;  // tiles per rasterisation panel
+    const int panel = tile / tpp;
+    int r = tile - panel * tpp;
+    const int tx = r % prm.ntx;
+    r /= prm.ntx;
+    const int tyi = r % prm.py, tzi = r / prm.py;
+    const int npy = prm.nty / prm.py;
+    Item it;
+    it.x0 = tx * P::BX;
+    it.y0 = ((panel % npy) * prm.py + tyi) * P::BY;
+    it.z0 = ((panel / npy) * prm.pz + tzi) * P::BZ;
+    it.t0 = chunk * prm.tchunk;
+    return it;
+}
+
+// ---------------------------------------------------------------- the kernel
+template <class P>
+__global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ TmaMaps maps, const TmaParams prm) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const uint32_t sbase = smem_u32(smem);
+    const uint32_t bar_full = sbase + P::OFF_BAR, bar_empty = bar_full + OB_COUNT * 8;
+    const int tid = threadIdx.x;
+    constexpr int BZ = P::BZ, BY = P::BY, BX = P::BX, N = P::N;
+    constexpr bool CLOVER = (P::SELF == SELF_CLOVER);
+
+    if (tid == 0) {
+        if (sbase & 127u) __trap();  // TMA destinations need 128-byte alignment
+        for (int k = 0; k < OB_COUNT; k++) {
+            mbar_init(bar_full + 8 * k, 1);        // the producer's arrive.expect_tx
+            mbar_init(bar_empty + 8 * k, P::NW);   // one arrive per compute warp
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    const int T = prm.n[0], Z = prm.n[1], Y = prm.n[2], X = prm.n[3];
+
+    if (tid >= N) {
+        // ======================= producer: one thread issues every TMA =======================
+        if (tid != N) return;
+        tma_prefetch_desc(&maps.psi_c); tma_prefetch_desc(&maps.psi_z); tma_prefetch_desc(&maps.psi_y);
+        tma_prefetch_desc(&maps.psi_x); tma_prefetch_desc(&maps.u_c);   tma_prefetch_desc(&maps.u_z);
+        tma_prefetch_desc(&maps.u_y);   tma_prefetch_desc(&maps.u_x);   tma_prefetch_desc(&maps.s_c);
+        uint32_t nC = 0, nT = 0, nF = 0;  // fills issued so far of C, T, and of the per-step objects
+        for (int item = blockIdx.x; item < prm.nitems; item += gridDim.x) {
+            const Item it = decode_item<P>(prm, item);
+            const int cx = 2 * it.x0, y0 = it.y0, z0 = it.z0;  // dim-0 coordinates count doubles
+            const int zlo = (z0 == 0) ? Z - 1 : z0 - 1, zhi = (z0 + BZ == Z) ? 0 : z0 + BZ;
+            const int ylo = (y0 == 0) ? Y - 1 : y0 - 1, yhi = (y0 + BY == Y) ? 0 : y0 + BY;
+            const int cxlo = 2 * ((it.x0 == 0) ? X - 1 : it.x0 - 1), cxhi = 2 * ((it.x0 + BX == X) ? 0 : it.x0 + BX);
+            int t = (it.t0 == 0) ? T - 1 : it.t0 - 1;
+            // prologue: psi(t0-1), only to seed the carried half-spinor
+            mbar_wait(bar_empty + 8 * OB_C, (nC & 1) ^ 1);
+            mbar_arrive_expect_tx(bar_full + 8 * OB_C, P::SZ_C);
+            tma_load_5d(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cx, y0, z0, t, 0);
+            nC++;
+            for (int j = 1; j <= prm.tchunk + 1; j++) {
+                const int tprev = t;
+                t = (t + 1 == T) ? 0 : t + 1;
+                const bool full = (j <= prm.tchunk);
+                // T object: U_T(t-1)
+                mbar_wait(bar_empty + 8 * OB_T, (nT & 1) ^ 1);
+                mbar_arrive_expect_tx(bar_full + 8 * OB_T, P::SZ_U);
+                tma_load_5d(sbase + P::OFF_T, &maps.u_c, bar_full + 8 * OB_T, cx, y0, z0, tprev, 0);
+                nT++;
+                if (full) {
+                    const uint32_t pe = (nF & 1) ^ 1;
+                    mbar_wait(bar_empty + 8 * OB_Z, pe);
+                    mbar_arrive_expect_tx(bar_full + 8 * OB_Z, P::SZ_Z);
+                    tma_load_5d(sbase + P::OFF_Z, &maps.u_c, bar_full + 8 * OB_Z, cx, y0, z0, t, 9);
+                    tma_load_5d(sbase + P::OFF_ZUF, &maps.u_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, 9);
+                    tma_load_5d(sbase + P::OFF_ZLO, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, 0);
+                    tma_load_5d(sbase + P::OFF_ZHI, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zhi, t, 0);
+                    mbar_wait(bar_empty + 8 * OB_Y, pe);
+                    mbar_arrive_expect_tx(bar_full + 8 * OB_Y, P::SZ_Y);
+                    tma_load_5d(sbase + P::OFF_Y, &maps.u_c, bar_full + 8 * OB_Y, cx, y0, z0, t, 18);
+                    tma_load_5d(sbase + P::OFF_YUF, &maps.u_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, 18);
+                    tma_load_5d(sbase + P::OFF_YLO, &maps.psi_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, 0);
+                    tma_load_5d(sbase + P::OFF_YHI, &maps.psi_y, bar_full + 8 * OB_Y, cx, yhi, z0, t, 0);
+                    mbar_wait(bar_empty + 8 * OB_X, pe);
+                    mbar_arrive_expect_tx(bar_full + 8 * OB_X, P::SZ_X);
+                    tma_load_5d(sbase + P::OFF_X, &maps.u_c, bar_full + 8 * OB_X, cx, y0, z0, t, 27);
+                    tma_load_5d(sbase + P::OFF_XUF, &maps.u_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, 27);
+                    tma_load_5d(sbase + P::OFF_XLO, &maps.psi_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, 0);
+                    tma_load_5d(sbase + P::OFF_XHI, &maps.psi_x, bar_full + 8 * OB_X, cxhi, y0, z0, t, 0);
+                }
+                // C object: psi(t).  Its buffer is released after the X phase of the previous step, so
+                // it has only the S phases to land: warm L2 one step ahead.
+                mbar_wait(bar_empty + 8 * OB_C, (nC & 1) ^ 1);
+                mbar_arrive_expect_tx(bar_full + 8 * OB_C, P::SZ_C);
+                tma_load_5d(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cx, y0, z0, t, 0);
+                nC++;
+                if (full) tma_prefetch_5d(&maps.psi_c, cx, y0, z0, (t + 1 == T) ? 0 : t + 1, 0);
+                if (full && CLOVER) {
+                    const uint32_t pe = (nF & 1) ^ 1;
+                    mbar_wait(bar_empty + 8 * OB_SA, pe);
+                    mbar_arrive_expect_tx(bar_full + 8 * OB_SA, P::SZ_S);
+                    tma_load_5d(sbase + P::OFF_SA, &maps.s_c, bar_full + 8 * OB_SA, cx, y0, z0, t, 0);
+                    mbar_wait(bar_empty + 8 * OB_SB, pe);
+                    mbar_arrive_expect_tx(bar_full + 8 * OB_SB, P::SZ_S);
+                    tma_load_5d(sbase + P::OFF_SB, &maps.s_c, bar_full + 8 * OB_SB, cx, y0, z0, t, 18);
+                }
+                if (full) nF++;
+            }
+        }
+        return;
+    }
+    // ======================= consumers: one thread per site of the tile =======================
+    const int lane = tid & 31;
+    const int lx = tid % BX, ly = (tid / BX) % BY, lz = tid / (BX * BY);
+    constexpr uint32_t E = P::E, NS = N * E;
+    const uint32_t own = tid * E;
+    // operand addresses (bytes from the start of shared memory): interior or face storage
+    const uint32_t fz = (ly * BX + lx) * E, fy = (lz * BX + lx) * E, fx = (lz * BY + ly) * E;
+    const bool zf_in = lz < BZ - 1, zb_in = lz > 0, yf_in = ly < BY - 1, yb_in = ly > 0, xf_in = lx < BX - 1, xb_in = lx > 0;
+    const uint32_t z_pf = zf_in ? P::OFF_C + own + P::FZ * E : P::OFF_ZHI + fz, z_pf_s = zf_in ? NS : P::FZ * E;
+    const uint32_t z_pb = zb_in ? P::OFF_C + own - P::FZ * E : P::OFF_ZLO + fz, z_b_s = zb_in ? NS : P::FZ * E;
+    const uint32_t z_ub = zb_in ? P::OFF_Z + own - P::FZ * E : P::OFF_ZUF + fz;
+    const uint32_t y_pf = yf_in ? P::OFF_C + own + BX * E : P::OFF_YHI + fy, y_pf_s = yf_in ? NS : P::FY * E;
+    const uint32_t y_pb = yb_in ? P::OFF_C + own - BX * E : P::OFF_YLO + fy, y_b_s = yb_in ? NS : P::FY * E;
+    const uint32_t y_ub = yb_in ? P::OFF_Y + own - BX * E : P::OFF_YUF + fy;
+    const uint32_t x_pf = xf_in ? P::OFF_C + own + E : P::OFF_XHI + fx, x_pf_s = xf_in ? NS : P::FX * E;
+    const uint32_t x_pb = xb_in ? P::OFF_C + own - E : P::OFF_XLO + fx, x_b_s = xb_in ? NS : P::FX * E;
+    const uint32_t x_ub = xb_in ? P::OFF_X + own - E : P::OFF_XUF + fx;
+
+    auto release = [&](int ob) {
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_empty + 8 * ob);
+    };
+
+    const long long V = prm.V;
+    const long long strideT = (long long)Z * Y * X;
+    cd *__restrict__ out = prm.out;
+    uint32_t nC = 0, nT = 0, nF = 0;  // fills consumed so far
+    cd hprev[6];                      // rows 0,1 of (1 + gamma_T) psi(t-1)
+    cd outp[12];                      // out(t-1) still missing its forward-T hop
+
+    for (int item = blockIdx.x; item < prm.nitems; item += gridDim.x) {
+        const Item it = decode_item<P>(prm, item);
+        const long long site0 = ((long long)(it.z0 + lz) * Y + (it.y0 + ly)) * X + (it.x0 + lx);
+        int t = (it.t0 == 0) ? T - 1 : it.t0 - 1;
+        {   // prologue: seed the carried half-spinor from psi(t0-1)
+            cd p[12];
+            mbar_wait(bar_full + 8 * OB_C, nC & 1);
+#pragma unroll
+            for (int c = 0; c < 12; c++) p[c] = lds(smem, P::OFF_C + own + c * NS);
+            project<0, +1>(hprev, p);
+            release(OB_C);
+            nC++;
+        }
+        for (int j = 1; j <= prm.tchunk + 1; j++) {
+            const int tprev = t;
+            t = (t + 1 == T) ? 0 : t + 1;
+            cd p[12], acc[12];
+            {   // T phase: finish out(t-1) with its forward hop, start out(t) with its backward hop
+                cd u[9];
+                mbar_wait(bar_full + 8 * OB_T, nT & 1);
+                mbar_wait(bar_full + 8 * OB_C, nC & 1);
+#pragma unroll
+                for (int k = 0; k < 9; k++) u[k] = lds(smem, P::OFF_T + own + k * NS);
+#pragma unroll
+                for (int c = 0; c < 12; c++) p[c] = lds(smem, P::OFF_C + own + c * NS);
+                if (j > 1) {
+                    cd f[12];
+#pragma unroll
+                    for (int c = 0; c < 12; c++) f[c] = make_double2(0.0, 0.0);
+                    hop_term<0, -1>(f, p, u);  // (1 - gamma_T) U_T(t-1) psi(t)
+                    const long long ip = (long long)tprev * strideT + site0;
+#pragma unroll
+                    for (int c = 0; c < 12; c++)
+                        __stcs(out + (long long)c * V + ip,
+                               make_double2(fma(-0.5, f[c].x, outp[c].x), fma(-0.5, f[c].y, outp[c].y)));
+                }
+                if (j == prm.tchunk + 1) {  // epilogue step: nothing else to do for slice t
+                    release(OB_T);
+                    release(OB_C);
+                    nT++;
+                    nC++;
+                    break;
+                }
+                cd g[6];
+                su3_mul<true>(g, u, hprev);  // U_T(t-1)^H (1 + gamma_T) psi(t-1)
+#pragma unroll
+                for (int c = 0; c < 12; c++) acc[c] = make_double2(0.0, 0.0);
+                reconstruct_add<0, +1>(acc, g);
+                project<0, +1>(hprev, p);
+                release(OB_T);
+                nT++;
+            }
+            const uint32_t pf = nF & 1;
+            mbar_wait(bar_full + 8 * OB_Z, pf);
+            hop_pair_smem<1>(acc, smem, P::OFF_Z + own, NS, z_pf, z_pf_s, z_ub, z_b_s, z_pb, z_b_s);
+            release(OB_Z);
+            mbar_wait(bar_full + 8 * OB_Y, pf);
+            hop_pair_smem<2>(acc, smem, P::OFF_Y + own, NS, y_pf, y_pf_s, y_ub, y_b_s, y_pb, y_b_s);
+            release(OB_Y);
+            mbar_wait(bar_full + 8 * OB_X, pf);
+            hop_pair_smem<3>(acc, smem, P::OFF_X + own, NS, x_pf, x_pf_s, x_ub, x_b_s, x_pb, x_b_s);
+            release(OB_X);
+            release(OB_C);
+            nC++;
+            // self-coupling (a5) and combination (a6); the store waits for the forward-T hop
+            if (CLOVER) {
+#pragma unroll
+                for (int b = 0; b < 2; b++) {
+                    const uint32_t so = (b == 0 ? P::OFF_SA : P::OFF_SB) + own;
+                    mbar_wait(bar_full + 8 * (OB_SA + b), pf);
+                    double d[6];
+                    cd a[15], r[6];
+#pragma unroll
+                    for (int q = 0; q < 3; q++) {
+                        const cd dd = lds(smem, so + q * NS);
+                        d[2 * q] = dd.x;
+                        d[2 * q + 1] = dd.y;
+                    }
+#pragma unroll
+                    for (int k = 0; k < 15; k++) a[k] = lds(smem, so + (3 + k) * NS);
+                    release(OB_SA + b);
+                    herm6_mul(r, d, a, p + 6 * b);
+#pragma unroll
+                    for (int c = 0; c < 6; c++)
+                        outp[6 * b + c] = make_double2(fma(-0.5, acc[6 * b + c].x, r[c].x), fma(-0.5, acc[6 * b + c].y, r[c].y));
+                }
+            } else if (P::SELF == SELF_MASS) {
+#pragma unroll
+                for (int c = 0; c < 12; c++)
+                    outp[c] = make_double2(fma(prm.mass, p[c].x, -0.5 * acc[c].x), fma(prm.mass, p[c].y, -0.5 * acc[c].y));
+            } else {
+#pragma unroll
+                for (int c = 0; c < 12; c++) outp[c] = make_double2(-0.5 * acc[c].x, -0.5 * acc[c].y);
+            }
+            nF++;
+        }
+    }
+}
+
+// ---------------------------------------------------------------- host side
+static int sm_count() {
+    static int n = 0;
+    if (!n) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1)
+            n = 148;
+    }
+    return n;
+}
+
+// Work decomposition.  An item = (tile, T chunk); a CTA marches one item at a time.  tchunk trades
+// the wave-quantisation tail (few items per SM) against the per-item prologue/epilogue (one extra
+// psi slice in, one extra psi + U_T slice at the end).  The panel (py x pz tiles, all of X) is the
+// set of tiles in flight together: as cubic as possible, at most one wave, so that most face
+// re-reads are L2 hits on data a neighbouring CTA is streaming at the same time.
+template <class P> static void plan_items(const KParams &p, TmaParams &prm) {
+    const int nsm = sm_count();
+    prm.ntx = p.n[3] / P::BX;
+    prm.nty = p.n[2] / P::BY;
+    prm.ntz = p.n[1] / P::BZ;
+    const int ntiles = prm.ntx * prm.nty * prm.ntz, T = p.n[0];
+    int best_tc = T;
+    if (p.opt_tchunk > 0 && T % p.opt_tchunk == 0) {
+        best_tc = p.opt_tchunk;
+    } else {
+        double best = 1e300;
+        for (int tc = 1; tc <= T; tc++) {
+            if (T % tc) continue;
+            const long long items = (long long)ntiles * (T / tc);
+            const double cost = (double)((items + nsm - 1) / nsm) * (tc + 1.5);
+            if (cost < best * 0.999) best = cost, best_tc = tc;
+        }
+    }
+    prm.tchunk = best_tc;
+    prm.ntc = T / best_tc;
+    prm.nitems = ntiles * prm.ntc;
+    int bpy = 1, bpz = 1;
+    double bscore = 1e300;
+    for (int py = 1; py <= prm.nty; py++) {
+        if (prm.nty % py) continue;
+        for (int pz = 1; pz <= prm.ntz; pz++) {
+            if (prm.ntz % pz) continue;
+            if (p.opt_zgroup > 0 && pz != p.opt_zgroup && prm.ntz % p.opt_zgroup == 0) continue;
+            const int tiles = prm.ntx * py * pz;
+            double score = 1.0 / (py * P::BY) + 1.0 / (pz * P::BZ);
+            if (tiles > nsm) score += 10.0 * tiles / nsm;  // over one wave: only if nothing smaller exists
+            if (score < bscore) bscore = score, bpy = py, bpz = pz;
+        }
+    }
+    prm.py = bpy;
+    prm.pz = bpz;
+}
+
+template <int BZ, int BY, int BX, int SELF> static cudaError_t launch_tma_self(const KParams &p, cudaStream_t st) {
+    using P = Plan<BZ, BY, BX, SELF>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(k_tma<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::SMEM);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    TmaMaps maps;
+    cudaError_t e;
+#define WD_ENC(m, base, nc, bx, by, bz, bc)                                      \
+    if ((e = encode_field_map(&maps.m, base, p.n, nc, bx, by, bz, bc)) != cudaSuccess) return e;
+    WD_ENC(psi_c, p.psi, 12, BX, BY, BZ, 12)
+    WD_ENC(psi_z, p.psi, 12, BX, BY, 1, 12)
+    WD_ENC(psi_y, p.psi, 12, BX, 1, BZ, 12)
+    WD_ENC(psi_x, p.psi, 12, 1, BY, BZ, 12)
+    WD_ENC(u_c, p.U, 36, BX, BY, BZ, 9)
+    WD_ENC(u_z, p.U, 36, BX, BY, 1, 9)
+    WD_ENC(u_y, p.U, 36, BX, 1, BZ, 9)
+    WD_ENC(u_x, p.U, 36, 1, BY, BZ, 9)
+    WD_ENC(s_c, (SELF == SELF_CLOVER) ? p.S : p.U, 36, BX, BY, BZ, 18)
+#undef WD_ENC
+    TmaParams prm;
+    prm.out = p.out;
+    prm.V = p.V;
+    for (int a = 0; a < 4; a++) prm.n[a] = p.n[a];
+    prm.mass = p.mass;
+    plan_items<P>(p, prm);
+    const int grid = (prm.nitems < sm_count()) ? prm.nitems : sm_count();
+    k_tma<P><<<grid, P::NTHREADS, P::SMEM, st>>>(maps, prm);
+    return cudaGetLastError();
+}
+
+template <int BZ, int BY, int BX> static cudaError_t launch_tma(const KParams &p, int self, cudaStream_t st) {
+    if (self == SELF_CLOVER) return launch_tma_self<BZ, BY, BX, SELF_CLOVER>(p, st);
+    if (self == SELF_MASS) return launch_tma_self<BZ, BY, BX, SELF_MASS>(p, st);
+    return launch_tma_self<BZ, BY, BX, SELF_NONE>(p, st);
+}
+
+cudaError_t launch_tma_2x4x16(const KParams &p, int self, cudaStream_t st) { return launch_tma<2, 4, 16>(p, self, st); }
+cudaError_t launch_tma_4x4x8(const KParams &p, int self, cudaStream_t st) { return launch_tma<4, 4, 8>(p, self, st); }
+}  // namespace wd

@@ -69,14 +69,18 @@ def test_host_packer_is_the_stated_permutation(V):
         back = np.empty_like(a)
         wd.wd_layout_unpack_host(field, V, packed, back)
         assert np.array_equal(back, a)
-    # self-coupling: 42 canonical -> 36 slots: 6 real-diagonal pairs, then the 30 off-diagonals
+    # self-coupling: 42 canonical -> 36 slots, 18 per chirality block (3 real-diagonal pairs, then
+    # the block's 15 strict-upper entries), block A first
     C = wdinputs.selfcoupling_random((1, 1, 1, V), 77)
     packed = np.empty((36, V, 2))
     assert wd.wd_layout_bytes(wd.WD_FIELD_CLOVER, V) == packed.nbytes == V * 576
     wd.wd_layout_pack_host(wd.WD_FIELD_CLOVER, V, C, packed)
-    for j in range(6):
-        assert np.array_equal(packed[j, :, 0], C[:, 2 * j, 0]) and np.array_equal(packed[j, :, 1], C[:, 2 * j + 1, 0])
-    assert np.array_equal(packed[6:], C[:, 12:].transpose(1, 0, 2))
+    for b in range(2):
+        for j in range(3):
+            q = 3 * b + j
+            assert np.array_equal(packed[18 * b + j, :, 0], C[:, 2 * q, 0])
+            assert np.array_equal(packed[18 * b + j, :, 1], C[:, 2 * q + 1, 0])
+        assert np.array_equal(packed[18 * b + 3:18 * b + 18], C[:, 12 + 15 * b:27 + 15 * b].transpose(1, 0, 2))
     back = np.empty_like(C)
     wd.wd_layout_unpack_host(wd.WD_FIELD_CLOVER, V, packed, back)
     assert np.array_equal(back, C)

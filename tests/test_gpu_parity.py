@@ -80,8 +80,8 @@ def kernels_fitting(dims):
         if name.startswith("linear"):
             out.append(k)
             continue
-        b = [int(v) for v in name.split("_")[1].split("x")]
-        if all(n % t == 0 for n, t in zip(dims, b)):
+        b = [int(v) for v in name.split("_")[1].split("x")]  # tile_TxZxYxX or tma_ZxYxX
+        if all(n % t == 0 for n, t in zip(dims[-len(b):], b)):
             out.append(k)
     return out
 
