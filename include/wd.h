@@ -103,8 +103,16 @@ int wd_apply(wd_handle *h, void *dev_out, const void *dev_in, int nrhs);
  * in host_out.  (Pinned host memory makes the copies faster but is not required.) */
 int wd_apply_host(wd_handle *h, double *host_out, const double *host_in, int nrhs);
 
-/* Size in bytes of a device spinor buffer for nrhs right-hand sides (0 on error). */
+/* Size in bytes of a device spinor buffer for nrhs right-hand sides (0 on error).  It is
+ * nrhs * 12 * wd_component_stride(h) * 16 — a little more than nrhs * V * 192, see below. */
 size_t wd_spinor_bytes(const wd_handle *h, int nrhs);
+
+/* Component stride Vs of the device layout, in complex elements (0 on error): component c of
+ * right-hand side r of a device spinor starts at element (12*r + c) * Vs and holds the V sites in
+ * canonical order, followed by Vs - V elements of padding that are never read or written.  The
+ * padding keeps the components of one site from aliasing onto one L2 slice when V*16 B is a
+ * power of two. */
+long long wd_component_stride(const wd_handle *h);
 
 /* HOST canonical [nrhs][V][12][2]  <->  DEVICE layout.  Synchronous. */
 int wd_pack_spinor(wd_handle *h, void *dev_dst, const double *host_src, int nrhs);

@@ -32,6 +32,7 @@ SIGNATURES = {
     "wd_apply": (_i, [_vp, _vp, _vp, _i]),
     "wd_apply_host": (_i, [_vp, _vp, _vp, _i]),
     "wd_spinor_bytes": (_sz, [_vp, _i]),
+    "wd_component_stride": (ctypes.c_longlong, [_vp]),
     "wd_pack_spinor": (_i, [_vp, _vp, _vp, _i]),
     "wd_unpack_spinor": (_i, [_vp, _vp, _vp, _i]),
     "wd_layout_bytes": (_sz, [_i, ctypes.c_longlong]),
@@ -128,6 +129,10 @@ def wd_apply_host(h, host_out, host_in, nrhs: int = 1) -> None:
 
 def wd_spinor_bytes(h, nrhs: int = 1) -> int:
     return int(lib().wd_spinor_bytes(h, nrhs))
+
+
+def wd_component_stride(h) -> int:
+    return int(lib().wd_component_stride(h))
 
 
 def wd_pack_spinor(h, dev_dst, host_src, nrhs: int = 1) -> None:

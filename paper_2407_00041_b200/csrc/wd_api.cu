@@ -14,11 +14,12 @@ using namespace wd;
 
 struct wd_handle {
     int n[4];
-    long long V;
+    long long V, Vs;  // sites; component stride of the device layout (elements)
     double m0, csw;
     int device;
     cudaStream_t stream;
     double2 *dU, *dS;
+    unsigned int *dsched;  // work-queue words of the TMA kernels
     bool has_gauge, has_clover;
     // options
     long variant, kernel_opt, tchunk_opt, zgroup_opt, device_pack;
@@ -34,6 +35,19 @@ struct wd_handle {
 };
 
 static thread_local std::string g_create_err = "";
+
+// Component stride of the device SoA layout.  V rounded up to 16 sites (256 B, keeps every component
+// 256-byte aligned for TMA / 128-bit access) plus 17 * 16 sites, so that consecutive components differ
+// in the low address bits that select the L2 slice and set.  WD_PAD_SITES overrides the padding
+// (experiments only; any multiple of 16 >= 0).
+long long wd::component_stride(long long V) {
+    long long pad = 16 * 17;
+    if (const char *e = getenv("WD_PAD_SITES")) {
+        const long long v = atoll(e);
+        if (v >= 0 && v % 16 == 0) pad = v;
+    }
+    return (V + 15) / 16 * 16 + pad;
+}
 
 static int fail(wd_handle *h, int code, const std::string &msg) {
     if (h) h->err = msg; else g_create_err = msg;
@@ -97,11 +111,13 @@ int wd_create(wd_handle **out, int T, int Z, int Y, int X, double m0, double csw
     if (!h) return fail(nullptr, WD_ENOMEM, "wd_create: out of host memory");
     h->n[0] = T; h->n[1] = Z; h->n[2] = Y; h->n[3] = X;
     h->V = V;
+    h->Vs = component_stride(V);
     h->m0 = m0;
     h->csw = csw;
     h->device = dev;
     h->stream = nullptr;
     h->dU = h->dS = nullptr;
+    h->dsched = nullptr;
     h->has_gauge = h->has_clover = false;
     h->variant = 0;
     h->kernel_opt = -1;
@@ -115,7 +131,9 @@ int wd_create(wd_handle **out, int T, int Z, int Y, int X, double m0, double csw
     h->dstage_bytes = 0;
     h->work_in = h->work_out = nullptr;
     h->launches = 0;
-    e = cudaMalloc((void **)&h->dU, (size_t)V * kGaugeComps * sizeof(double2));
+    e = cudaMalloc((void **)&h->dU, (size_t)h->Vs * kGaugeComps * sizeof(double2));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&h->dsched, 2 * sizeof(unsigned int));
+    if (e == cudaSuccess) e = cudaMemset(h->dsched, 0, 2 * sizeof(unsigned int));
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->pinned_ev[0], cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->pinned_ev[1], cudaEventDisableTiming);
     if (e != cudaSuccess) {
@@ -134,6 +152,7 @@ int wd_destroy(wd_handle *h) {
     cudaStreamSynchronize(h->stream);
     if (h->dU) cudaFree(h->dU);
     if (h->dS) cudaFree(h->dS);
+    if (h->dsched) cudaFree(h->dsched);
     if (h->dstage) cudaFree(h->dstage);
     if (h->work_in) cudaFree(h->work_in);
     if (h->work_out) cudaFree(h->work_out);
@@ -180,7 +199,7 @@ static int load_chunked(wd_handle *h, double2 *dev, const double2 *host, int nco
         const long long cnt = (V - i0 < chunk) ? V - i0 : chunk;
         WD_CUDA(h, cudaEventSynchronize(h->pinned_ev[b]));
         pack(h->pinned[b], host, i0, cnt);
-        WD_CUDA(h, cudaMemcpy2DAsync(dev + i0, (size_t)V * sizeof(double2), h->pinned[b], (size_t)cnt * sizeof(double2),
+        WD_CUDA(h, cudaMemcpy2DAsync(dev + i0, (size_t)h->Vs * sizeof(double2), h->pinned[b], (size_t)cnt * sizeof(double2),
                                      (size_t)cnt * sizeof(double2), ncomp_dev, cudaMemcpyHostToDevice, h->stream));
         WD_CUDA(h, cudaEventRecord(h->pinned_ev[b], h->stream));
     }
@@ -200,7 +219,7 @@ static int store_chunked(wd_handle *h, double2 *host, const double2 *dev, int nc
     if (rc) return rc;
     for (long long i0 = 0; i0 < V; i0 += chunk) {
         const long long cnt = (V - i0 < chunk) ? V - i0 : chunk;
-        WD_CUDA(h, cudaMemcpy2DAsync(h->pinned[0], (size_t)cnt * sizeof(double2), dev + i0, (size_t)V * sizeof(double2),
+        WD_CUDA(h, cudaMemcpy2DAsync(h->pinned[0], (size_t)cnt * sizeof(double2), dev + i0, (size_t)h->Vs * sizeof(double2),
                                      (size_t)cnt * sizeof(double2), ncomp_dev, cudaMemcpyDeviceToHost, h->stream));
         WD_CUDA(h, cudaStreamSynchronize(h->stream));
         unpack(host, h->pinned[0], i0, cnt);
@@ -216,7 +235,7 @@ int wd_load_gauge(wd_handle *h, const double *host_U) {
         int rc = ensure_dstage(h, bytes);
         if (rc) return rc;
         WD_CUDA(h, cudaMemcpyAsync(h->dstage, host_U, bytes, cudaMemcpyHostToDevice, h->stream));
-        WD_CUDA(h, launch_aos_to_soa(h->dU, h->dstage, h->V, kGaugeComps, h->stream));
+        WD_CUDA(h, launch_aos_to_soa(h->dU, h->dstage, h->V, h->Vs, kGaugeComps, h->stream));
         h->launches++;
         WD_CUDA(h, cudaStreamSynchronize(h->stream));
         release_dstage(h);
@@ -229,7 +248,7 @@ int wd_load_gauge(wd_handle *h, const double *host_U) {
 }
 
 static int ensure_clover_storage(wd_handle *h) {
-    if (!h->dS) WD_CUDA(h, cudaMalloc((void **)&h->dS, (size_t)h->V * kCloverSlots * sizeof(double2)));
+    if (!h->dS) WD_CUDA(h, cudaMalloc((void **)&h->dS, (size_t)h->Vs * kCloverSlots * sizeof(double2)));
     return WD_OK;
 }
 
@@ -243,7 +262,7 @@ int wd_load_clover(wd_handle *h, const double *host_C) {
         rc = ensure_dstage(h, bytes);
         if (rc) return rc;
         WD_CUDA(h, cudaMemcpyAsync(h->dstage, host_C, bytes, cudaMemcpyHostToDevice, h->stream));
-        WD_CUDA(h, launch_clover_canon_to_dev(h->dS, h->dstage, h->V, h->stream));
+        WD_CUDA(h, launch_clover_canon_to_dev(h->dS, h->dstage, h->V, h->Vs, h->stream));
         h->launches++;
         WD_CUDA(h, cudaStreamSynchronize(h->stream));
         release_dstage(h);
@@ -260,7 +279,7 @@ int wd_build_clover(wd_handle *h) {
     if (!h->has_gauge) return fail(h, WD_ESTATE, "wd_build_clover: no gauge field loaded");
     int rc = ensure_clover_storage(h);
     if (rc) return rc;
-    WD_CUDA(h, launch_build_clover(h->dS, h->dU, h->n, h->V, h->m0 + 4.0, h->csw, h->stream));
+    WD_CUDA(h, launch_build_clover(h->dS, h->dU, h->n, h->V, h->Vs, h->m0 + 4.0, h->csw, h->stream));
     h->launches++;
     h->has_clover = true;
     return WD_OK;
@@ -276,23 +295,25 @@ int wd_get_clover(wd_handle *h, double *host_C) {
 // ---- spinors ------------------------------------------------------------------------------------
 size_t wd_spinor_bytes(const wd_handle *h, int nrhs) {
     if (!h || nrhs < 1) return 0;
-    return (size_t)nrhs * (size_t)h->V * kSpinorComps * sizeof(double2);
+    return (size_t)nrhs * (size_t)h->Vs * kSpinorComps * sizeof(double2);
 }
+
+long long wd_component_stride(const wd_handle *h) { return h ? h->Vs : 0; }
 
 static bool misaligned(const void *p) { return ((size_t)p & 15) != 0; }
 
 int wd_pack_spinor(wd_handle *h, void *dev_dst, const double *host_src, int nrhs) {
     if (!h) return WD_EINVAL;
     if (!dev_dst || !host_src || nrhs < 1 || misaligned(dev_dst)) return fail(h, WD_EINVAL, "wd_pack_spinor: bad argument");
-    const size_t per = (size_t)h->V * kSpinorComps;
+    const size_t per = (size_t)h->V * kSpinorComps, dper = (size_t)h->Vs * kSpinorComps;
     for (int r = 0; r < nrhs; r++) {
-        double2 *dst = (double2 *)dev_dst + r * per;
+        double2 *dst = (double2 *)dev_dst + r * dper;
         const double2 *src = (const double2 *)host_src + r * per;
         if (h->device_pack) {
             int rc = ensure_dstage(h, per * sizeof(double2));
             if (rc) return rc;
             WD_CUDA(h, cudaMemcpyAsync(h->dstage, src, per * sizeof(double2), cudaMemcpyHostToDevice, h->stream));
-            WD_CUDA(h, launch_aos_to_soa(dst, h->dstage, h->V, kSpinorComps, h->stream));
+            WD_CUDA(h, launch_aos_to_soa(dst, h->dstage, h->V, h->Vs, kSpinorComps, h->stream));
             h->launches++;
             WD_CUDA(h, cudaStreamSynchronize(h->stream));
         } else {
@@ -306,14 +327,14 @@ int wd_pack_spinor(wd_handle *h, void *dev_dst, const double *host_src, int nrhs
 int wd_unpack_spinor(wd_handle *h, double *host_dst, const void *dev_src, int nrhs) {
     if (!h) return WD_EINVAL;
     if (!host_dst || !dev_src || nrhs < 1 || misaligned(dev_src)) return fail(h, WD_EINVAL, "wd_unpack_spinor: bad argument");
-    const size_t per = (size_t)h->V * kSpinorComps;
+    const size_t per = (size_t)h->V * kSpinorComps, dper = (size_t)h->Vs * kSpinorComps;
     for (int r = 0; r < nrhs; r++) {
         double2 *dst = (double2 *)host_dst + r * per;
-        const double2 *src = (const double2 *)dev_src + r * per;
+        const double2 *src = (const double2 *)dev_src + r * dper;
         if (h->device_pack) {
             int rc = ensure_dstage(h, per * sizeof(double2));
             if (rc) return rc;
-            WD_CUDA(h, launch_soa_to_aos(h->dstage, src, h->V, kSpinorComps, h->stream));
+            WD_CUDA(h, launch_soa_to_aos(h->dstage, src, h->V, h->Vs, kSpinorComps, h->stream));
             h->launches++;
             WD_CUDA(h, cudaMemcpyAsync(dst, h->dstage, per * sizeof(double2), cudaMemcpyDeviceToHost, h->stream));
             WD_CUDA(h, cudaStreamSynchronize(h->stream));
@@ -364,7 +385,7 @@ static bool geometry_fits(const wd_handle *h, const KernelInfo &k) {
 
 static int auto_kernel(const wd_handle *h) {
     // preference order among the tiled geometries; linear256 always fits
-    static const char *pref[] = {"tile_1x4x4x16", "tile_1x4x8x8", "tile_1x2x4x32", "tile_2x4x4x8", "tile_4x4x4x4",
+    static const char *pref[] = {"tma_2x4x16", "tma_4x4x8", "tile_1x4x4x16", "tile_1x4x8x8", "tile_1x2x4x32", "tile_2x4x4x8", "tile_4x4x4x4",
                                  "tile_1x4x4x8", "tile_1x4x4x4"};
     for (const char *name : pref)
         for (int id = 0; id < kernel_count(); id++)
@@ -429,6 +450,7 @@ static int fill_params(wd_handle *h, KParams &p, const KernelInfo &k) {
     p.U = h->dU;
     p.S = h->dS;
     p.V = h->V;
+    p.Vs = h->Vs;
     for (int a = 0; a < 4; a++) p.n[a] = h->n[a];
     p.stride[3] = 1;
     p.stride[2] = h->n[3];
@@ -438,6 +460,7 @@ static int fill_params(wd_handle *h, KParams &p, const KernelInfo &k) {
     p.ntx = p.nty = p.ntz = p.ntc = p.gz = p.tchunk = 1;
     p.opt_tchunk = (int)h->tchunk_opt;
     p.opt_zgroup = (int)h->zgroup_opt;
+    p.sched = h->dsched;
     if (k.bx) {
         p.ntx = h->n[3] / k.bx;
         p.nty = h->n[2] / k.by;
@@ -475,7 +498,7 @@ int wd_apply(wd_handle *h, void *dev_out, const void *dev_in, int nrhs) {
     int rc = fill_params(h, p, k);
     if (rc) return rc;
     const int self = h->has_clover ? SELF_CLOVER : SELF_MASS;
-    const size_t per = (size_t)h->V * kSpinorComps;
+    const size_t per = (size_t)h->Vs * kSpinorComps;
     for (int r = 0; r < nrhs; r++) {
         p.psi = (const double2 *)dev_in + r * per;
         p.out = (double2 *)dev_out + r * per;
@@ -495,17 +518,18 @@ int wd_apply_host(wd_handle *h, double *host_out, const double *host_in, int nrh
     if (!h) return WD_EINVAL;
     if (!host_out || !host_in || nrhs < 1) return fail(h, WD_EINVAL, "wd_apply_host: null pointer or nrhs < 1");
     const size_t per = (size_t)h->V * kSpinorComps, bytes = per * sizeof(double2);
-    if (!h->work_in) WD_CUDA(h, cudaMalloc((void **)&h->work_in, bytes));
-    if (!h->work_out) WD_CUDA(h, cudaMalloc((void **)&h->work_out, bytes));
+    const size_t dbytes = wd_spinor_bytes(h, 1);
+    if (!h->work_in) WD_CUDA(h, cudaMalloc((void **)&h->work_in, dbytes));
+    if (!h->work_out) WD_CUDA(h, cudaMalloc((void **)&h->work_out, dbytes));
     int rc = ensure_dstage(h, bytes);
     if (rc) return rc;
     for (int r = 0; r < nrhs; r++) {
         WD_CUDA(h, cudaMemcpyAsync(h->dstage, (const double2 *)host_in + r * per, bytes, cudaMemcpyHostToDevice, h->stream));
-        WD_CUDA(h, launch_aos_to_soa(h->work_in, h->dstage, h->V, kSpinorComps, h->stream));
+        WD_CUDA(h, launch_aos_to_soa(h->work_in, h->dstage, h->V, h->Vs, kSpinorComps, h->stream));
         h->launches++;
         rc = wd_apply(h, h->work_out, h->work_in, 1);
         if (rc) return rc;
-        WD_CUDA(h, launch_soa_to_aos(h->dstage, h->work_out, h->V, kSpinorComps, h->stream));
+        WD_CUDA(h, launch_soa_to_aos(h->dstage, h->work_out, h->V, h->Vs, kSpinorComps, h->stream));
         h->launches++;
         WD_CUDA(h, cudaMemcpyAsync((double2 *)host_out + r * per, h->dstage, bytes, cudaMemcpyDeviceToHost, h->stream));
     }

@@ -55,7 +55,7 @@ __device__ static long long shift(long long i, const int n[4], const int stride[
 struct CloverParams {
     double2 *S;
     const double2 *U;
-    long long V;
+    long long V, Vs;
     int n[4], stride[4];
     double mass, csw;
 };
@@ -77,7 +77,7 @@ __global__ void __launch_bounds__(128) k_build_clover(const CloverParams p) {
             for (int q = 0; q < 6; q++) blk[b][r][q] = make_double2((r == q) ? p.mass : 0.0, 0.0);
 
     const cd *U = p.U;
-    const long long V = p.V;
+    const long long V = p.Vs;  // component stride
     for (int mu = 0; mu < 4; mu++)
         for (int nu = mu + 1; nu < 4; nu++) {
             int cm[4] = {c[0], c[1], c[2], c[3]};  // coordinates of x - mu
@@ -141,12 +141,13 @@ __global__ void __launch_bounds__(128) k_build_clover(const CloverParams p) {
     }
 }
 
-cudaError_t launch_build_clover(double2 *S_slots, const double2 *U, const int n[4], long long V, double mass,
-                                double csw, cudaStream_t st) {
+cudaError_t launch_build_clover(double2 *S_slots, const double2 *U, const int n[4], long long V, long long Vs,
+                                double mass, double csw, cudaStream_t st) {
     CloverParams p;
     p.S = S_slots;
     p.U = U;
     p.V = V;
+    p.Vs = Vs;
     for (int a = 0; a < 4; a++) p.n[a] = n[a];
     p.stride[3] = 1;
     p.stride[2] = n[3];

@@ -11,15 +11,20 @@ namespace wd {
 // double = double2 = 16 B; the site index i (canonical order, X fastest) is the fastest index of
 // every array, so a warp that handles 32 consecutive sites reads 512 contiguous bytes per
 // component:
-//   spinor  double2 [nrhs][12][V]       component c = 3*spin + colour
-//   gauge   double2 [4][9][V]           mu = T,Z,Y,X; k = 3*row + col; forward links only, each
+// The component stride is Vs = V + padding (component_stride()): with Vs = V the components of one
+// site sit a power of two apart on the paper-sized lattices (2^28 B at 64^4) and alias onto the same
+// L2 slice and set; measured at 64^4: 38 % extra DRAM reads (profiles/r1b_*.md).
+//   spinor  double2 [nrhs][12][Vs]      component c = 3*spin + colour
+//   gauge   double2 [4][9][Vs]          mu = T,Z,Y,X; k = 3*row + col; forward links only, each
 //                                       link stored ONCE (U_mu(x-mu) is read from site x-mu)
-//   selfcpl double2 [36][V]             18 slots per chirality block b (A = 0, B = 1), block-contiguous
+//   selfcpl double2 [36][Vs]            18 slots per chirality block b (A = 0, B = 1), block-contiguous
 //                                       so that one block is one TMA box: slot 18b+j (j<3) holds the
 //                                       real diagonal pair (B_{2j,2j}, B_{2j+1,2j+1}); slot 18b+3+k the
 //                                       k-th strict-upper entry (row-major) of the 6x6 block
 //                                       (72 reals = 576 B per site, R6/R7)
 // ---------------------------------------------------------------------------------------------
+long long component_stride(long long V);  // wd_api.cu
+
 constexpr int kSpinorComps = 12;
 constexpr int kGaugeComps = 36;
 constexpr int kCloverSlots = 36;
@@ -35,7 +40,8 @@ struct KParams {
     const double2 *U;
     const double2 *S;
     double2 *out;
-    long long V;
+    long long V;    // sites
+    long long Vs;   // component stride in elements (V plus padding, see component_stride())
     int n[4];       // T, Z, Y, X
     int stride[4];  // site-index strides of T, Z, Y, X
     double mass;    // m0 + 4
@@ -44,6 +50,7 @@ struct KParams {
     int gz;                  // Z-tiles per rasterisation group
     int tchunk;              // T-extent marched by one CTA
     int opt_tchunk, opt_zgroup;  // the raw WD_OPT_TCHUNK / WD_OPT_ZGROUP values (0 = automatic)
+    unsigned int *sched;         // device, 2 words, zero between launches: work queue of the TMA kernels
 };
 
 struct KernelInfo {
@@ -63,11 +70,11 @@ cudaError_t launch_tma_4x4x8(const KParams &p, int self, cudaStream_t st);
 // self-coupling kernel of the unfused variant: out += S psi (clover) or out += mass * psi
 cudaError_t launch_selfcoupling(const KParams &p, int self, cudaStream_t st);
 
-// device-side layout transposes (wd_pack.cu): canonical AoS <-> device SoA, on device buffers
-cudaError_t launch_aos_to_soa(double2 *dst_soa, const double2 *src_aos, long long V, int ncomp, cudaStream_t st);
-cudaError_t launch_soa_to_aos(double2 *dst_aos, const double2 *src_soa, long long V, int ncomp, cudaStream_t st);
-cudaError_t launch_clover_canon_to_dev(double2 *dst_slots, const double2 *src42, long long V, cudaStream_t st);
-cudaError_t launch_clover_dev_to_canon(double2 *dst42, const double2 *src_slots, long long V, cudaStream_t st);
+// device-side layout transposes (wd_pack.cu): canonical AoS <-> device SoA (component stride Vs)
+cudaError_t launch_aos_to_soa(double2 *dst_soa, const double2 *src_aos, long long V, long long Vs, int ncomp, cudaStream_t st);
+cudaError_t launch_soa_to_aos(double2 *dst_aos, const double2 *src_soa, long long V, long long Vs, int ncomp, cudaStream_t st);
+cudaError_t launch_clover_canon_to_dev(double2 *dst_slots, const double2 *src42, long long V, long long Vs, cudaStream_t st);
+cudaError_t launch_clover_dev_to_canon(double2 *dst42, const double2 *src_slots, long long V, long long Vs, cudaStream_t st);
 
 // host packers (wd_pack.cu): canonical AoS chunk [i0, i0+cnt) -> SoA staging [ncomp][cnt]
 void host_pack_aos_to_soa(double2 *dst, const double2 *src_aos, long long i0, long long cnt, int ncomp);
@@ -76,7 +83,7 @@ void host_pack_clover(double2 *dst, const double2 *src42, long long i0, long lon
 void host_unpack_clover(double2 *dst42, const double2 *src, long long i0, long long cnt);
 
 // device clover construction (wd_clover.cu): S slots from the device gauge field
-cudaError_t launch_build_clover(double2 *S_slots, const double2 *U, const int n[4], long long V, double mass,
-                                double csw, cudaStream_t st);
+cudaError_t launch_build_clover(double2 *S_slots, const double2 *U, const int n[4], long long V, long long Vs,
+                                double mass, double csw, cudaStream_t st);
 
 }  // namespace wd

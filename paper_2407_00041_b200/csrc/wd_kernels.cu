@@ -42,7 +42,7 @@ template <int SELF>
 __device__ __forceinline__ void site_apply(const KParams &p, long long i, int t, int z, int y, int x) {
     const cd *__restrict__ psi = p.psi;
     const cd *__restrict__ U = p.U;
-    const long long V = p.V;
+    const long long V = p.Vs;  // component stride
     cd acc[12];
 #pragma unroll
     for (int c = 0; c < 12; c++) acc[c] = make_double2(0.0, 0.0);
@@ -167,7 +167,7 @@ template <int BT, int BZ, int BY, int BX> static cudaError_t launch_tiled(const 
 template <int SELF> __global__ void __launch_bounds__(256) k_selfcoupling(const KParams p) {
     const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
     if (i >= p.V) return;
-    const long long V = p.V;
+    const long long V = p.Vs;  // component stride
     const cd *__restrict__ psi = p.psi;
     cd *__restrict__ out = p.out;
     if (SELF == SELF_MASS) {

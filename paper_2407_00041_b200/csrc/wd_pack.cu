@@ -66,7 +66,7 @@ constexpr int TS = 64;
 
 template <bool TO_SOA>
 __global__ void __launch_bounds__(256) k_transpose(double2 *__restrict__ dst, const double2 *__restrict__ src,
-                                                  long long V, int ncomp) {
+                                                  long long V, long long Vs, int ncomp) {
     extern __shared__ double2 tile[];  // [TS][ncomp + 1]
     const long long i0 = (long long)blockIdx.x * TS;
     const int cnt = (int)((V - i0 < TS) ? (V - i0) : TS);
@@ -77,32 +77,33 @@ __global__ void __launch_bounds__(256) k_transpose(double2 *__restrict__ dst, co
         __syncthreads();
         for (int e = threadIdx.x; e < ncomp * TS; e += blockDim.x) {
             const int c = e / TS, j = e % TS;
-            if (j < cnt) dst[(long long)c * V + i0 + j] = tile[j * pitch + c];
+            if (j < cnt) dst[(long long)c * Vs + i0 + j] = tile[j * pitch + c];
         }
     } else {
         for (int e = threadIdx.x; e < ncomp * TS; e += blockDim.x) {
             const int c = e / TS, j = e % TS;
-            if (j < cnt) tile[j * pitch + c] = src[(long long)c * V + i0 + j];
+            if (j < cnt) tile[j * pitch + c] = src[(long long)c * Vs + i0 + j];
         }
         __syncthreads();
         for (int e = threadIdx.x; e < n; e += blockDim.x) dst[i0 * ncomp + e] = tile[(e / ncomp) * pitch + (e % ncomp)];
     }
 }
 
-cudaError_t launch_aos_to_soa(double2 *dst_soa, const double2 *src_aos, long long V, int ncomp, cudaStream_t st) {
+cudaError_t launch_aos_to_soa(double2 *dst_soa, const double2 *src_aos, long long V, long long Vs, int ncomp, cudaStream_t st) {
     const unsigned grid = (unsigned)((V + TS - 1) / TS);
-    k_transpose<true><<<grid, 256, TS * (ncomp + 1) * sizeof(double2), st>>>(dst_soa, src_aos, V, ncomp);
+    k_transpose<true><<<grid, 256, TS * (ncomp + 1) * sizeof(double2), st>>>(dst_soa, src_aos, V, Vs, ncomp);
     return cudaGetLastError();
 }
 
-cudaError_t launch_soa_to_aos(double2 *dst_aos, const double2 *src_soa, long long V, int ncomp, cudaStream_t st) {
+cudaError_t launch_soa_to_aos(double2 *dst_aos, const double2 *src_soa, long long V, long long Vs, int ncomp, cudaStream_t st) {
     const unsigned grid = (unsigned)((V + TS - 1) / TS);
-    k_transpose<false><<<grid, 256, TS * (ncomp + 1) * sizeof(double2), st>>>(dst_aos, src_soa, V, ncomp);
+    k_transpose<false><<<grid, 256, TS * (ncomp + 1) * sizeof(double2), st>>>(dst_aos, src_soa, V, Vs, ncomp);
     return cudaGetLastError();
 }
 
 template <bool TO_DEV>
-__global__ void __launch_bounds__(256) k_clover_convert(double2 *__restrict__ dst, const double2 *__restrict__ src, long long V) {
+__global__ void __launch_bounds__(256) k_clover_convert(double2 *__restrict__ dst, const double2 *__restrict__ src, long long V,
+                                                       long long Vs) {
     __shared__ double2 tile[TS * (kCloverCanon + 1)];
     const long long i0 = (long long)blockIdx.x * TS;
     const int cnt = (int)((V - i0 < TS) ? (V - i0) : TS);
@@ -118,14 +119,14 @@ __global__ void __launch_bounds__(256) k_clover_convert(double2 *__restrict__ ds
             if (q < 6) v = make_double2(tile[j * pitch + 2 * q].x, tile[j * pitch + 2 * q + 1].x);
             else v = tile[j * pitch + 6 + q];
             const int slot = (q < 6) ? slot_of_pair(q) : slot_of_upper(q - 6);
-            dst[(long long)slot * V + i0 + j] = v;
+            dst[(long long)slot * Vs + i0 + j] = v;
         }
     } else {
         for (int e = threadIdx.x; e < kCloverSlots * TS; e += blockDim.x) {
             const int q = e / TS, j = e % TS;
             if (j >= cnt) continue;
             const int slot = (q < 6) ? slot_of_pair(q) : slot_of_upper(q - 6);
-            const double2 v = src[(long long)slot * V + i0 + j];
+            const double2 v = src[(long long)slot * Vs + i0 + j];
             if (q < 6) {
                 tile[j * pitch + 2 * q] = make_double2(v.x, 0.0);
                 tile[j * pitch + 2 * q + 1] = make_double2(v.y, 0.0);
@@ -139,13 +140,13 @@ __global__ void __launch_bounds__(256) k_clover_convert(double2 *__restrict__ ds
     }
 }
 
-cudaError_t launch_clover_canon_to_dev(double2 *dst_slots, const double2 *src42, long long V, cudaStream_t st) {
-    k_clover_convert<true><<<(unsigned)((V + TS - 1) / TS), 256, 0, st>>>(dst_slots, src42, V);
+cudaError_t launch_clover_canon_to_dev(double2 *dst_slots, const double2 *src42, long long V, long long Vs, cudaStream_t st) {
+    k_clover_convert<true><<<(unsigned)((V + TS - 1) / TS), 256, 0, st>>>(dst_slots, src42, V, Vs);
     return cudaGetLastError();
 }
 
-cudaError_t launch_clover_dev_to_canon(double2 *dst42, const double2 *src_slots, long long V, cudaStream_t st) {
-    k_clover_convert<false><<<(unsigned)((V + TS - 1) / TS), 256, 0, st>>>(dst42, src_slots, V);
+cudaError_t launch_clover_dev_to_canon(double2 *dst42, const double2 *src_slots, long long V, long long Vs, cudaStream_t st) {
+    k_clover_convert<false><<<(unsigned)((V + TS - 1) / TS), 256, 0, st>>>(dst42, src_slots, V, Vs);
     return cudaGetLastError();
 }
 

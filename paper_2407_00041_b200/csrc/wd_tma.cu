@@ -23,6 +23,8 @@
 // algorithmic 1536 B, plus face re-reads that hit L2 (neighbouring tiles march concurrently).
 // Neighbour indexing and the periodic wrap (a1) are box coordinates computed by the producer.
 #include <cstdio>
+#include <cstdlib>
+#include <vector>
 
 #include "wd_internal.h"
 #include "wd_math.cuh"
@@ -49,13 +51,13 @@ static EncodeTiledFn encode_fn() {
     return fn;
 }
 
-cudaError_t encode_field_map(CUtensorMap *map, const void *base, const int n[4], int ncomp, int bx, int by, int bz,
-                             int bc) {
+cudaError_t encode_field_map(CUtensorMap *map, const void *base, const int n[4], long long Vs, int ncomp, int bx,
+                             int by, int bz, int bc) {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return cudaErrorNotSupported;
     const cuuint64_t T = n[0], Z = n[1], Y = n[2], X = n[3];
     const cuuint64_t dims[5] = {2 * X, Y, Z, T, (cuuint64_t)ncomp};
-    const cuuint64_t strides[4] = {X * 16, X * Y * 16, X * Y * Z * 16, X * Y * Z * T * 16};  // bytes, dims 1..4
+    const cuuint64_t strides[4] = {X * 16, X * Y * 16, X * Y * Z * 16, (cuuint64_t)Vs * 16};  // bytes, dims 1..4
     const cuuint32_t box[5] = {(cuuint32_t)(2 * bx), (cuuint32_t)by, (cuuint32_t)bz, 1u, (cuuint32_t)bc};
     const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
     const CUtensorMapL2promotion promo = (bx * 16 >= 256)   ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B
@@ -74,7 +76,7 @@ cudaError_t encode_field_map(CUtensorMap *map, const void *base, const int n[4],
 //   Z  U_Z(t) interior | U_Z face z0-1 | psi faces z0-1, z0+BZ      [9][N] [9][FZ] [12][FZ] [12][FZ]
 //   Y  same for Y;  X  same for X
 //   SA, SB  the two 6x6 blocks of S(t)                    [18][N] each
-enum { OB_C = 0, OB_T, OB_Z, OB_Y, OB_X, OB_SA, OB_SB, OB_COUNT };
+enum { OB_C = 0, OB_T, OB_Z, OB_Y, OB_X, OB_SA, OB_SB, OB_ITEM0, OB_ITEM1, OB_COUNT };  // ITEM: work-item mailbox
 
 template <int BZ_, int BY_, int BX_, int SELF_> struct Plan {
     static constexpr int BZ = BZ_, BY = BY_, BX = BX_, SELF = SELF_;
@@ -98,7 +100,8 @@ template <int BZ_, int BY_, int BX_, int SELF_> struct Plan {
     static constexpr uint32_t OFF_SA = OFF_X + SZ_X;
     static constexpr uint32_t OFF_SB = OFF_SA + SZ_S;
     static constexpr uint32_t OFF_BAR = (SELF == SELF_CLOVER) ? OFF_SB + SZ_S : OFF_SA;
-    static constexpr uint32_t SMEM = OFF_BAR + 2 * OB_COUNT * 8;
+    static constexpr uint32_t OFF_MAIL = OFF_BAR + 2 * OB_COUNT * 8;  // int[2]: item index per mailbox slot
+    static constexpr uint32_t SMEM = OFF_MAIL + 16;
     static_assert(N % 32 == 0 && FZ % 8 == 0 && FY % 8 == 0 && FX % 8 == 0, "tile faces must keep 128-byte alignment");
     static_assert(SMEM <= 232448, "shared-memory plan exceeds 227 KB");
 };
@@ -111,14 +114,19 @@ struct TmaMaps {
 
 struct TmaParams {
     double2 *out;
-    long long V;
+    long long V, Vs;     // sites, component stride
     int n[4];
     int ntx, nty, ntz;   // tiles per direction
     int py, pz;          // rasterisation panel (in tiles); py | nty, pz | ntz
     int tchunk, ntc;     // T steps per work item, items per tile
     int nitems;          // ntx*nty*ntz*ntc
     double mass;
+    int flags;           // WD_TMA_FLAGS (experiments; 0 = production): 1 S evict_normal instead of evict_first,
+                         // 2 U evict_first, 4 psi evict_last, 8 L2-prefetch psi(t+1), 16 static round-robin items
+    unsigned int *sched; // [0] next item, [1] CTAs finished (dynamic work distribution; both 0 between launches)
+    unsigned long long *trace;  // diagnostics (WD_TMA_TRACE): [cta][kTraceLen] globaltimer per step, or null
 };
+constexpr int kTraceLen = 1024;
 
 // ---------------------------------------------------------------- shared-memory operand fetch
 __device__ __forceinline__ cd lds(const unsigned char *smem, uint32_t off) {
@@ -185,7 +193,7 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
     if (tid == 0) {
         if (sbase & 127u) __trap();  // TMA destinations need 128-byte alignment
         for (int k = 0; k < OB_COUNT; k++) {
-            mbar_init(bar_full + 8 * k, 1);        // the producer's arrive.expect_tx
+            mbar_init(bar_full + 8 * k, 1);        // the producer's arrive(.expect_tx)
             mbar_init(bar_empty + 8 * k, P::NW);   // one arrive per compute warp
         }
         mbar_fence_init();
@@ -200,8 +208,29 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
         tma_prefetch_desc(&maps.psi_c); tma_prefetch_desc(&maps.psi_z); tma_prefetch_desc(&maps.psi_y);
         tma_prefetch_desc(&maps.psi_x); tma_prefetch_desc(&maps.u_c);   tma_prefetch_desc(&maps.u_z);
         tma_prefetch_desc(&maps.u_y);   tma_prefetch_desc(&maps.u_x);   tma_prefetch_desc(&maps.s_c);
+        const uint64_t pol_n = l2_policy_evict_normal();
+        const uint64_t pol_s = (prm.flags & 1) ? pol_n : l2_policy_evict_first();  // S is used exactly once
+        const uint64_t pol_u = (prm.flags & 2) ? l2_policy_evict_first() : pol_n;
+        const uint64_t pol_p = (prm.flags & 4) ? l2_policy_evict_last() : pol_n;
         uint32_t nC = 0, nT = 0, nF = 0;  // fills issued so far of C, T, and of the per-step objects
-        for (int item = blockIdx.x; item < prm.nitems; item += gridDim.x) {
+        volatile int *mail = reinterpret_cast<volatile int *>(smem + P::OFF_MAIL);
+        const bool dynamic = !(prm.flags & 16);
+        for (uint32_t seq = 0;; seq++) {
+            // next work item: atomic queue (fast SMs take more items; measured SM-to-SM spread of the
+            // streaming rate is ~20 %), handed to the consumers through a two-slot mailbox
+            int item = dynamic ? (int)atomicAdd(prm.sched, 1u) : (int)(blockIdx.x + seq * gridDim.x);
+            if (item >= prm.nitems) item = -1;
+            const uint32_t slot = seq & 1, mpar = (seq >> 1) & 1;
+            mbar_wait(bar_empty + 8 * (OB_ITEM0 + slot), mpar ^ 1);
+            mail[slot] = item;
+            mbar_arrive(bar_full + 8 * (OB_ITEM0 + slot));
+            if (item < 0) {
+                if (dynamic && atomicAdd(prm.sched + 1, 1u) == gridDim.x - 1) {  // last CTA out re-arms the queue
+                    prm.sched[0] = 0;
+                    prm.sched[1] = 0;
+                }
+                break;
+            }
             const Item it = decode_item<P>(prm, item);
             const int cx = 2 * it.x0, y0 = it.y0, z0 = it.z0;  // dim-0 coordinates count doubles
             const int zlo = (z0 == 0) ? Z - 1 : z0 - 1, zhi = (z0 + BZ == Z) ? 0 : z0 + BZ;
@@ -211,7 +240,7 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
             // prologue: psi(t0-1), only to seed the carried half-spinor
             mbar_wait(bar_empty + 8 * OB_C, (nC & 1) ^ 1);
             mbar_arrive_expect_tx(bar_full + 8 * OB_C, P::SZ_C);
-            tma_load_5d(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cx, y0, z0, t, 0);
+            tma_load_5d_hint(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cx, y0, z0, t, 0, pol_p);
             nC++;
             for (int j = 1; j <= prm.tchunk + 1; j++) {
                 const int tprev = t;
@@ -220,44 +249,45 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
                 // T object: U_T(t-1)
                 mbar_wait(bar_empty + 8 * OB_T, (nT & 1) ^ 1);
                 mbar_arrive_expect_tx(bar_full + 8 * OB_T, P::SZ_U);
-                tma_load_5d(sbase + P::OFF_T, &maps.u_c, bar_full + 8 * OB_T, cx, y0, z0, tprev, 0);
+                tma_load_5d_hint(sbase + P::OFF_T, &maps.u_c, bar_full + 8 * OB_T, cx, y0, z0, tprev, 0, pol_u);
                 nT++;
                 if (full) {
                     const uint32_t pe = (nF & 1) ^ 1;
                     mbar_wait(bar_empty + 8 * OB_Z, pe);
                     mbar_arrive_expect_tx(bar_full + 8 * OB_Z, P::SZ_Z);
-                    tma_load_5d(sbase + P::OFF_Z, &maps.u_c, bar_full + 8 * OB_Z, cx, y0, z0, t, 9);
-                    tma_load_5d(sbase + P::OFF_ZUF, &maps.u_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, 9);
-                    tma_load_5d(sbase + P::OFF_ZLO, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, 0);
-                    tma_load_5d(sbase + P::OFF_ZHI, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zhi, t, 0);
+                    tma_load_5d_hint(sbase + P::OFF_Z, &maps.u_c, bar_full + 8 * OB_Z, cx, y0, z0, t, 9, pol_u);
+                    tma_load_5d_hint(sbase + P::OFF_ZUF, &maps.u_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, 9, pol_u);
+                    tma_load_5d_hint(sbase + P::OFF_ZLO, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, 0, pol_p);
+                    tma_load_5d_hint(sbase + P::OFF_ZHI, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zhi, t, 0, pol_p);
                     mbar_wait(bar_empty + 8 * OB_Y, pe);
                     mbar_arrive_expect_tx(bar_full + 8 * OB_Y, P::SZ_Y);
-                    tma_load_5d(sbase + P::OFF_Y, &maps.u_c, bar_full + 8 * OB_Y, cx, y0, z0, t, 18);
-                    tma_load_5d(sbase + P::OFF_YUF, &maps.u_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, 18);
-                    tma_load_5d(sbase + P::OFF_YLO, &maps.psi_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, 0);
-                    tma_load_5d(sbase + P::OFF_YHI, &maps.psi_y, bar_full + 8 * OB_Y, cx, yhi, z0, t, 0);
+                    tma_load_5d_hint(sbase + P::OFF_Y, &maps.u_c, bar_full + 8 * OB_Y, cx, y0, z0, t, 18, pol_u);
+                    tma_load_5d_hint(sbase + P::OFF_YUF, &maps.u_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, 18, pol_u);
+                    tma_load_5d_hint(sbase + P::OFF_YLO, &maps.psi_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, 0, pol_p);
+                    tma_load_5d_hint(sbase + P::OFF_YHI, &maps.psi_y, bar_full + 8 * OB_Y, cx, yhi, z0, t, 0, pol_p);
                     mbar_wait(bar_empty + 8 * OB_X, pe);
                     mbar_arrive_expect_tx(bar_full + 8 * OB_X, P::SZ_X);
-                    tma_load_5d(sbase + P::OFF_X, &maps.u_c, bar_full + 8 * OB_X, cx, y0, z0, t, 27);
-                    tma_load_5d(sbase + P::OFF_XUF, &maps.u_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, 27);
-                    tma_load_5d(sbase + P::OFF_XLO, &maps.psi_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, 0);
-                    tma_load_5d(sbase + P::OFF_XHI, &maps.psi_x, bar_full + 8 * OB_X, cxhi, y0, z0, t, 0);
+                    tma_load_5d_hint(sbase + P::OFF_X, &maps.u_c, bar_full + 8 * OB_X, cx, y0, z0, t, 27, pol_u);
+                    tma_load_5d_hint(sbase + P::OFF_XUF, &maps.u_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, 27, pol_u);
+                    tma_load_5d_hint(sbase + P::OFF_XLO, &maps.psi_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, 0, pol_p);
+                    tma_load_5d_hint(sbase + P::OFF_XHI, &maps.psi_x, bar_full + 8 * OB_X, cxhi, y0, z0, t, 0, pol_p);
                 }
-                // C object: psi(t).  Its buffer is released after the X phase of the previous step, so
-                // it has only the S phases to land: warm L2 one step ahead.
+                // C object: psi(t).  Its buffer is released after the X phase of the previous step, so it
+                // has only the S phases to land.  (Warming L2 one step ahead with a TMA prefetch was
+                // measured to cost 20 % at 64^4 — flag 8, profiles/r1b — so it is off.)
                 mbar_wait(bar_empty + 8 * OB_C, (nC & 1) ^ 1);
                 mbar_arrive_expect_tx(bar_full + 8 * OB_C, P::SZ_C);
-                tma_load_5d(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cx, y0, z0, t, 0);
+                tma_load_5d_hint(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cx, y0, z0, t, 0, pol_p);
                 nC++;
-                if (full) tma_prefetch_5d(&maps.psi_c, cx, y0, z0, (t + 1 == T) ? 0 : t + 1, 0);
+                if (full && (prm.flags & 8)) tma_prefetch_5d(&maps.psi_c, cx, y0, z0, (t + 1 == T) ? 0 : t + 1, 0);
                 if (full && CLOVER) {
                     const uint32_t pe = (nF & 1) ^ 1;
                     mbar_wait(bar_empty + 8 * OB_SA, pe);
                     mbar_arrive_expect_tx(bar_full + 8 * OB_SA, P::SZ_S);
-                    tma_load_5d(sbase + P::OFF_SA, &maps.s_c, bar_full + 8 * OB_SA, cx, y0, z0, t, 0);
+                    tma_load_5d_hint(sbase + P::OFF_SA, &maps.s_c, bar_full + 8 * OB_SA, cx, y0, z0, t, 0, pol_s);
                     mbar_wait(bar_empty + 8 * OB_SB, pe);
                     mbar_arrive_expect_tx(bar_full + 8 * OB_SB, P::SZ_S);
-                    tma_load_5d(sbase + P::OFF_SB, &maps.s_c, bar_full + 8 * OB_SB, cx, y0, z0, t, 18);
+                    tma_load_5d_hint(sbase + P::OFF_SB, &maps.s_c, bar_full + 8 * OB_SB, cx, y0, z0, t, 18, pol_s);
                 }
                 if (full) nF++;
             }
@@ -287,14 +317,21 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
         if (lane == 0) mbar_arrive(bar_empty + 8 * ob);
     };
 
-    const long long V = prm.V;
+    const long long V = prm.Vs;  // component stride
     const long long strideT = (long long)Z * Y * X;
     cd *__restrict__ out = prm.out;
     uint32_t nC = 0, nT = 0, nF = 0;  // fills consumed so far
+    int ntrace = 0;
     cd hprev[6];                      // rows 0,1 of (1 + gamma_T) psi(t-1)
     cd outp[12];                      // out(t-1) still missing its forward-T hop
 
-    for (int item = blockIdx.x; item < prm.nitems; item += gridDim.x) {
+    const volatile int *mail = reinterpret_cast<const volatile int *>(smem + P::OFF_MAIL);
+    for (uint32_t seq = 0;; seq++) {
+        const uint32_t slot = seq & 1, mpar = (seq >> 1) & 1;
+        mbar_wait(bar_full + 8 * (OB_ITEM0 + slot), mpar);
+        const int item = mail[slot];
+        release(OB_ITEM0 + slot);
+        if (item < 0) break;
         const Item it = decode_item<P>(prm, item);
         const long long site0 = ((long long)(it.z0 + lz) * Y + (it.y0 + ly)) * X + (it.x0 + lx);
         int t = (it.t0 == 0) ? T - 1 : it.t0 - 1;
@@ -315,6 +352,11 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
                 cd u[9];
                 mbar_wait(bar_full + 8 * OB_T, nT & 1);
                 mbar_wait(bar_full + 8 * OB_C, nC & 1);
+                if (prm.trace && tid == 0 && ntrace < kTraceLen) {
+                    unsigned long long now;
+                    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+                    prm.trace[(size_t)blockIdx.x * kTraceLen + ntrace++] = now;
+                }
 #pragma unroll
                 for (int k = 0; k < 9; k++) u[k] = lds(smem, P::OFF_T + own + k * NS);
 #pragma unroll
@@ -404,9 +446,9 @@ static int sm_count() {
     return n;
 }
 
-// Work decomposition.  An item = (tile, T chunk); a CTA marches one item at a time.  tchunk trades
-// the wave-quantisation tail (few items per SM) against the per-item prologue/epilogue (one extra
-// psi slice in, one extra psi + U_T slice at the end).  The panel (py x pz tiles, all of X) is the
+// Work decomposition.  An item = (tile, T chunk); a CTA marches one item at a time and takes the
+// next from an atomic queue.  tchunk trades the tail (the last items finish unevenly) against the
+// per-item prologue/epilogue (one extra psi slice in, one extra psi + U_T slice at the end).  The panel (py x pz tiles, all of X) is the
 // set of tiles in flight together: as cubic as possible, at most one wave, so that most face
 // re-reads are L2 hits on data a neighbouring CTA is streaming at the same time.
 template <class P> static void plan_items(const KParams &p, TmaParams &prm) {
@@ -423,7 +465,8 @@ template <class P> static void plan_items(const KParams &p, TmaParams &prm) {
         for (int tc = 1; tc <= T; tc++) {
             if (T % tc) continue;
             const long long items = (long long)ntiles * (T / tc);
-            const double cost = (double)((items + nsm - 1) / nsm) * (tc + 1.5);
+            // dynamic queue: work = items * (steps + prologue/epilogue) / SMs, plus an expected tail of half an item
+            const double cost = (double)items * (tc + 0.5) / nsm + 0.5 * (tc + 1);
             if (cost < best * 0.999) best = cost, best_tc = tc;
         }
     }
@@ -458,7 +501,7 @@ template <int BZ, int BY, int BX, int SELF> static cudaError_t launch_tma_self(c
     TmaMaps maps;
     cudaError_t e;
 #define WD_ENC(m, base, nc, bx, by, bz, bc)                                      \
-    if ((e = encode_field_map(&maps.m, base, p.n, nc, bx, by, bz, bc)) != cudaSuccess) return e;
+    if ((e = encode_field_map(&maps.m, base, p.n, p.Vs, nc, bx, by, bz, bc)) != cudaSuccess) return e;
     WD_ENC(psi_c, p.psi, 12, BX, BY, BZ, 12)
     WD_ENC(psi_z, p.psi, 12, BX, BY, 1, 12)
     WD_ENC(psi_y, p.psi, 12, BX, 1, BZ, 12)
@@ -472,12 +515,34 @@ template <int BZ, int BY, int BX, int SELF> static cudaError_t launch_tma_self(c
     TmaParams prm;
     prm.out = p.out;
     prm.V = p.V;
+    prm.Vs = p.Vs;
     for (int a = 0; a < 4; a++) prm.n[a] = p.n[a];
     prm.mass = p.mass;
     plan_items<P>(p, prm);
     const int grid = (prm.nitems < sm_count()) ? prm.nitems : sm_count();
+    prm.trace = nullptr;
+    prm.sched = p.sched;
+    prm.flags = getenv("WD_TMA_FLAGS") ? atoi(getenv("WD_TMA_FLAGS")) : 0;
+    const char *trace_path = getenv("WD_TMA_TRACE");
+    if (trace_path) {
+        if ((e = cudaMalloc((void **)&prm.trace, (size_t)grid * kTraceLen * 8)) != cudaSuccess) return e;
+        cudaMemsetAsync(prm.trace, 0, (size_t)grid * kTraceLen * 8, st);
+    }
     k_tma<P><<<grid, P::NTHREADS, P::SMEM, st>>>(maps, prm);
-    return cudaGetLastError();
+    e = cudaGetLastError();
+    if (trace_path && e == cudaSuccess) {  // diagnostics only: synchronous dump of the last launch's step times
+        std::vector<unsigned long long> host((size_t)grid * kTraceLen);
+        cudaStreamSynchronize(st);
+        cudaMemcpy(host.data(), prm.trace, host.size() * 8, cudaMemcpyDeviceToHost);
+        if (FILE *f = fopen(trace_path, "wb")) {
+            const int hdr[4] = {grid, kTraceLen, prm.tchunk, prm.nitems};
+            fwrite(hdr, sizeof(int), 4, f);
+            fwrite(host.data(), 8, host.size(), f);
+            fclose(f);
+        }
+    }
+    if (prm.trace) cudaFree(prm.trace);
+    return e;
 }
 
 template <int BZ, int BY, int BX> static cudaError_t launch_tma(const KParams &p, int self, cudaStream_t st) {

@@ -70,6 +70,11 @@ __device__ __forceinline__ uint64_t l2_policy_evict_first() {
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
     return p;
 }
+__device__ __forceinline__ uint64_t l2_policy_evict_normal() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
 __device__ __forceinline__ uint64_t l2_policy_evict_last() {
     uint64_t p;
     asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
@@ -77,9 +82,10 @@ __device__ __forceinline__ uint64_t l2_policy_evict_last() {
 }
 
 // ---------------------------------------------------------------- host side
-// A field of double2 [ncomp][T][Z][Y][X] seen as a 5-D FP64 tensor (2X, Y, Z, T, ncomp); a box is
-// (2*bx, by, bz, 1, bc) and lands in shared memory densely as double2 [bc][bz][by][bx].
-cudaError_t encode_field_map(CUtensorMap *map, const void *base, const int n[4], int ncomp, int bx, int by, int bz,
-                             int bc);
+// A field of double2 [ncomp][Vs] (Vs >= T*Z*Y*X, site index X fastest) seen as a 5-D FP64 tensor
+// (2X, Y, Z, T, ncomp); a box is (2*bx, by, bz, 1, bc) and lands in shared memory densely as
+// double2 [bc][bz][by][bx].
+cudaError_t encode_field_map(CUtensorMap *map, const void *base, const int n[4], long long Vs, int ncomp, int bx,
+                             int by, int bz, int bc);
 
 }  // namespace wd
