@@ -231,8 +231,8 @@ def run_ours(args):
     clover = cfg["csw"] != 0.0
     flop = FLOP_WILSON + (FLOP_CLOVER if clover else 0)
     gauge_b, self_b = 576, (576 if clover else 0)
-    alg_bytes_site_rhs = (gauge_b + self_b) / nrhs + 384  # per site and RHS
-    alg_bytes_launch = V * (gauge_b + self_b + 384)       # one launch processes V sites of ONE rhs
+    alg_bytes_site_rhs = (gauge_b + self_b) / nrhs + 384  # per site and RHS: links and S once for all RHS (a8)
+    alg_bytes_step = V * (gauge_b + self_b + 384 * nrhs)  # one step = all nrhs right-hand sides
 
     # ---- setup (untimed): fields become device resident in device layout
     h = wd.wd_create(*dims, cfg["m0"], cfg["csw"])
@@ -301,6 +301,7 @@ def run_ours(args):
     peak, peak_src = peak_hbm()
     launches_per_step = launches / args.steps
     avg_launch_ms = (sum(per_step) / len(per_step)) / launches_per_step
+    alg_bytes_launch = alg_bytes_step / launches_per_step  # tma_*: one launch per step, all RHS
     achieved = alg_bytes_launch / (avg_launch_ms * 1e-3) / 1e9
     roofline = {
         "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,

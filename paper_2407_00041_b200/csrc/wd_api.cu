@@ -499,6 +499,15 @@ int wd_apply(wd_handle *h, void *dev_out, const void *dev_in, int nrhs) {
     if (rc) return rc;
     const int self = h->has_clover ? SELF_CLOVER : SELF_MASS;
     const size_t per = (size_t)h->Vs * kSpinorComps;
+    p.nrhs = 1;
+    if (k.multi_rhs && h->variant == 0) {  // a8: one launch, links and S shared by the right-hand sides
+        p.psi = (const double2 *)dev_in;
+        p.out = (double2 *)dev_out;
+        p.nrhs = nrhs;
+        WD_CUDA(h, k.launch(p, self, h->stream));
+        h->launches++;
+        return WD_OK;
+    }
     for (int r = 0; r < nrhs; r++) {
         p.psi = (const double2 *)dev_in + r * per;
         p.out = (double2 *)dev_out + r * per;

@@ -36,7 +36,8 @@ __host__ __device__ constexpr int slot_off(int b, int k) { return 18 * b + 3 + k
 enum SelfMode { SELF_NONE = 0, SELF_MASS = 1, SELF_CLOVER = 2 };
 
 struct KParams {
-    const double2 *psi;
+    const double2 *psi;  // right-hand side 0; RHS r at + r * 12 * Vs (same for out)
+    int nrhs;            // right-hand sides of this launch (> 1 only for kernels with multi_rhs)
     const double2 *U;
     const double2 *S;
     double2 *out;
@@ -57,6 +58,7 @@ struct KernelInfo {
     const char *name;
     int bt, bz, by, bx;  // tile extents (all 0: linear geometry, any lattice)
     int threads;
+    bool multi_rhs;      // one launch applies the operator to all p.nrhs right-hand sides
     cudaError_t (*launch)(const KParams &p, int self, cudaStream_t st);
 };
 

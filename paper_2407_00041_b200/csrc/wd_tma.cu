@@ -119,7 +119,8 @@ struct TmaParams {
     int ntx, nty, ntz;   // tiles per direction
     int py, pz;          // rasterisation panel (in tiles); py | nty, pz | ntz
     int tchunk, ntc;     // T steps per work item, items per tile
-    int nitems;          // ntx*nty*ntz*ntc
+    int nrhs, rb;        // right-hand sides in this launch; RHS per block of the item order
+    int nitems;          // ntx*nty*ntz*ntc*nrhs
     double mass;
     int flags;           // WD_TMA_FLAGS (experiments; 0 = production): 1 S evict_normal instead of evict_first,
                          // 2 U evict_first, 4 psi evict_last, 8 L2-prefetch psi(t+1), 16 static round-robin items
@@ -158,13 +159,23 @@ __device__ __forceinline__ void hop_pair_smem(cd acc[12], const unsigned char *s
 namespace wd {
 
 struct Item {
-    int x0, y0, z0, t0;
+    int x0, y0, z0, t0, rhs;
 };
 
+// Item order (slowest to fastest): T chunk, block of up to `rb` right-hand sides, tile (panel
+// order), right-hand side within the block.  The CTAs in flight therefore work on the same few
+// tiles for rb right-hand sides at once: the links and S of a tile are fetched from HBM by the
+// first of them and are L2 hits for the others (a8: +384 B per extra RHS instead of +1536 B).
 template <class P> __device__ __forceinline__ Item decode_item(const TmaParams &prm, int item) {
     const int ntiles = prm.ntx * prm.nty * prm.ntz;
-    const int chunk = item / ntiles;
-    const int tile = item - chunk * ntiles;
+    const int per_chunk = ntiles * prm.nrhs;
+    const int chunk = item / per_chunk;
+    int rem = item - chunk * per_chunk;
+    const int blk = rem / (ntiles * prm.rb);
+    rem -= blk * ntiles * prm.rb;
+    const int rb_here = min(prm.rb, prm.nrhs - blk * prm.rb);
+    const int tile = rem / rb_here;
+    const int rhs = blk * prm.rb + (rem - tile * rb_here);
     const int tpp = prm.ntx * prm.py * prm.pz;  // tiles per rasterisation panel
     const int panel = tile / tpp;
     int r = tile - panel * tpp;
@@ -177,6 +188,7 @@ template <class P> __device__ __forceinline__ Item decode_item(const TmaParams &
     it.y0 = ((panel % npy) * prm.py + tyi) * P::BY;
     it.z0 = ((panel / npy) * prm.pz + tzi) * P::BZ;
     it.t0 = chunk * prm.tchunk;
+    it.rhs = rhs;
     return it;
 }
 
@@ -233,6 +245,7 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
             }
             const Item it = decode_item<P>(prm, item);
             const int cx = 2 * it.x0, y0 = it.y0, z0 = it.z0;  // dim-0 coordinates count doubles
+            const int pc = 12 * it.rhs;                        // first component of this right-hand side
             const int zlo = (z0 == 0) ? Z - 1 : z0 - 1, zhi = (z0 + BZ == Z) ? 0 : z0 + BZ;
             const int ylo = (y0 == 0) ? Y - 1 : y0 - 1, yhi = (y0 + BY == Y) ? 0 : y0 + BY;
             const int cxlo = 2 * ((it.x0 == 0) ? X - 1 : it.x0 - 1), cxhi = 2 * ((it.x0 + BX == X) ? 0 : it.x0 + BX);
@@ -240,7 +253,7 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
             // prologue: psi(t0-1), only to seed the carried half-spinor
             mbar_wait(bar_empty + 8 * OB_C, (nC & 1) ^ 1);
             mbar_arrive_expect_tx(bar_full + 8 * OB_C, P::SZ_C);
-            tma_load_5d_hint(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cx, y0, z0, t, 0, pol_p);
+            tma_load_5d_hint(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cx, y0, z0, t, pc, pol_p);
             nC++;
             for (int j = 1; j <= prm.tchunk + 1; j++) {
                 const int tprev = t;
@@ -257,29 +270,29 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
                     mbar_arrive_expect_tx(bar_full + 8 * OB_Z, P::SZ_Z);
                     tma_load_5d_hint(sbase + P::OFF_Z, &maps.u_c, bar_full + 8 * OB_Z, cx, y0, z0, t, 9, pol_u);
                     tma_load_5d_hint(sbase + P::OFF_ZUF, &maps.u_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, 9, pol_u);
-                    tma_load_5d_hint(sbase + P::OFF_ZLO, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, 0, pol_p);
-                    tma_load_5d_hint(sbase + P::OFF_ZHI, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zhi, t, 0, pol_p);
+                    tma_load_5d_hint(sbase + P::OFF_ZLO, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, pc, pol_p);
+                    tma_load_5d_hint(sbase + P::OFF_ZHI, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zhi, t, pc, pol_p);
                     mbar_wait(bar_empty + 8 * OB_Y, pe);
                     mbar_arrive_expect_tx(bar_full + 8 * OB_Y, P::SZ_Y);
                     tma_load_5d_hint(sbase + P::OFF_Y, &maps.u_c, bar_full + 8 * OB_Y, cx, y0, z0, t, 18, pol_u);
                     tma_load_5d_hint(sbase + P::OFF_YUF, &maps.u_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, 18, pol_u);
-                    tma_load_5d_hint(sbase + P::OFF_YLO, &maps.psi_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, 0, pol_p);
-                    tma_load_5d_hint(sbase + P::OFF_YHI, &maps.psi_y, bar_full + 8 * OB_Y, cx, yhi, z0, t, 0, pol_p);
+                    tma_load_5d_hint(sbase + P::OFF_YLO, &maps.psi_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, pc, pol_p);
+                    tma_load_5d_hint(sbase + P::OFF_YHI, &maps.psi_y, bar_full + 8 * OB_Y, cx, yhi, z0, t, pc, pol_p);
                     mbar_wait(bar_empty + 8 * OB_X, pe);
                     mbar_arrive_expect_tx(bar_full + 8 * OB_X, P::SZ_X);
                     tma_load_5d_hint(sbase + P::OFF_X, &maps.u_c, bar_full + 8 * OB_X, cx, y0, z0, t, 27, pol_u);
                     tma_load_5d_hint(sbase + P::OFF_XUF, &maps.u_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, 27, pol_u);
-                    tma_load_5d_hint(sbase + P::OFF_XLO, &maps.psi_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, 0, pol_p);
-                    tma_load_5d_hint(sbase + P::OFF_XHI, &maps.psi_x, bar_full + 8 * OB_X, cxhi, y0, z0, t, 0, pol_p);
+                    tma_load_5d_hint(sbase + P::OFF_XLO, &maps.psi_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, pc, pol_p);
+                    tma_load_5d_hint(sbase + P::OFF_XHI, &maps.psi_x, bar_full + 8 * OB_X, cxhi, y0, z0, t, pc, pol_p);
                 }
                 // C object: psi(t).  Its buffer is released after the X phase of the previous step, so it
                 // has only the S phases to land.  (Warming L2 one step ahead with a TMA prefetch was
                 // measured to cost 20 % at 64^4 — flag 8, profiles/r1b — so it is off.)
                 mbar_wait(bar_empty + 8 * OB_C, (nC & 1) ^ 1);
                 mbar_arrive_expect_tx(bar_full + 8 * OB_C, P::SZ_C);
-                tma_load_5d_hint(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cx, y0, z0, t, 0, pol_p);
+                tma_load_5d_hint(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cx, y0, z0, t, pc, pol_p);
                 nC++;
-                if (full && (prm.flags & 8)) tma_prefetch_5d(&maps.psi_c, cx, y0, z0, (t + 1 == T) ? 0 : t + 1, 0);
+                if (full && (prm.flags & 8)) tma_prefetch_5d(&maps.psi_c, cx, y0, z0, (t + 1 == T) ? 0 : t + 1, pc);
                 if (full && CLOVER) {
                     const uint32_t pe = (nF & 1) ^ 1;
                     mbar_wait(bar_empty + 8 * OB_SA, pe);
@@ -319,7 +332,6 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
 
     const long long V = prm.Vs;  // component stride
     const long long strideT = (long long)Z * Y * X;
-    cd *__restrict__ out = prm.out;
     uint32_t nC = 0, nT = 0, nF = 0;  // fills consumed so far
     int ntrace = 0;
     cd hprev[6];                      // rows 0,1 of (1 + gamma_T) psi(t-1)
@@ -334,6 +346,7 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
         if (item < 0) break;
         const Item it = decode_item<P>(prm, item);
         const long long site0 = ((long long)(it.z0 + lz) * Y + (it.y0 + ly)) * X + (it.x0 + lx);
+        cd *__restrict__ out = prm.out + (long long)it.rhs * 12 * V;
         int t = (it.t0 == 0) ? T - 1 : it.t0 - 1;
         {   // prologue: seed the carried half-spinor from psi(t0-1)
             cd p[12];
@@ -448,8 +461,8 @@ static int sm_count() {
 
 // Work decomposition.  An item = (tile, T chunk); a CTA marches one item at a time and takes the
 // next from an atomic queue.  tchunk trades the tail (the last items finish unevenly) against the
-// per-item prologue/epilogue (one extra psi slice in, one extra psi + U_T slice at the end).  The panel (py x pz tiles, all of X) is the
-// set of tiles in flight together: as cubic as possible, at most one wave, so that most face
+// per-item prologue/epilogue (one extra psi slice in, one extra psi + U_T slice at the end).
+// The panel (py x pz tiles, all of X) is the set of tiles in flight together: as cubic as possible, at most one wave, so that most face
 // re-reads are L2 hits on data a neighbouring CTA is streaming at the same time.
 template <class P> static void plan_items(const KParams &p, TmaParams &prm) {
     const int nsm = sm_count();
@@ -464,7 +477,7 @@ template <class P> static void plan_items(const KParams &p, TmaParams &prm) {
         double best = 1e300;
         for (int tc = 1; tc <= T; tc++) {
             if (T % tc) continue;
-            const long long items = (long long)ntiles * (T / tc);
+            const long long items = (long long)ntiles * (T / tc) * p.nrhs;
             // dynamic queue: work = items * (steps + prologue/epilogue) / SMs, plus an expected tail of half an item
             const double cost = (double)items * (tc + 0.5) / nsm + 0.5 * (tc + 1);
             if (cost < best * 0.999) best = cost, best_tc = tc;
@@ -472,7 +485,14 @@ template <class P> static void plan_items(const KParams &p, TmaParams &prm) {
     }
     prm.tchunk = best_tc;
     prm.ntc = T / best_tc;
-    prm.nitems = ntiles * prm.ntc;
+    prm.nrhs = p.nrhs;
+    prm.rb = (p.nrhs < 4) ? p.nrhs : 4;  // RHS sharing the links of a tile through L2 (WD_TMA_RB: experiments)
+    if (const char *e = getenv("WD_TMA_RB")) {
+        const int v = atoi(e);
+        if (v >= 1) prm.rb = (v < p.nrhs) ? v : p.nrhs;
+    }
+    prm.nitems = ntiles * prm.ntc * p.nrhs;
+    const int wave = (nsm / prm.rb > 0) ? nsm / prm.rb : 1;  // tiles in flight together
     int bpy = 1, bpz = 1;
     double bscore = 1e300;
     for (int py = 1; py <= prm.nty; py++) {
@@ -482,7 +502,7 @@ template <class P> static void plan_items(const KParams &p, TmaParams &prm) {
             if (p.opt_zgroup > 0 && pz != p.opt_zgroup && prm.ntz % p.opt_zgroup == 0) continue;
             const int tiles = prm.ntx * py * pz;
             double score = 1.0 / (py * P::BY) + 1.0 / (pz * P::BZ);
-            if (tiles > nsm) score += 10.0 * tiles / nsm;  // over one wave: only if nothing smaller exists
+            if (tiles > wave) score += 10.0 * tiles / wave;  // over one wave: only if nothing smaller exists
             if (score < bscore) bscore = score, bpy = py, bpz = pz;
         }
     }
@@ -502,10 +522,10 @@ template <int BZ, int BY, int BX, int SELF> static cudaError_t launch_tma_self(c
     cudaError_t e;
 #define WD_ENC(m, base, nc, bx, by, bz, bc)                                      \
     if ((e = encode_field_map(&maps.m, base, p.n, p.Vs, nc, bx, by, bz, bc)) != cudaSuccess) return e;
-    WD_ENC(psi_c, p.psi, 12, BX, BY, BZ, 12)
-    WD_ENC(psi_z, p.psi, 12, BX, BY, 1, 12)
-    WD_ENC(psi_y, p.psi, 12, BX, 1, BZ, 12)
-    WD_ENC(psi_x, p.psi, 12, 1, BY, BZ, 12)
+    WD_ENC(psi_c, p.psi, 12 * p.nrhs, BX, BY, BZ, 12)
+    WD_ENC(psi_z, p.psi, 12 * p.nrhs, BX, BY, 1, 12)
+    WD_ENC(psi_y, p.psi, 12 * p.nrhs, BX, 1, BZ, 12)
+    WD_ENC(psi_x, p.psi, 12 * p.nrhs, 1, BY, BZ, 12)
     WD_ENC(u_c, p.U, 36, BX, BY, BZ, 9)
     WD_ENC(u_z, p.U, 36, BX, BY, 1, 9)
     WD_ENC(u_y, p.U, 36, BX, 1, BZ, 9)
