@@ -23,7 +23,7 @@ def tma_kernels(dims):
     out = []
     for k in range(wd.wd_kernel_count()):
         name = wd.wd_kernel_name(k)
-        if name.startswith("tma_"):
+        if name.startswith("tma"):
             b = [int(v) for v in name.split("_")[1].split("x")]
             if all(n % t == 0 for n, t in zip(dims[-3:], b)):
                 out.append(k)
