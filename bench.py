@@ -206,6 +206,22 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def reduce_over_ranks(total_ms, units, dist=None, device="cpu"):
+    """Replicas only: every rank ran the same independent job.  Whole-job time =
+    MAX over ranks of the device time, whole-job work = SUM over ranks of the units (site x RHS
+    applications) each processed.  No data-path collective: these two scalars are all that is exchanged."""
+    if dist is None:
+        return float(total_ms), int(units)
+    import torch
+
+    t = torch.tensor([float(total_ms)], dtype=torch.float64, device=device)
+    u = torch.tensor([int(units)], dtype=torch.int64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    dist.barrier()
+    return float(t.item()), int(u.item())
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -287,14 +303,10 @@ def run_ours(args):
     sampler.join()
     per_step = [evs[k].elapsed_time(evs[k + 1]) for k in range(args.steps)]
     total_ms = evs[0].elapsed_time(evs[-1])
-    if dist:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.barrier()
-        total_ms = float(t.item())
+    total_ms, units = reduce_over_ranks(total_ms, V * nrhs * args.steps, dist, "cuda")
     torch.cuda.synchronize()
     ms_per_step = total_ms / args.steps
-    site_rhs_per_s = world * V * nrhs * args.steps / (total_ms * 1e-3)
+    site_rhs_per_s = units / (total_ms * 1e-3)
     value = site_rhs_per_s * flop / 1e9
 
     # ---- roofline of the dominant kernel (the fused kernel is the whole step)
