@@ -65,11 +65,11 @@ struct KernelInfo {
 int kernel_count();
 const KernelInfo &kernel_info(int id);
 
-// TMA-staged T-marching kernels (wd_tma.cu)
+// TMA-staged T-marching kernels: first generation (wd_tma.cu), second generation (wd_tmb.cu)
 cudaError_t launch_tma_2x4x16(const KParams &p, int self, cudaStream_t st);
 cudaError_t launch_tma_4x4x8(const KParams &p, int self, cudaStream_t st);
-cudaError_t launch_tma2_2x4x16(const KParams &p, int self, cudaStream_t st);  // two compute groups per tile
-cudaError_t launch_tma2_4x4x8(const KParams &p, int self, cudaStream_t st);
+cudaError_t launch_tmb_4x4x8(const KParams &p, int self, cudaStream_t st);
+cudaError_t launch_tmb_2x8x8(const KParams &p, int self, cudaStream_t st);
 
 // self-coupling kernel of the unfused variant: out += S psi (clover) or out += mass * psi
 cudaError_t launch_selfcoupling(const KParams &p, int self, cudaStream_t st);

@@ -230,8 +230,8 @@ static const KernelInfo kKernels[] = {
     {"tile_1x4x4x4", 1, 4, 4, 4, 64, false, launch_tiled<1, 4, 4, 4>},
     {"tma_2x4x16", 1, 2, 4, 16, 160, true, launch_tma_2x4x16},
     {"tma_4x4x8", 1, 4, 4, 8, 160, true, launch_tma_4x4x8},
-    {"tma2_2x4x16", 1, 2, 4, 16, 288, true, launch_tma2_2x4x16},
-    {"tma2_4x4x8", 1, 4, 4, 8, 288, true, launch_tma2_4x4x8},
+    {"tmb_4x4x8", 1, 4, 4, 8, 160, true, launch_tmb_4x4x8},
+    {"tmb_2x8x8", 1, 2, 8, 8, 160, true, launch_tmb_2x8x8},
 };
 
 int kernel_count() { return (int)(sizeof(kKernels) / sizeof(kKernels[0])); }

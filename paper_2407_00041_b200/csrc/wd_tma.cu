@@ -76,19 +76,13 @@ cudaError_t encode_field_map(CUtensorMap *map, const void *base, const int n[4],
 //   Z  U_Z(t) interior | U_Z face z0-1 | psi faces z0-1, z0+BZ      [9][N] [9][FZ] [12][FZ] [12][FZ]
 //   Y  same for Y;  X  same for X
 //   SA, SB  the two 6x6 blocks of S(t)                    [18][N] each
-enum { OB_C = 0, OB_T, OB_Z, OB_Y, OB_X, OB_SA, OB_SB, OB_ITEM0, OB_ITEM1, OB_Q, OB_COUNT };
-// ITEM: work-item mailbox.  Q (two compute groups only): group 1's half of the result handed to group 0;
-// its "full" barrier is arrived on by group 1's warps, its "empty" barrier by group 0's.
+enum { OB_C = 0, OB_T, OB_Z, OB_Y, OB_X, OB_SA, OB_SB, OB_ITEM0, OB_ITEM1, OB_COUNT };  // ITEM: work-item mailbox
 
-template <int BZ_, int BY_, int BX_, int SELF_, int G_> struct Plan {
+template <int BZ_, int BY_, int BX_, int SELF_> struct Plan {
     static constexpr int BZ = BZ_, BY = BY_, BX = BX_, SELF = SELF_;
-    static constexpr int G = G_;            // compute groups: 1 = a thread does a whole site; 2 = a site is split
-                                            // between a thread of group 0 (T, Z hops, block A) and one of
-                                            // group 1 (Y, X hops, block B)
-    static constexpr int N = BZ * BY * BX;  // sites per tile = threads per compute group
-    static constexpr int NW = N / 32;       // warps per compute group
-    static constexpr int NCOMPUTE = G * N;
-    static constexpr int NTHREADS = NCOMPUTE + 32;  // + the producer warp
+    static constexpr int N = BZ * BY * BX;  // sites per tile = compute threads
+    static constexpr int NW = N / 32;       // compute warps
+    static constexpr int NTHREADS = N + 32; // + the producer warp
     static constexpr int FZ = BY * BX, FY = BZ * BX, FX = BZ * BY;  // sites per face
     static constexpr uint32_t E = 16;                               // bytes per element
     static constexpr uint32_t SZ_C = 12 * N * E, SZ_U = 9 * N * E, SZ_S = 18 * N * E;
@@ -105,10 +99,7 @@ template <int BZ_, int BY_, int BX_, int SELF_, int G_> struct Plan {
     static constexpr uint32_t SZ_X = SZ_U + (9 + 24) * FX * E;
     static constexpr uint32_t OFF_SA = OFF_X + SZ_X;
     static constexpr uint32_t OFF_SB = OFF_SA + SZ_S;
-    // exchange buffer of the two-group kernels, [12][N]: aliases the SB buffer once group 1 has read it
-    // (clover), else it has room of its own where S would be
-    static constexpr uint32_t OFF_Q = (SELF == SELF_CLOVER) ? OFF_SB : OFF_SA;
-    static constexpr uint32_t OFF_BAR = (SELF == SELF_CLOVER) ? OFF_SB + SZ_S : OFF_SA + (G == 2 ? SZ_C : 0);
+    static constexpr uint32_t OFF_BAR = (SELF == SELF_CLOVER) ? OFF_SB + SZ_S : OFF_SA;
     static constexpr uint32_t OFF_MAIL = OFF_BAR + 2 * OB_COUNT * 8;  // int[2]: item index per mailbox slot
     static constexpr uint32_t SMEM = OFF_MAIL + 16;
     static_assert(N % 32 == 0 && FZ % 8 == 0 && FY % 8 == 0 && FX % 8 == 0, "tile faces must keep 128-byte alignment");
@@ -146,7 +137,7 @@ __device__ __forceinline__ cd lds(const unsigned char *smem, uint32_t off) {
 // One direction MU != T of the stencil for the thread's site: both hops, operands from shared
 // memory.  (base, stride) pairs select interior or face storage per thread (no divergence: both
 // are shared-memory addresses).
-template <int MU, bool FENCE = false>
+template <int MU>
 __device__ __forceinline__ void hop_pair_smem(cd acc[12], const unsigned char *smem, uint32_t u_own, uint32_t u_own_stride,
                                               uint32_t pf, uint32_t pf_stride, uint32_t ub, uint32_t ub_stride,
                                               uint32_t pb, uint32_t pb_stride) {
@@ -156,10 +147,6 @@ __device__ __forceinline__ void hop_pair_smem(cd acc[12], const unsigned char *s
 #pragma unroll
     for (int c = 0; c < 12; c++) p[c] = lds(smem, pf + c * pf_stride);
     hop_term<MU, -1>(acc, p, u);
-    // FENCE (kernels capped at 168 registers): keep the compiler from hoisting the second hop's 21 loads
-    // above the first hop's arithmetic — with ~1 KB of L1 left beside 227 KB of shared memory a spill costs
-    // an L2 round trip
-    if (FENCE) asm volatile("" ::: "memory");
 #pragma unroll
     for (int k = 0; k < 9; k++) u[k] = lds(smem, ub + k * ub_stride);
 #pragma unroll
@@ -205,104 +192,6 @@ template <class P> __device__ __forceinline__ Item decode_item(const TmaParams &
     return it;
 }
 
-// ---------------------------------------------------------------- the producer (one thread)
-template <class P>
-__device__ __forceinline__ void producer_loop(const TmaMaps &maps, const TmaParams &prm, unsigned char *smem,
-                                              uint32_t sbase, uint32_t bar_full, uint32_t bar_empty) {
-    constexpr int BZ = P::BZ, BY = P::BY, BX = P::BX;
-    constexpr bool CLOVER = (P::SELF == SELF_CLOVER);
-    const int T = prm.n[0], Z = prm.n[1], Y = prm.n[2], X = prm.n[3];
-    // ======================= producer: one thread issues every TMA =======================
-    tma_prefetch_desc(&maps.psi_c); tma_prefetch_desc(&maps.psi_z); tma_prefetch_desc(&maps.psi_y);
-    tma_prefetch_desc(&maps.psi_x); tma_prefetch_desc(&maps.u_c);   tma_prefetch_desc(&maps.u_z);
-    tma_prefetch_desc(&maps.u_y);   tma_prefetch_desc(&maps.u_x);   tma_prefetch_desc(&maps.s_c);
-    const uint64_t pol_n = l2_policy_evict_normal();
-    const uint64_t pol_s = (prm.flags & 1) ? pol_n : l2_policy_evict_first();  // S is used exactly once
-    const uint64_t pol_u = (prm.flags & 2) ? l2_policy_evict_first() : pol_n;
-    const uint64_t pol_p = (prm.flags & 4) ? l2_policy_evict_last() : pol_n;
-    uint32_t nC = 0, nT = 0, nF = 0;  // fills issued so far of C, T, and of the per-step objects
-    volatile int *mail = reinterpret_cast<volatile int *>(smem + P::OFF_MAIL);
-    const bool dynamic = !(prm.flags & 16);
-    for (uint32_t seq = 0;; seq++) {
-        // next work item: atomic queue (fast SMs take more items; measured SM-to-SM spread of the
-        // streaming rate is ~20 %), handed to the consumers through a two-slot mailbox
-        int item = dynamic ? (int)atomicAdd(prm.sched, 1u) : (int)(blockIdx.x + seq * gridDim.x);
-        if (item >= prm.nitems) item = -1;
-        const uint32_t slot = seq & 1, mpar = (seq >> 1) & 1;
-        mbar_wait(bar_empty + 8 * (OB_ITEM0 + slot), mpar ^ 1);
-        mail[slot] = item;
-        mbar_arrive(bar_full + 8 * (OB_ITEM0 + slot));
-        if (item < 0) {
-            if (dynamic && atomicAdd(prm.sched + 1, 1u) == gridDim.x - 1) {  // last CTA out re-arms the queue
-                prm.sched[0] = 0;
-                prm.sched[1] = 0;
-            }
-            break;
-        }
-        const Item it = decode_item<P>(prm, item);
-        const int cx = 2 * it.x0, y0 = it.y0, z0 = it.z0;  // dim-0 coordinates count doubles
-        const int pc = 12 * it.rhs;                        // first component of this right-hand side
-        const int zlo = (z0 == 0) ? Z - 1 : z0 - 1, zhi = (z0 + BZ == Z) ? 0 : z0 + BZ;
-        const int ylo = (y0 == 0) ? Y - 1 : y0 - 1, yhi = (y0 + BY == Y) ? 0 : y0 + BY;
-        const int cxlo = 2 * ((it.x0 == 0) ? X - 1 : it.x0 - 1), cxhi = 2 * ((it.x0 + BX == X) ? 0 : it.x0 + BX);
-        int t = (it.t0 == 0) ? T - 1 : it.t0 - 1;
-        // prologue: psi(t0-1), only to seed the carried half-spinor
-        mbar_wait(bar_empty + 8 * OB_C, (nC & 1) ^ 1);
-        mbar_arrive_expect_tx(bar_full + 8 * OB_C, P::SZ_C);
-        tma_load_5d_hint(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cx, y0, z0, t, pc, pol_p);
-        nC++;
-        for (int j = 1; j <= prm.tchunk + 1; j++) {
-            const int tprev = t;
-            t = (t + 1 == T) ? 0 : t + 1;
-            const bool full = (j <= prm.tchunk);
-            // T object: U_T(t-1)
-            mbar_wait(bar_empty + 8 * OB_T, (nT & 1) ^ 1);
-            mbar_arrive_expect_tx(bar_full + 8 * OB_T, P::SZ_U);
-            tma_load_5d_hint(sbase + P::OFF_T, &maps.u_c, bar_full + 8 * OB_T, cx, y0, z0, tprev, 0, pol_u);
-            nT++;
-            if (full) {
-                const uint32_t pe = (nF & 1) ^ 1;
-                mbar_wait(bar_empty + 8 * OB_Z, pe);
-                mbar_arrive_expect_tx(bar_full + 8 * OB_Z, P::SZ_Z);
-                tma_load_5d_hint(sbase + P::OFF_Z, &maps.u_c, bar_full + 8 * OB_Z, cx, y0, z0, t, 9, pol_u);
-                tma_load_5d_hint(sbase + P::OFF_ZUF, &maps.u_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, 9, pol_u);
-                tma_load_5d_hint(sbase + P::OFF_ZLO, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, pc, pol_p);
-                tma_load_5d_hint(sbase + P::OFF_ZHI, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zhi, t, pc, pol_p);
-                mbar_wait(bar_empty + 8 * OB_Y, pe);
-                mbar_arrive_expect_tx(bar_full + 8 * OB_Y, P::SZ_Y);
-                tma_load_5d_hint(sbase + P::OFF_Y, &maps.u_c, bar_full + 8 * OB_Y, cx, y0, z0, t, 18, pol_u);
-                tma_load_5d_hint(sbase + P::OFF_YUF, &maps.u_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, 18, pol_u);
-                tma_load_5d_hint(sbase + P::OFF_YLO, &maps.psi_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, pc, pol_p);
-                tma_load_5d_hint(sbase + P::OFF_YHI, &maps.psi_y, bar_full + 8 * OB_Y, cx, yhi, z0, t, pc, pol_p);
-                mbar_wait(bar_empty + 8 * OB_X, pe);
-                mbar_arrive_expect_tx(bar_full + 8 * OB_X, P::SZ_X);
-                tma_load_5d_hint(sbase + P::OFF_X, &maps.u_c, bar_full + 8 * OB_X, cx, y0, z0, t, 27, pol_u);
-                tma_load_5d_hint(sbase + P::OFF_XUF, &maps.u_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, 27, pol_u);
-                tma_load_5d_hint(sbase + P::OFF_XLO, &maps.psi_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, pc, pol_p);
-                tma_load_5d_hint(sbase + P::OFF_XHI, &maps.psi_x, bar_full + 8 * OB_X, cxhi, y0, z0, t, pc, pol_p);
-            }
-            // C object: psi(t).  Its buffer is released after the X phase of the previous step, so it
-            // has only the S phases to land.  (Warming L2 one step ahead with a TMA prefetch was
-            // measured to cost 20 % at 64^4 — flag 8, profiles/r1b — so it is off.)
-            mbar_wait(bar_empty + 8 * OB_C, (nC & 1) ^ 1);
-            mbar_arrive_expect_tx(bar_full + 8 * OB_C, P::SZ_C);
-            tma_load_5d_hint(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cx, y0, z0, t, pc, pol_p);
-            nC++;
-            if (full && (prm.flags & 8)) tma_prefetch_5d(&maps.psi_c, cx, y0, z0, (t + 1 == T) ? 0 : t + 1, pc);
-            if (full && CLOVER) {
-                const uint32_t pe = (nF & 1) ^ 1;
-                mbar_wait(bar_empty + 8 * OB_SA, pe);
-                mbar_arrive_expect_tx(bar_full + 8 * OB_SA, P::SZ_S);
-                tma_load_5d_hint(sbase + P::OFF_SA, &maps.s_c, bar_full + 8 * OB_SA, cx, y0, z0, t, 0, pol_s);
-                mbar_wait(bar_empty + 8 * OB_SB, pe);
-                mbar_arrive_expect_tx(bar_full + 8 * OB_SB, P::SZ_S);
-                tma_load_5d_hint(sbase + P::OFF_SB, &maps.s_c, bar_full + 8 * OB_SB, cx, y0, z0, t, 18, pol_s);
-            }
-            if (full) nF++;
-        }
-    }
-}
-
 // ---------------------------------------------------------------- the kernel
 template <class P>
 __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ TmaMaps maps, const TmaParams prm) {
@@ -316,10 +205,8 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
     if (tid == 0) {
         if (sbase & 127u) __trap();  // TMA destinations need 128-byte alignment
         for (int k = 0; k < OB_COUNT; k++) {
-            // full: the producer's arrive(.expect_tx); empty: one arrive per warp that reads the object
-            const bool both = (k == OB_C || k == OB_ITEM0 || k == OB_ITEM1);
-            mbar_init(bar_full + 8 * k, (k == OB_Q) ? P::NW : 1);
-            mbar_init(bar_empty + 8 * k, (both ? P::G : 1) * P::NW);
+            mbar_init(bar_full + 8 * k, 1);        // the producer's arrive(.expect_tx)
+            mbar_init(bar_empty + 8 * k, P::NW);   // one arrive per compute warp
         }
         mbar_fence_init();
     }
@@ -327,21 +214,104 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
 
     const int T = prm.n[0], Z = prm.n[1], Y = prm.n[2], X = prm.n[3];
 
-    if (tid >= P::NCOMPUTE) {
+    if (tid >= N) {
         // ======================= producer: one thread issues every TMA =======================
-        if (tid == P::NCOMPUTE) producer_loop<P>(maps, prm, smem, sbase, bar_full, bar_empty);
+        if (tid != N) return;
+        tma_prefetch_desc(&maps.psi_c); tma_prefetch_desc(&maps.psi_z); tma_prefetch_desc(&maps.psi_y);
+        tma_prefetch_desc(&maps.psi_x); tma_prefetch_desc(&maps.u_c);   tma_prefetch_desc(&maps.u_z);
+        tma_prefetch_desc(&maps.u_y);   tma_prefetch_desc(&maps.u_x);   tma_prefetch_desc(&maps.s_c);
+        const uint64_t pol_n = l2_policy_evict_normal();
+        const uint64_t pol_s = (prm.flags & 1) ? pol_n : l2_policy_evict_first();  // S is used exactly once
+        const uint64_t pol_u = (prm.flags & 2) ? l2_policy_evict_first() : pol_n;
+        const uint64_t pol_p = (prm.flags & 4) ? l2_policy_evict_last() : pol_n;
+        uint32_t nC = 0, nT = 0, nF = 0;  // fills issued so far of C, T, and of the per-step objects
+        volatile int *mail = reinterpret_cast<volatile int *>(smem + P::OFF_MAIL);
+        const bool dynamic = !(prm.flags & 16);
+        for (uint32_t seq = 0;; seq++) {
+            // next work item: atomic queue (fast SMs take more items; measured SM-to-SM spread of the
+            // streaming rate is ~20 %), handed to the consumers through a two-slot mailbox
+            int item = dynamic ? (int)atomicAdd(prm.sched, 1u) : (int)(blockIdx.x + seq * gridDim.x);
+            if (item >= prm.nitems) item = -1;
+            const uint32_t slot = seq & 1, mpar = (seq >> 1) & 1;
+            mbar_wait(bar_empty + 8 * (OB_ITEM0 + slot), mpar ^ 1);
+            mail[slot] = item;
+            mbar_arrive(bar_full + 8 * (OB_ITEM0 + slot));
+            if (item < 0) {
+                if (dynamic && atomicAdd(prm.sched + 1, 1u) == gridDim.x - 1) {  // last CTA out re-arms the queue
+                    prm.sched[0] = 0;
+                    prm.sched[1] = 0;
+                }
+                break;
+            }
+            const Item it = decode_item<P>(prm, item);
+            const int cx = 2 * it.x0, y0 = it.y0, z0 = it.z0;  // dim-0 coordinates count doubles
+            const int pc = 12 * it.rhs;                        // first component of this right-hand side
+            const int zlo = (z0 == 0) ? Z - 1 : z0 - 1, zhi = (z0 + BZ == Z) ? 0 : z0 + BZ;
+            const int ylo = (y0 == 0) ? Y - 1 : y0 - 1, yhi = (y0 + BY == Y) ? 0 : y0 + BY;
+            const int cxlo = 2 * ((it.x0 == 0) ? X - 1 : it.x0 - 1), cxhi = 2 * ((it.x0 + BX == X) ? 0 : it.x0 + BX);
+            int t = (it.t0 == 0) ? T - 1 : it.t0 - 1;
+            // prologue: psi(t0-1), only to seed the carried half-spinor
+            mbar_wait(bar_empty + 8 * OB_C, (nC & 1) ^ 1);
+            mbar_arrive_expect_tx(bar_full + 8 * OB_C, P::SZ_C);
+            tma_load_5d_hint(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cx, y0, z0, t, pc, pol_p);
+            nC++;
+            for (int j = 1; j <= prm.tchunk + 1; j++) {
+                const int tprev = t;
+                t = (t + 1 == T) ? 0 : t + 1;
+                const bool full = (j <= prm.tchunk);
+                // T object: U_T(t-1)
+                mbar_wait(bar_empty + 8 * OB_T, (nT & 1) ^ 1);
+                mbar_arrive_expect_tx(bar_full + 8 * OB_T, P::SZ_U);
+                tma_load_5d_hint(sbase + P::OFF_T, &maps.u_c, bar_full + 8 * OB_T, cx, y0, z0, tprev, 0, pol_u);
+                nT++;
+                if (full) {
+                    const uint32_t pe = (nF & 1) ^ 1;
+                    mbar_wait(bar_empty + 8 * OB_Z, pe);
+                    mbar_arrive_expect_tx(bar_full + 8 * OB_Z, P::SZ_Z);
+                    tma_load_5d_hint(sbase + P::OFF_Z, &maps.u_c, bar_full + 8 * OB_Z, cx, y0, z0, t, 9, pol_u);
+                    tma_load_5d_hint(sbase + P::OFF_ZUF, &maps.u_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, 9, pol_u);
+                    tma_load_5d_hint(sbase + P::OFF_ZLO, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, pc, pol_p);
+                    tma_load_5d_hint(sbase + P::OFF_ZHI, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zhi, t, pc, pol_p);
+                    mbar_wait(bar_empty + 8 * OB_Y, pe);
+                    mbar_arrive_expect_tx(bar_full + 8 * OB_Y, P::SZ_Y);
+                    tma_load_5d_hint(sbase + P::OFF_Y, &maps.u_c, bar_full + 8 * OB_Y, cx, y0, z0, t, 18, pol_u);
+                    tma_load_5d_hint(sbase + P::OFF_YUF, &maps.u_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, 18, pol_u);
+                    tma_load_5d_hint(sbase + P::OFF_YLO, &maps.psi_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, pc, pol_p);
+                    tma_load_5d_hint(sbase + P::OFF_YHI, &maps.psi_y, bar_full + 8 * OB_Y, cx, yhi, z0, t, pc, pol_p);
+                    mbar_wait(bar_empty + 8 * OB_X, pe);
+                    mbar_arrive_expect_tx(bar_full + 8 * OB_X, P::SZ_X);
+                    tma_load_5d_hint(sbase + P::OFF_X, &maps.u_c, bar_full + 8 * OB_X, cx, y0, z0, t, 27, pol_u);
+                    tma_load_5d_hint(sbase + P::OFF_XUF, &maps.u_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, 27, pol_u);
+                    tma_load_5d_hint(sbase + P::OFF_XLO, &maps.psi_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, pc, pol_p);
+                    tma_load_5d_hint(sbase + P::OFF_XHI, &maps.psi_x, bar_full + 8 * OB_X, cxhi, y0, z0, t, pc, pol_p);
+                }
+                // C object: psi(t).  Its buffer is released after the X phase of the previous step, so it
+                // has only the S phases to land.  (Warming L2 one step ahead with a TMA prefetch was
+                // measured to cost 20 % at 64^4 — flag 8, profiles/r1b — so it is off.)
+                mbar_wait(bar_empty + 8 * OB_C, (nC & 1) ^ 1);
+                mbar_arrive_expect_tx(bar_full + 8 * OB_C, P::SZ_C);
+                tma_load_5d_hint(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cx, y0, z0, t, pc, pol_p);
+                nC++;
+                if (full && (prm.flags & 8)) tma_prefetch_5d(&maps.psi_c, cx, y0, z0, (t + 1 == T) ? 0 : t + 1, pc);
+                if (full && CLOVER) {
+                    const uint32_t pe = (nF & 1) ^ 1;
+                    mbar_wait(bar_empty + 8 * OB_SA, pe);
+                    mbar_arrive_expect_tx(bar_full + 8 * OB_SA, P::SZ_S);
+                    tma_load_5d_hint(sbase + P::OFF_SA, &maps.s_c, bar_full + 8 * OB_SA, cx, y0, z0, t, 0, pol_s);
+                    mbar_wait(bar_empty + 8 * OB_SB, pe);
+                    mbar_arrive_expect_tx(bar_full + 8 * OB_SB, P::SZ_S);
+                    tma_load_5d_hint(sbase + P::OFF_SB, &maps.s_c, bar_full + 8 * OB_SB, cx, y0, z0, t, 18, pol_s);
+                }
+                if (full) nF++;
+            }
+        }
         return;
     }
-    // ======================= consumers =======================
-    // G = 1: one thread per site does everything.  G = 2: thread s of group 0 does the T and Z hops
-    // and block A of site s, thread s of group 1 the Y and X hops and block B; group 1 hands its half
-    // (q) to group 0 through the exchange buffer, group 0 owns the carried state and the stores.
+    // ======================= consumers: one thread per site of the tile =======================
     const int lane = tid & 31;
-    const int grp = tid / N, stid = tid - grp * N;  // compute group, site of the tile
-    constexpr bool do_tz = true, do_yx = (P::G == 1);  // in the main loop below (group 1 has its own loop)
-    const int lx = stid % BX, ly = (stid / BX) % BY, lz = stid / (BX * BY);
+    const int lx = tid % BX, ly = (tid / BX) % BY, lz = tid / (BX * BY);
     constexpr uint32_t E = P::E, NS = N * E;
-    const uint32_t own = stid * E;
+    const uint32_t own = tid * E;
     // operand addresses (bytes from the start of shared memory): interior or face storage
     const uint32_t fz = (ly * BX + lx) * E, fy = (lz * BX + lx) * E, fx = (lz * BY + ly) * E;
     const bool zf_in = lz < BZ - 1, zb_in = lz > 0, yf_in = ly < BY - 1, yb_in = ly > 0, xf_in = lx < BX - 1, xb_in = lx > 0;
@@ -359,92 +329,15 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_empty + 8 * ob);
     };
-    // r = B p for the 6x6 block in the SA / SB buffer; the buffer is released (rel) once it is in registers
-    auto block_mul = [&](cd r[6], uint32_t so, const cd *pp, int ob, bool rel, uint32_t parity) {
-        mbar_wait(bar_full + 8 * ob, parity);
-        double d[6];
-        cd a[15];
-#pragma unroll
-        for (int q = 0; q < 3; q++) {
-            const cd dd = lds(smem, so + q * NS);
-            d[2 * q] = dd.x;
-            d[2 * q + 1] = dd.y;
-        }
-#pragma unroll
-        for (int k = 0; k < 15; k++) a[k] = lds(smem, so + (3 + k) * NS);
-        if (rel) release(ob);
-        herm6_mul(r, d, a, pp);
-    };
 
     const long long V = prm.Vs;  // component stride
     const long long strideT = (long long)Z * Y * X;
-    const volatile int *mail = reinterpret_cast<const volatile int *>(smem + P::OFF_MAIL);
-
-    if (P::G == 2 && grp == 1) {
-        // ---- group 1: Y and X hops, block B; its half q goes to group 0 through the exchange buffer
-        uint32_t nC = 0, nF = 0;
-        for (uint32_t seq = 0;; seq++) {
-            const uint32_t slot = seq & 1, mpar = (seq >> 1) & 1;
-            mbar_wait(bar_full + 8 * (OB_ITEM0 + slot), mpar);
-            const int item = mail[slot];
-            release(OB_ITEM0 + slot);
-            if (item < 0) break;
-            mbar_wait(bar_full + 8 * OB_C, nC & 1);  // prologue slice: nothing to do here
-            release(OB_C);
-            nC++;
-            for (int j = 1; j <= prm.tchunk + 1; j++) {
-                mbar_wait(bar_full + 8 * OB_C, nC & 1);
-                if (j == prm.tchunk + 1) {  // epilogue slice: nothing to do here
-                    release(OB_C);
-                    nC++;
-                    break;
-                }
-                const uint32_t pf = nF & 1;
-                cd q[12];
-#pragma unroll
-                for (int c = 0; c < 12; c++) q[c] = make_double2(0.0, 0.0);
-                mbar_wait(bar_full + 8 * OB_Y, pf);
-                hop_pair_smem<2, true>(q, smem, P::OFF_Y + own, NS, y_pf, y_pf_s, y_ub, y_b_s, y_pb, y_b_s);
-                release(OB_Y);
-                mbar_wait(bar_full + 8 * OB_X, pf);
-                hop_pair_smem<3, true>(q, smem, P::OFF_X + own, NS, x_pf, x_pf_s, x_ub, x_b_s, x_pb, x_b_s);
-                release(OB_X);
-                cd pb[6];  // rows 6..11 of psi(t)
-#pragma unroll
-                for (int c = 0; c < 6; c++) pb[c] = lds(smem, P::OFF_C + own + (6 + c) * NS);
-                release(OB_C);
-                nC++;
-#pragma unroll
-                for (int c = 0; c < 12; c++) q[c] = make_double2(-0.5 * q[c].x, -0.5 * q[c].y);
-                if (CLOVER) {
-                    cd r[6];
-                    block_mul(r, P::OFF_SB + own, pb, OB_SB, false, pf);  // SB is released by group 0 (q aliases it)
-#pragma unroll
-                    for (int c = 0; c < 6; c++) q[6 + c] = make_double2(q[6 + c].x + r[c].x, q[6 + c].y + r[c].y);
-                } else if (P::SELF == SELF_MASS) {
-#pragma unroll
-                    for (int c = 0; c < 6; c++)
-                        q[6 + c] = make_double2(fma(prm.mass, pb[c].x, q[6 + c].x), fma(prm.mass, pb[c].y, q[6 + c].y));
-                }
-                mbar_wait(bar_empty + 8 * OB_Q, pf ^ 1);  // group 0 has read the previous q
-                // (clover: q overwrites SB, but a thread writes only the column of its own site, whose S
-                // values it already holds in registers)
-#pragma unroll
-                for (int c = 0; c < 12; c++) *reinterpret_cast<cd *>(smem + P::OFF_Q + own + c * NS) = q[c];
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar_full + 8 * OB_Q);
-                nF++;
-            }
-        }
-        return;
-    }
-
-    // ---- group 0 (or the only group)
     uint32_t nC = 0, nT = 0, nF = 0;  // fills consumed so far
     int ntrace = 0;
     cd hprev[6];                      // rows 0,1 of (1 + gamma_T) psi(t-1)
     cd outp[12];                      // out(t-1) still missing its forward-T hop
+
+    const volatile int *mail = reinterpret_cast<const volatile int *>(smem + P::OFF_MAIL);
     for (uint32_t seq = 0;; seq++) {
         const uint32_t slot = seq & 1, mpar = (seq >> 1) & 1;
         mbar_wait(bar_full + 8 * (OB_ITEM0 + slot), mpar);
@@ -456,27 +349,22 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
         cd *__restrict__ out = prm.out + (long long)it.rhs * 12 * V;
         int t = (it.t0 == 0) ? T - 1 : it.t0 - 1;
         {   // prologue: seed the carried half-spinor from psi(t0-1)
+            cd p[12];
             mbar_wait(bar_full + 8 * OB_C, nC & 1);
-            if (do_tz) {
-                cd p[12];
 #pragma unroll
-                for (int c = 0; c < 12; c++) p[c] = lds(smem, P::OFF_C + own + c * NS);
-                project<0, +1>(hprev, p);
-            }
+            for (int c = 0; c < 12; c++) p[c] = lds(smem, P::OFF_C + own + c * NS);
+            project<0, +1>(hprev, p);
             release(OB_C);
             nC++;
         }
         for (int j = 1; j <= prm.tchunk + 1; j++) {
             const int tprev = t;
             t = (t + 1 == T) ? 0 : t + 1;
-            const bool last = (j == prm.tchunk + 1);  // epilogue step: only the forward-T hop of slice t-1
             cd p[12], acc[12];
-#pragma unroll
-            for (int c = 0; c < 12; c++) acc[c] = make_double2(0.0, 0.0);
-            mbar_wait(bar_full + 8 * OB_C, nC & 1);
-            if (do_tz) {  // T phase: finish out(t-1) with its forward hop, start out(t) with its backward hop
+            {   // T phase: finish out(t-1) with its forward hop, start out(t) with its backward hop
                 cd u[9];
                 mbar_wait(bar_full + 8 * OB_T, nT & 1);
+                mbar_wait(bar_full + 8 * OB_C, nC & 1);
                 if (prm.trace && tid == 0 && ntrace < kTraceLen) {
                     unsigned long long now;
                     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
@@ -497,84 +385,63 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
                         __stcs(out + (long long)c * V + ip,
                                make_double2(fma(-0.5, f[c].x, outp[c].x), fma(-0.5, f[c].y, outp[c].y)));
                 }
-                if (!last) {
-                    cd g[6];
-                    su3_mul<true>(g, u, hprev);  // U_T(t-1)^H (1 + gamma_T) psi(t-1)
-                    reconstruct_add<0, +1>(acc, g);
-                    project<0, +1>(hprev, p);
+                if (j == prm.tchunk + 1) {  // epilogue step: nothing else to do for slice t
+                    release(OB_T);
+                    release(OB_C);
+                    nT++;
+                    nC++;
+                    break;
                 }
+                cd g[6];
+                su3_mul<true>(g, u, hprev);  // U_T(t-1)^H (1 + gamma_T) psi(t-1)
+#pragma unroll
+                for (int c = 0; c < 12; c++) acc[c] = make_double2(0.0, 0.0);
+                reconstruct_add<0, +1>(acc, g);
+                project<0, +1>(hprev, p);
                 release(OB_T);
                 nT++;
             }
-            if (last) {
-                release(OB_C);
-                nC++;
-                break;
-            }
             const uint32_t pf = nF & 1;
-            if (do_tz) {
-                mbar_wait(bar_full + 8 * OB_Z, pf);
-                hop_pair_smem<1, (P::G == 2)>(acc, smem, P::OFF_Z + own, NS, z_pf, z_pf_s, z_ub, z_b_s, z_pb, z_b_s);
-                release(OB_Z);
-            }
-            if (do_yx) {
-                mbar_wait(bar_full + 8 * OB_Y, pf);
-                hop_pair_smem<2>(acc, smem, P::OFF_Y + own, NS, y_pf, y_pf_s, y_ub, y_b_s, y_pb, y_b_s);
-                release(OB_Y);
-                mbar_wait(bar_full + 8 * OB_X, pf);
-                hop_pair_smem<3>(acc, smem, P::OFF_X + own, NS, x_pf, x_pf_s, x_ub, x_b_s, x_pb, x_b_s);
-                release(OB_X);
-            }
-            if (P::G == 2) {  // re-read rows 0..5 of psi(t) for block A instead of keeping psi(t) live through the hops
-#pragma unroll
-                for (int c = 0; c < 6; c++) p[c] = lds(smem, P::OFF_C + own + c * NS);
-            }
+            mbar_wait(bar_full + 8 * OB_Z, pf);
+            hop_pair_smem<1>(acc, smem, P::OFF_Z + own, NS, z_pf, z_pf_s, z_ub, z_b_s, z_pb, z_b_s);
+            release(OB_Z);
+            mbar_wait(bar_full + 8 * OB_Y, pf);
+            hop_pair_smem<2>(acc, smem, P::OFF_Y + own, NS, y_pf, y_pf_s, y_ub, y_b_s, y_pb, y_b_s);
+            release(OB_Y);
+            mbar_wait(bar_full + 8 * OB_X, pf);
+            hop_pair_smem<3>(acc, smem, P::OFF_X + own, NS, x_pf, x_pf_s, x_ub, x_b_s, x_pb, x_b_s);
+            release(OB_X);
             release(OB_C);
             nC++;
             // self-coupling (a5) and combination (a6); the store waits for the forward-T hop
-            if (P::G == 1) {
-                if (CLOVER) {
+            if (CLOVER) {
 #pragma unroll
-                    for (int b = 0; b < 2; b++) {
-                        cd r[6];
-                        block_mul(r, (b == 0 ? P::OFF_SA : P::OFF_SB) + own, p + 6 * b, OB_SA + b, true, pf);
+                for (int b = 0; b < 2; b++) {
+                    const uint32_t so = (b == 0 ? P::OFF_SA : P::OFF_SB) + own;
+                    mbar_wait(bar_full + 8 * (OB_SA + b), pf);
+                    double d[6];
+                    cd a[15], r[6];
 #pragma unroll
-                        for (int c = 0; c < 6; c++)
-                            outp[6 * b + c] = make_double2(fma(-0.5, acc[6 * b + c].x, r[c].x), fma(-0.5, acc[6 * b + c].y, r[c].y));
+                    for (int q = 0; q < 3; q++) {
+                        const cd dd = lds(smem, so + q * NS);
+                        d[2 * q] = dd.x;
+                        d[2 * q + 1] = dd.y;
                     }
-                } else if (P::SELF == SELF_MASS) {
 #pragma unroll
-                    for (int c = 0; c < 12; c++)
-                        outp[c] = make_double2(fma(prm.mass, p[c].x, -0.5 * acc[c].x), fma(prm.mass, p[c].y, -0.5 * acc[c].y));
-                } else {
-#pragma unroll
-                    for (int c = 0; c < 12; c++) outp[c] = make_double2(-0.5 * acc[c].x, -0.5 * acc[c].y);
-                }
-            } else {
-                // group 0: rows 0..5 of S psi, own hops, plus group 1's half
-                cd r[6];
-                if (CLOVER) {
-                    block_mul(r, P::OFF_SA + own, p, OB_SA, true, pf);
-                } else {
+                    for (int k = 0; k < 15; k++) a[k] = lds(smem, so + (3 + k) * NS);
+                    release(OB_SA + b);
+                    herm6_mul(r, d, a, p + 6 * b);
 #pragma unroll
                     for (int c = 0; c < 6; c++)
-                        r[c] = (P::SELF == SELF_MASS) ? make_double2(prm.mass * p[c].x, prm.mass * p[c].y) : make_double2(0.0, 0.0);
+                        outp[6 * b + c] = make_double2(fma(-0.5, acc[6 * b + c].x, r[c].x), fma(-0.5, acc[6 * b + c].y, r[c].y));
                 }
+            } else if (P::SELF == SELF_MASS) {
 #pragma unroll
-                for (int c = 0; c < 6; c++) {
-                    outp[c] = make_double2(fma(-0.5, acc[c].x, r[c].x), fma(-0.5, acc[c].y, r[c].y));
-                    outp[6 + c] = make_double2(-0.5 * acc[6 + c].x, -0.5 * acc[6 + c].y);
-                }
-                mbar_wait(bar_full + 8 * OB_Q, pf);
+                for (int c = 0; c < 12; c++)
+                    outp[c] = make_double2(fma(prm.mass, p[c].x, -0.5 * acc[c].x), fma(prm.mass, p[c].y, -0.5 * acc[c].y));
+            } else {
 #pragma unroll
-                for (int c = 0; c < 12; c++) {
-                    const cd q = lds(smem, P::OFF_Q + own + c * NS);
-                    outp[c].x += q.x;
-                    outp[c].y += q.y;
-                }
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                release(OB_Q);
-                if (CLOVER) release(OB_SB);  // the next S block B may now overwrite q
+                for (int c = 0; c < 12; c++) outp[c] = make_double2(-0.5 * acc[c].x, -0.5 * acc[c].y);
             }
             nF++;
         }
@@ -643,8 +510,8 @@ template <class P> static void plan_items(const KParams &p, TmaParams &prm) {
     prm.pz = bpz;
 }
 
-template <int BZ, int BY, int BX, int SELF, int G> static cudaError_t launch_tma_self(const KParams &p, cudaStream_t st) {
-    using P = Plan<BZ, BY, BX, SELF, G>;
+template <int BZ, int BY, int BX, int SELF> static cudaError_t launch_tma_self(const KParams &p, cudaStream_t st) {
+    using P = Plan<BZ, BY, BX, SELF>;
     static bool attr_done = false;
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(k_tma<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::SMEM);
@@ -698,14 +565,12 @@ template <int BZ, int BY, int BX, int SELF, int G> static cudaError_t launch_tma
     return e;
 }
 
-template <int BZ, int BY, int BX, int G> static cudaError_t launch_tma(const KParams &p, int self, cudaStream_t st) {
-    if (self == SELF_CLOVER) return launch_tma_self<BZ, BY, BX, SELF_CLOVER, G>(p, st);
-    if (self == SELF_MASS) return launch_tma_self<BZ, BY, BX, SELF_MASS, G>(p, st);
-    return launch_tma_self<BZ, BY, BX, SELF_NONE, G>(p, st);
+template <int BZ, int BY, int BX> static cudaError_t launch_tma(const KParams &p, int self, cudaStream_t st) {
+    if (self == SELF_CLOVER) return launch_tma_self<BZ, BY, BX, SELF_CLOVER>(p, st);
+    if (self == SELF_MASS) return launch_tma_self<BZ, BY, BX, SELF_MASS>(p, st);
+    return launch_tma_self<BZ, BY, BX, SELF_NONE>(p, st);
 }
 
-cudaError_t launch_tma_2x4x16(const KParams &p, int self, cudaStream_t st) { return launch_tma<2, 4, 16, 1>(p, self, st); }
-cudaError_t launch_tma_4x4x8(const KParams &p, int self, cudaStream_t st) { return launch_tma<4, 4, 8, 1>(p, self, st); }
-cudaError_t launch_tma2_2x4x16(const KParams &p, int self, cudaStream_t st) { return launch_tma<2, 4, 16, 2>(p, self, st); }
-cudaError_t launch_tma2_4x4x8(const KParams &p, int self, cudaStream_t st) { return launch_tma<4, 4, 8, 2>(p, self, st); }
+cudaError_t launch_tma_2x4x16(const KParams &p, int self, cudaStream_t st) { return launch_tma<2, 4, 16>(p, self, st); }
+cudaError_t launch_tma_4x4x8(const KParams &p, int self, cudaStream_t st) { return launch_tma<4, 4, 8>(p, self, st); }
 }  // namespace wd

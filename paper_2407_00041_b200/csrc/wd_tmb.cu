@@ -1,0 +1,653 @@
+// wd_tmb.cu — second generation of the TMA-staged fused kernel ("tmb_*"): psi double-buffered, the
+// accumulator is the only state a thread carries.
+//
+// Same operator, same decomposition (persistent CTA per SM, one producer thread, one compute thread per
+// site of a 128-site tile marching along T, atomic work queue) as wd_tma.cu.  What changed:
+//   * psi(t) sits in one of TWO buffers for the whole of step t, and psi(t+1) lands in the other one
+//     during the step: no operand has less than a full step to arrive (in wd_tma.cu psi(t+1) had only the
+//     S phases, and consumers spent 23 % of their samples waiting for it, profiles/r1c);
+//   * at the end of step t both T hops that involve U_T(t) are done together: the forward hop completes
+//     out(t), which is stored at once, and the backward hop of slice t+1 initialises the next accumulator.
+//     Nothing but acc[12] lives across phases (wd_tma.cu also carried out(t-1), (1+gamma_T) psi(t-1) and
+//     psi(t): 120 more registers), psi of the own site is re-read from shared memory where it is needed;
+//   * S psi is folded into the accumulator (out = -1/2 (hops - 2 S psi)), S arrives as four 9-component
+//     objects through a ring of four slots that also carries U_T.
+// Measured at 64^4 (profiles/r1c): pure Wilson 3.66 -> 2.96 ms; Wilson-clover 4.17 -> 4.36 ms (the ring and
+// the 4x4x8 tile cost more than the registers bring), which is why wd_api.cu picks tma_* when there is a
+// clover term and tmb_* when there is none.
+#include <cstdio>
+#include <cstdlib>
+#include <vector>
+
+#include "wd_internal.h"
+#include "wd_math.cuh"
+#include "wd_tma.cuh"
+
+namespace wd {
+namespace tmb {
+
+// ---------------------------------------------------------------- shared-memory plan
+// Objects (each with a full/empty mbarrier pair):
+//   C   psi(t) interior [12][N], TWO buffers (fill n in buffer n & 1): psi(t) is read during the whole of
+//       step t and psi(t+1) at its end, so the next slice lands while the current one is in use
+//   Z   U_Z(t) interior | U_Z face z0-1 | psi faces z0-1, z0+BZ      [9][N] [9][FZ] [12][FZ] [12][FZ]
+//   Y   same for Y;  X  same for X
+//   R   a ring of four [9][N] slots shared by the five 9-component objects of a step, in this order:
+//       S1, S2 (block A of S(t): 3 diagonal pairs + 6 entries | 9 entries), S3, S4 (block B), T = U_T(t)
+//       (consumed between the Y and X hops, and at the end of the step)
+enum { OB_C = 0, OB_C1, OB_Z, OB_Y, OB_X, OB_R, OB_R1, OB_R2, OB_R3, OB_ITEM0, OB_ITEM1, OB_COUNT };
+
+template <int BZ_, int BY_, int BX_, int SELF_> struct Plan {
+    static constexpr int BZ = BZ_, BY = BY_, BX = BX_, SELF = SELF_;
+    static constexpr int N = BZ * BY * BX;   // sites per tile = compute threads
+    static constexpr int NW = N / 32;        // compute warps
+    static constexpr int NTHREADS = N + 32;  // + the producer warp
+    static constexpr int FZ = BY * BX, FY = BZ * BX, FX = BZ * BY;  // sites per face
+    static constexpr uint32_t E = 16;                               // bytes per element
+    static constexpr uint32_t SZ_C = 12 * N * E, SZ_U = 9 * N * E;
+    static constexpr uint32_t OFF_C = 0;
+    static constexpr uint32_t OFF_Z = OFF_C + 2 * SZ_C;
+    static constexpr uint32_t OFF_ZUF = OFF_Z + SZ_U, OFF_ZLO = OFF_ZUF + 9 * FZ * E, OFF_ZHI = OFF_ZLO + 12 * FZ * E;
+    static constexpr uint32_t SZ_Z = SZ_U + (9 + 24) * FZ * E;
+    static constexpr uint32_t OFF_Y = OFF_Z + SZ_Z;
+    static constexpr uint32_t OFF_YUF = OFF_Y + SZ_U, OFF_YLO = OFF_YUF + 9 * FY * E, OFF_YHI = OFF_YLO + 12 * FY * E;
+    static constexpr uint32_t SZ_Y = SZ_U + (9 + 24) * FY * E;
+    static constexpr uint32_t OFF_X = OFF_Y + SZ_Y;
+    static constexpr uint32_t OFF_XUF = OFF_X + SZ_U, OFF_XLO = OFF_XUF + 9 * FX * E, OFF_XHI = OFF_XLO + 12 * FX * E;
+    static constexpr uint32_t SZ_X = SZ_U + (9 + 24) * FX * E;
+    static constexpr uint32_t OFF_R = OFF_X + SZ_X;
+    static constexpr uint32_t OFF_BAR = OFF_R + 4 * SZ_U;
+    static constexpr uint32_t OFF_MAIL = OFF_BAR + 2 * OB_COUNT * 8;  // int[2]: item index per mailbox slot
+    static constexpr uint32_t SMEM = OFF_MAIL + 16;
+    static constexpr int RING_PER_STEP = (SELF == SELF_CLOVER) ? 5 : 1;  // S1..S4 and T, or T alone
+    static_assert(N % 32 == 0 && FZ % 8 == 0 && FY % 8 == 0 && FX % 8 == 0, "tile faces must keep 128-byte alignment");
+    static_assert(SMEM <= 232448, "shared-memory plan exceeds 227 KB");
+};
+
+struct TmaMaps {
+    CUtensorMap psi_c, psi_z, psi_y, psi_x;  // boxes: interior, z-face, y-face, x-face (12 components)
+    CUtensorMap u_c, u_z, u_y, u_x;          // same shapes, 9 components (one link)
+    CUtensorMap s_c;                         // interior box, 9 components (half of a 6x6 block)
+};
+
+struct TmaParams {
+    double2 *out;
+    long long V, Vs;     // sites, component stride
+    int n[4];
+    int ntx, nty, ntz;   // tiles per direction
+    int py, pz;          // rasterisation panel (in tiles); py | nty, pz | ntz
+    int tchunk, ntc;     // T steps per work item, items per tile
+    int nrhs, rb;        // right-hand sides in this launch; RHS per block of the item order
+    int nitems;          // ntx*nty*ntz*ntc*nrhs
+    double mass;
+    int flags;           // WD_TMA_FLAGS (experiments; 0 = production): 1 S evict_normal instead of evict_first,
+                         // 2 U evict_first, 4 psi evict_last, 16 static round-robin items
+    unsigned int *sched; // [0] next item, [1] CTAs finished (dynamic work distribution; both 0 between launches)
+    unsigned long long *trace;  // diagnostics (WD_TMA_TRACE): [cta][kTraceLen] globaltimer per step, or null
+};
+constexpr int kTraceLen = 1024;
+
+// ---------------------------------------------------------------- shared-memory operand fetch
+__device__ __forceinline__ cd lds(const unsigned char *smem, uint32_t off) {
+    return *reinterpret_cast<const cd *>(smem + off);
+}
+
+// One direction MU != T of the stencil for the thread's site: both hops, operands from shared
+// memory.  (base, stride) pairs select interior or face storage per thread (no divergence: both
+// are shared-memory addresses).
+template <int MU>
+__device__ __forceinline__ void hop_pair_smem(cd acc[12], const unsigned char *smem, uint32_t u_own, uint32_t u_own_stride,
+                                              uint32_t pf, uint32_t pf_stride, uint32_t ub, uint32_t ub_stride,
+                                              uint32_t pb, uint32_t pb_stride) {
+    cd p[12], u[9];
+#pragma unroll
+    for (int k = 0; k < 9; k++) u[k] = lds(smem, u_own + k * u_own_stride);
+#pragma unroll
+    for (int c = 0; c < 12; c++) p[c] = lds(smem, pf + c * pf_stride);
+    hop_term<MU, -1>(acc, p, u);
+#pragma unroll
+    for (int k = 0; k < 9; k++) u[k] = lds(smem, ub + k * ub_stride);
+#pragma unroll
+    for (int c = 0; c < 12; c++) p[c] = lds(smem, pb + c * pb_stride);
+    hop_term<MU, +1>(acc, p, u);
+}
+
+// acc[0..5] += (part of B) q for one 6x6 Hermitian block B.  H = 0: the 6 real diagonal entries (slots
+// 0..2, as pairs) and strict-upper entries 0..5 (slots 3..8); H = 1: strict-upper entries 6..14 (slots
+// 0..8).  q is the block's half of psi already scaled by -2 (out = S psi - 1/2 hops = -1/2 (hops - 2 S psi)).
+template <int H>
+__device__ __forceinline__ void herm6_half_add(cd acc[6], const unsigned char *smem, uint32_t so, uint32_t stride,
+                                               const cd q[6]) {
+    cd a[9];
+#pragma unroll
+    for (int k = 0; k < 9; k++) a[k] = lds(smem, so + k * stride);
+    if (H == 0) {
+#pragma unroll
+        for (int i = 0; i < 3; i++) {
+            acc[2 * i].x = fma(a[i].x, q[2 * i].x, acc[2 * i].x);
+            acc[2 * i].y = fma(a[i].x, q[2 * i].y, acc[2 * i].y);
+            acc[2 * i + 1].x = fma(a[i].y, q[2 * i + 1].x, acc[2 * i + 1].x);
+            acc[2 * i + 1].y = fma(a[i].y, q[2 * i + 1].y, acc[2 * i + 1].y);
+        }
+    }
+    int k = 0;
+#pragma unroll
+    for (int i = 0; i < 6; i++)
+#pragma unroll
+        for (int j = i + 1; j < 6; j++, k++) {
+            const int slot = (H == 0) ? k + 3 : k - 6;
+            if ((H == 0 && k < 6) || (H == 1 && k >= 6)) {
+                cfma(acc[i], a[slot], q[j]);
+                cfma_conj(acc[j], a[slot], q[i]);
+            }
+        }
+}
+
+struct Item {
+    int x0, y0, z0, t0, rhs;
+};
+
+// Item order (slowest to fastest): T chunk, block of up to `rb` right-hand sides, tile (panel
+// order), right-hand side within the block.  The CTAs in flight therefore work on the same few
+// tiles for rb right-hand sides at once: the links and S of a tile are fetched from HBM by the
+// first of them and are L2 hits for the others (a8: +384 B per extra RHS instead of +1536 B).
+template <class P> __device__ __forceinline__ Item decode_item(const TmaParams &prm, int item) {
+    const int ntiles = prm.ntx * prm.nty * prm.ntz;
+    const int per_chunk = ntiles * prm.nrhs;
+    const int chunk = item / per_chunk;
+    int rem = item - chunk * per_chunk;
+    const int blk = rem / (ntiles * prm.rb);
+    rem -= blk * ntiles * prm.rb;
+    const int rb_here = min(prm.rb, prm.nrhs - blk * prm.rb);
+    const int tile = rem / rb_here;
+    const int rhs = blk * prm.rb + (rem - tile * rb_here);
+    const int tpp = prm.ntx * prm.py * prm.pz;  // tiles per rasterisation panel
+    const int panel = tile / tpp;
+    int r = tile - panel * tpp;
+    const int tx = r % prm.ntx;
+    r /= prm.ntx;
+    const int tyi = r % prm.py, tzi = r / prm.py;
+    const int npy = prm.nty / prm.py;
+    Item it;
+    it.x0 = tx * P::BX;
+    it.y0 = ((panel % npy) * prm.py + tyi) * P::BY;
+    it.z0 = ((panel / npy) * prm.pz + tzi) * P::BZ;
+    it.t0 = chunk * prm.tchunk;
+    it.rhs = rhs;
+    return it;
+}
+
+// ---------------------------------------------------------------- the producer (one thread)
+// A resumable state machine: advance() performs the next load of the fixed sequence if the buffer it
+// targets has been released, else returns false.  Sequence per work item:
+//   [fetch item] [psi(t0-1)] [U_T(t0-1)] [psi(t0)]  then per step t:  [Z] [Y] [S1] [S2] [S3] [S4] [X] [psi(t+1)] [U_T(t)]
+// — the order in which the consumers release the buffers of the previous step.
+enum { ST_FETCH = 0, ST_PRO_C, ST_PRO_T, ST_PRO_C2, ST_Z, ST_S1, ST_Y, ST_S2, ST_X, ST_S3, ST_S4, ST_C, ST_T };
+
+template <class P> struct Producer {
+    uint32_t nC, nR, nF, seq;  // fills issued so far: C buffers, ring slots, per-step objects; items fetched
+    int stage, j, t;           // j = step within the item (1..tchunk), t = its T slice
+    int cx, y0, z0, pc, zlo, zhi, ylo, yhi, cxlo, cxhi;
+    bool done;
+    uint64_t pol_n, pol_s, pol_u, pol_p;
+
+    __device__ __forceinline__ void init(const TmaMaps &maps, const TmaParams &prm) {
+        tma_prefetch_desc(&maps.psi_c); tma_prefetch_desc(&maps.psi_z); tma_prefetch_desc(&maps.psi_y);
+        tma_prefetch_desc(&maps.psi_x); tma_prefetch_desc(&maps.u_c);   tma_prefetch_desc(&maps.u_z);
+        tma_prefetch_desc(&maps.u_y);   tma_prefetch_desc(&maps.u_x);   tma_prefetch_desc(&maps.s_c);
+        pol_n = l2_policy_evict_normal();
+        pol_s = (prm.flags & 1) ? pol_n : l2_policy_evict_first();  // S is used exactly once
+        pol_u = (prm.flags & 2) ? l2_policy_evict_first() : pol_n;
+        pol_p = (prm.flags & 4) ? l2_policy_evict_last() : pol_n;
+        nC = nR = nF = seq = 0;
+        stage = ST_FETCH;
+        j = t = 0;
+        done = false;
+    }
+
+    // psi(tt) interior into C buffer nC & 1 (its previous content was fill nC - 2)
+    __device__ __forceinline__ bool load_c(const TmaMaps &maps, uint32_t sbase, uint32_t bar_full, uint32_t bar_empty, int tt) {
+        const uint32_t b = nC & 1, ob = OB_C + b;
+        if (!mbar_try_wait(bar_empty + 8 * ob, ((nC >> 1) & 1) ^ 1)) return false;
+        mbar_arrive_expect_tx(bar_full + 8 * ob, P::SZ_C);
+        tma_load_5d_hint(sbase + P::OFF_C + b * P::SZ_C, &maps.psi_c, bar_full + 8 * ob, cx, y0, z0, tt, pc, pol_p);
+        nC++;
+        return true;
+    }
+    // nine components of U or S into ring slot nR & 3 (its previous content was fill nR - 4)
+    __device__ __forceinline__ bool load_ring(const CUtensorMap *map, uint32_t sbase, uint32_t bar_full, uint32_t bar_empty,
+                                              int tt, int comp, uint64_t pol) {
+        const uint32_t b = nR & 3, ob = OB_R + b;
+        if (!mbar_try_wait(bar_empty + 8 * ob, ((nR >> 2) & 1) ^ 1)) return false;
+        mbar_arrive_expect_tx(bar_full + 8 * ob, P::SZ_U);
+        tma_load_5d_hint(sbase + P::OFF_R + b * P::SZ_U, map, bar_full + 8 * ob, cx, y0, z0, tt, comp, pol);
+        nR++;
+        return true;
+    }
+
+    __device__ __forceinline__ bool advance(const TmaMaps &maps, const TmaParams &prm, unsigned char *smem, uint32_t sbase,
+                                            uint32_t bar_full, uint32_t bar_empty) {
+        constexpr int BZ = P::BZ, BY = P::BY, BX = P::BX;
+        constexpr bool CLOVER = (P::SELF == SELF_CLOVER);
+        if (done) return false;
+        const int T = prm.n[0];
+        const uint32_t pe = (nF & 1) ^ 1;
+        switch (stage) {
+        case ST_FETCH: {
+            // next work item: atomic queue (fast SMs take more items; measured SM-to-SM spread of the
+            // streaming rate is ~20 %), handed to the consumers through a two-slot mailbox
+            const uint32_t slot = seq & 1, mpar = (seq >> 1) & 1;
+            if (!mbar_try_wait(bar_empty + 8 * (OB_ITEM0 + slot), mpar ^ 1)) return false;
+            const bool dynamic = !(prm.flags & 16);
+            int item = dynamic ? (int)atomicAdd(prm.sched, 1u) : (int)(blockIdx.x + seq * gridDim.x);
+            if (item >= prm.nitems) item = -1;
+            reinterpret_cast<volatile int *>(smem + P::OFF_MAIL)[slot] = item;
+            mbar_arrive(bar_full + 8 * (OB_ITEM0 + slot));
+            seq++;
+            if (item < 0) {
+                if (dynamic && atomicAdd(prm.sched + 1, 1u) == gridDim.x - 1) {  // last CTA out re-arms the queue
+                    prm.sched[0] = 0;
+                    prm.sched[1] = 0;
+                }
+                done = true;
+                return false;
+            }
+            const Item it = decode_item<P>(prm, item);
+            const int Z = prm.n[1], Y = prm.n[2], X = prm.n[3];
+            cx = 2 * it.x0, y0 = it.y0, z0 = it.z0;  // dim-0 coordinates count doubles
+            pc = 12 * it.rhs;                        // first component of this right-hand side
+            zlo = (z0 == 0) ? Z - 1 : z0 - 1, zhi = (z0 + BZ == Z) ? 0 : z0 + BZ;
+            ylo = (y0 == 0) ? Y - 1 : y0 - 1, yhi = (y0 + BY == Y) ? 0 : y0 + BY;
+            cxlo = 2 * ((it.x0 == 0) ? X - 1 : it.x0 - 1), cxhi = 2 * ((it.x0 + BX == X) ? 0 : it.x0 + BX);
+            t = it.t0;
+            j = 1;
+            stage = ST_PRO_C;
+            return true;
+        }
+        case ST_PRO_C:  // psi(t0-1) and U_T(t0-1): the backward-T hop of the first slice
+            if (!load_c(maps, sbase, bar_full, bar_empty, (t == 0) ? T - 1 : t - 1)) return false;
+            stage = ST_PRO_T;
+            return true;
+        case ST_PRO_T:
+            if (!load_ring(&maps.u_c, sbase, bar_full, bar_empty, (t == 0) ? T - 1 : t - 1, 0, pol_u)) return false;
+            stage = ST_PRO_C2;
+            return true;
+        case ST_PRO_C2:  // psi(t0)
+            if (!load_c(maps, sbase, bar_full, bar_empty, t)) return false;
+            stage = ST_Z;
+            return true;
+        case ST_Z:
+            if (!mbar_try_wait(bar_empty + 8 * OB_Z, pe)) return false;
+            mbar_arrive_expect_tx(bar_full + 8 * OB_Z, P::SZ_Z);
+            tma_load_5d_hint(sbase + P::OFF_Z, &maps.u_c, bar_full + 8 * OB_Z, cx, y0, z0, t, 9, pol_u);
+            tma_load_5d_hint(sbase + P::OFF_ZUF, &maps.u_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, 9, pol_u);
+            tma_load_5d_hint(sbase + P::OFF_ZLO, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, pc, pol_p);
+            tma_load_5d_hint(sbase + P::OFF_ZHI, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zhi, t, pc, pol_p);
+            stage = ST_Y;
+            return true;
+        case ST_S1:
+            if (!load_ring(&maps.s_c, sbase, bar_full, bar_empty, t, 0, pol_s)) return false;
+            stage = ST_S2;
+            return true;
+        case ST_Y:
+            if (!mbar_try_wait(bar_empty + 8 * OB_Y, pe)) return false;
+            mbar_arrive_expect_tx(bar_full + 8 * OB_Y, P::SZ_Y);
+            tma_load_5d_hint(sbase + P::OFF_Y, &maps.u_c, bar_full + 8 * OB_Y, cx, y0, z0, t, 18, pol_u);
+            tma_load_5d_hint(sbase + P::OFF_YUF, &maps.u_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, 18, pol_u);
+            tma_load_5d_hint(sbase + P::OFF_YLO, &maps.psi_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, pc, pol_p);
+            tma_load_5d_hint(sbase + P::OFF_YHI, &maps.psi_y, bar_full + 8 * OB_Y, cx, yhi, z0, t, pc, pol_p);
+            stage = CLOVER ? ST_S1 : ST_X;
+            return true;
+        case ST_S2:
+            if (!load_ring(&maps.s_c, sbase, bar_full, bar_empty, t, 9, pol_s)) return false;
+            stage = ST_S3;
+            return true;
+        case ST_X:
+            if (!mbar_try_wait(bar_empty + 8 * OB_X, pe)) return false;
+            mbar_arrive_expect_tx(bar_full + 8 * OB_X, P::SZ_X);
+            tma_load_5d_hint(sbase + P::OFF_X, &maps.u_c, bar_full + 8 * OB_X, cx, y0, z0, t, 27, pol_u);
+            tma_load_5d_hint(sbase + P::OFF_XUF, &maps.u_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, 27, pol_u);
+            tma_load_5d_hint(sbase + P::OFF_XLO, &maps.psi_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, pc, pol_p);
+            tma_load_5d_hint(sbase + P::OFF_XHI, &maps.psi_x, bar_full + 8 * OB_X, cxhi, y0, z0, t, pc, pol_p);
+            stage = ST_C;
+            return true;
+        case ST_S3:
+            if (!load_ring(&maps.s_c, sbase, bar_full, bar_empty, t, 18, pol_s)) return false;
+            stage = ST_S4;
+            return true;
+        case ST_S4:
+            if (!load_ring(&maps.s_c, sbase, bar_full, bar_empty, t, 27, pol_s)) return false;
+            stage = ST_X;
+            return true;
+        case ST_C:  // psi(t+1): forward-T hop of this slice, then the next step's centre
+            if (!load_c(maps, sbase, bar_full, bar_empty, (t + 1 == T) ? 0 : t + 1)) return false;
+            stage = ST_T;
+            return true;
+        default:  // ST_T: U_T(t)
+            if (!load_ring(&maps.u_c, sbase, bar_full, bar_empty, t, 0, pol_u)) return false;
+            nF++;
+            j++;
+            t = (t + 1 == T) ? 0 : t + 1;
+            stage = (j > prm.tchunk) ? ST_FETCH : ST_Z;
+            return true;
+        }
+    }
+};
+
+// ---------------------------------------------------------------- the kernel
+template <class P>
+__global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ TmaMaps maps, const TmaParams prm) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const uint32_t sbase = smem_u32(smem);
+    const uint32_t bar_full = sbase + P::OFF_BAR, bar_empty = bar_full + OB_COUNT * 8;
+    const int tid = threadIdx.x;
+    constexpr int BZ = P::BZ, BY = P::BY, BX = P::BX, N = P::N;
+    constexpr bool CLOVER = (P::SELF == SELF_CLOVER);
+
+    if (tid == 0) {
+        if (sbase & 127u) __trap();  // TMA destinations need 128-byte alignment
+        for (int k = 0; k < OB_COUNT; k++) {
+            mbar_init(bar_full + 8 * k, 1);        // the producer's arrive(.expect_tx)
+            mbar_init(bar_empty + 8 * k, P::NW);   // one arrive per compute warp
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    const int T = prm.n[0], Z = prm.n[1], Y = prm.n[2], X = prm.n[3];
+
+    if (tid >= N) {
+        // ======================= producer: one thread issues every TMA =======================
+        if (tid == N) {
+            Producer<P> prod;
+            prod.init(maps, prm);
+            while (!prod.done) prod.advance(maps, prm, smem, sbase, bar_full, bar_empty);
+        }
+        return;
+    }
+    // ======================= consumers: one thread per site of the tile =======================
+    // The only state a thread carries from phase to phase is acc[12]: the hops of the current slice summed
+    // so far, with -2 S psi folded in (out = S psi - 1/2 hops = -1/2 (hops - 2 S psi)).  psi of the own site
+    // is re-read from the C buffer where it is needed instead of being kept in registers.
+    const int lane = tid & 31;
+    const int lx = tid % BX, ly = (tid / BX) % BY, lz = tid / (BX * BY);
+    constexpr uint32_t E = P::E, NS = N * E;
+    const uint32_t own = tid * E;
+    // operand addresses (bytes from the start of shared memory): interior (relative to the C buffer in use)
+    // or face storage
+    const uint32_t fz = (ly * BX + lx) * E, fy = (lz * BX + lx) * E, fx = (lz * BY + ly) * E;
+    const bool zf_in = lz < BZ - 1, zb_in = lz > 0, yf_in = ly < BY - 1, yb_in = ly > 0, xf_in = lx < BX - 1, xb_in = lx > 0;
+    const uint32_t z_pf = zf_in ? P::OFF_C + own + P::FZ * E : P::OFF_ZHI + fz, z_pf_s = zf_in ? NS : P::FZ * E;
+    const uint32_t z_pb = zb_in ? P::OFF_C + own - P::FZ * E : P::OFF_ZLO + fz, z_b_s = zb_in ? NS : P::FZ * E;
+    const uint32_t z_ub = zb_in ? P::OFF_Z + own - P::FZ * E : P::OFF_ZUF + fz;
+    const uint32_t y_pf = yf_in ? P::OFF_C + own + BX * E : P::OFF_YHI + fy, y_pf_s = yf_in ? NS : P::FY * E;
+    const uint32_t y_pb = yb_in ? P::OFF_C + own - BX * E : P::OFF_YLO + fy, y_b_s = yb_in ? NS : P::FY * E;
+    const uint32_t y_ub = yb_in ? P::OFF_Y + own - BX * E : P::OFF_YUF + fy;
+    const uint32_t x_pf = xf_in ? P::OFF_C + own + E : P::OFF_XHI + fx, x_pf_s = xf_in ? NS : P::FX * E;
+    const uint32_t x_pb = xb_in ? P::OFF_C + own - E : P::OFF_XLO + fx, x_b_s = xb_in ? NS : P::FX * E;
+    const uint32_t x_ub = xb_in ? P::OFF_X + own - E : P::OFF_XUF + fx;
+
+    auto release = [&](int ob) {
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_empty + 8 * ob);
+    };
+    auto wait_full = [&](int ob, uint32_t parity) { mbar_wait(bar_full + 8 * ob, parity); };
+
+    const long long V = prm.Vs;  // component stride
+    const long long strideT = (long long)Z * Y * X;
+    uint32_t nC = 0, nR = 0, nF = 0;  // fills consumed so far: C buffers, ring slots, per-step objects
+    int ntrace = 0;
+    cd acc[12];
+
+    // own-site psi of C fill n, rows r0..r0+5 scaled by s
+    auto load_half = [&](cd q[6], uint32_t cb, int r0, double s) {
+#pragma unroll
+        for (int c = 0; c < 6; c++) {
+            const cd v = lds(smem, P::OFF_C + cb + own + (r0 + c) * NS);
+            q[c] = make_double2(s * v.x, s * v.y);
+        }
+    };
+    // one 6x6 block of S (two consecutive ring objects): acc[6b..6b+5] += B_b * (-2 psi)
+    auto s_phase = [&](uint32_t cb, int b) {
+        const uint32_t s0 = nR & 3, s1 = (nR + 1) & 3;
+        cd q[6];
+        load_half(q, cb, 6 * b, -2.0);
+        wait_full(OB_R + s0, (nR >> 2) & 1);
+        herm6_half_add<0>(acc + 6 * b, smem, P::OFF_R + s0 * P::SZ_U + own, NS, q);
+        wait_full(OB_R + s1, ((nR + 1) >> 2) & 1);
+        herm6_half_add<1>(acc + 6 * b, smem, P::OFF_R + s1 * P::SZ_U + own, NS, q);
+        release(OB_R + s0);
+        release(OB_R + s1);
+        nR += 2;
+    };
+
+    const volatile int *mail = reinterpret_cast<const volatile int *>(smem + P::OFF_MAIL);
+    for (uint32_t seq = 0;; seq++) {
+        const uint32_t mslot = seq & 1, mpar = (seq >> 1) & 1;
+        wait_full(OB_ITEM0 + mslot, mpar);
+        const int item = mail[mslot];
+        release(OB_ITEM0 + mslot);
+        if (item < 0) break;
+        const Item it = decode_item<P>(prm, item);
+        const long long site0 = ((long long)(it.z0 + lz) * Y + (it.y0 + ly)) * X + (it.x0 + lx);
+        cd *__restrict__ out = prm.out + (long long)it.rhs * 12 * V;
+        int t = it.t0;
+        {   // prologue: acc = backward-T hop of slice t0, (1 + gamma_T) U_T(t0-1)^H psi(t0-1)
+            const uint32_t cb = (nC & 1) ? P::SZ_C : 0, slot = nR & 3;
+            wait_full(OB_C + (nC & 1), (nC >> 1) & 1);
+            wait_full(OB_R + slot, (nR >> 2) & 1);
+            cd p[12], u[9], h[6], g[6];
+#pragma unroll
+            for (int k = 0; k < 9; k++) u[k] = lds(smem, P::OFF_R + slot * P::SZ_U + own + k * NS);
+#pragma unroll
+            for (int c = 0; c < 12; c++) p[c] = lds(smem, P::OFF_C + cb + own + c * NS);
+            release(OB_C + (nC & 1));
+            release(OB_R + slot);
+            nC++;
+            nR++;
+            project<0, +1>(h, p);
+            su3_mul<true>(g, u, h);
+#pragma unroll
+            for (int c = 0; c < 12; c++) acc[c] = make_double2(0.0, 0.0);
+            reconstruct_add<0, +1>(acc, g);
+        }
+        for (int j = 1; j <= prm.tchunk; j++) {
+            const bool last = (j == prm.tchunk);
+            const uint32_t cb = (nC & 1) ? P::SZ_C : 0;  // C buffer holding psi(t) (waited for at the end of the
+            if (j == 1) wait_full(OB_C + (nC & 1), (nC >> 1) & 1);  // previous step, except for the first slice)
+            const uint32_t pf = nF & 1;
+            wait_full(OB_Z, pf);
+            hop_pair_smem<1>(acc, smem, P::OFF_Z + own, NS, z_pf + (zf_in ? cb : 0), z_pf_s, z_ub, z_b_s,
+                             z_pb + (zb_in ? cb : 0), z_b_s);
+            release(OB_Z);
+            wait_full(OB_Y, pf);
+            hop_pair_smem<2>(acc, smem, P::OFF_Y + own, NS, y_pf + (yf_in ? cb : 0), y_pf_s, y_ub, y_b_s,
+                             y_pb + (yb_in ? cb : 0), y_b_s);
+            release(OB_Y);
+            if (CLOVER) {  // between the Y and X hops, so that neither S4 nor the next U_T waits on a just-freed slot
+                s_phase(cb, 0);
+                s_phase(cb, 1);
+            }
+            wait_full(OB_X, pf);
+            hop_pair_smem<3>(acc, smem, P::OFF_X + own, NS, x_pf + (xf_in ? cb : 0), x_pf_s, x_ub, x_b_s,
+                             x_pb + (xb_in ? cb : 0), x_b_s);
+            release(OB_X);
+            nF++;
+            {   // T phase: forward hop (1 - gamma_T) U_T(t) psi(t+1) completes out(t); the backward hop of slice
+                // t+1, (1 + gamma_T) U_T(t)^H psi(t), starts the next accumulator
+                const uint32_t cn = cb ^ P::SZ_C, slot = nR & 3;  // psi(t+1) is in the other C buffer
+                wait_full(OB_C + ((nC + 1) & 1), ((nC + 1) >> 1) & 1);
+                wait_full(OB_R + slot, (nR >> 2) & 1);
+                if (prm.trace && tid == 0 && ntrace < kTraceLen) {
+                    unsigned long long now;
+                    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+                    prm.trace[(size_t)blockIdx.x * kTraceLen + ntrace++] = now;
+                }
+                cd u[9], p[12];
+#pragma unroll
+                for (int k = 0; k < 9; k++) u[k] = lds(smem, P::OFF_R + slot * P::SZ_U + own + k * NS);
+#pragma unroll
+                for (int c = 0; c < 12; c++) p[c] = lds(smem, P::OFF_C + cn + own + c * NS);
+                hop_term<0, -1>(acc, p, u);
+                if (P::SELF == SELF_MASS || !last) {
+#pragma unroll
+                    for (int c = 0; c < 12; c++) p[c] = lds(smem, P::OFF_C + cb + own + c * NS);  // psi(t)
+                }
+                const long long ip = (long long)t * strideT + site0;
+#pragma unroll
+                for (int c = 0; c < 12; c++) {
+                    cd o = make_double2(-0.5 * acc[c].x, -0.5 * acc[c].y);
+                    if (P::SELF == SELF_MASS) o = make_double2(fma(prm.mass, p[c].x, o.x), fma(prm.mass, p[c].y, o.y));
+                    __stcs(out + (long long)c * V + ip, o);
+                }
+                if (!last) {
+                    cd h[6], g[6];
+                    project<0, +1>(h, p);
+                    su3_mul<true>(g, u, h);
+#pragma unroll
+                    for (int c = 0; c < 12; c++) acc[c] = make_double2(0.0, 0.0);
+                    reconstruct_add<0, +1>(acc, g);
+                }
+                release(OB_R + slot);
+                nR++;
+                release(OB_C + (nC & 1));  // psi(t) is done; psi(t+1) stays for the next step
+                nC++;
+                if (last) {                // ... unless this was the item's last slice
+                    release(OB_C + (nC & 1));
+                    nC++;
+                }
+            }
+            t = (t + 1 == T) ? 0 : t + 1;
+        }
+    }
+}
+
+// ---------------------------------------------------------------- host side
+static int sm_count() {
+    static int n = 0;
+    if (!n) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1)
+            n = 148;
+    }
+    return n;
+}
+
+// Work decomposition.  An item = (tile, T chunk); a CTA marches one item at a time and takes the
+// next from an atomic queue.  tchunk trades the tail (the last items finish unevenly) against the
+// per-item prologue/epilogue (one extra psi slice in, one extra psi + U_T slice at the end).
+// The panel (py x pz tiles, all of X) is the set of tiles in flight together: as cubic as possible, at most one wave, so that most face
+// re-reads are L2 hits on data a neighbouring CTA is streaming at the same time.
+template <class P> static void plan_items(const KParams &p, TmaParams &prm) {
+    const int nsm = sm_count();
+    prm.ntx = p.n[3] / P::BX;
+    prm.nty = p.n[2] / P::BY;
+    prm.ntz = p.n[1] / P::BZ;
+    const int ntiles = prm.ntx * prm.nty * prm.ntz, T = p.n[0];
+    int best_tc = T;
+    if (p.opt_tchunk > 0 && T % p.opt_tchunk == 0) {
+        best_tc = p.opt_tchunk;
+    } else {
+        double best = 1e300;
+        for (int tc = 1; tc <= T; tc++) {
+            if (T % tc) continue;
+            const long long items = (long long)ntiles * (T / tc) * p.nrhs;
+            // dynamic queue: work = items * (steps + prologue/epilogue) / SMs, plus an expected tail of half an item
+            const double cost = (double)items * (tc + 0.5) / nsm + 0.5 * (tc + 1);
+            if (cost < best * 0.999) best = cost, best_tc = tc;
+        }
+    }
+    prm.tchunk = best_tc;
+    prm.ntc = T / best_tc;
+    prm.nrhs = p.nrhs;
+    prm.rb = (p.nrhs < 4) ? p.nrhs : 4;  // RHS sharing the links of a tile through L2 (WD_TMA_RB: experiments)
+    if (const char *e = getenv("WD_TMA_RB")) {
+        const int v = atoi(e);
+        if (v >= 1) prm.rb = (v < p.nrhs) ? v : p.nrhs;
+    }
+    prm.nitems = ntiles * prm.ntc * p.nrhs;
+    const int wave = (nsm / prm.rb > 0) ? nsm / prm.rb : 1;  // tiles in flight together
+    int bpy = 1, bpz = 1;
+    double bscore = 1e300;
+    for (int py = 1; py <= prm.nty; py++) {
+        if (prm.nty % py) continue;
+        for (int pz = 1; pz <= prm.ntz; pz++) {
+            if (prm.ntz % pz) continue;
+            if (p.opt_zgroup > 0 && pz != p.opt_zgroup && prm.ntz % p.opt_zgroup == 0) continue;
+            const int tiles = prm.ntx * py * pz;
+            double score = 1.0 / (py * P::BY) + 1.0 / (pz * P::BZ);
+            if (tiles > wave) score += 10.0 * tiles / wave;  // over one wave: only if nothing smaller exists
+            if (score < bscore) bscore = score, bpy = py, bpz = pz;
+        }
+    }
+    prm.py = bpy;
+    prm.pz = bpz;
+}
+
+template <int BZ, int BY, int BX, int SELF> static cudaError_t launch_tma_self(const KParams &p, cudaStream_t st) {
+    using P = Plan<BZ, BY, BX, SELF>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(k_tma<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::SMEM);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    TmaMaps maps;
+    cudaError_t e;
+#define WD_ENC(m, base, nc, bx, by, bz, bc)                                      \
+    if ((e = encode_field_map(&maps.m, base, p.n, p.Vs, nc, bx, by, bz, bc)) != cudaSuccess) return e;
+    WD_ENC(psi_c, p.psi, 12 * p.nrhs, BX, BY, BZ, 12)
+    WD_ENC(psi_z, p.psi, 12 * p.nrhs, BX, BY, 1, 12)
+    WD_ENC(psi_y, p.psi, 12 * p.nrhs, BX, 1, BZ, 12)
+    WD_ENC(psi_x, p.psi, 12 * p.nrhs, 1, BY, BZ, 12)
+    WD_ENC(u_c, p.U, 36, BX, BY, BZ, 9)
+    WD_ENC(u_z, p.U, 36, BX, BY, 1, 9)
+    WD_ENC(u_y, p.U, 36, BX, 1, BZ, 9)
+    WD_ENC(u_x, p.U, 36, 1, BY, BZ, 9)
+    WD_ENC(s_c, (SELF == SELF_CLOVER) ? p.S : p.U, 36, BX, BY, BZ, 9)
+#undef WD_ENC
+    TmaParams prm;
+    prm.out = p.out;
+    prm.V = p.V;
+    prm.Vs = p.Vs;
+    for (int a = 0; a < 4; a++) prm.n[a] = p.n[a];
+    prm.mass = p.mass;
+    plan_items<P>(p, prm);
+    const int grid = (prm.nitems < sm_count()) ? prm.nitems : sm_count();
+    prm.trace = nullptr;
+    prm.sched = p.sched;
+    prm.flags = getenv("WD_TMA_FLAGS") ? atoi(getenv("WD_TMA_FLAGS")) : 0;
+    const char *trace_path = getenv("WD_TMA_TRACE");
+    if (trace_path) {
+        if ((e = cudaMalloc((void **)&prm.trace, (size_t)grid * kTraceLen * 8)) != cudaSuccess) return e;
+        cudaMemsetAsync(prm.trace, 0, (size_t)grid * kTraceLen * 8, st);
+    }
+    k_tma<P><<<grid, P::NTHREADS, P::SMEM, st>>>(maps, prm);
+    e = cudaGetLastError();
+    if (trace_path && e == cudaSuccess) {  // diagnostics only: synchronous dump of the last launch's step times
+        std::vector<unsigned long long> host((size_t)grid * kTraceLen);
+        cudaStreamSynchronize(st);
+        cudaMemcpy(host.data(), prm.trace, host.size() * 8, cudaMemcpyDeviceToHost);
+        if (FILE *f = fopen(trace_path, "wb")) {
+            const int hdr[4] = {grid, kTraceLen, prm.tchunk, prm.nitems};
+            fwrite(hdr, sizeof(int), 4, f);
+            fwrite(host.data(), 8, host.size(), f);
+            fclose(f);
+        }
+    }
+    if (prm.trace) cudaFree(prm.trace);
+    return e;
+}
+
+template <int BZ, int BY, int BX> static cudaError_t launch_tma(const KParams &p, int self, cudaStream_t st) {
+    if (self == SELF_CLOVER) return launch_tma_self<BZ, BY, BX, SELF_CLOVER>(p, st);
+    if (self == SELF_MASS) return launch_tma_self<BZ, BY, BX, SELF_MASS>(p, st);
+    return launch_tma_self<BZ, BY, BX, SELF_NONE>(p, st);
+}
+
+// Tiles of 128 sites whose shared-memory plan fits 227 KB (2x4x16 is 816 B too large)
+}  // namespace tmb
+
+cudaError_t launch_tmb_4x4x8(const KParams &p, int self, cudaStream_t st) { return tmb::launch_tma<4, 4, 8>(p, self, st); }
+cudaError_t launch_tmb_2x8x8(const KParams &p, int self, cudaStream_t st) { return tmb::launch_tma<2, 8, 8>(p, self, st); }
+}  // namespace wd

@@ -23,14 +23,14 @@ def tma_kernels(dims):
     out = []
     for k in range(wd.wd_kernel_count()):
         name = wd.wd_kernel_name(k)
-        if name.startswith("tma"):
+        if name.startswith(("tma_", "tmb_")):
             b = [int(v) for v in name.split("_")[1].split("x")]
             if all(n % t == 0 for n, t in zip(dims[-3:], b)):
                 out.append(k)
     return out
 
 
-@pytest.mark.parametrize("dims", [(4, 2, 4, 16), (3, 4, 4, 16), (4, 4, 8, 32), (6, 8, 8, 16), (1, 4, 4, 8), (5, 8, 12, 24)])
+@pytest.mark.parametrize("dims", [(4, 2, 8, 16), (4, 2, 4, 16), (3, 4, 4, 16), (4, 4, 8, 32), (6, 8, 8, 16), (1, 4, 4, 8), (5, 8, 12, 24)])
 def test_tma_kernels_match_oracle(torch, dims):
     m0, csw = -0.4, 1.0
     U = wdinputs.gauge_haar(dims, 401)
