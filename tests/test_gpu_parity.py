@@ -329,3 +329,39 @@ def test_cfg4_full_size_sampled_outputs(torch):
         assert rel_l2(out[sites], ref) <= TOL
         worst = np.abs(out[sites] - ref).max() / np.abs(ref).max()
         assert worst <= 1e-13
+
+
+def test_cfg5_full_size_multi_rhs_sampled_outputs(torch):
+    """48^3 x 96 Wilson-clover with 12 right-hand sides in ONE wd_apply (the launch configuration bench.py
+    --config 5 times: automatic kernel, RHS-blocked item order, S built on the device), checked on sampled
+    sites of every right-hand side that the oracle computes one by one from (U, psi_r) alone.  The host
+    streams one RHS at a time through the oracle."""
+    import psutil
+
+    cfg = wdinputs.CONFIGS[5]
+    dims, nrhs = cfg["dims"], cfg["nrhs"]
+    if psutil.virtual_memory().available < 80e9 or torch.cuda.mem_get_info()[0] < 80e9 or os.environ.get("WD_TEST_SMALL"):
+        dims, nrhs = (24, 16, 16, 48), 5
+    V = wdinputs.volume(dims)
+    T, Z, Y, X = dims
+    U = wdinputs.gauge_haar(dims, cfg["gauge"][1])
+    rng = np.random.default_rng(5)
+    corners = [0, V - 1, X - 1, X, Y * X - 1, Z * Y * X - 1, Z * Y * X, (T - 1) * Z * Y * X, V - X, V // 2]
+    sites = np.unique(np.concatenate([np.array(corners), rng.integers(0, V, size=600)])).astype(np.int64)
+    with Op(torch, dims, cfg["m0"], cfg["csw"], U, build_clover=True, device_pack=1) as op:
+        Vs = wd.wd_component_stride(op.h)
+        din, dout = op.dev_spinor(nrhs), op.dev_spinor(nrhs)
+        dout.fill_(float("nan"))
+        refs = []
+        for r in range(nrhs):  # one RHS at a time: generate, pack into its slot, keep only the sampled reference
+            psi_r = wdinputs.spinor(dims, cfg["spinor_seed"] + r)
+            wd.wd_pack_spinor(op.h, din[r * 24 * Vs:(r + 1) * 24 * Vs], psi_r, 1)
+            refs.append(oracle.apply_sites(dims, cfg["m0"], cfg["csw"], U, psi_r[0], sites))
+            del psi_r
+        wd.wd_apply(op.h, dout, din, nrhs)
+        wd.wd_synchronize(op.h)
+        out_r = np.empty((1, V, 12, 2))
+        for r in range(nrhs):
+            wd.wd_unpack_spinor(op.h, out_r, dout[r * 24 * Vs:(r + 1) * 24 * Vs], 1)
+            assert np.isfinite(out_r).all(), r
+            assert rel_l2(out_r[0][sites], refs[r]) <= TOL, r
