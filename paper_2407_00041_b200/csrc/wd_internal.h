@@ -70,6 +70,9 @@ cudaError_t launch_tma_2x4x16(const KParams &p, int self, cudaStream_t st);
 cudaError_t launch_tma_4x4x8(const KParams &p, int self, cudaStream_t st);
 cudaError_t launch_tmb_4x4x8(const KParams &p, int self, cudaStream_t st);
 cudaError_t launch_tmb_2x8x8(const KParams &p, int self, cudaStream_t st);
+// multi-RHS kernel: G right-hand sides of a 64-site tile share U and S in shared memory (wd_tmr.cu)
+cudaError_t launch_tmr_2x4x8_g3(const KParams &p, int self, cudaStream_t st);
+cudaError_t launch_tmr_2x4x8_g2(const KParams &p, int self, cudaStream_t st);
 
 // self-coupling kernel of the unfused variant: out += S psi (clover) or out += mass * psi
 cudaError_t launch_selfcoupling(const KParams &p, int self, cudaStream_t st);

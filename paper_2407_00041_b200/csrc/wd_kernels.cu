@@ -232,6 +232,8 @@ static const KernelInfo kKernels[] = {
     {"tma_4x4x8", 1, 4, 4, 8, 160, true, launch_tma_4x4x8},
     {"tmb_4x4x8", 1, 4, 4, 8, 160, true, launch_tmb_4x4x8},
     {"tmb_2x8x8", 1, 2, 8, 8, 160, true, launch_tmb_2x8x8},
+    {"tmr3_2x4x8", 1, 2, 4, 8, 224, true, launch_tmr_2x4x8_g3},
+    {"tmr2_2x4x8", 1, 2, 4, 8, 160, true, launch_tmr_2x4x8_g2},
 };
 
 int kernel_count() { return (int)(sizeof(kKernels) / sizeof(kKernels[0])); }

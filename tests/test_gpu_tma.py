@@ -23,7 +23,7 @@ def tma_kernels(dims):
     out = []
     for k in range(wd.wd_kernel_count()):
         name = wd.wd_kernel_name(k)
-        if name.startswith(("tma_", "tmb_")):
+        if name.startswith(("tma_", "tmb_", "tmr")):
             b = [int(v) for v in name.split("_")[1].split("x")]
             if all(n % t == 0 for n, t in zip(dims[-3:], b)):
                 out.append(k)
@@ -78,3 +78,25 @@ def test_tma_many_items_per_cta_and_multi_rhs(torch):
     for kid in tma_kernels(dims):
         with Op(torch, dims, m0, csw, U, C, kernel=kid, tchunk=1) as op:
             assert rel_l2(op.apply(psi, nrhs), ref) <= TOL, wd.wd_kernel_name(kid)
+
+
+@pytest.mark.parametrize("nrhs", [2, 5, 7])
+def test_multi_rhs_groups_share_links(torch, nrhs):
+    """tmr kernels: G right-hand sides of a tile are processed by G thread groups that share U and S in shared
+    memory; nrhs that is not a multiple of G leaves groups without a right-hand side in the last block."""
+    dims, m0, csw = (6, 4, 8, 16), -0.4, 1.0
+    U = wdinputs.gauge_haar(dims, 431)
+    psi = wdinputs.spinor(dims, 432, nrhs=nrhs)
+    C = wdinputs.selfcoupling_random(dims, 433)
+    ref_c = oracle.apply(dims, m0, U, C, psi)
+    ref_w = oracle.apply(dims, m0, U, None, psi)
+    kids = [k for k in tma_kernels(dims) if wd.wd_kernel_name(k).startswith("tmr")]
+    assert kids
+    for kid in kids:
+        for tchunk in (0, 2):
+            with Op(torch, dims, m0, csw, U, C, kernel=kid, tchunk=tchunk) as op:
+                out = op.apply(psi, nrhs)
+                for r in range(nrhs):
+                    assert rel_l2(out[r], ref_c[r]) <= TOL, (wd.wd_kernel_name(kid), r)
+        with Op(torch, dims, m0, 0.0, U, None, kernel=kid) as op:
+            assert rel_l2(op.apply(psi, nrhs), ref_w) <= TOL, wd.wd_kernel_name(kid)
