@@ -99,8 +99,12 @@ int wd_get_clover(wd_handle *h, double *host_C);
 int wd_apply(wd_handle *h, void *dev_out, const void *dev_in, int nrhs);
 
 /* Same operation on HOST arrays in canonical spinor layout: host->device copy, on-device
- * repack, wd_apply, repack, device->host copy, all inside the call; returns after the result is
- * in host_out.  (Pinned host memory makes the copies faster but is not required.) */
+ * repack, operator, repack, device->host copy, all inside the call; returns after the result is
+ * in host_out.  With a TMA kernel the lattice is cut into up to 16 chunks along T and upload,
+ * compute and download of different chunks overlap on three streams (the library's own two plus
+ * the handle's); otherwise the steps run one after the other on the handle's stream.  Pinned
+ * host memory lets the copies overlap and is faster, but is not required.  Result identical bit
+ * for bit to wd_pack_spinor / wd_apply / wd_unpack_spinor. */
 int wd_apply_host(wd_handle *h, double *host_out, const double *host_in, int nrhs);
 
 /* Size in bytes of a device spinor buffer for nrhs right-hand sides (0 on error).  It is

@@ -12,6 +12,8 @@
 
 using namespace wd;
 
+static const int kMaxPipeChunks = 16;  // T chunks of the pipelined wd_apply_host
+
 struct wd_handle {
     int n[4];
     long long V, Vs;  // sites; component stride of the device layout (elements)
@@ -30,6 +32,10 @@ struct wd_handle {
     double2 *dstage;
     size_t dstage_bytes;
     double2 *work_in, *work_out;  // wd_apply_host
+    double2 *dstage_out;          // pipelined wd_apply_host: AoS staging of the result
+    cudaStream_t s_up, s_dn;      // its upload and download streams
+    cudaEvent_t ev_up[kMaxPipeChunks], ev_cmp[kMaxPipeChunks], ev_misc[2];
+    bool pipe_ready;
     long launches;
     std::string err;
 };
@@ -130,6 +136,9 @@ int wd_create(wd_handle **out, int T, int Z, int Y, int X, double m0, double csw
     h->dstage = nullptr;
     h->dstage_bytes = 0;
     h->work_in = h->work_out = nullptr;
+    h->dstage_out = nullptr;
+    h->s_up = h->s_dn = nullptr;
+    h->pipe_ready = false;
     h->launches = 0;
     e = cudaMalloc((void **)&h->dU, (size_t)h->Vs * kGaugeComps * sizeof(double2));
     if (e == cudaSuccess) e = cudaMalloc((void **)&h->dsched, 2 * sizeof(unsigned int));
@@ -156,6 +165,17 @@ int wd_destroy(wd_handle *h) {
     if (h->dstage) cudaFree(h->dstage);
     if (h->work_in) cudaFree(h->work_in);
     if (h->work_out) cudaFree(h->work_out);
+    if (h->dstage_out) cudaFree(h->dstage_out);
+    if (h->pipe_ready) {
+        cudaStreamDestroy(h->s_up);
+        cudaStreamDestroy(h->s_dn);
+        for (int k = 0; k < kMaxPipeChunks; k++) {
+            cudaEventDestroy(h->ev_up[k]);
+            cudaEventDestroy(h->ev_cmp[k]);
+        }
+        cudaEventDestroy(h->ev_misc[0]);
+        cudaEventDestroy(h->ev_misc[1]);
+    }
     for (int b = 0; b < 2; b++) {
         if (h->pinned[b]) cudaFreeHost(h->pinned[b]);
         if (h->pinned_ev[b]) cudaEventDestroy(h->pinned_ev[b]);
@@ -466,6 +486,7 @@ static int fill_params(wd_handle *h, KParams &p, const KernelInfo &k) {
     p.ntx = p.nty = p.ntz = p.ntc = p.gz = p.tchunk = 1;
     p.opt_tchunk = (int)h->tchunk_opt;
     p.opt_zgroup = (int)h->zgroup_opt;
+    p.tc_begin = p.tc_count = 0;
     p.sched = h->dsched;
     if (k.bx) {
         p.ntx = h->n[3] / k.bx;
@@ -529,15 +550,101 @@ int wd_apply(wd_handle *h, void *dev_out, const void *dev_in, int nrhs) {
     return WD_OK;
 }
 
+// Pipelined host-to-host application (TMA kernels, fused variant): the lattice is cut into C chunks along T; chunk
+// k is computed as soon as chunks k-1, k, k+1 of the input are on the device and in device layout, and is
+// repacked and copied back while the next chunks are computed.  Upload (s_up), compute (the handle's stream) and
+// download (s_dn) overlap, so a PCIe-bound application costs about max(H2D, D2H) instead of H2D + D2H.
+static int apply_host_pipelined(wd_handle *h, double *host_out, const double *host_in, int nrhs, int C) {
+    const int T = h->n[0], tcs = T / C;               // slices per chunk
+    const long long Vc = h->V / T * tcs;              // sites per chunk (a T range is a contiguous site range)
+    const size_t per = (size_t)h->V * kSpinorComps, cbytes = (size_t)Vc * kSpinorComps * sizeof(double2);
+    if (!h->pipe_ready) {
+        WD_CUDA(h, cudaStreamCreateWithFlags(&h->s_up, cudaStreamNonBlocking));
+        WD_CUDA(h, cudaStreamCreateWithFlags(&h->s_dn, cudaStreamNonBlocking));
+        for (int k = 0; k < kMaxPipeChunks; k++) {
+            WD_CUDA(h, cudaEventCreateWithFlags(&h->ev_up[k], cudaEventDisableTiming));
+            WD_CUDA(h, cudaEventCreateWithFlags(&h->ev_cmp[k], cudaEventDisableTiming));
+        }
+        WD_CUDA(h, cudaEventCreateWithFlags(&h->ev_misc[0], cudaEventDisableTiming));
+        WD_CUDA(h, cudaEventCreateWithFlags(&h->ev_misc[1], cudaEventDisableTiming));
+        h->pipe_ready = true;
+    }
+    if (!h->dstage_out) WD_CUDA(h, cudaMalloc((void **)&h->dstage_out, per * sizeof(double2)));
+    const KernelInfo &kinfo = kernel_info(wd_kernel_in_use(h));
+    KParams p;
+    const long saved_tchunk = h->tchunk_opt;
+    h->tchunk_opt = tcs;
+    int rc = fill_params(h, p, kinfo);
+    h->tchunk_opt = saved_tchunk;
+    if (rc) return rc;
+    p.psi = h->work_in;
+    p.out = h->work_out;
+    p.nrhs = 1;
+    p.tc_count = 1;
+    const int self = h->has_clover ? SELF_CLOVER : SELF_MASS;
+    // everything issued so far on the handle's stream comes first
+    WD_CUDA(h, cudaEventRecord(h->ev_misc[0], h->stream));
+    WD_CUDA(h, cudaStreamWaitEvent(h->s_up, h->ev_misc[0], 0));
+    WD_CUDA(h, cudaStreamWaitEvent(h->s_dn, h->ev_misc[0], 0));
+    for (int r = 0; r < nrhs; r++) {
+        const double2 *src = (const double2 *)host_in + r * per;
+        double2 *dst = (double2 *)host_out + r * per;
+        if (r > 0) {  // the previous right-hand side must be out of work_in (compute) and work_out (repack)
+            WD_CUDA(h, cudaStreamWaitEvent(h->s_up, h->ev_cmp[C - 1], 0));
+            WD_CUDA(h, cudaStreamWaitEvent(h->stream, h->ev_misc[1], 0));
+        }
+        for (int i = 0; i < C; i++) {  // upload order: last chunk first (chunk 0 needs slice T-1), then 0, 1, ...
+            const int k = (i == 0) ? C - 1 : i - 1;
+            const long long s0 = (long long)k * Vc;
+            WD_CUDA(h, cudaMemcpyAsync(h->dstage + s0 * kSpinorComps, src + s0 * kSpinorComps, cbytes, cudaMemcpyHostToDevice, h->s_up));
+            WD_CUDA(h, launch_aos_to_soa(h->work_in + s0, h->dstage + s0 * kSpinorComps, Vc, h->Vs, kSpinorComps, h->s_up));
+            WD_CUDA(h, cudaEventRecord(h->ev_up[k], h->s_up));
+            h->launches++;
+        }
+        for (int k = 0; k < C; k++) {
+            WD_CUDA(h, cudaStreamWaitEvent(h->stream, h->ev_up[(k + C - 1) % C], 0));
+            WD_CUDA(h, cudaStreamWaitEvent(h->stream, h->ev_up[k], 0));
+            WD_CUDA(h, cudaStreamWaitEvent(h->stream, h->ev_up[(k + 1) % C], 0));
+            p.tc_begin = k;
+            WD_CUDA(h, kinfo.launch(p, self, h->stream));
+            WD_CUDA(h, cudaEventRecord(h->ev_cmp[k], h->stream));
+            h->launches++;
+            const long long s0 = (long long)k * Vc;
+            WD_CUDA(h, cudaStreamWaitEvent(h->s_dn, h->ev_cmp[k], 0));
+            WD_CUDA(h, launch_soa_to_aos(h->dstage_out + s0 * kSpinorComps, h->work_out + s0, Vc, h->Vs, kSpinorComps, h->s_dn));
+            h->launches++;
+            if (k == C - 1) WD_CUDA(h, cudaEventRecord(h->ev_misc[1], h->s_dn));
+            WD_CUDA(h, cudaMemcpyAsync(dst + s0 * kSpinorComps, h->dstage_out + s0 * kSpinorComps, cbytes, cudaMemcpyDeviceToHost, h->s_dn));
+        }
+    }
+    WD_CUDA(h, cudaStreamSynchronize(h->s_dn));
+    WD_CUDA(h, cudaStreamSynchronize(h->s_up));
+    WD_CUDA(h, cudaStreamSynchronize(h->stream));
+    return WD_OK;
+}
+
 int wd_apply_host(wd_handle *h, double *host_out, const double *host_in, int nrhs) {
     if (!h) return WD_EINVAL;
     if (!host_out || !host_in || nrhs < 1) return fail(h, WD_EINVAL, "wd_apply_host: null pointer or nrhs < 1");
+    if (!h->has_gauge) return fail(h, WD_ESTATE, "wd_apply_host: no gauge field loaded");
+    if (h->csw != 0.0 && !h->has_clover)
+        return fail(h, WD_ESTATE, "wd_apply_host: csw != 0 but no self-coupling field (wd_load_clover / wd_build_clover)");
     const size_t per = (size_t)h->V * kSpinorComps, bytes = per * sizeof(double2);
     const size_t dbytes = wd_spinor_bytes(h, 1);
     if (!h->work_in) WD_CUDA(h, cudaMalloc((void **)&h->work_in, dbytes));
     if (!h->work_out) WD_CUDA(h, cudaMalloc((void **)&h->work_out, dbytes));
     int rc = ensure_dstage(h, bytes);
     if (rc) return rc;
+    // pipelined path: a TMA kernel, fused variant, and T splits into 4..16 equal chunks (WD_HOST_CHUNKS: experiments)
+    const KernelInfo &kinfo = kernel_info(wd_kernel_in_use(h));
+    int C = 0;
+    if (kinfo.multi_rhs && h->variant == 0 && strncmp(kinfo.name, "tmr", 3) != 0 && !getenv("WD_HOST_SERIAL"))
+    {
+        const int cmax = getenv("WD_HOST_CHUNKS") ? atoi(getenv("WD_HOST_CHUNKS")) : kMaxPipeChunks;
+        for (int c = (cmax < kMaxPipeChunks ? cmax : kMaxPipeChunks); c >= 4 && !C; c--)
+            if (h->n[0] % c == 0) C = c;
+    }
+    if (C) return apply_host_pipelined(h, host_out, host_in, nrhs, C);
     for (int r = 0; r < nrhs; r++) {
         WD_CUDA(h, cudaMemcpyAsync(h->dstage, (const double2 *)host_in + r * per, bytes, cudaMemcpyHostToDevice, h->stream));
         WD_CUDA(h, launch_aos_to_soa(h->work_in, h->dstage, h->V, h->Vs, kSpinorComps, h->stream));

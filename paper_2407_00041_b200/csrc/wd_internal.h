@@ -52,6 +52,8 @@ struct KParams {
     int tchunk;              // T-extent marched by one CTA
     int opt_tchunk, opt_zgroup;  // the raw WD_OPT_TCHUNK / WD_OPT_ZGROUP values (0 = automatic)
     unsigned int *sched;         // device, 2 words, zero between launches: work queue of the TMA kernels
+    int tc_begin, tc_count;      // TMA kernels: apply only to T chunks [tc_begin, tc_begin + tc_count) of opt_tchunk
+                                 // slices each (tc_count = 0: the whole lattice); used by the pipelined wd_apply_host
 };
 
 struct KernelInfo {

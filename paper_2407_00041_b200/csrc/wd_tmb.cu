@@ -79,7 +79,8 @@ struct TmaParams {
     int py, pz;          // rasterisation panel (in tiles); py | nty, pz | ntz
     int tchunk, ntc;     // T steps per work item, items per tile
     int nrhs, rb;        // right-hand sides in this launch; RHS per block of the item order
-    int nitems;          // ntx*nty*ntz*ntc*nrhs
+    int chunk0;          // first T chunk of this launch (0 unless a T range was asked for)
+    int nitems;          // ntx*nty*ntz*(chunks of this launch)*nrhs
     double mass;
     int flags;           // WD_TMA_FLAGS (experiments; 0 = production): 1 S evict_normal instead of evict_first,
                          // 2 U evict_first, 4 psi evict_last, 16 static round-robin items
@@ -99,8 +100,9 @@ struct Item {
 template <class P> __device__ __forceinline__ Item decode_item(const TmaParams &prm, int item) {
     const int ntiles = prm.ntx * prm.nty * prm.ntz;
     const int per_chunk = ntiles * prm.nrhs;
-    const int chunk = item / per_chunk;
-    int rem = item - chunk * per_chunk;
+    const int chunk_rel = item / per_chunk;
+    const int chunk = chunk_rel + prm.chunk0;
+    int rem = item - chunk_rel * per_chunk;
     const int blk = rem / (ntiles * prm.rb);
     rem -= blk * ntiles * prm.rb;
     const int rb_here = min(prm.rb, prm.nrhs - blk * prm.rb);
@@ -509,7 +511,8 @@ template <class P> static void plan_items(const KParams &p, TmaParams &prm) {
         const int v = atoi(e);
         if (v >= 1) prm.rb = (v < p.nrhs) ? v : p.nrhs;
     }
-    prm.nitems = ntiles * prm.ntc * p.nrhs;
+    prm.chunk0 = (p.tc_count > 0) ? p.tc_begin : 0;
+    prm.nitems = ntiles * ((p.tc_count > 0) ? p.tc_count : prm.ntc) * p.nrhs;
     const int wave = (nsm / prm.rb > 0) ? nsm / prm.rb : 1;  // tiles in flight together
     int bpy = 1, bpz = 1;
     double bscore = 1e300;
