@@ -326,6 +326,11 @@ def run_ours(args):
         "frac_of_8000_spec": achieved / 8000.0,
     }
 
+    # second roof: FP64 FMA peak measured on this GPU with a register-only microbenchmark
+    fp64_peak, _ = wd.wd_measure_fp64(1024, 8, False)
+    roofline["fp64_peak_tflops_measured"] = fp64_peak
+    roofline["frac_of_fp64_peak"] = (value / 1e3) / fp64_peak
+
     line = {
         "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",

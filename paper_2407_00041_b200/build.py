@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJDIR = os.path.join(HERE, "build")
 SO = os.path.join(HERE, "libwd.so")
-SOURCES = ["wd_api.cu", "wd_kernels.cu", "wd_tma.cu", "wd_tmb.cu", "wd_tmr.cu", "wd_pack.cu", "wd_clover.cu"]
+SOURCES = ["wd_api.cu", "wd_kernels.cu", "wd_tma.cu", "wd_tmb.cu", "wd_tmr.cu", "wd_pack.cu", "wd_clover.cu", "wd_peaks.cu"]
 HEADERS = ["wd_internal.h", "wd_math.cuh", "wd_tma.cuh", "wd_smem_ops.cuh", os.path.join("..", "..", "include", "wd.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
