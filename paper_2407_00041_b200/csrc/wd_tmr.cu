@@ -480,13 +480,10 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tmr(const __grid_constant__ 
 }
 
 // ---------------------------------------------------------------- host side
-static int sm_count() {
-    static int n = 0;
-    if (!n) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1)
-            n = 148;
-    }
+static int sm_count() {  // of the current device
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1)
+        n = 148;
     return n;
 }
 
@@ -531,11 +528,13 @@ template <class P> static void plan_items(const KParams &p, TmaParams &prm) {
 
 template <int BZ, int BY, int BX, int SELF, int G> static cudaError_t launch_self(const KParams &p, cudaStream_t st) {
     using P = Plan<BZ, BY, BX, SELF, G>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(k_tmr<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::SMEM);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
+    static bool attr_done[64] = {};  // per device: the attribute belongs to the device's copy of the kernel
+    int dev_id = 0;
+    cudaGetDevice(&dev_id);
+    if (dev_id < 0 || dev_id >= 64 || !attr_done[dev_id]) {
+        cudaError_t e0 = cudaFuncSetAttribute(k_tmr<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::SMEM);
+        if (e0 != cudaSuccess) return e0;
+        if (dev_id >= 0 && dev_id < 64) attr_done[dev_id] = true;
     }
     TmaMaps maps;
     cudaError_t e;

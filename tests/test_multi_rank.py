@@ -20,14 +20,14 @@ dist.init_process_group("gloo")
 r = dist.get_rank()
 ms, units = bench.reduce_over_ranks([3.0, 7.5][r], [1000, 1024][r], dist, "cpu")
 lone = bench.reduce_over_ranks(2.0, 10)          # no process group: passthrough
-print(json.dumps({{"rank": r, "ms": ms, "units": units, "lone": lone}}), flush=True)
+open(os.path.join({out!r}, "rank%d.json" % r), "w").write(json.dumps({{"rank": r, "ms": ms, "units": units, "lone": lone}}))
 dist.destroy_process_group()
 '''
 
 
 def test_replica_aggregation_max_time_sum_work_gloo_world2(tmp_path):
     script = tmp_path / "worker.py"
-    script.write_text(WORKER.format(root=ROOT))
+    script.write_text(WORKER.format(root=ROOT, out=str(tmp_path)))
     import socket
 
     with socket.socket() as sk:  # a free rendezvous port
@@ -38,7 +38,7 @@ def test_replica_aggregation_max_time_sum_work_gloo_world2(tmp_path):
            "127.0.0.1", "--master-port", str(port), str(script)]
     r = subprocess.run(cmd, capture_output=True, text=True, env=env, timeout=240)
     assert r.returncode == 0, r.stderr[-2000:]
-    lines = [json.loads(l) for l in r.stdout.splitlines() if l.startswith("{")]
+    lines = [json.loads((tmp_path / ("rank%d.json" % k)).read_text()) for k in (0, 1)]  # one file per rank
     assert sorted(l["rank"] for l in lines) == [0, 1]
     for l in lines:
         assert l["ms"] == 7.5 and l["units"] == 2024 and l["lone"] == [2.0, 10]
