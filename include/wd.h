@@ -136,9 +136,11 @@ int wd_layout_unpack_host(int field, long long nsites, const double *packed, dou
 /* Register-only FP64 FMA microbenchmark (the paper's section 3.1 method): the FP64 roof that
  * co-limits a multi-RHS application.  Launches threads_per_sm-thread CTAs (a multiple of 32, <= 1024) filling
  * every SM (one_cta_per_sm = 0) or exactly one per SM (1), each thread running `ilp` (1, 2, 4, 8, 16) independent
- * FMA chains.  *tflops = achieved 2*FMA/s; *cycles_per_fma_per_warp (may be NULL) = cycles of the nominal
+ * FMA chains; distinct_operands = 0: a = fma(a, b, c) with b, c common to all chains, 1: every operand of every
+ * chain a register pair of its own.  *tflops = achieved 2*FMA/s; *cycles_per_fma_per_warp (may be NULL) = cycles of the nominal
  * maximum SM clock between two FMAs issued on one SM sub-partition.  Synchronous, default stream. */
-int wd_measure_fp64(int threads_per_sm, int ilp, int one_cta_per_sm, double *tflops, double *cycles_per_fma_per_warp);
+int wd_measure_fp64(int threads_per_sm, int ilp, int one_cta_per_sm, int distinct_operands, double *tflops,
+                    double *cycles_per_fma_per_warp);
 
 /* cudaStream_t passed as void* (NULL = legacy default stream).  PyTorch supplies memory and
  * streams only. */

@@ -38,7 +38,7 @@ SIGNATURES = {
     "wd_layout_bytes": (_sz, [_i, ctypes.c_longlong]),
     "wd_layout_pack_host": (_i, [_i, ctypes.c_longlong, _vp, _vp]),
     "wd_layout_unpack_host": (_i, [_i, ctypes.c_longlong, _vp, _vp]),
-    "wd_measure_fp64": (_i, [_i, _i, _i, ctypes.POINTER(_d), ctypes.POINTER(_d)]),
+    "wd_measure_fp64": (_i, [_i, _i, _i, _i, ctypes.POINTER(_d), ctypes.POINTER(_d)]),
     "wd_set_stream": (_i, [_vp, _vp]),
     "wd_synchronize": (_i, [_vp]),
     "wd_set_option": (_i, [_vp, _i, _l]),
@@ -160,9 +160,11 @@ def wd_layout_unpack_host(field: int, nsites: int, packed, canonical) -> None:
         raise WDError(rc, "wd_layout_unpack_host: bad argument")
 
 
-def wd_measure_fp64(threads_per_sm: int, ilp: int, one_cta_per_sm: bool = False) -> tuple[float, float]:
+def wd_measure_fp64(threads_per_sm: int, ilp: int, one_cta_per_sm: bool = False,
+                    distinct_operands: bool = False) -> tuple[float, float]:
     tf, cyc = _d(0.0), _d(0.0)
-    rc = lib().wd_measure_fp64(threads_per_sm, ilp, 1 if one_cta_per_sm else 0, ctypes.byref(tf), ctypes.byref(cyc))
+    rc = lib().wd_measure_fp64(threads_per_sm, ilp, 1 if one_cta_per_sm else 0, 1 if distinct_operands else 0,
+                               ctypes.byref(tf), ctypes.byref(cyc))
     if rc != WD_OK:
         raise WDError(rc, "wd_measure_fp64")
     return tf.value, cyc.value

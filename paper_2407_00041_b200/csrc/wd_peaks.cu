@@ -7,14 +7,21 @@
 
 namespace {
 
-template <int ILP> __global__ void k_dfma(double *out, int iters, double b, double c) {
+// DISTINCT = false: a = fma(a, b, c) with b, c shared by all chains (two of the three operands are re-used
+// registers).  DISTINCT = true: a_j = fma(x_j, y_j, a_j) with every operand a register pair of its own, which is
+// what the SU(3) and 6x6 arithmetic of the operator looks like to the register file.
+template <int ILP, bool DISTINCT> __global__ void k_dfma(double *out, int iters, double b, double c) {
     extern __shared__ unsigned char pad[];  // only sizes the CTA so that one CTA fits per SM when asked to
-    double a[ILP];
+    double a[ILP], x[ILP], y[ILP];
 #pragma unroll
-    for (int j = 0; j < ILP; j++) a[j] = 1.0 + 1e-3 * (threadIdx.x + j);
+    for (int j = 0; j < ILP; j++) {
+        a[j] = 1.0 + 1e-3 * (threadIdx.x + j);
+        x[j] = b + 1e-9 * j;
+        y[j] = c * (j + 1);
+    }
     for (int i = 0; i < iters; i++) {
 #pragma unroll
-        for (int j = 0; j < ILP; j++) a[j] = fma(a[j], b, c);
+        for (int j = 0; j < ILP; j++) a[j] = DISTINCT ? fma(x[j], y[(j + 1) % ILP], a[j]) : fma(a[j], b, c);
     }
     double s = 0.0;
 #pragma unroll
@@ -22,15 +29,15 @@ template <int ILP> __global__ void k_dfma(double *out, int iters, double b, doub
     if (s == 123.456) out[blockIdx.x * blockDim.x + threadIdx.x] = s;  // never true: keeps the chain alive
 }
 
-template <int ILP> cudaError_t run(int grid, int threads, size_t smem, int iters, double *out, float *ms) {
-    cudaError_t e = cudaFuncSetAttribute(k_dfma<ILP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+template <int ILP, bool D> cudaError_t run(int grid, int threads, size_t smem, int iters, double *out, float *ms) {
+    cudaError_t e = cudaFuncSetAttribute(k_dfma<ILP, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
-    k_dfma<ILP><<<grid, threads, smem>>>(out, iters / 8, 1.0000001, 1e-9);  // warm-up
+    k_dfma<ILP, D><<<grid, threads, smem>>>(out, iters / 8, 1.0000001, 1e-9);  // warm-up
     cudaEventRecord(e0);
-    k_dfma<ILP><<<grid, threads, smem>>>(out, iters, 1.0000001, 1e-9);
+    k_dfma<ILP, D><<<grid, threads, smem>>>(out, iters, 1.0000001, 1e-9);
     cudaEventRecord(e1);
     e = cudaEventSynchronize(e1);
     if (e == cudaSuccess) e = cudaGetLastError();
@@ -42,7 +49,8 @@ template <int ILP> cudaError_t run(int grid, int threads, size_t smem, int iters
 
 }  // namespace
 
-extern "C" int wd_measure_fp64(int threads_per_sm, int ilp, int one_cta_per_sm, double *tflops, double *cycles_per_fma_per_warp) {
+extern "C" int wd_measure_fp64(int threads_per_sm, int ilp, int one_cta_per_sm, int distinct_operands, double *tflops,
+                               double *cycles_per_fma_per_warp) {
     if (!tflops || threads_per_sm < 32 || threads_per_sm > 1024 || threads_per_sm % 32) return WD_EINVAL;
     int dev = 0, nsm = 0, khz = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return WD_ECUDA;
@@ -55,14 +63,16 @@ extern "C" int wd_measure_fp64(int threads_per_sm, int ilp, int one_cta_per_sm, 
     if (cudaMalloc((void **)&out, (size_t)grid * threads_per_sm * sizeof(double)) != cudaSuccess) return WD_ENOMEM;
     float ms = 0.f;
     cudaError_t e;
+#define WD_RUN(I) (distinct_operands ? run<I, true>(grid, threads_per_sm, smem, iters, out, &ms) : run<I, false>(grid, threads_per_sm, smem, iters, out, &ms))
     switch (ilp) {
-    case 1: e = run<1>(grid, threads_per_sm, smem, iters, out, &ms); break;
-    case 2: e = run<2>(grid, threads_per_sm, smem, iters, out, &ms); break;
-    case 4: e = run<4>(grid, threads_per_sm, smem, iters, out, &ms); break;
-    case 8: e = run<8>(grid, threads_per_sm, smem, iters, out, &ms); break;
-    case 16: e = run<16>(grid, threads_per_sm, smem, iters, out, &ms); break;
+    case 1: e = WD_RUN(1); break;
+    case 2: e = WD_RUN(2); break;
+    case 4: e = WD_RUN(4); break;
+    case 8: e = WD_RUN(8); break;
+    case 16: e = WD_RUN(16); break;
     default: cudaFree(out); return WD_EINVAL;
     }
+#undef WD_RUN
     cudaFree(out);
     if (e != cudaSuccess) return WD_ECUDA;
     const double fmas = (double)grid * threads_per_sm * (double)iters * ilp;

@@ -30,9 +30,11 @@ namespace tmr {
 
 // ---------------------------------------------------------------- shared-memory plan
 // shared objects:  UZ = U_Z(t) interior [9][N] | face z0-1 [9][FZ];  UY, UX alike;
-//                  R  = ring of four [9][N] slots: S1, S2 (block A), S3, S4 (block B), T = U_T(t)
+//                  R  = ring of kRing [9][N] slots: S1, S2 (block A), S3, S4 (block B), T = U_T(t)
 // per group g:     C  = psi_g(t) interior [12][N], two buffers;  PZ = psi_g faces z0-1 | z0+BZ [12][FZ] each;  PY, PX
-enum { OB_UZ = 0, OB_UY, OB_UX, OB_R, OB_R1, OB_R2, OB_R3, OB_ITEM0, OB_ITEM1, OB_GROUP };  // then 5 per group:
+constexpr int kRing = 6;  // ring slots: all groups must be done with a slot before it is refilled, so the ring is
+                          // what couples the groups; six slots for five objects per step let them drift by a step
+enum { OB_UZ = 0, OB_UY, OB_UX, OB_R, OB_ITEM0 = OB_R + kRing, OB_ITEM1, OB_GROUP };  // then 5 per group:
 enum { GB_C = 0, GB_C1, GB_PZ, GB_PY, GB_PX, GB_COUNT };
 
 template <int BZ_, int BY_, int BX_, int SELF_, int G_> struct Plan {
@@ -47,7 +49,7 @@ template <int BZ_, int BY_, int BX_, int SELF_, int G_> struct Plan {
     static constexpr uint32_t OFF_UY = OFF_UZ + SZ_UZ, OFF_UYF = OFF_UY + SZ_U, SZ_UY = SZ_U + 9 * FY * E;
     static constexpr uint32_t OFF_UX = OFF_UY + SZ_UY, OFF_UXF = OFF_UX + SZ_U, SZ_UX = SZ_U + 9 * FX * E;
     static constexpr uint32_t OFF_R = OFF_UX + SZ_UX;
-    static constexpr uint32_t OFF_G = OFF_R + 4 * SZ_U;  // group regions start here
+    static constexpr uint32_t OFF_G = OFF_R + kRing * SZ_U;  // group regions start here
     // offsets inside a group region
     static constexpr uint32_t GO_C = 0;
     static constexpr uint32_t GO_ZLO = GO_C + 2 * SZ_C, GO_ZHI = GO_ZLO + 12 * FZ * E, SZ_PZ = 24 * FZ * E;
@@ -152,11 +154,11 @@ template <class P> struct Producer {
         tma_load_5d_hint(sbase + gbase() + P::GO_C + b * P::SZ_C, &maps.psi_c, bar_full + ob, cx, y0, z0, tt, pc(), pol_p);
         return true;
     }
-    // nine components of U or S into ring slot nR & 3
+    // nine components of U or S into ring slot nR % kRing
     __device__ __forceinline__ bool load_ring(const CUtensorMap *map, uint32_t sbase, uint32_t bar_full, uint32_t bar_empty,
                                               int tt, int comp, uint64_t pol) {
-        const uint32_t b = nR & 3, ob = 8 * (OB_R + b);
-        if (!mbar_try_wait(bar_empty + ob, ((nR >> 2) & 1) ^ 1)) return false;
+        const uint32_t b = nR % kRing, ob = 8 * (OB_R + b);
+        if (!mbar_try_wait(bar_empty + ob, ((nR / kRing) & 1) ^ 1)) return false;
         mbar_arrive_expect_tx(bar_full + ob, P::SZ_U);
         tma_load_5d_hint(sbase + P::OFF_R + b * P::SZ_U, map, bar_full + ob, cx, y0, z0, tt, comp, pol);
         nR++;
@@ -354,9 +356,9 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tmr(const __grid_constant__ 
 
     // one 6x6 block of S (two consecutive ring objects): acc[6b..6b+5] += B_b * (-2 psi)
     auto s_phase = [&](uint32_t cb, int b, bool active) {
-        const uint32_t s0 = nR & 3, s1 = (nR + 1) & 3;
-        wait_full(8 * (OB_R + s0), (nR >> 2) & 1);
-        wait_full(8 * (OB_R + s1), ((nR + 1) >> 2) & 1);
+        const uint32_t s0 = nR % kRing, s1 = (nR + 1) % kRing;
+        wait_full(8 * (OB_R + s0), (nR / kRing) & 1);
+        wait_full(8 * (OB_R + s1), ((nR + 1) / kRing) & 1);
         if (active) {
             cd q[6];
 #pragma unroll
@@ -385,9 +387,9 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tmr(const __grid_constant__ 
         cd *__restrict__ out = prm.out + (long long)(it.rhs0 + (active ? grp : 0)) * 12 * V;
         int t = it.t0;
         {   // prologue: acc = backward-T hop of slice t0, (1 + gamma_T) U_T(t0-1)^H psi(t0-1)
-            const uint32_t cb = (nC & 1) ? P::SZ_C : 0, slot = nR & 3;
+            const uint32_t cb = (nC & 1) ? P::SZ_C : 0, slot = nR % kRing;
             wait_full(gbar + 8 * (GB_C + (nC & 1)), (nC >> 1) & 1);
-            wait_full(8 * (OB_R + slot), (nR >> 2) & 1);
+            wait_full(8 * (OB_R + slot), (nR / kRing) & 1);
             cd p[12], u[9], h[6], g[6];
 #pragma unroll
             for (int k = 0; k < 9; k++) u[k] = lds(smem, P::OFF_R + slot * P::SZ_U + own + k * NS);
@@ -435,9 +437,9 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tmr(const __grid_constant__ 
             release(gbar + 8 * GB_PX);
             nF++;
             {   // T phase: forward hop completes out(t); the backward hop of slice t+1 starts the next accumulator
-                const uint32_t cn = cb ^ P::SZ_C, slot = nR & 3;  // psi(t+1) is in the other C buffer
+                const uint32_t cn = cb ^ P::SZ_C, slot = nR % kRing;  // psi(t+1) is in the other C buffer
                 wait_full(gbar + 8 * (GB_C + ((nC + 1) & 1)), ((nC + 1) >> 1) & 1);
-                wait_full(8 * (OB_R + slot), (nR >> 2) & 1);
+                wait_full(8 * (OB_R + slot), (nR / kRing) & 1);
                 if (active) {
                     cd u[9], p[12];
 #pragma unroll
