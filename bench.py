@@ -278,7 +278,7 @@ def run_ours(args):
     ins[1].mul_(1.0 / 8.0)
     ins[2].mul_(1.0 / 64.0)
     torch.cuda.synchronize()
-    kname = wd.wd_kernel_name(wd.wd_kernel_in_use(h))
+    kname = wd.wd_kernel_name(wd.wd_kernel_for(h, nrhs))
 
     def step(k):
         wd.wd_apply(h, outs[k % 2], ins[k % 3], nrhs)

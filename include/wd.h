@@ -157,6 +157,9 @@ int wd_get_option(const wd_handle *h, int option, long *value);
 int wd_kernel_count(void);
 const char *wd_kernel_name(int id);
 int wd_kernel_in_use(const wd_handle *h);
+/* The kernel wd_apply(h, ..., nrhs) launches (the automatic choice depends on whether there is a clover term and on
+ * whether several right-hand sides are applied in one call); wd_kernel_in_use(h) = wd_kernel_for(h, 1). */
+int wd_kernel_for(const wd_handle *h, int nrhs);
 
 /* Number of kernel launches issued by this handle so far (all kernels of this library). */
 long wd_launch_count(const wd_handle *h);

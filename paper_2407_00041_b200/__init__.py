@@ -46,6 +46,7 @@ SIGNATURES = {
     "wd_kernel_count": (_i, []),
     "wd_kernel_name": (_cp, [_i]),
     "wd_kernel_in_use": (_i, [_vp]),
+    "wd_kernel_for": (_i, [_vp, _i]),
     "wd_launch_count": (_l, [_vp]),
     "wd_last_error": (_cp, [_vp]),
     "wd_version": (_cp, []),
@@ -199,6 +200,10 @@ def wd_kernel_name(kid: int) -> str | None:
 
 def wd_kernel_in_use(h) -> int:
     return lib().wd_kernel_in_use(h)
+
+
+def wd_kernel_for(h, nrhs: int) -> int:
+    return int(lib().wd_kernel_for(h, nrhs))
 
 
 def wd_launch_count(h) -> int:

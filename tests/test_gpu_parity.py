@@ -179,7 +179,11 @@ def test_multi_rhs_equals_repeated_single_rhs(torch):
         out = op.apply(psi, nrhs)
         for r in range(nrhs):
             assert rel_l2(out[r], ref[r]) <= TOL
-            assert np.array_equal(out[r], op.apply(psi[r:r + 1])[0])
+            single = op.apply(psi[r:r + 1])[0]
+            if wd.wd_kernel_for(op.h, nrhs) == wd.wd_kernel_for(op.h, 1):
+                assert np.array_equal(out[r], single)  # same kernel: same arithmetic, bit for bit
+            else:  # the automatic choice differs for several right-hand sides: only the summation order may differ
+                assert rel_l2(out[r], single) <= 1e-14
 
 
 # ---------------------------------------------------------------- packers, host path, options
