@@ -49,7 +49,10 @@ def parse_args():
     ap.add_argument("--zgroup", type=int, default=0)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-ceilings", action="store_true", help="skip the streaming / FP64 ceiling microbenchmarks")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--graph", action="store_true",
+                    help="also time the K steps captured as ONE CUDA graph (cfg 3: 100 back-to-back applies)")
     return ap.parse_args()
 
 
@@ -75,14 +78,20 @@ def peak_hbm():
 
 
 def ncu_traffic(name):
-    """dram bytes per launch of the dominant kernel from the committed ncu capture, or None."""
+    """(dram bytes per launch of the dominant kernel, where that number comes from): a CONSTANT read from the
+    committed ncu capture table profiles/roofline_traffic.json (ncu cannot run inside a timed bench), or (None, None)."""
     p = os.path.join(ROOT, "profiles", "roofline_traffic.json")
     if os.path.exists(p):
         try:
-            return json.load(open(p)).get(name)
+            tab = json.load(open(p))
+            ent = tab.get(name)
+            if isinstance(ent, dict):
+                return ent.get("bytes"), "profiles/roofline_traffic.json: " + ent.get("source", "?")
+            if ent is not None:
+                return ent, "profiles/roofline_traffic.json: " + str(tab.get("_source", "?"))
         except Exception:
-            return None
-    return None
+            pass
+    return None, None
 
 
 class ClockSampler(threading.Thread):
@@ -91,6 +100,7 @@ class ClockSampler(threading.Thread):
     def __init__(self, index):
         super().__init__(daemon=True)
         self.index, self.samples, self.reasons, self.stop_flag, self.max_mhz = index, [], set(), False, None
+        self.power = []
         self.ok = False
         try:
             import pynvml
@@ -118,6 +128,10 @@ class ClockSampler(threading.Thread):
             try:
                 self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
                 try:
+                    self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1e3)
+                except Exception:
+                    pass
+                try:
                     r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
                 except Exception:
                     r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
@@ -132,38 +146,68 @@ class ClockSampler(threading.Thread):
         if not self.samples:
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": 0}
         s = sorted(self.samples)
+        pw = sorted(self.power)
         return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
-                "samples": len(s)}
+                "samples": len(s), "sm_mhz_min": s[0], "power_w": pw[len(pw) // 2] if pw else None,
+                "power_w_max": pw[-1] if pw else None}
 
 
-def cpu_baseline_sample(cfg, max_seconds=25.0):
-    """The oracle, as it stands, on the host cores, on a bounded sample of the workload: the same
-    recipe on a lattice of at most 32^3 x 64 sites (a 1/8 .. 1/16 sub-volume of the 64^4 job), S
-    prebuilt by the oracle (untimed), whole-lattice applies timed for <= ~25 s."""
+def oracle_inputs(cfg):
+    """Host inputs of the oracle timing legs on the bench lattice ITSELF (same dims, same links and spinor recipe).
+    S: the 42-entry field is filled with seeded random Hermitian blocks instead of being built from the links —
+    building it with the oracle costs minutes at 64^4 and the values do not change the cost of an apply."""
+    import wdinputs
+
+    dims = tuple(cfg["dims"])
+    U = wdinputs.config_gauge(cfg, dims)
+    psi = wdinputs.spinor(dims, cfg["spinor_seed"])
+    C = wdinputs.selfcoupling_random(dims, 7) if cfg["csw"] else None
+    return dims, U, C, psi
+
+
+def time_oracle(dims, m0, U, C, psi, reps, threads=None):
+    """Seconds per whole-lattice oracle apply (best of reps), with `threads` OpenMP threads (None: all)."""
+    import oracle
+
+    nall = oracle.num_threads()
+    if threads:
+        oracle.set_num_threads(threads)
+    try:
+        best = 1e30
+        for _ in range(reps):
+            t0 = time.perf_counter()
+            oracle.apply(dims, m0, U, C, psi)
+            best = min(best, time.perf_counter() - t0)
+    finally:
+        oracle.set_num_threads(nall)
+    return best
+
+
+def cpu_baseline_sample(cfg):
+    """The oracle, as it stands, on the host cores, on the bench lattice itself (one right-hand side): best of 2
+    whole-lattice applies on all cores after one warm-up, and one apply on a single thread (skipped above 2^25 sites
+    x RHS to keep the default run within minutes)."""
     import oracle
     import wdinputs
 
-    dims = tuple(min(n, 32) for n in cfg["dims"])
+    dims, U, C, psi = oracle_inputs(cfg)
     V = wdinputs.volume(dims)
-    U = wdinputs.config_gauge(cfg, dims)
-    psi = wdinputs.spinor(dims, cfg["spinor_seed"])
-    C = oracle.build_clover(dims, cfg["m0"], cfg["csw"], U) if cfg["csw"] else None
-    oracle.apply(dims, cfg["m0"], U, C, psi)  # warm
-    n, t0 = 0, time.perf_counter()
-    while True:
-        oracle.apply(dims, cfg["m0"], U, C, psi)
-        n += 1
-        el = time.perf_counter() - t0
-        if el > 10.0 or n >= 20 or el > max_seconds:
-            break
     flop = FLOP_WILSON + (FLOP_CLOVER if cfg["csw"] else 0)
-    sites_per_s = n * V / el
-    return {
-        "value": sites_per_s * flop / 1e9, "unit": "GFLOP/s", "sites_per_s": sites_per_s,
-        "cores": oracle.num_threads(), "kind": "oracle",
-        "sample": f"{n} whole-lattice oracle applies of a {'x'.join(map(str, dims))} lattice "
-                  f"({V} sites, same recipe: m0={cfg['m0']} csw={cfg['csw']}, S prebuilt untimed), {el:.1f} s",
-    }, el / n
+    time_oracle(dims, cfg["m0"], U, C, psi, 1)  # warm
+    t_all = time_oracle(dims, cfg["m0"], U, C, psi, 2)
+    t_one = time_oracle(dims, cfg["m0"], U, C, psi, 1, threads=1) if V <= (1 << 25) else None
+    lat = "x".join(map(str, dims))
+    base = {
+        "value": V / t_all * flop / 1e9, "unit": "GFLOP/s", "sites_per_s": V / t_all,
+        "cores": oracle.num_threads(), "kind": "oracle", "seconds_per_apply": t_all,
+        "sample": f"whole-lattice oracle applies of the bench lattice itself, {lat} ({V} sites, one right-hand side, "
+                  f"m0={cfg['m0']} csw={cfg['csw']}; S = seeded random Hermitian blocks, untimed set-up): best of 2 on "
+                  f"all cores, 1 on one thread",
+    }
+    if t_one:
+        base["single_thread"] = {"value": V / t_one * flop / 1e9, "unit": "GFLOP/s", "sites_per_s": V / t_one,
+                                 "cores": 1, "seconds_per_apply": t_one}
+    return base
 
 
 def run_reference(args):
@@ -174,14 +218,13 @@ def run_reference(args):
     import oracle
     import wdinputs
 
-    dims = tuple(min(n, 32) for n in cfg["dims"])
+    dims, U, C, psi = oracle_inputs(cfg)
     V = wdinputs.volume(dims)
-    U = wdinputs.config_gauge(cfg, dims)
-    psi = wdinputs.spinor(dims, cfg["spinor_seed"])
-    C = oracle.build_clover(dims, cfg["m0"], cfg["csw"], U) if cfg["csw"] else None
-    steps = max(1, min(args.steps, 20))
+    # bounded: every step is one whole-lattice apply of ONE right-hand side of the bench lattice; at most 20 steps
+    per = time_oracle(dims, cfg["m0"], U, C, psi, 1)  # warm-up 1
+    steps = max(1, min(args.steps, 20, int(120.0 / max(per, 1e-3)) or 1))
     warm = max(1, min(args.warmup, 3))
-    for _ in range(warm):
+    for _ in range(warm - 1):
         oracle.apply(dims, cfg["m0"], U, C, psi)
     t0 = time.perf_counter()
     for _ in range(steps):
@@ -189,8 +232,9 @@ def run_reference(args):
     el = time.perf_counter() - t0
     flop = FLOP_WILSON + (FLOP_CLOVER if cfg["csw"] else 0)
     val = steps * V / el * flop / 1e9
-    sample = (f"each step = one whole-lattice oracle apply of a {'x'.join(map(str, dims))} lattice "
-              f"({V} sites; bounded sample of {cfg['name']}), S prebuilt untimed")
+    sample = (f"each step = one whole-lattice oracle apply of ONE right-hand side of the bench lattice itself "
+              f"({'x'.join(map(str, dims))}, {V} sites); S = seeded random Hermitian blocks (values do not change the "
+              f"cost), untimed set-up; steps capped at 20")
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": "GFLOP/s", "n_gpus": args.gpus,
         "steps": steps, "warmup": warm, "ms_per_step": el / steps * 1e3, "higher_is_better": True,
@@ -315,21 +359,17 @@ def run_ours(args):
     avg_launch_ms = (sum(per_step) / len(per_step)) / launches_per_step
     alg_bytes_launch = alg_bytes_step / launches_per_step  # tma_*: one launch per step, all RHS
     achieved = alg_bytes_launch / (avg_launch_ms * 1e-3) / 1e9
+    traffic, traffic_src = (ncu_traffic(kname + ("/clover" if clover else "/wilson") + ("" if nrhs == 1 else f"/x{nrhs}")
+                                        + "@" + "x".join(map(str, dims))))
     roofline = {
         "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-        "traffic": (ncu_traffic(kname + ("/clover" if clover else "/wilson"))
-                    if tuple(dims) == (64, 64, 64, 64) and nrhs == 1 else None),  # captured for that workload only
-        "peak_source": peak_src,
+        "traffic": traffic, "traffic_source": traffic_src,  # a constant from the committed ncu capture of this
+        "peak_source": peak_src,                            # kernel on this workload — not measured in this run
         "kernel": kname + ("/fused" if args.variant == 0 else "/unfused"),
         "algorithmic_bytes_per_launch": alg_bytes_launch, "avg_launch_ms": avg_launch_ms,
         "best_launch_ms": min(per_step) / launches_per_step,
         "frac_of_8000_spec": achieved / 8000.0,
     }
-
-    # second roof: FP64 FMA peak measured on this GPU with a register-only microbenchmark
-    fp64_peak, _ = wd.wd_measure_fp64(1024, 8, False)
-    roofline["fp64_peak_tflops_measured"] = fp64_peak
-    roofline["frac_of_fp64_peak"] = (value / 1e3) / fp64_peak
 
     line = {
         "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
@@ -339,7 +379,8 @@ def run_ours(args):
         "config": {"workload": cfg["name"], "lattice": list(dims), "m0": cfg["m0"], "csw": cfg["csw"],
                    "nrhs": nrhs, "kernel": kname, "variant": "fused" if args.variant == 0 else "unfused",
                    "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "l2": "inputs larger than L2 (25.8 GB touched per step at 64^4); 3 inputs / 2 outputs rotate"},
+                   "l2": f"inputs larger than L2 ({alg_bytes_step / 1e9:.2f} GB touched per step); "
+                         "3 inputs / 2 outputs rotate"},
         "roofline": roofline, "gpu_launches": launches, "clocks": sampler.summary(),
     }
 
@@ -362,12 +403,59 @@ def run_ours(args):
                        "ms_per_step": ms, "steps": args.e2e_steps,
                        "api": "wd_apply_host (pinned host buffers, canonical layout)"}
         del hin, hout
+    # ---- the K steps as ONE CUDA graph (cfg 3: "100 back-to-back applies ... also as one CUDA graph")
+    if args.graph and rank == 0:
+        gs = torch.cuda.Stream()
+        wd.wd_set_stream(h, gs.cuda_stream)
+        with torch.cuda.stream(gs):
+            for k in range(3):
+                step(k)
+            gs.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=gs):
+                for k in range(args.steps):
+                    step(k)
+            graph.replay()
+            gs.synchronize()
+            g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            g0.record(gs)
+            graph.replay()
+            g1.record(gs)
+            gs.synchronize()
+        gms = g0.elapsed_time(g1) / args.steps
+        line["graph"] = {"ms_per_step": gms, "steps_in_graph": args.steps,
+                         "value": V * nrhs * flop / (gms * 1e-3) / 1e9, "unit": "GFLOP/s"}
+        wd.wd_set_stream(h, stream.cuda_stream)
+        del graph
     wd.wd_destroy(h)
     del ins, outs
     torch.cuda.empty_cache()
 
+    # ---- ceilings measured on this GPU in this run (bench-only library, include/wd_bench.h): streaming read-only /
+    # copy / 7 reads per write (the operator's mix), and the FP64 FMA roof that co-limits a multi-RHS application
+    if rank == 0 and not args.no_ceilings:
+        from paper_2407_00041_b200 import benchlib
+
+        try:
+            nb = 8 << 30
+            roofline["stream_read_only_gbs"] = benchlib.wdb_measure_stream(0, nb, 5)
+            roofline["stream_copy_gbs"] = benchlib.wdb_measure_stream(1, nb // 2, 5)
+            roofline["stream_7r1w_gbs"] = benchlib.wdb_measure_stream(2, nb, 5)
+            roofline["frac_of_stream_7r1w"] = achieved / roofline["stream_7r1w_gbs"]
+            fs = ClockSampler(local)
+            fs.start()
+            fp64 = max(benchlib.wdb_measure_fp64(1024, 8, False)[0] for _ in range(5))
+            fs.stop_flag = True
+            fs.join()
+            roofline["fp64_peak_tflops_measured"] = fp64
+            roofline["fp64_peak_clocks"] = fs.summary()
+            roofline["fp64_peak_how"] = "best of 5, 1024 threads x 8 chains per SM, register-only DFMA"
+            roofline["frac_of_fp64_peak"] = (value / 1e3) / fp64
+        except Exception as exc:  # the ceilings are context, never the reason a bench line is lost
+            roofline["ceilings_error"] = repr(exc)
+
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        line["cpu_baseline"], _ = cpu_baseline_sample(cfg)
+        line["cpu_baseline"] = cpu_baseline_sample(cfg)
     if dist:
         dist.barrier()
         dist.destroy_process_group()

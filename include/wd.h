@@ -25,8 +25,9 @@
  *                   conjugates (R6).
  *
  * DEVICE LAYOUT: chosen by the library, opaque to the caller.
- * A device spinor buffer holds wd_spinor_bytes(h, nrhs) bytes, is 256-byte aligned, and is
- * filled / read with wd_pack_spinor / wd_unpack_spinor (or wd_apply_host).  Fields stay
+ * A device spinor buffer holds wd_spinor_bytes(h, nrhs) bytes, is at least 16-byte aligned (checked;
+ * cudaMalloc and PyTorch give 256 bytes or more), and is filled / read with wd_pack_spinor /
+ * wd_unpack_spinor (or wd_apply_host).  Fields stay
  * device-resident in device layout between applications: wd_apply never repacks (the lesson of
  * PAPER.md:1015, where per-application reordering ate the gain).
  *
@@ -36,6 +37,9 @@
  *
  * THREADING: a handle is used by one host thread at a time.  All device work of a handle is
  * issued on the handle's stream (default: the legacy default stream; see wd_set_stream).
+ *
+ * DEVICE: a handle belongs to the CUDA device that was current in wd_create.  Every entry point
+ * switches to that device for the duration of the call and restores the caller's current device.
  */
 #ifndef WD_H
 #define WD_H
@@ -62,7 +66,9 @@ enum {
     WD_OPT_KERNEL = 2,    /* hopping/fused kernel geometry id; -1 = automatic (default); see wd_kernel_name        */
     WD_OPT_TCHUNK = 3,    /* T-extent marched by one CTA in tiled geometries; 0 = automatic                       */
     WD_OPT_ZGROUP = 4,    /* number of Z-tiles per rasterisation group in tiled geometries; 0 = automatic         */
-    WD_OPT_DEVICE_PACK = 5/* 1 = wd_load_* / wd_pack_* transpose on the device instead of on the host (default 0) */
+    WD_OPT_DEVICE_PACK = 5,/* 1 = wd_load_* / wd_pack_* transpose on the device instead of on the host (default 0) */
+    WD_OPT_HOST_PIPELINE = 6,/* wd_apply_host: 1 = overlap upload, compute and download over T chunks (default), 0 = serial */
+    WD_OPT_GMRES_GRAPH = 7 /* wd_gmres: 1 = replay restart cycles as one CUDA graph (default; needs a non-default stream), 0 = launch by launch */
 };
 
 /* Create an operator for a T x Z x Y x X periodic lattice.  Every extent >= 1 (n = 2, where
@@ -77,7 +83,10 @@ int wd_destroy(wd_handle *h);
 
 /* HOST pointer, canonical gauge layout.  Packed into the device layout and copied; the caller
  * keeps ownership.  Links are treated as general 3x3 complex matrices (U and U^H are used,
- * never U^-1; R11).  Synchronous w.r.t. the host array. */
+ * never U^-1; R11).  Synchronous w.r.t. the host array.
+ * A self-coupling field that wd_build_clover derived from the PREVIOUS links is discarded: with
+ * csw != 0 the next wd_apply returns WD_ESTATE until wd_build_clover or wd_load_clover is called
+ * again.  A field supplied with wd_load_clover is the caller's and is kept. */
 int wd_load_gauge(wd_handle *h, const double *host_U);
 
 /* HOST pointer, canonical self-coupling layout (the whole S(x), eq. 2.5).  Required iff csw != 0
@@ -93,10 +102,31 @@ int wd_build_clover(wd_handle *h);
 int wd_get_clover(wd_handle *h, double *host_C);
 
 /* out = D in for nrhs right-hand sides (eq. 1.13).  DEVICE pointers in DEVICE layout, each
- * wd_spinor_bytes(h, nrhs) bytes, 256-byte aligned; out must not overlap in.  Asynchronous:
+ * wd_spinor_bytes(h, nrhs) bytes, 16-byte aligned; out must not overlap in.  Asynchronous:
  * enqueued on the handle's stream, no host synchronisation, no host<->device copies, no
  * repacking.  Errors: WD_EINVAL, WD_ESTATE (no gauge; csw != 0 and no self-coupling), WD_ECUDA. */
 int wd_apply(wd_handle *h, void *dev_out, const void *dev_in, int nrhs);
+
+/* Restarted GMRES(m) with right preconditioning M = I for D x = b (Algorithm 1 of the paper, PAPER.md:240-289;
+ * modified Gram-Schmidt, h_ij = v_i^H w, R16), entirely on the device: the operator is wd_apply, the
+ * orthogonalisation, norms, the (m+1) x m least-squares problem and the solution update are kernels of this library
+ * that keep every scalar in device memory.  dev_x: DEVICE spinor (device layout, one right-hand side), the initial
+ * guess x_0 on entry and the approximate solution on return; dev_b: DEVICE spinor, not modified; 1 <= m <= 64.
+ * Termination (R17): ||b - D x|| < tol * ||b - D x_0||, tested on the true residual at the top
+ * of every restart cycle, or max_cycles cycles done; inside a cycle |h_{j+1,j}| < tol / 10 ends the Arnoldi loop
+ * (R18).  *cycles_done (may be NULL) = cycles performed; host_resid (HOST, may be NULL, max_cycles + 1
+ * doubles): host_resid[k] = ||b - D x|| after k cycles.  The library owns (m + 2) work spinors, kept for the next
+ * call.  Synchronises the handle's stream once per cycle (to read the residual norm); with a non-default stream the
+ * second and later cycles are one CUDA graph launch each (WD_OPT_GMRES_GRAPH).
+ * Errors: WD_EINVAL, WD_ESTATE (no gauge / no self-coupling field), WD_ENOMEM, WD_ECUDA. */
+int wd_gmres(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_cycles, double tol, int *cycles_done,
+             double *host_resid);
+
+/* The Hessenberg matrix of the LAST restart cycle of the last wd_gmres call as the Arnoldi process produced it:
+ * host_H (HOST, may be NULL): (m+1) * m complex numbers, column-major with leading dimension m + 1
+ * (host_H[2 * (i + (m+1) * j)] = Re h_{i+1,j+1}); *kdim (may be NULL) = Krylov dimension of that cycle (m unless the
+ * breakdown rule ended it); *lsq_resid (may be NULL) = min_y ||beta e_1 - H y||, the recurrence residual. */
+int wd_gmres_last_hessenberg(wd_handle *h, double *host_H, int *kdim, double *lsq_resid);
 
 /* Same operation on HOST arrays in canonical spinor layout: host->device copy, on-device
  * repack, operator, repack, device->host copy, all inside the call; returns after the result is
@@ -133,17 +163,9 @@ size_t wd_layout_bytes(int field, long long nsites);
 int wd_layout_pack_host(int field, long long nsites, const double *canonical, double *packed);
 int wd_layout_unpack_host(int field, long long nsites, const double *packed, double *canonical);
 
-/* Register-only FP64 FMA microbenchmark (the paper's section 3.1 method): the FP64 roof that
- * co-limits a multi-RHS application.  Launches threads_per_sm-thread CTAs (a multiple of 32, <= 1024) filling
- * every SM (one_cta_per_sm = 0) or exactly one per SM (1), each thread running `ilp` (1, 2, 4, 8, 16) independent
- * FMA chains; distinct_operands = 0: a = fma(a, b, c) with b, c common to all chains, 1: every operand of every
- * chain a register pair of its own.  *tflops = achieved 2*FMA/s; *cycles_per_fma_per_warp (may be NULL) = cycles of the nominal
- * maximum SM clock between two FMAs issued on one SM sub-partition.  Synchronous, default stream. */
-int wd_measure_fp64(int threads_per_sm, int ilp, int one_cta_per_sm, int distinct_operands, double *tflops,
-                    double *cycles_per_fma_per_warp);
-
 /* cudaStream_t passed as void* (NULL = legacy default stream).  PyTorch supplies memory and
- * streams only. */
+ * streams only.  Waits for the work already enqueued on the previous stream (the handle's work
+ * queue and staging buffers are shared by all its launches). */
 int wd_set_stream(wd_handle *h, void *cuda_stream);
 
 /* Block the host until all work enqueued on the handle's stream has finished. */

@@ -17,7 +17,8 @@ LIB_PATH = os.path.join(_HERE, "libwd.so")
 
 WD_OK, WD_EINVAL, WD_ENOMEM, WD_ESTATE, WD_ECUDA = 0, -1, -2, -3, -4
 WD_FIELD_SPINOR, WD_FIELD_GAUGE, WD_FIELD_CLOVER = 0, 1, 2
-WD_OPT_VARIANT, WD_OPT_KERNEL, WD_OPT_TCHUNK, WD_OPT_ZGROUP, WD_OPT_DEVICE_PACK = 1, 2, 3, 4, 5
+WD_OPT_VARIANT, WD_OPT_KERNEL, WD_OPT_TCHUNK, WD_OPT_ZGROUP, WD_OPT_DEVICE_PACK, WD_OPT_HOST_PIPELINE = 1, 2, 3, 4, 5, 6
+WD_OPT_GMRES_GRAPH = 7
 
 # name -> (restype, argtypes); mirrors include/wd.h declaration by declaration
 _vp, _i, _d, _l, _sz, _cp = (ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_long,
@@ -31,6 +32,8 @@ SIGNATURES = {
     "wd_get_clover": (_i, [_vp, _vp]),
     "wd_apply": (_i, [_vp, _vp, _vp, _i]),
     "wd_apply_host": (_i, [_vp, _vp, _vp, _i]),
+    "wd_gmres": (_i, [_vp, _vp, _vp, _i, _i, _d, ctypes.POINTER(_i), _vp]),
+    "wd_gmres_last_hessenberg": (_i, [_vp, _vp, ctypes.POINTER(_i), ctypes.POINTER(_d)]),
     "wd_spinor_bytes": (_sz, [_vp, _i]),
     "wd_component_stride": (ctypes.c_longlong, [_vp]),
     "wd_pack_spinor": (_i, [_vp, _vp, _vp, _i]),
@@ -38,7 +41,6 @@ SIGNATURES = {
     "wd_layout_bytes": (_sz, [_i, ctypes.c_longlong]),
     "wd_layout_pack_host": (_i, [_i, ctypes.c_longlong, _vp, _vp]),
     "wd_layout_unpack_host": (_i, [_i, ctypes.c_longlong, _vp, _vp]),
-    "wd_measure_fp64": (_i, [_i, _i, _i, _i, ctypes.POINTER(_d), ctypes.POINTER(_d)]),
     "wd_set_stream": (_i, [_vp, _vp]),
     "wd_synchronize": (_i, [_vp]),
     "wd_set_option": (_i, [_vp, _i, _l]),
@@ -129,6 +131,20 @@ def wd_apply_host(h, host_out, host_in, nrhs: int = 1) -> None:
     _check(h, lib().wd_apply_host(h, _ptr(host_out), _ptr(host_in), nrhs))
 
 
+def wd_gmres(h, dev_x, dev_b, m: int, max_cycles: int, tol: float, host_resid=None) -> int:
+    """Returns the number of restart cycles done; host_resid: float64 array of max_cycles + 1 entries, or None."""
+    n = _i(0)
+    _check(h, lib().wd_gmres(h, _ptr(dev_x), _ptr(dev_b), m, max_cycles, tol, ctypes.byref(n), _ptr(host_resid)))
+    return n.value
+
+
+def wd_gmres_last_hessenberg(h, host_H=None) -> tuple[int, float]:
+    """(Krylov dimension, recurrence residual) of the last cycle; host_H: float64 array [(m+1)*m*2] or None."""
+    kd, lr = _i(0), _d(0.0)
+    _check(h, lib().wd_gmres_last_hessenberg(h, _ptr(host_H), ctypes.byref(kd), ctypes.byref(lr)))
+    return kd.value, lr.value
+
+
 def wd_spinor_bytes(h, nrhs: int = 1) -> int:
     return int(lib().wd_spinor_bytes(h, nrhs))
 
@@ -159,16 +175,6 @@ def wd_layout_unpack_host(field: int, nsites: int, packed, canonical) -> None:
     rc = lib().wd_layout_unpack_host(field, nsites, _ptr(packed), _ptr(canonical))
     if rc != WD_OK:
         raise WDError(rc, "wd_layout_unpack_host: bad argument")
-
-
-def wd_measure_fp64(threads_per_sm: int, ilp: int, one_cta_per_sm: bool = False,
-                    distinct_operands: bool = False) -> tuple[float, float]:
-    tf, cyc = _d(0.0), _d(0.0)
-    rc = lib().wd_measure_fp64(threads_per_sm, ilp, 1 if one_cta_per_sm else 0, 1 if distinct_operands else 0,
-                               ctypes.byref(tf), ctypes.byref(cyc))
-    if rc != WD_OK:
-        raise WDError(rc, "wd_measure_fp64")
-    return tf.value, cyc.value
 
 
 def wd_set_stream(h, cuda_stream) -> None:

@@ -13,8 +13,11 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJDIR = os.path.join(HERE, "build")
 SO = os.path.join(HERE, "libwd.so")
-SOURCES = ["wd_api.cu", "wd_kernels.cu", "wd_tma.cu", "wd_tmb.cu", "wd_tmr.cu", "wd_pack.cu", "wd_clover.cu", "wd_peaks.cu"]
-HEADERS = ["wd_internal.h", "wd_math.cuh", "wd_tma.cuh", "wd_smem_ops.cuh", os.path.join("..", "..", "include", "wd.h")]
+BENCH_SO = os.path.join(HERE, "libwdbench.so")  # measurement helpers of bench.py (include/wd_bench.h), not the product
+SOURCES = ["wd_api.cu", "wd_kernels.cu", "wd_tma.cu", "wd_tmb.cu", "wd_tmc.cu", "wd_pack.cu", "wd_clover.cu", "wd_gmres.cu"]
+BENCH_SOURCES = [os.path.join("bench", "wd_peaks.cu")]
+HEADERS = ["wd_internal.h", "wd_handle.h", "wd_math.cuh", "wd_tma.cuh", "wd_tma_common.cuh", "wd_smem_ops.cuh",
+           os.path.join("..", "..", "include", "wd.h"), os.path.join("..", "..", "include", "wd_bench.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC,-fopenmp,-O2", "--expt-relaxed-constexpr"]
@@ -26,11 +29,15 @@ def _newest(paths):
 
 def build(force: bool = False, verbose: bool = False) -> str:
     srcs = [os.path.join(CSRC, s) for s in SOURCES]
-    deps = srcs + [os.path.normpath(os.path.join(CSRC, h)) for h in HEADERS]
-    if not force and os.path.exists(SO) and os.path.getmtime(SO) >= _newest(deps):
+    bsrcs = [os.path.join(CSRC, s) for s in BENCH_SOURCES]
+    deps = srcs + bsrcs + [os.path.normpath(os.path.join(CSRC, h)) for h in HEADERS]
+    if (not force and os.path.exists(SO) and os.path.exists(BENCH_SO)
+            and min(os.path.getmtime(SO), os.path.getmtime(BENCH_SO)) >= _newest(deps)):
         return SO
     os.makedirs(OBJDIR, exist_ok=True)
     extra = ["-Xptxas", "-v"] if verbose else []
+    if os.environ.get("WD_EXPERIMENTS"):  # tracing / policy knobs of the TMA kernels (never in the default build)
+        extra += ["-DWD_EXPERIMENTS"]
 
     def compile_one(src):
         obj = os.path.join(OBJDIR, os.path.basename(src) + ".o")
@@ -42,12 +49,14 @@ def build(force: bool = False, verbose: bool = False) -> str:
             sys.stderr.write(r.stderr)
         return obj
 
-    with concurrent.futures.ThreadPoolExecutor(max_workers=len(srcs)) as ex:
-        objs = list(ex.map(compile_one, srcs))
-    cmd = [NVCC, "-shared", "-o", SO, *objs, "-Xcompiler", "-fopenmp", "-lgomp", "-cudart", "static"]
-    r = subprocess.run(cmd, capture_output=True, text=True)
-    if r.returncode != 0:
-        raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
+    with concurrent.futures.ThreadPoolExecutor(max_workers=len(srcs) + len(bsrcs)) as ex:
+        allobjs = list(ex.map(compile_one, srcs + bsrcs))
+    objs, bobjs = allobjs[:len(srcs)], allobjs[len(srcs):]
+    for so, oo in ((SO, objs), (BENCH_SO, bobjs)):
+        cmd = [NVCC, "-shared", "-o", so, *oo, "-Xcompiler", "-fopenmp", "-lgomp", "-cudart", "static"]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode != 0:
+            raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
     return SO
 
 

@@ -1,9 +1,13 @@
-// wd_peaks.cu — register-only FP64 FMA microbenchmark (the paper's section 3.1 method): the
+// wd_peaks.cu (libwdbench.so, bench-only) — streaming ceilings of the device memory, and a register-only FP64 FMA microbenchmark (the paper's section 3.1 method): the
 // second roof of the multi-RHS application (cfg 5) and the issue rate one warp per SM
 // sub-partition can reach, which is what the TMA kernels' compute side runs on.
 #include <cuda_runtime.h>
 
-#include "../../include/wd.h"
+#include <stddef.h>
+
+#include "../../../include/wd_bench.h"
+
+enum { WD_OK = 0, WD_EINVAL = -1, WD_ENOMEM = -2, WD_ECUDA = -4 };
 
 namespace {
 
@@ -49,7 +53,7 @@ template <int ILP, bool D> cudaError_t run(int grid, int threads, size_t smem, i
 
 }  // namespace
 
-extern "C" int wd_measure_fp64(int threads_per_sm, int ilp, int one_cta_per_sm, int distinct_operands, double *tflops,
+extern "C" int wdb_measure_fp64(int threads_per_sm, int ilp, int one_cta_per_sm, int distinct_operands, double *tflops,
                                double *cycles_per_fma_per_warp) {
     if (!tflops || threads_per_sm < 32 || threads_per_sm > 1024 || threads_per_sm % 32) return WD_EINVAL;
     int dev = 0, nsm = 0, khz = 0;
@@ -82,5 +86,81 @@ extern "C" int wd_measure_fp64(int threads_per_sm, int ilp, int one_cta_per_sm, 
         const double warp_fmas_per_sm = (double)iters * ilp * warps_per_sm;
         *cycles_per_fma_per_warp = (ms * 1e-3) * (khz * 1e3) / warp_fmas_per_sm * (warps_per_sm < 4 ? warps_per_sm : 4.0);
     }
+    return WD_OK;
+}
+
+// ---------------------------------------------------------------- streaming ceilings
+namespace {
+// MODE 0: read only.  1: copy.  2: seven 16-byte reads per 16-byte write (the operator's mix).
+template <int MODE> __global__ void __launch_bounds__(256) k_stream(const double2 *__restrict__ src, double2 *__restrict__ dst, size_t n,
+                                                                     double *sink) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    double s = 0.0;
+    if (MODE == 0) {
+        size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+        for (; i + 3 * stride < n; i += 4 * stride) {  // four independent 16-byte loads in flight per thread
+            const double2 a = __ldcs(src + i), b = __ldcs(src + i + stride), c = __ldcs(src + i + 2 * stride),
+                          d = __ldcs(src + i + 3 * stride);
+            s += a.x + b.y + c.x + d.y;
+        }
+        for (; i < n; i += stride) s += __ldcs(src + i).x;
+    } else if (MODE == 1) {
+        for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) __stcs(dst + i, __ldcs(src + i));
+    } else {
+        const size_t m = n / 7;  // 7 source planes of m elements, one destination plane
+        for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < m; i += stride) {
+            double2 v = __ldcs(src + i);
+#pragma unroll
+            for (int k = 1; k < 7; k++) {
+                const double2 w = __ldcs(src + (size_t)k * m + i);
+                v.x += w.x;
+                v.y += w.y;
+            }
+            __stcs(dst + i, v);
+        }
+    }
+    if (s == 123.456) *sink = s;  // never true
+}
+}  // namespace
+
+extern "C" int wdb_measure_stream(int mode, size_t bytes, int reps, double *gbs) {
+    if (!gbs || mode < 0 || mode > 2 || bytes < (1u << 20) || reps < 1) return WD_EINVAL;
+    int dev = 0, nsm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return WD_ECUDA;
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    const size_t n = bytes / sizeof(double2);
+    double2 *src = nullptr, *dst = nullptr;
+    double *sink = nullptr;
+    const size_t dst_n = (mode == 1) ? n : (mode == 2) ? n / 7 : 1;
+    if (cudaMalloc((void **)&src, n * sizeof(double2)) != cudaSuccess) return WD_ENOMEM;
+    if (cudaMalloc((void **)&dst, dst_n * sizeof(double2)) != cudaSuccess) { cudaFree(src); return WD_ENOMEM; }
+    cudaMalloc((void **)&sink, sizeof(double));
+    cudaMemset(src, 0, n * sizeof(double2));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    const int grid = nsm * 8;
+    float best = 1e30f;
+    cudaError_t e = cudaSuccess;
+    for (int r = 0; r < reps + 1 && e == cudaSuccess; r++) {  // first repetition = warm-up
+        cudaEventRecord(e0);
+        if (mode == 0) k_stream<0><<<grid, 256>>>(src, dst, n, sink);
+        else if (mode == 1) k_stream<1><<<grid, 256>>>(src, dst, n, sink);
+        else k_stream<2><<<grid, 256>>>(src, dst, n, sink);
+        cudaEventRecord(e1);
+        e = cudaEventSynchronize(e1);
+        if (e == cudaSuccess) e = cudaGetLastError();
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (r > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(src);
+    cudaFree(dst);
+    cudaFree(sink);
+    if (e != cudaSuccess) return WD_ECUDA;
+    const double moved = (mode == 0) ? (double)n * 16 : (mode == 1) ? 2.0 * n * 16 : (double)(n / 7) * 8 * 16;
+    *gbs = moved / (best * 1e-3) / 1e9;
     return WD_OK;
 }

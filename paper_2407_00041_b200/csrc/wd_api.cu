@@ -7,66 +7,31 @@
 #include <new>
 #include <string>
 
-#include "../../include/wd.h"
-#include "wd_internal.h"
+#include "wd_handle.h"
 
 using namespace wd;
-
-static const int kMaxPipeChunks = 16;  // T chunks of the pipelined wd_apply_host
-
-struct wd_handle {
-    int n[4];
-    long long V, Vs;  // sites; component stride of the device layout (elements)
-    double m0, csw;
-    int device;
-    cudaStream_t stream;
-    double2 *dU, *dS;
-    unsigned int *dsched;  // work-queue words of the TMA kernels
-    bool has_gauge, has_clover;
-    // options
-    long variant, kernel_opt, tchunk_opt, zgroup_opt, device_pack;
-    // staging
-    double2 *pinned[2];
-    size_t pinned_bytes;
-    cudaEvent_t pinned_ev[2];
-    double2 *dstage;
-    size_t dstage_bytes;
-    double2 *work_in, *work_out;  // wd_apply_host
-    double2 *dstage_out;          // pipelined wd_apply_host: AoS staging of the result
-    cudaStream_t s_up, s_dn;      // its upload and download streams
-    cudaEvent_t ev_up[kMaxPipeChunks], ev_cmp[kMaxPipeChunks], ev_misc[2];
-    bool pipe_ready;
-    long launches;
-    std::string err;
-};
 
 static thread_local std::string g_create_err = "";
 
 // Component stride of the device SoA layout.  V rounded up to 16 sites (256 B, keeps every component
 // 256-byte aligned for TMA / 128-bit access) plus 17 * 16 sites, so that consecutive components differ
-// in the low address bits that select the L2 slice and set.  WD_PAD_SITES overrides the padding
-// (experiments only; any multiple of 16 >= 0).
+// in the low address bits that select the L2 slice and set (measured: no effect on B200; kept
+// because it is free).  With -DWD_EXPERIMENTS, WD_PAD_SITES overrides the padding (any multiple of 16 >= 0).
 long long wd::component_stride(long long V) {
     long long pad = 16 * 17;
+#ifdef WD_EXPERIMENTS
     if (const char *e = getenv("WD_PAD_SITES")) {
         const long long v = atoll(e);
         if (v >= 0 && v % 16 == 0) pad = v;
     }
+#endif
     return (V + 15) / 16 * 16 + pad;
 }
 
-static int fail(wd_handle *h, int code, const std::string &msg) {
+int wd::fail(wd_handle *h, int code, const std::string &msg) {
     if (h) h->err = msg; else g_create_err = msg;
     return code;
 }
-
-#define WD_CUDA(h, call)                                                                          \
-    do {                                                                                          \
-        cudaError_t e_ = (call);                                                                  \
-        if (e_ != cudaSuccess)                                                                    \
-            return fail(h, (e_ == cudaErrorMemoryAllocation) ? WD_ENOMEM : WD_ECUDA,              \
-                        std::string(#call) + ": " + cudaGetErrorString(e_));                     \
-    } while (0)
 
 static const size_t kStageSites = 1 << 16;  // sites per host staging chunk
 
@@ -109,7 +74,8 @@ int wd_create(wd_handle **out, int T, int Z, int Y, int X, double m0, double csw
     *out = nullptr;
     if (T < 1 || Z < 1 || Y < 1 || X < 1) return fail(nullptr, WD_EINVAL, "wd_create: every lattice extent must be >= 1");
     const long long V = (long long)T * Z * Y * X;
-    if (V > (1LL << 31) / 42) return fail(nullptr, WD_EINVAL, "wd_create: lattice too large for 32-bit element indexing");
+    // site indices are 64-bit everywhere; a T slice (the stride of T) must fit an int, the whole field the device
+    if ((long long)Z * Y * X >= (1LL << 31) || V >= (1LL << 40)) return fail(nullptr, WD_EINVAL, "wd_create: lattice too large");
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return fail(nullptr, WD_ECUDA, std::string("wd_create: no CUDA device: ") + cudaGetErrorString(e));
@@ -124,7 +90,13 @@ int wd_create(wd_handle **out, int T, int Z, int Y, int X, double m0, double csw
     h->stream = nullptr;
     h->dU = h->dS = nullptr;
     h->dsched = nullptr;
-    h->has_gauge = h->has_clover = false;
+    h->sched_dirty = false;
+    h->has_gauge = h->has_clover = h->clover_built = false;
+    h->nsm = 148;
+    if (cudaDeviceGetAttribute(&h->nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || h->nsm < 1) h->nsm = 148;
+    h->maps = map_cache_new();
+    h->host_pipeline = 1;
+    h->gmres_graph = 1;
     h->variant = 0;
     h->kernel_opt = -1;
     h->tchunk_opt = 0;
@@ -140,6 +112,8 @@ int wd_create(wd_handle **out, int T, int Z, int Y, int X, double m0, double csw
     h->s_up = h->s_dn = nullptr;
     h->pipe_ready = false;
     h->launches = 0;
+    h->gmres = nullptr;
+    h->dd = nullptr;
     e = cudaMalloc((void **)&h->dU, (size_t)h->Vs * kGaugeComps * sizeof(double2));
     if (e == cudaSuccess) e = cudaMalloc((void **)&h->dsched, 2 * sizeof(unsigned int));
     if (e == cudaSuccess) e = cudaMemset(h->dsched, 0, 2 * sizeof(unsigned int));
@@ -157,8 +131,11 @@ int wd_create(wd_handle **out, int T, int Z, int Y, int X, double m0, double csw
 }
 
 int wd_destroy(wd_handle *h) {
-    if (!h) return WD_EINVAL;
+    WD_ENTER(h);
     cudaStreamSynchronize(h->stream);
+    gmres_free(h);
+    dd_free(h);
+    map_cache_delete(h->maps);
     if (h->dU) cudaFree(h->dU);
     if (h->dS) cudaFree(h->dS);
     if (h->dsched) cudaFree(h->dsched);
@@ -185,13 +162,16 @@ int wd_destroy(wd_handle *h) {
 }
 
 int wd_set_stream(wd_handle *h, void *cuda_stream) {
-    if (!h) return WD_EINVAL;
+    WD_ENTER(h);
+    if ((cudaStream_t)cuda_stream == h->stream) return WD_OK;
+    // work pending on the old stream still uses the handle's work queue and staging: let it finish first
+    WD_CUDA(h, cudaStreamSynchronize(h->stream));
     h->stream = (cudaStream_t)cuda_stream;
     return WD_OK;
 }
 
 int wd_synchronize(wd_handle *h) {
-    if (!h) return WD_EINVAL;
+    WD_ENTER(h);
     WD_CUDA(h, cudaStreamSynchronize(h->stream));
     return WD_OK;
 }
@@ -248,8 +228,12 @@ static int store_chunked(wd_handle *h, double2 *host, const double2 *dev, int nc
 }
 
 int wd_load_gauge(wd_handle *h, const double *host_U) {
-    if (!h) return WD_EINVAL;
+    WD_ENTER(h);
     if (!host_U) return fail(h, WD_EINVAL, "wd_load_gauge: null pointer");
+    if (h->clover_built) {  // S was built from the links that are being replaced: it must be rebuilt (or loaded)
+        h->has_clover = h->clover_built = false;
+    }
+    h->has_gauge = false;
     const size_t bytes = (size_t)h->V * kGaugeComps * sizeof(double2);
     if (h->device_pack) {
         int rc = ensure_dstage(h, bytes);
@@ -273,7 +257,7 @@ static int ensure_clover_storage(wd_handle *h) {
 }
 
 int wd_load_clover(wd_handle *h, const double *host_C) {
-    if (!h) return WD_EINVAL;
+    WD_ENTER(h);
     if (!host_C) return fail(h, WD_EINVAL, "wd_load_clover: null pointer");
     int rc = ensure_clover_storage(h);
     if (rc) return rc;
@@ -291,22 +275,24 @@ int wd_load_clover(wd_handle *h, const double *host_C) {
         if (rc) return rc;
     }
     h->has_clover = true;
+    h->clover_built = false;
     return WD_OK;
 }
 
 int wd_build_clover(wd_handle *h) {
-    if (!h) return WD_EINVAL;
+    WD_ENTER(h);
     if (!h->has_gauge) return fail(h, WD_ESTATE, "wd_build_clover: no gauge field loaded");
     int rc = ensure_clover_storage(h);
     if (rc) return rc;
     WD_CUDA(h, launch_build_clover(h->dS, h->dU, h->n, h->V, h->Vs, h->m0 + 4.0, h->csw, h->stream));
     h->launches++;
     h->has_clover = true;
+    h->clover_built = true;
     return WD_OK;
 }
 
 int wd_get_clover(wd_handle *h, double *host_C) {
-    if (!h) return WD_EINVAL;
+    WD_ENTER(h);
     if (!host_C) return fail(h, WD_EINVAL, "wd_get_clover: null pointer");
     if (!h->has_clover) return fail(h, WD_ESTATE, "wd_get_clover: no self-coupling field present");
     return store_chunked(h, (double2 *)host_C, h->dS, kCloverSlots, host_unpack_clover);
@@ -323,7 +309,7 @@ long long wd_component_stride(const wd_handle *h) { return h ? h->Vs : 0; }
 static bool misaligned(const void *p) { return ((size_t)p & 15) != 0; }
 
 int wd_pack_spinor(wd_handle *h, void *dev_dst, const double *host_src, int nrhs) {
-    if (!h) return WD_EINVAL;
+    WD_ENTER(h);
     if (!dev_dst || !host_src || nrhs < 1 || misaligned(dev_dst)) return fail(h, WD_EINVAL, "wd_pack_spinor: bad argument");
     const size_t per = (size_t)h->V * kSpinorComps, dper = (size_t)h->Vs * kSpinorComps;
     for (int r = 0; r < nrhs; r++) {
@@ -345,7 +331,7 @@ int wd_pack_spinor(wd_handle *h, void *dev_dst, const double *host_src, int nrhs
 }
 
 int wd_unpack_spinor(wd_handle *h, double *host_dst, const void *dev_src, int nrhs) {
-    if (!h) return WD_EINVAL;
+    WD_ENTER(h);
     if (!host_dst || !dev_src || nrhs < 1 || misaligned(dev_src)) return fail(h, WD_EINVAL, "wd_unpack_spinor: bad argument");
     const size_t per = (size_t)h->V * kSpinorComps, dper = (size_t)h->Vs * kSpinorComps;
     for (int r = 0; r < nrhs; r++) {
@@ -404,17 +390,16 @@ static bool geometry_fits(const wd_handle *h, const KernelInfo &k) {
 }
 
 static int auto_kernel(const wd_handle *h, int nrhs) {
-    // Preference order: with a clover term in the fused variant the first-generation TMA
-    // kernel is the fastest (64^4: 4.17 ms vs 4.36 ms); for the hopping term alone (csw = 0, or the unfused
-    // variant) the second generation is (3.66 ms vs 2.96 ms).  linear256 always fits.
-    static const char *pref_clover[] = {"tma_2x4x16", "tma_4x4x8", "tmb_2x8x8", "tile_1x4x4x16", "tile_1x4x8x8", "tile_1x2x4x32",
-                                        "tile_2x4x4x8", "tile_4x4x4x4", "tile_1x4x4x8", "tile_1x4x4x4"};
-    static const char *pref_hop[] = {"tmb_4x4x8", "tmb_2x8x8", "tma_2x4x16", "tile_1x4x4x16", "tile_1x4x8x8", "tile_1x2x4x32",
-                                     "tile_2x4x4x8", "tile_4x4x4x4", "tile_1x4x4x8", "tile_1x4x4x4"};
-    // several right-hand sides in one launch: the second generation is 7 % faster on cfg 5 (26.5 vs 28.5 ms)
-    const bool clover_fused = (h->csw != 0.0) && h->variant == 0 && nrhs == 1;
-    const char **pref = clover_fused ? pref_clover : pref_hop;
-    for (int i = 0; i < 10; i++)
+    // Preference order: one right-hand side with a clover term, fused: the first-generation
+    // TMA kernel (64^4: 4.17 ms vs 4.36 ms); the hopping term alone (csw = 0, or the unfused variant): the second
+    // generation (3.66 ms vs 2.96 ms); several right-hand sides in one call: wd_tmc.cu (two per thread, links in
+    // registers).  linear256 always fits.
+    static const char *pref_clover[] = {"tma_2x4x16", "tmb_4x4x8", "tmb_2x8x8", "tile_1x4x4x16", "tile_2x4x4x4"};
+    static const char *pref_hop[] = {"tmb_4x4x8", "tmb_2x8x8", "tma_2x4x16", "tile_1x4x4x16", "tile_2x4x4x4"};
+    static const char *pref_multi[] = {"tmb_4x4x8", "tmb_2x8x8", "tmc_2x4x16", "tile_1x4x4x16", "tile_2x4x4x4"};
+    const bool clover_fused = (h->csw != 0.0 || h->has_clover) && h->variant == 0;
+    const char **pref = (nrhs > 1 && h->variant == 0) ? pref_multi : clover_fused ? pref_clover : pref_hop;
+    for (int i = 0; i < 5; i++)
         for (int id = 0; id < kernel_count(); id++)
             if (!strcmp(kernel_info(id).name, pref[i]) && geometry_fits(h, kernel_info(id))) return id;
     return 0;
@@ -457,6 +442,12 @@ int wd_set_option(wd_handle *h, int option, long value) {
     case WD_OPT_DEVICE_PACK:
         h->device_pack = value ? 1 : 0;
         return WD_OK;
+    case WD_OPT_HOST_PIPELINE:
+        h->host_pipeline = value ? 1 : 0;
+        return WD_OK;
+    case WD_OPT_GMRES_GRAPH:
+        h->gmres_graph = value ? 1 : 0;
+        return WD_OK;
     default:
         return fail(h, WD_EINVAL, "wd_set_option: unknown option");
     }
@@ -470,12 +461,16 @@ int wd_get_option(const wd_handle *h, int option, long *value) {
     case WD_OPT_TCHUNK: *value = h->tchunk_opt; return WD_OK;
     case WD_OPT_ZGROUP: *value = h->zgroup_opt; return WD_OK;
     case WD_OPT_DEVICE_PACK: *value = h->device_pack; return WD_OK;
+    case WD_OPT_HOST_PIPELINE: *value = h->host_pipeline; return WD_OK;
+    case WD_OPT_GMRES_GRAPH: *value = h->gmres_graph; return WD_OK;
     default: return WD_EINVAL;
     }
 }
 
 // ---- apply ------------------------------------------------------------------------------------------
-static int fill_params(wd_handle *h, KParams &p, const KernelInfo &k) {
+}  // extern "C"
+
+int wd::fill_params(wd_handle *h, KParams &p, const KernelInfo &k) {
     p.U = h->dU;
     p.S = h->dS;
     p.V = h->V;
@@ -491,6 +486,11 @@ static int fill_params(wd_handle *h, KParams &p, const KernelInfo &k) {
     p.opt_zgroup = (int)h->zgroup_opt;
     p.tc_begin = p.tc_count = 0;
     p.sched = h->dsched;
+    p.nsm = h->nsm;
+    p.device = h->device;
+    p.maps = h->maps;
+    p.open_mask = 0;
+    p.gauge_rows = 3;
     if (k.bx) {
         p.ntx = h->n[3] / k.bx;
         p.nty = h->n[2] / k.by;
@@ -512,8 +512,27 @@ static int fill_params(wd_handle *h, KParams &p, const KernelInfo &k) {
     return WD_OK;
 }
 
+// The TMA kernels expect the two work-queue words to be zero at launch; the last CTA of every launch re-arms them.
+// After a failed launch (or a stream change with work pending, see wd_set_stream) they are zeroed explicitly.
+int wd::launch_op(wd_handle *h, const KernelInfo &k, const KParams &p, int self) {
+    if (h->sched_dirty) {
+        WD_CUDA(h, cudaMemsetAsync(h->dsched, 0, 2 * sizeof(unsigned int), h->stream));
+        h->sched_dirty = false;
+    }
+    const cudaError_t e = k.launch(p, self, h->stream);
+    if (e != cudaSuccess) {
+        h->sched_dirty = true;
+        map_cache_clear(h->maps);
+        return fail(h, (e == cudaErrorMemoryAllocation) ? WD_ENOMEM : WD_ECUDA, std::string("kernel launch (") + k.name + "): " + cudaGetErrorString(e));
+    }
+    h->launches++;
+    return WD_OK;
+}
+
+extern "C" {
+
 int wd_apply(wd_handle *h, void *dev_out, const void *dev_in, int nrhs) {
-    if (!h) return WD_EINVAL;
+    WD_ENTER(h);
     if (!dev_out || !dev_in || nrhs < 1) return fail(h, WD_EINVAL, "wd_apply: null pointer or nrhs < 1");
     if (misaligned(dev_out) || misaligned(dev_in)) return fail(h, WD_EINVAL, "wd_apply: spinor buffers must be 16-byte aligned");
     const size_t bytes = wd_spinor_bytes(h, nrhs);
@@ -534,20 +553,19 @@ int wd_apply(wd_handle *h, void *dev_out, const void *dev_in, int nrhs) {
         p.psi = (const double2 *)dev_in;
         p.out = (double2 *)dev_out;
         p.nrhs = nrhs;
-        WD_CUDA(h, k.launch(p, self, h->stream));
-        h->launches++;
-        return WD_OK;
+        return launch_op(h, k, p, self);
     }
     for (int r = 0; r < nrhs; r++) {
         p.psi = (const double2 *)dev_in + r * per;
         p.out = (double2 *)dev_out + r * per;
         if (h->variant == 0) {
-            WD_CUDA(h, k.launch(p, self, h->stream));
-            h->launches++;
+            rc = launch_op(h, k, p, self);
+            if (rc) return rc;
         } else {
-            WD_CUDA(h, k.launch(p, SELF_NONE, h->stream));
+            rc = launch_op(h, k, p, SELF_NONE);
+            if (rc) return rc;
             WD_CUDA(h, launch_selfcoupling(p, self, h->stream));
-            h->launches += 2;
+            h->launches++;
         }
     }
     return WD_OK;
@@ -609,9 +627,9 @@ static int apply_host_pipelined(wd_handle *h, double *host_out, const double *ho
             WD_CUDA(h, cudaStreamWaitEvent(h->stream, h->ev_up[k], 0));
             WD_CUDA(h, cudaStreamWaitEvent(h->stream, h->ev_up[(k + 1) % C], 0));
             p.tc_begin = k;
-            WD_CUDA(h, kinfo.launch(p, self, h->stream));
+            rc = launch_op(h, kinfo, p, self);
+            if (rc) return rc;
             WD_CUDA(h, cudaEventRecord(h->ev_cmp[k], h->stream));
-            h->launches++;
             const long long s0 = (long long)k * Vc;
             WD_CUDA(h, cudaStreamWaitEvent(h->s_dn, h->ev_cmp[k], 0));
             WD_CUDA(h, launch_soa_to_aos(h->dstage_out + s0 * kSpinorComps, h->work_out + s0, Vc, h->Vs, kSpinorComps, h->s_dn));
@@ -627,7 +645,7 @@ static int apply_host_pipelined(wd_handle *h, double *host_out, const double *ho
 }
 
 int wd_apply_host(wd_handle *h, double *host_out, const double *host_in, int nrhs) {
-    if (!h) return WD_EINVAL;
+    WD_ENTER(h);
     if (!host_out || !host_in || nrhs < 1) return fail(h, WD_EINVAL, "wd_apply_host: null pointer or nrhs < 1");
     if (!h->has_gauge) return fail(h, WD_ESTATE, "wd_apply_host: no gauge field loaded");
     if (h->csw != 0.0 && !h->has_clover)
@@ -638,13 +656,11 @@ int wd_apply_host(wd_handle *h, double *host_out, const double *host_in, int nrh
     if (!h->work_out) WD_CUDA(h, cudaMalloc((void **)&h->work_out, dbytes));
     int rc = ensure_dstage(h, bytes);
     if (rc) return rc;
-    // pipelined path: a TMA kernel, fused variant, and T splits into 4..16 equal chunks (WD_HOST_CHUNKS: experiments)
+    // pipelined path (WD_OPT_HOST_PIPELINE, default on): a TMA kernel, fused variant, and T splits into 4..16 equal chunks
     const KernelInfo &kinfo = kernel_info(wd_kernel_in_use(h));
     int C = 0;
-    if (kinfo.multi_rhs && h->variant == 0 && strncmp(kinfo.name, "tmr", 3) != 0 && !getenv("WD_HOST_SERIAL"))
-    {
-        const int cmax = getenv("WD_HOST_CHUNKS") ? atoi(getenv("WD_HOST_CHUNKS")) : kMaxPipeChunks;
-        for (int c = (cmax < kMaxPipeChunks ? cmax : kMaxPipeChunks); c >= 4 && !C; c--)
+    if (kinfo.multi_rhs && h->variant == 0 && h->host_pipeline) {
+        for (int c = kMaxPipeChunks; c >= 4 && !C; c--)
             if (h->n[0] % c == 0) C = c;
     }
     if (C) return apply_host_pipelined(h, host_out, host_in, nrhs, C);
@@ -663,3 +679,5 @@ int wd_apply_host(wd_handle *h, double *host_out, const double *host_in, int nrh
 }
 
 }  // extern "C"
+
+void wd::dd_free(wd_handle *) {}

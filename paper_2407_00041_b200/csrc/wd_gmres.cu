@@ -1,0 +1,434 @@
+// wd_gmres.cu — restarted GMRES(m) on the device around the operator: Algorithm 1 of the paper
+// with M = I, in the paper's order:
+//
+//     r = b - A x;  beta = ||r||;  v_1 = r / beta                                     (lines 4-6)
+//     for j = 1..m:  w = A v_j                                                        (line 9: wd_apply, the hot path)
+//                    for i = 1..j:  h_ij = <w, v_i> = v_i^H w;  w = w - h_ij v_i      (lines 10-12, modified Gram-Schmidt)
+//                    h_{j+1,j} = ||w||;  v_{j+1} = w / h_{j+1,j}                       (lines 14-15)
+//     y = argmin || beta e_1 - H y ||;  x = x + V y                                   (lines 18-20)
+//
+// Termination as DDalphaAMG's (R17, R18): ||b - A x|| < tol ||b - A x_0|| tested on
+// the true residual at the top of the restart loop, or max_cycles; |h_{j+1,j}| < tol/10 ends the Arnoldi loop.
+//
+// Vectors are device spinors in DEVICE layout ([12][Vs], the padding between components is never touched).
+// The BLAS-1 work is fused so that every pass over memory does as much as the sequential dependence of modified
+// Gram-Schmidt allows:  [w -= h_{i-1,j} v_{i-1}  and  h_ij = <w, v_i>]  is ONE kernel (3 reads + 1 write instead of
+// 2 + 3 reads and 1 write), the last subtraction is fused with the norm, the solution update reads all basis
+// vectors in one pass.  Every scalar (h_ij, beta, 1/h, y, the breakdown flag) lives in device memory and is
+// produced by the last block of the kernel that reduces it (fixed summation order: results are deterministic),
+// so a whole restart cycle is a fixed sequence of launches without host synchronisation: it is captured once
+// into a CUDA graph and replayed (the consumer of cfg 3's "100 back-to-back applications", SURVEY.md:399).
+#include <cmath>
+#include <cstddef>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "wd_handle.h"
+#include "wd_math.cuh"
+
+using namespace wd;
+
+namespace {
+constexpr int kMaxM = 64;
+constexpr int kThreads = 256;
+
+struct Scalars {          // device-resident scalars of the iteration
+    double2 H[(kMaxM + 1) * kMaxM];  // H[i + (m+1) * j]
+    double2 y[kMaxM];
+    double beta, inv;     // ||r||, and the reciprocal the next scaling uses (1/beta or 1/h_{j+1,j})
+    double lsq_resid;     // |g_{kdim+1}|: the recurrence residual of the cycle
+    int active, kdim;     // Arnoldi still running; Krylov dimension of this cycle
+    unsigned int ticket;  // last-block detection of the reductions (zero between kernels)
+};
+}  // namespace
+
+struct wd_gmres_state {
+    int m;
+    double2 *basis;       // (m + 2) device spinors: v_0 .. v_m, w
+    Scalars *sc;          // device
+    double2 *partials;    // per-block partial sums of the reductions
+    int nbx;              // blocks per component
+    cudaGraphExec_t graph;
+    const void *gx, *gb;  // what the captured cycle was built for
+    int gm;
+    double gtol;
+    cudaStream_t gstream;
+    long graph_launches;  // kernel launches inside one captured cycle
+    int last_m, last_kdim;
+    std::vector<double2> hostH;
+};
+
+namespace {
+
+__device__ __forceinline__ double2 block_reduce(double2 v, double2 *sh) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        v.x += __shfl_xor_sync(0xffffffffu, v.x, o);
+        v.y += __shfl_xor_sync(0xffffffffu, v.y, o);
+    }
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    __syncthreads();
+    if (l == 0) sh[w] = v;
+    __syncthreads();
+    v = (threadIdx.x < kThreads / 32) ? sh[threadIdx.x] : make_double2(0.0, 0.0);
+    if (w == 0) {
+#pragma unroll
+        for (int o = 4; o > 0; o >>= 1) {
+            v.x += __shfl_xor_sync(0xffffffffu, v.x, o);
+            v.y += __shfl_xor_sync(0xffffffffu, v.y, o);
+        }
+    }
+    return v;  // valid in thread 0
+}
+
+// Grid-wide sum in a fixed order: every block leaves its partial, the last block to finish adds them up.
+// Returns true in thread 0 of that last block, with the total in *total.
+__device__ __forceinline__ bool grid_reduce(double2 mine, double2 *partials, unsigned int *ticket, double2 *total) {
+    __shared__ double2 sh[kThreads / 32];
+    __shared__ bool last;
+    const unsigned int nblk = gridDim.x * gridDim.y, blk = blockIdx.y * gridDim.x + blockIdx.x;
+    const double2 b = block_reduce(mine, sh);
+    if (threadIdx.x == 0) {
+        partials[blk] = b;
+        __threadfence();
+        last = (atomicAdd(ticket, 1u) == nblk - 1);
+    }
+    __syncthreads();
+    if (!last) return false;
+    __threadfence();
+    double2 s = make_double2(0.0, 0.0);
+    for (unsigned int k = threadIdx.x; k < nblk; k += kThreads) {
+        const double2 p = partials[k];
+        s.x += p.x;
+        s.y += p.y;
+    }
+    s = block_reduce(s, sh);
+    if (threadIdx.x == 0) {
+        *total = s;
+        *ticket = 0;
+        return true;
+    }
+    return false;
+}
+
+enum { OP_DOT = 0, OP_AXPY_DOT, OP_AXPY_NORM, OP_RESID_NORM };
+
+// One fused pass (see the header): the vectors are [12][Vs], blockIdx.y is the component.
+//   OP_DOT        : h_out = <w, vn>
+//   OP_AXPY_DOT   : w -= h_in * vp;  h_out = <w, vn>
+//   OP_AXPY_NORM  : w -= h_in * vp;  h_out = ||w|| (real), inv = 1 / h_out, breakdown rule
+//   OP_RESID_NORM : w = bvec - w;    beta = ||w||, inv = 1 / beta; starts a cycle (active = 1, kdim = m)
+template <int OP>
+__global__ void __launch_bounds__(kThreads) k_fused(double2 *__restrict__ w, const double2 *__restrict__ vp,
+                                                    const double2 *__restrict__ vn, long long V, long long Vs, Scalars *sc,
+                                                    int h_in, int h_out, int j, int m, double tol10) {
+    if (OP != OP_RESID_NORM && !sc->active) return;
+    const long long base = (long long)blockIdx.y * Vs;
+    double2 h = make_double2(0.0, 0.0);
+    if (OP == OP_AXPY_DOT || OP == OP_AXPY_NORM) h = sc->H[h_in];
+    double2 acc = make_double2(0.0, 0.0);
+    for (long long i = (long long)blockIdx.x * kThreads + threadIdx.x; i < V; i += (long long)gridDim.x * kThreads) {
+        double2 x = w[base + i];
+        if (OP == OP_AXPY_DOT || OP == OP_AXPY_NORM) {
+            const double2 p = vp[base + i];
+            x.x = fma(-h.x, p.x, fma(h.y, p.y, x.x));
+            x.y = fma(-h.x, p.y, fma(-h.y, p.x, x.y));
+            w[base + i] = x;
+        } else if (OP == OP_RESID_NORM) {
+            const double2 b = vp[base + i];
+            x = make_double2(b.x - x.x, b.y - x.y);
+            w[base + i] = x;
+        }
+        if (OP == OP_DOT || OP == OP_AXPY_DOT) {  // conj(vn) * x
+            const double2 q = vn[base + i];
+            acc.x = fma(q.x, x.x, fma(q.y, x.y, acc.x));
+            acc.y = fma(q.x, x.y, fma(-q.y, x.x, acc.y));
+        } else {
+            acc.x = fma(x.x, x.x, fma(x.y, x.y, acc.x));
+        }
+    }
+    double2 total;
+    if (!grid_reduce(acc, reinterpret_cast<double2 *>(sc + 1), &sc->ticket, &total)) return;
+    if (OP == OP_DOT || OP == OP_AXPY_DOT) {
+        sc->H[h_out] = total;
+    } else if (OP == OP_AXPY_NORM) {
+        const double hn = sqrt(total.x);
+        sc->H[h_out] = make_double2(hn, 0.0);
+        sc->inv = (hn > 0.0) ? 1.0 / hn : 0.0;
+        if (hn < tol10) {  // near breakdown: the Krylov dimension of this cycle is j + 1
+            sc->active = 0;
+            sc->kdim = j + 1;
+        }
+    } else {
+        const double beta = sqrt(total.x);
+        sc->beta = beta;
+        sc->inv = (beta > 0.0) ? 1.0 / beta : 0.0;
+        sc->active = 1;
+        sc->kdim = m;
+    }
+}
+
+// dst = inv * src (v_1 = r / beta, v_{j+1} = w / h_{j+1,j}); `always`: also when the Arnoldi loop has ended
+__global__ void __launch_bounds__(kThreads) k_scale(double2 *__restrict__ dst, const double2 *__restrict__ src, long long V,
+                                                    long long Vs, const Scalars *sc, int always) {
+    if (!always && !sc->active) return;
+    const double s = sc->inv;
+    const long long base = (long long)blockIdx.y * Vs;
+    for (long long i = (long long)blockIdx.x * kThreads + threadIdx.x; i < V; i += (long long)gridDim.x * kThreads) {
+        const double2 x = src[base + i];
+        dst[base + i] = make_double2(s * x.x, s * x.y);
+    }
+}
+
+// y = argmin || beta e_1 - H y ||_2 over the kdim columns of this cycle: Givens QR of the (kdim+1) x kdim Hessenberg
+// matrix, one thread (kdim <= 64).  Rotation [[c, s], [-conj(s), c]], c real, zeroes the sub-diagonal entry.
+__global__ void k_lsq(Scalars *sc, int m) {
+    if (threadIdx.x || blockIdx.x) return;
+    const int kd = sc->kdim, ld = m + 1;
+    double2 g[kMaxM + 1];
+    double2 *H = sc->H;
+    for (int k = 0; k <= kd; k++) g[k] = make_double2(0.0, 0.0);
+    g[0].x = sc->beta;
+    for (int k = 0; k < kd; k++) {
+        const double2 a = H[k + ld * k];
+        const double b = H[k + 1 + ld * k].x;
+        const double na = hypot(a.x, a.y), r = hypot(na, b);
+        double c = 1.0;
+        double2 s = make_double2(0.0, 0.0);
+        if (r > 0.0) {
+            if (na > 0.0) {
+                c = na / r;
+                s = make_double2(b * a.x / (na * r), b * a.y / (na * r));
+            } else {
+                c = 0.0;
+                s = make_double2(1.0, 0.0);
+            }
+        }
+        for (int col = k; col < kd; col++) {  // rows k, k+1 of the remaining columns (and of column k itself)
+            const double2 p = H[k + ld * col], q = H[k + 1 + ld * col];
+            H[k + ld * col] = make_double2(c * p.x + s.x * q.x - s.y * q.y, c * p.y + s.x * q.y + s.y * q.x);
+            H[k + 1 + ld * col] = make_double2(-(s.x * p.x + s.y * p.y) + c * q.x, -(s.x * p.y - s.y * p.x) + c * q.y);
+        }
+        const double2 p = g[k];
+        g[k] = make_double2(c * p.x, c * p.y);
+        g[k + 1] = make_double2(-(s.x * p.x + s.y * p.y), -(s.x * p.y - s.y * p.x));
+    }
+    sc->lsq_resid = hypot(g[kd].x, g[kd].y);
+    for (int k = kd - 1; k >= 0; k--) {  // back substitution R y = g
+        double2 t = g[k];
+        for (int col = k + 1; col < kd; col++) {
+            const double2 rr = H[k + ld * col], yy = sc->y[col];
+            t.x -= rr.x * yy.x - rr.y * yy.y;
+            t.y -= rr.x * yy.y + rr.y * yy.x;
+        }
+        const double2 d = H[k + ld * k];
+        const double dd = d.x * d.x + d.y * d.y;
+        sc->y[k] = (dd > 0.0) ? make_double2((t.x * d.x + t.y * d.y) / dd, (t.y * d.x - t.x * d.y) / dd) : make_double2(0.0, 0.0);
+    }
+}
+
+// x += sum_i y_i v_i over the kdim basis vectors of this cycle, one pass (line 19)
+__global__ void __launch_bounds__(kThreads) k_update(double2 *__restrict__ x, const double2 *__restrict__ basis, long long V,
+                                                     long long Vs, long long vec_stride, const Scalars *sc) {
+    const int kd = sc->kdim;
+    const long long base = (long long)blockIdx.y * Vs;
+    for (long long i = (long long)blockIdx.x * kThreads + threadIdx.x; i < V; i += (long long)gridDim.x * kThreads) {
+        double2 s = x[base + i];
+        for (int k = 0; k < kd; k++) {
+            const double2 yk = sc->y[k], v = basis[(long long)k * vec_stride + base + i];
+            s.x = fma(yk.x, v.x, fma(-yk.y, v.y, s.x));
+            s.y = fma(yk.x, v.y, fma(yk.y, v.x, s.y));
+        }
+        x[base + i] = s;
+    }
+}
+
+// Hessenberg matrix of the cycle as the Arnoldi process produced it (before k_lsq rotates it in place)
+__global__ void k_copy_h(double2 *dst, const Scalars *sc, int n) {
+    for (int k = threadIdx.x; k < n; k += blockDim.x) dst[k] = sc->H[k];
+}
+
+int ensure_workspace(wd_handle *h, int m) {
+    wd_gmres_state *g = h->gmres;
+    if (g && g->m >= m) return WD_OK;
+    gmres_free(h);
+    g = new (std::nothrow) wd_gmres_state();
+    if (!g) return fail(h, WD_ENOMEM, "wd_gmres: out of host memory");
+    g->m = m;
+    g->basis = nullptr;
+    g->sc = nullptr;
+    g->graph = nullptr;
+    g->gx = g->gb = nullptr;
+    g->graph_launches = 0;
+    g->last_m = g->last_kdim = 0;
+    long long nbx = (h->V + kThreads * 8 - 1) / (kThreads * 8);  // ~8 elements per thread, at most ~8 blocks per SM
+    const long long cap = (long long)h->nsm * 8 / 12 + 1;
+    if (nbx > cap) nbx = cap;
+    if (nbx < 1) nbx = 1;
+    g->nbx = (int)nbx;
+    h->gmres = g;
+    const size_t vec = (size_t)h->Vs * kSpinorComps * sizeof(double2);
+    WD_CUDA(h, cudaMalloc((void **)&g->basis, (size_t)(m + 2) * vec));
+    // the scalars, followed by the per-block partial sums and room for a copy of H
+    const size_t extra = (size_t)g->nbx * 12 * sizeof(double2) + (size_t)(kMaxM + 1) * kMaxM * sizeof(double2);
+    WD_CUDA(h, cudaMalloc((void **)&g->sc, sizeof(Scalars) + extra));
+    WD_CUDA(h, cudaMemsetAsync(g->sc, 0, sizeof(Scalars) + extra, h->stream));
+    return WD_OK;
+}
+
+struct Cycle {  // issues the launches of the algorithm on the handle's stream; counts them
+    wd_handle *h;
+    wd_gmres_state *g;
+    int m;
+    double tol10;
+    long launches = 0;
+    double2 *vec(int k) const { return g->basis + (size_t)k * h->Vs * kSpinorComps; }
+    double2 *w() const { return vec(m + 1); }
+    dim3 grid() const { return dim3((unsigned)g->nbx, 12); }
+    template <int OP> int fused(double2 *wv, const double2 *vp, const double2 *vn, int h_in, int h_out, int j) {
+        k_fused<OP><<<grid(), kThreads, 0, h->stream>>>(wv, vp, vn, h->V, h->Vs, g->sc, h_in, h_out, j, m, tol10);
+        WD_CUDA(h, cudaGetLastError());
+        launches++;
+        return WD_OK;
+    }
+    int apply(double2 *out, const double2 *in) {
+        const long before = h->launches;
+        const int rc = wd_apply(h, out, in, 1);
+        launches += h->launches - before;
+        h->launches = before;  // the caller adds `launches` once per executed cycle (graph replays included)
+        return rc;
+    }
+    // w = b - A x;  beta = ||w||
+    int residual(const double2 *x, const double2 *b) {
+        int rc = apply(w(), x);
+        if (rc) return rc;
+        return fused<OP_RESID_NORM>(w(), b, nullptr, 0, 0, 0);
+    }
+    // lines 6-20 of Algorithm 1, then line 4-5 for the new x
+    int body(double2 *x, const double2 *b) {
+        const int ld = m + 1;
+        int rc;
+        k_scale<<<grid(), kThreads, 0, h->stream>>>(vec(0), w(), h->V, h->Vs, g->sc, 1);  // v_1 = r / beta
+        WD_CUDA(h, cudaGetLastError());
+        launches++;
+        WD_CUDA(h, cudaMemsetAsync(g->sc->H, 0, sizeof(double2) * (size_t)ld * m, h->stream));
+        for (int j = 0; j < m; j++) {
+            if ((rc = apply(w(), vec(j)))) return rc;                                      // w = A v_j
+            if ((rc = fused<OP_DOT>(w(), nullptr, vec(0), 0, 0 + ld * j, j))) return rc;   // h_1j
+            for (int i = 1; i <= j; i++)                                                   // w -= h_{i-1,j} v_{i-1}; h_ij
+                if ((rc = fused<OP_AXPY_DOT>(w(), vec(i - 1), vec(i), (i - 1) + ld * j, i + ld * j, j))) return rc;
+            if ((rc = fused<OP_AXPY_NORM>(w(), vec(j), nullptr, j + ld * j, (j + 1) + ld * j, j))) return rc;
+            k_scale<<<grid(), kThreads, 0, h->stream>>>(vec(j + 1), w(), h->V, h->Vs, g->sc, 0);  // v_{j+1}
+            WD_CUDA(h, cudaGetLastError());
+            launches++;
+        }
+        double2 *Hcopy = reinterpret_cast<double2 *>(g->sc + 1) + (size_t)g->nbx * 12;
+        k_copy_h<<<1, 256, 0, h->stream>>>(Hcopy, g->sc, ld * m);
+        k_lsq<<<1, 32, 0, h->stream>>>(g->sc, m);
+        k_update<<<grid(), kThreads, 0, h->stream>>>(x, g->basis, h->V, h->Vs, h->Vs * kSpinorComps, g->sc);
+        WD_CUDA(h, cudaGetLastError());
+        launches += 3;
+        return residual(x, b);
+    }
+};
+
+}  // namespace
+
+void wd::gmres_free(wd_handle *h) {
+    wd_gmres_state *g = h->gmres;
+    if (!g) return;
+    if (g->graph) cudaGraphExecDestroy(g->graph);
+    if (g->basis) cudaFree(g->basis);
+    if (g->sc) cudaFree(g->sc);
+    delete g;
+    h->gmres = nullptr;
+}
+
+extern "C" {
+
+int wd_gmres(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_cycles, double tol, int *cycles_done,
+             double *host_resid) {
+    WD_ENTER(h);
+    if (!dev_x || !dev_b || m < 1 || m > kMaxM || max_cycles < 0 || !(tol > 0.0))
+        return fail(h, WD_EINVAL, "wd_gmres: null pointer, m outside 1..64, max_cycles < 0 or tol <= 0");
+    if (((size_t)dev_x | (size_t)dev_b) & 15) return fail(h, WD_EINVAL, "wd_gmres: spinor buffers must be 16-byte aligned");
+    if (dev_x == dev_b) return fail(h, WD_EINVAL, "wd_gmres: x overlaps b");
+    if (!h->has_gauge) return fail(h, WD_ESTATE, "wd_gmres: no gauge field loaded");
+    int rc = ensure_workspace(h, m);
+    if (rc) return rc;
+    wd_gmres_state *g = h->gmres;
+    Cycle cyc{h, g, m, tol / 10.0};
+    double2 *x = (double2 *)dev_x;
+    const double2 *b = (const double2 *)dev_b;
+    struct { double beta, inv, lsq; int active, kdim; } hs;
+    auto read_scalars = [&]() -> int {
+        WD_CUDA(h, cudaMemcpyAsync(&hs, &g->sc->beta, sizeof(hs), cudaMemcpyDeviceToHost, h->stream));
+        WD_CUDA(h, cudaStreamSynchronize(h->stream));
+        return WD_OK;
+    };
+    static_assert(offsetof(Scalars, kdim) - offsetof(Scalars, beta) == 3 * sizeof(double) + sizeof(int), "layout of Scalars");
+    // lines 4-5 for x_0
+    if ((rc = cyc.residual(x, b))) return rc;
+    h->launches += cyc.launches;
+    if ((rc = read_scalars())) return rc;
+    const double r0 = hs.beta;
+    if (host_resid) host_resid[0] = r0;
+    int k = 0;
+    const bool can_graph = (h->stream != nullptr) && h->gmres_graph;
+    while (!(hs.beta < tol * r0) && k < max_cycles && hs.beta != 0.0) {
+        const bool have_graph = g->graph && g->gx == dev_x && g->gb == dev_b && g->gm == m && g->gtol == tol && g->gstream == h->stream;
+        if (have_graph) {
+            WD_CUDA(h, cudaGraphLaunch(g->graph, h->stream));
+            h->launches += g->graph_launches;
+        } else if (can_graph && k >= 1) {  // the first cycle ran eagerly (all caches warm): capture the second, replay it
+            if (g->graph) cudaGraphExecDestroy(g->graph);
+            g->graph = nullptr;
+            cudaGraph_t graph = nullptr;
+            WD_CUDA(h, cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
+            cyc.launches = 0;
+            rc = cyc.body(x, b);
+            const cudaError_t ce = cudaStreamEndCapture(h->stream, &graph);
+            if (rc) {
+                if (graph) cudaGraphDestroy(graph);
+                return rc;
+            }
+            WD_CUDA(h, ce);
+            const cudaError_t ie = cudaGraphInstantiate(&g->graph, graph, 0);
+            cudaGraphDestroy(graph);
+            WD_CUDA(h, ie);
+            g->gx = dev_x, g->gb = dev_b, g->gm = m, g->gtol = tol, g->gstream = h->stream;
+            g->graph_launches = cyc.launches;
+            WD_CUDA(h, cudaGraphLaunch(g->graph, h->stream));
+            h->launches += g->graph_launches;
+        } else {
+            cyc.launches = 0;
+            if ((rc = cyc.body(x, b))) return rc;
+            h->launches += cyc.launches;
+        }
+        if ((rc = read_scalars())) return rc;
+        k++;
+        if (host_resid) host_resid[k] = hs.beta;
+    }
+    if (cycles_done) *cycles_done = k;
+    g->last_m = m;
+    g->last_kdim = (k > 0) ? hs.kdim : 0;
+    return WD_OK;
+}
+
+int wd_gmres_last_hessenberg(wd_handle *h, double *host_H, int *kdim, double *lsq_resid) {
+    WD_ENTER(h);
+    wd_gmres_state *g = h->gmres;
+    if (!g || g->last_m < 1) return fail(h, WD_ESTATE, "wd_gmres_last_hessenberg: no GMRES cycle has run on this handle");
+    const int m = g->last_m;
+    if (host_H) {
+        const double2 *Hcopy = reinterpret_cast<const double2 *>(g->sc + 1) + (size_t)g->nbx * 12;
+        WD_CUDA(h, cudaMemcpyAsync(host_H, Hcopy, sizeof(double2) * (size_t)(m + 1) * m, cudaMemcpyDeviceToHost, h->stream));
+    }
+    if (lsq_resid) WD_CUDA(h, cudaMemcpyAsync(lsq_resid, &g->sc->lsq_resid, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    WD_CUDA(h, cudaStreamSynchronize(h->stream));
+    if (kdim) *kdim = g->last_kdim;
+    return WD_OK;
+}
+
+}  // extern "C"

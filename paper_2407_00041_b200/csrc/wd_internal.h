@@ -11,9 +11,9 @@ namespace wd {
 // double = double2 = 16 B; the site index i (canonical order, X fastest) is the fastest index of
 // every array, so a warp that handles 32 consecutive sites reads 512 contiguous bytes per
 // component:
-// The component stride is Vs = V + padding (component_stride()): with Vs = V the components of one
-// site sit a power of two apart on the paper-sized lattices (2^28 B at 64^4) and alias onto the same
-// L2 slice and set; measured at 64^4: 38 % extra DRAM reads (profiles/r1b_*.md).
+// The component stride is Vs = V rounded up to 16 sites + 272 sites of padding (component_stride()): every
+// component starts 256-byte aligned and the components of one site are not a power of two apart.  Measured
+// at 64^4 (profiles/r1b_*.md): padding of 0 .. 16400 sites all within 1 % — kept because it is free.
 //   spinor  double2 [nrhs][12][Vs]      component c = 3*spin + colour
 //   gauge   double2 [4][9][Vs]          mu = T,Z,Y,X; k = 3*row + col; forward links only, each
 //                                       link stored ONCE (U_mu(x-mu) is read from site x-mu)
@@ -35,6 +35,8 @@ __host__ __device__ constexpr int slot_off(int b, int k) { return 18 * b + 3 + k
 
 enum SelfMode { SELF_NONE = 0, SELF_MASS = 1, SELF_CLOVER = 2 };
 
+struct MapCache;  // wd_tma_common.cuh: per-handle cache of tensor maps
+
 struct KParams {
     const double2 *psi;  // right-hand side 0; RHS r at + r * 12 * Vs (same for out)
     int nrhs;            // right-hand sides of this launch (> 1 only for kernels with multi_rhs)
@@ -54,6 +56,10 @@ struct KParams {
     unsigned int *sched;         // device, 2 words, zero between launches: work queue of the TMA kernels
     int tc_begin, tc_count;      // TMA kernels: apply only to T chunks [tc_begin, tc_begin + tc_count) of opt_tchunk
                                  // slices each (tc_count = 0: the whole lattice); used by the pipelined wd_apply_host
+    int nsm, device;             // SM count and ordinal of the handle's device (read once in wd_create)
+    MapCache *maps;              // tensor-map cache of the handle (may be null: encode per launch)
+    int open_mask;               // bit mu: direction mu does not wrap (sub-lattice of a domain decomposition, wd_dd.cu)
+    int gauge_rows;              // 3: links stored as 9 complex; 2: two-row storage, third row rebuilt in the kernel
 };
 
 struct KernelInfo {
@@ -69,12 +75,13 @@ const KernelInfo &kernel_info(int id);
 
 // TMA-staged T-marching kernels: first generation (wd_tma.cu), second generation (wd_tmb.cu)
 cudaError_t launch_tma_2x4x16(const KParams &p, int self, cudaStream_t st);
-cudaError_t launch_tma_4x4x8(const KParams &p, int self, cudaStream_t st);
 cudaError_t launch_tmb_4x4x8(const KParams &p, int self, cudaStream_t st);
 cudaError_t launch_tmb_2x8x8(const KParams &p, int self, cudaStream_t st);
-// multi-RHS kernel: G right-hand sides of a 64-site tile share U and S in shared memory (wd_tmr.cu)
-cudaError_t launch_tmr_2x4x8_g3(const KParams &p, int self, cudaStream_t st);
-cudaError_t launch_tmr_2x4x8_g2(const KParams &p, int self, cudaStream_t st);
+// multi-RHS kernel: two right-hand sides per thread, links and S by LDG into registers (wd_tmc.cu)
+cudaError_t launch_tmc_2x4x16(const KParams &p, int self, cudaStream_t st);
+MapCache *map_cache_new();
+void map_cache_delete(MapCache *c);
+void map_cache_clear(MapCache *c);
 
 // self-coupling kernel of the unfused variant: out += S psi (clover) or out += mass * psi
 cudaError_t launch_selfcoupling(const KParams &p, int self, cudaStream_t st);

@@ -215,25 +215,15 @@ cudaError_t launch_selfcoupling(const KParams &p, int self, cudaStream_t st) {
 }
 
 // ---- registry -------------------------------------------------------------------------------
+// linear: any lattice.  tile_*: LDG kernels for lattices no TMA tile divides (cfg 1: 4^4).  tma/tmb/tmc: the TMA kernels.
 static const KernelInfo kKernels[] = {
     {"linear256", 0, 0, 0, 0, 256, false, launch_linear<256>},
-    {"linear128", 0, 0, 0, 0, 128, false, launch_linear<128>},
     {"tile_1x4x4x16", 1, 4, 4, 16, 256, false, launch_tiled<1, 4, 4, 16>},
-    {"tile_1x2x4x32", 1, 2, 4, 32, 256, false, launch_tiled<1, 2, 4, 32>},
-    {"tile_1x4x8x8", 1, 4, 8, 8, 256, false, launch_tiled<1, 4, 8, 8>},
-    {"tile_1x2x2x64", 1, 2, 2, 64, 256, false, launch_tiled<1, 2, 2, 64>},
-    {"tile_2x4x4x8", 2, 4, 4, 8, 256, false, launch_tiled<2, 4, 4, 8>},
-    {"tile_4x4x4x4", 4, 4, 4, 4, 256, false, launch_tiled<4, 4, 4, 4>},
-    {"tile_1x4x4x8", 1, 4, 4, 8, 128, false, launch_tiled<1, 4, 4, 8>},
-    {"tile_1x2x4x16", 1, 2, 4, 16, 128, false, launch_tiled<1, 2, 4, 16>},
-    {"tile_1x2x2x32", 1, 2, 2, 32, 128, false, launch_tiled<1, 2, 2, 32>},
-    {"tile_1x4x4x4", 1, 4, 4, 4, 64, false, launch_tiled<1, 4, 4, 4>},
+    {"tile_2x4x4x4", 2, 4, 4, 4, 128, false, launch_tiled<2, 4, 4, 4>},
     {"tma_2x4x16", 1, 2, 4, 16, 160, true, launch_tma_2x4x16},
-    {"tma_4x4x8", 1, 4, 4, 8, 160, true, launch_tma_4x4x8},
     {"tmb_4x4x8", 1, 4, 4, 8, 160, true, launch_tmb_4x4x8},
     {"tmb_2x8x8", 1, 2, 8, 8, 160, true, launch_tmb_2x8x8},
-    {"tmr3_2x4x8", 1, 2, 4, 8, 224, true, launch_tmr_2x4x8_g3},
-    {"tmr2_2x4x8", 1, 2, 4, 8, 160, true, launch_tmr_2x4x8_g2},
+    {"tmc_2x4x16", 1, 2, 4, 16, 160, true, launch_tmc_2x4x16},
 };
 
 int kernel_count() { return (int)(sizeof(kKernels) / sizeof(kKernels[0])); }

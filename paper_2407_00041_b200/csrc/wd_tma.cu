@@ -24,11 +24,10 @@
 // Neighbour indexing and the periodic wrap (a1) are box coordinates computed by the producer.
 #include <cstdio>
 #include <cstdlib>
-#include <vector>
+#include <new>
 
-#include "wd_internal.h"
-#include "wd_math.cuh"
-#include "wd_tma.cuh"
+#include "wd_tma_common.cuh"
+#include "wd_smem_ops.cuh"
 
 namespace wd {
 
@@ -69,6 +68,12 @@ cudaError_t encode_field_map(CUtensorMap *map, const void *base, const int n[4],
     return (r == CUDA_SUCCESS) ? cudaSuccess : cudaErrorInvalidValue;
 }
 
+MapCache *map_cache_new() { return new (std::nothrow) MapCache(); }
+void map_cache_delete(MapCache *c) { delete c; }
+void map_cache_clear(MapCache *c) {
+    if (c) c->clear();
+}
+
 // ---------------------------------------------------------------- shared-memory plan
 // Objects (each with a full/empty mbarrier pair), refilled once per T step:
 //   C  psi(t) interior                                    [12][N]
@@ -80,6 +85,7 @@ enum { OB_C = 0, OB_T, OB_Z, OB_Y, OB_X, OB_SA, OB_SB, OB_ITEM0, OB_ITEM1, OB_CO
 
 template <int BZ_, int BY_, int BX_, int SELF_> struct Plan {
     static constexpr int BZ = BZ_, BY = BY_, BX = BX_, SELF = SELF_;
+    static constexpr int G = 1;             // right-hand sides per work item
     static constexpr int N = BZ * BY * BX;  // sites per tile = compute threads
     static constexpr int NW = N / 32;       // compute warps
     static constexpr int NTHREADS = N + 32; // + the producer warp
@@ -105,94 +111,6 @@ template <int BZ_, int BY_, int BX_, int SELF_> struct Plan {
     static_assert(N % 32 == 0 && FZ % 8 == 0 && FY % 8 == 0 && FX % 8 == 0, "tile faces must keep 128-byte alignment");
     static_assert(SMEM <= 232448, "shared-memory plan exceeds 227 KB");
 };
-
-struct TmaMaps {
-    CUtensorMap psi_c, psi_z, psi_y, psi_x;  // boxes: interior, z-face, y-face, x-face (12 components)
-    CUtensorMap u_c, u_z, u_y, u_x;          // same shapes, 9 components (one link)
-    CUtensorMap s_c;                         // interior box, 18 components (one 6x6 block)
-};
-
-struct TmaParams {
-    double2 *out;
-    long long V, Vs;     // sites, component stride
-    int n[4];
-    int ntx, nty, ntz;   // tiles per direction
-    int py, pz;          // rasterisation panel (in tiles); py | nty, pz | ntz
-    int tchunk, ntc;     // T steps per work item, items per tile
-    int nrhs, rb;        // right-hand sides in this launch; RHS per block of the item order
-    int chunk0;          // first T chunk of this launch (0 unless a T range was asked for)
-    int nitems;          // ntx*nty*ntz*(chunks of this launch)*nrhs
-    double mass;
-    int flags;           // WD_TMA_FLAGS (experiments; 0 = production): 1 S evict_normal instead of evict_first,
-                         // 2 U evict_first, 4 psi evict_last, 8 L2-prefetch psi(t+1), 16 static round-robin items
-    unsigned int *sched; // [0] next item, [1] CTAs finished (dynamic work distribution; both 0 between launches)
-    unsigned long long *trace;  // diagnostics (WD_TMA_TRACE): [cta][kTraceLen] globaltimer per step, or null
-};
-constexpr int kTraceLen = 1024;
-
-// ---------------------------------------------------------------- shared-memory operand fetch
-__device__ __forceinline__ cd lds(const unsigned char *smem, uint32_t off) {
-    return *reinterpret_cast<const cd *>(smem + off);
-}
-
-// One direction MU != T of the stencil for the thread's site: both hops, operands from shared
-// memory.  (base, stride) pairs select interior or face storage per thread (no divergence: both
-// are shared-memory addresses).
-template <int MU>
-__device__ __forceinline__ void hop_pair_smem(cd acc[12], const unsigned char *smem, uint32_t u_own, uint32_t u_own_stride,
-                                              uint32_t pf, uint32_t pf_stride, uint32_t ub, uint32_t ub_stride,
-                                              uint32_t pb, uint32_t pb_stride) {
-    cd p[12], u[9];
-#pragma unroll
-    for (int k = 0; k < 9; k++) u[k] = lds(smem, u_own + k * u_own_stride);
-#pragma unroll
-    for (int c = 0; c < 12; c++) p[c] = lds(smem, pf + c * pf_stride);
-    hop_term<MU, -1>(acc, p, u);
-#pragma unroll
-    for (int k = 0; k < 9; k++) u[k] = lds(smem, ub + k * ub_stride);
-#pragma unroll
-    for (int c = 0; c < 12; c++) p[c] = lds(smem, pb + c * pb_stride);
-    hop_term<MU, +1>(acc, p, u);
-}
-
-}  // namespace wd
-
-namespace wd {
-
-struct Item {
-    int x0, y0, z0, t0, rhs;
-};
-
-// Item order (slowest to fastest): T chunk, block of up to `rb` right-hand sides, tile (panel
-// order), right-hand side within the block.  The CTAs in flight therefore work on the same few
-// tiles for rb right-hand sides at once: the links and S of a tile are fetched from HBM by the
-// first of them and are L2 hits for the others (a8: +384 B per extra RHS instead of +1536 B).
-template <class P> __device__ __forceinline__ Item decode_item(const TmaParams &prm, int item) {
-    const int ntiles = prm.ntx * prm.nty * prm.ntz;
-    const int per_chunk = ntiles * prm.nrhs;
-    const int chunk_rel = item / per_chunk;
-    const int chunk = chunk_rel + prm.chunk0;
-    int rem = item - chunk_rel * per_chunk;
-    const int blk = rem / (ntiles * prm.rb);
-    rem -= blk * ntiles * prm.rb;
-    const int rb_here = min(prm.rb, prm.nrhs - blk * prm.rb);
-    const int tile = rem / rb_here;
-    const int rhs = blk * prm.rb + (rem - tile * rb_here);
-    const int tpp = prm.ntx * prm.py * prm.pz;  // tiles per rasterisation panel
-    const int panel = tile / tpp;
-    int r = tile - panel * tpp;
-    const int tx = r % prm.ntx;
-    r /= prm.ntx;
-    const int tyi = r % prm.py, tzi = r / prm.py;
-    const int npy = prm.nty / prm.py;
-    Item it;
-    it.x0 = tx * P::BX;
-    it.y0 = ((panel % npy) * prm.py + tyi) * P::BY;
-    it.z0 = ((panel / npy) * prm.pz + tzi) * P::BZ;
-    it.t0 = chunk * prm.tchunk;
-    it.rhs = rhs;
-    return it;
-}
 
 // ---------------------------------------------------------------- the kernel
 template <class P>
@@ -223,31 +141,22 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
         tma_prefetch_desc(&maps.psi_x); tma_prefetch_desc(&maps.u_c);   tma_prefetch_desc(&maps.u_z);
         tma_prefetch_desc(&maps.u_y);   tma_prefetch_desc(&maps.u_x);   tma_prefetch_desc(&maps.s_c);
         const uint64_t pol_n = l2_policy_evict_normal();
-        const uint64_t pol_s = (prm.flags & 1) ? pol_n : l2_policy_evict_first();  // S is used exactly once
-        const uint64_t pol_u = (prm.flags & 2) ? l2_policy_evict_first() : pol_n;
-        const uint64_t pol_p = (prm.flags & 4) ? l2_policy_evict_last() : pol_n;
+        const uint64_t pol_s = WD_FLAG(prm, 1) ? pol_n : l2_policy_evict_first();  // S is used exactly once
+        const uint64_t pol_u = WD_FLAG(prm, 2) ? l2_policy_evict_first() : pol_n;
+        const uint64_t pol_p = WD_FLAG(prm, 4) ? l2_policy_evict_last() : pol_n;
         uint32_t nC = 0, nT = 0, nF = 0;  // fills issued so far of C, T, and of the per-step objects
         volatile int *mail = reinterpret_cast<volatile int *>(smem + P::OFF_MAIL);
-        const bool dynamic = !(prm.flags & 16);
         for (uint32_t seq = 0;; seq++) {
-            // next work item: atomic queue (fast SMs take more items; measured SM-to-SM spread of the
-            // streaming rate is ~20 %), handed to the consumers through a two-slot mailbox
-            int item = dynamic ? (int)atomicAdd(prm.sched, 1u) : (int)(blockIdx.x + seq * gridDim.x);
-            if (item >= prm.nitems) item = -1;
+            // next work item from the atomic queue, handed to the consumers through a two-slot mailbox
+            const int item = fetch_item(prm, seq);
             const uint32_t slot = seq & 1, mpar = (seq >> 1) & 1;
             mbar_wait(bar_empty + 8 * (OB_ITEM0 + slot), mpar ^ 1);
             mail[slot] = item;
             mbar_arrive(bar_full + 8 * (OB_ITEM0 + slot));
-            if (item < 0) {
-                if (dynamic && atomicAdd(prm.sched + 1, 1u) == gridDim.x - 1) {  // last CTA out re-arms the queue
-                    prm.sched[0] = 0;
-                    prm.sched[1] = 0;
-                }
-                break;
-            }
+            if (item < 0) break;
             const Item it = decode_item<P>(prm, item);
             const int cx = 2 * it.x0, y0 = it.y0, z0 = it.z0;  // dim-0 coordinates count doubles
-            const int pc = 12 * it.rhs;                        // first component of this right-hand side
+            const int pc = 12 * it.rhs0;                       // first component of this right-hand side
             const int zlo = (z0 == 0) ? Z - 1 : z0 - 1, zhi = (z0 + BZ == Z) ? 0 : z0 + BZ;
             const int ylo = (y0 == 0) ? Y - 1 : y0 - 1, yhi = (y0 + BY == Y) ? 0 : y0 + BY;
             const int cxlo = 2 * ((it.x0 == 0) ? X - 1 : it.x0 - 1), cxhi = 2 * ((it.x0 + BX == X) ? 0 : it.x0 + BX);
@@ -294,7 +203,7 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
                 mbar_arrive_expect_tx(bar_full + 8 * OB_C, P::SZ_C);
                 tma_load_5d_hint(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cx, y0, z0, t, pc, pol_p);
                 nC++;
-                if (full && (prm.flags & 8)) tma_prefetch_5d(&maps.psi_c, cx, y0, z0, (t + 1 == T) ? 0 : t + 1, pc);
+                if (full && WD_FLAG(prm, 8)) tma_prefetch_5d(&maps.psi_c, cx, y0, z0, (t + 1 == T) ? 0 : t + 1, pc);
                 if (full && CLOVER) {
                     const uint32_t pe = (nF & 1) ^ 1;
                     mbar_wait(bar_empty + 8 * OB_SA, pe);
@@ -335,7 +244,9 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
     const long long V = prm.Vs;  // component stride
     const long long strideT = (long long)Z * Y * X;
     uint32_t nC = 0, nT = 0, nF = 0;  // fills consumed so far
+#ifdef WD_EXPERIMENTS
     int ntrace = 0;
+#endif
     cd hprev[6];                      // rows 0,1 of (1 + gamma_T) psi(t-1)
     cd outp[12];                      // out(t-1) still missing its forward-T hop
 
@@ -348,7 +259,7 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
         if (item < 0) break;
         const Item it = decode_item<P>(prm, item);
         const long long site0 = ((long long)(it.z0 + lz) * Y + (it.y0 + ly)) * X + (it.x0 + lx);
-        cd *__restrict__ out = prm.out + (long long)it.rhs * 12 * V;
+        cd *__restrict__ out = prm.out + (long long)it.rhs0 * 12 * V;
         int t = (it.t0 == 0) ? T - 1 : it.t0 - 1;
         {   // prologue: seed the carried half-spinor from psi(t0-1)
             cd p[12];
@@ -367,11 +278,13 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
                 cd u[9];
                 mbar_wait(bar_full + 8 * OB_T, nT & 1);
                 mbar_wait(bar_full + 8 * OB_C, nC & 1);
+#ifdef WD_EXPERIMENTS
                 if (prm.trace && tid == 0 && ntrace < kTraceLen) {
                     unsigned long long now;
                     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
                     prm.trace[(size_t)blockIdx.x * kTraceLen + ntrace++] = now;
                 }
+#endif
 #pragma unroll
                 for (int k = 0; k < 9; k++) u[k] = lds(smem, P::OFF_T + own + k * NS);
 #pragma unroll
@@ -451,120 +364,9 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
 }
 
 // ---------------------------------------------------------------- host side
-static int sm_count() {  // of the current device
-    int dev = 0, n = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1)
-        n = 148;
-    return n;
-}
-
-// Work decomposition.  An item = (tile, T chunk); a CTA marches one item at a time and takes the
-// next from an atomic queue.  tchunk trades the tail (the last items finish unevenly) against the
-// per-item prologue/epilogue (one extra psi slice in, one extra psi + U_T slice at the end).
-// The panel (py x pz tiles, all of X) is the set of tiles in flight together: as cubic as possible, at most one wave, so that most face
-// re-reads are L2 hits on data a neighbouring CTA is streaming at the same time.
-template <class P> static void plan_items(const KParams &p, TmaParams &prm) {
-    const int nsm = sm_count();
-    prm.ntx = p.n[3] / P::BX;
-    prm.nty = p.n[2] / P::BY;
-    prm.ntz = p.n[1] / P::BZ;
-    const int ntiles = prm.ntx * prm.nty * prm.ntz, T = p.n[0];
-    int best_tc = T;
-    if (p.opt_tchunk > 0 && T % p.opt_tchunk == 0) {
-        best_tc = p.opt_tchunk;
-    } else {
-        double best = 1e300;
-        for (int tc = 1; tc <= T; tc++) {
-            if (T % tc) continue;
-            const long long items = (long long)ntiles * (T / tc) * p.nrhs;
-            // dynamic queue: work = items * (steps + prologue/epilogue) / SMs, plus an expected tail of half an item
-            const double cost = (double)items * (tc + 0.5) / nsm + 0.5 * (tc + 1);
-            if (cost < best * 0.999) best = cost, best_tc = tc;
-        }
-    }
-    prm.tchunk = best_tc;
-    prm.ntc = T / best_tc;
-    prm.nrhs = p.nrhs;
-    prm.rb = (p.nrhs < 4) ? p.nrhs : 4;  // RHS sharing the links of a tile through L2 (WD_TMA_RB: experiments)
-    if (const char *e = getenv("WD_TMA_RB")) {
-        const int v = atoi(e);
-        if (v >= 1) prm.rb = (v < p.nrhs) ? v : p.nrhs;
-    }
-    prm.chunk0 = (p.tc_count > 0) ? p.tc_begin : 0;
-    prm.nitems = ntiles * ((p.tc_count > 0) ? p.tc_count : prm.ntc) * p.nrhs;
-    const int wave = (nsm / prm.rb > 0) ? nsm / prm.rb : 1;  // tiles in flight together
-    int bpy = 1, bpz = 1;
-    double bscore = 1e300;
-    for (int py = 1; py <= prm.nty; py++) {
-        if (prm.nty % py) continue;
-        for (int pz = 1; pz <= prm.ntz; pz++) {
-            if (prm.ntz % pz) continue;
-            if (p.opt_zgroup > 0 && pz != p.opt_zgroup && prm.ntz % p.opt_zgroup == 0) continue;
-            const int tiles = prm.ntx * py * pz;
-            double score = 1.0 / (py * P::BY) + 1.0 / (pz * P::BZ);
-            if (tiles > wave) score += 10.0 * tiles / wave;  // over one wave: only if nothing smaller exists
-            if (score < bscore) bscore = score, bpy = py, bpz = pz;
-        }
-    }
-    prm.py = bpy;
-    prm.pz = bpz;
-}
-
 template <int BZ, int BY, int BX, int SELF> static cudaError_t launch_tma_self(const KParams &p, cudaStream_t st) {
     using P = Plan<BZ, BY, BX, SELF>;
-    static bool attr_done[64] = {};  // per device: the attribute belongs to the device's copy of the kernel
-    int dev_id = 0;
-    cudaGetDevice(&dev_id);
-    if (dev_id < 0 || dev_id >= 64 || !attr_done[dev_id]) {
-        cudaError_t e0 = cudaFuncSetAttribute(k_tma<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::SMEM);
-        if (e0 != cudaSuccess) return e0;
-        if (dev_id >= 0 && dev_id < 64) attr_done[dev_id] = true;
-    }
-    TmaMaps maps;
-    cudaError_t e;
-#define WD_ENC(m, base, nc, bx, by, bz, bc)                                      \
-    if ((e = encode_field_map(&maps.m, base, p.n, p.Vs, nc, bx, by, bz, bc)) != cudaSuccess) return e;
-    WD_ENC(psi_c, p.psi, 12 * p.nrhs, BX, BY, BZ, 12)
-    WD_ENC(psi_z, p.psi, 12 * p.nrhs, BX, BY, 1, 12)
-    WD_ENC(psi_y, p.psi, 12 * p.nrhs, BX, 1, BZ, 12)
-    WD_ENC(psi_x, p.psi, 12 * p.nrhs, 1, BY, BZ, 12)
-    WD_ENC(u_c, p.U, 36, BX, BY, BZ, 9)
-    WD_ENC(u_z, p.U, 36, BX, BY, 1, 9)
-    WD_ENC(u_y, p.U, 36, BX, 1, BZ, 9)
-    WD_ENC(u_x, p.U, 36, 1, BY, BZ, 9)
-    WD_ENC(s_c, (SELF == SELF_CLOVER) ? p.S : p.U, 36, BX, BY, BZ, 18)
-#undef WD_ENC
-    TmaParams prm;
-    prm.out = p.out;
-    prm.V = p.V;
-    prm.Vs = p.Vs;
-    for (int a = 0; a < 4; a++) prm.n[a] = p.n[a];
-    prm.mass = p.mass;
-    plan_items<P>(p, prm);
-    const int grid = (prm.nitems < sm_count()) ? prm.nitems : sm_count();
-    prm.trace = nullptr;
-    prm.sched = p.sched;
-    prm.flags = getenv("WD_TMA_FLAGS") ? atoi(getenv("WD_TMA_FLAGS")) : 0;
-    const char *trace_path = getenv("WD_TMA_TRACE");
-    if (trace_path) {
-        if ((e = cudaMalloc((void **)&prm.trace, (size_t)grid * kTraceLen * 8)) != cudaSuccess) return e;
-        cudaMemsetAsync(prm.trace, 0, (size_t)grid * kTraceLen * 8, st);
-    }
-    k_tma<P><<<grid, P::NTHREADS, P::SMEM, st>>>(maps, prm);
-    e = cudaGetLastError();
-    if (trace_path && e == cudaSuccess) {  // diagnostics only: synchronous dump of the last launch's step times
-        std::vector<unsigned long long> host((size_t)grid * kTraceLen);
-        cudaStreamSynchronize(st);
-        cudaMemcpy(host.data(), prm.trace, host.size() * 8, cudaMemcpyDeviceToHost);
-        if (FILE *f = fopen(trace_path, "wb")) {
-            const int hdr[4] = {grid, kTraceLen, prm.tchunk, prm.nitems};
-            fwrite(hdr, sizeof(int), 4, f);
-            fwrite(host.data(), 8, host.size(), f);
-            fclose(f);
-        }
-    }
-    if (prm.trace) cudaFree(prm.trace);
-    return e;
+    return launch_tma_kernel<P>(k_tma<P>, p, st, /*ucomp*/ 9, /*scomp*/ 18, CHUNK_COST_MODEL, /*rb*/ 4);
 }
 
 template <int BZ, int BY, int BX> static cudaError_t launch_tma(const KParams &p, int self, cudaStream_t st) {
@@ -574,5 +376,4 @@ template <int BZ, int BY, int BX> static cudaError_t launch_tma(const KParams &p
 }
 
 cudaError_t launch_tma_2x4x16(const KParams &p, int self, cudaStream_t st) { return launch_tma<2, 4, 16>(p, self, st); }
-cudaError_t launch_tma_4x4x8(const KParams &p, int self, cudaStream_t st) { return launch_tma<4, 4, 8>(p, self, st); }
 }  // namespace wd

@@ -17,11 +17,8 @@
 // clover term and tmb_* when there is none.
 #include <cstdio>
 #include <cstdlib>
-#include <vector>
 
-#include "wd_internal.h"
-#include "wd_math.cuh"
-#include "wd_tma.cuh"
+#include "wd_tma_common.cuh"
 #include "wd_smem_ops.cuh"
 
 namespace wd {
@@ -40,6 +37,7 @@ enum { OB_C = 0, OB_C1, OB_Z, OB_Y, OB_X, OB_R, OB_R1, OB_R2, OB_R3, OB_ITEM0, O
 
 template <int BZ_, int BY_, int BX_, int SELF_> struct Plan {
     static constexpr int BZ = BZ_, BY = BY_, BX = BX_, SELF = SELF_;
+    static constexpr int G = 1;              // right-hand sides per work item
     static constexpr int N = BZ * BY * BX;   // sites per tile = compute threads
     static constexpr int NW = N / 32;        // compute warps
     static constexpr int NTHREADS = N + 32;  // + the producer warp
@@ -65,65 +63,6 @@ template <int BZ_, int BY_, int BX_, int SELF_> struct Plan {
     static_assert(SMEM <= 232448, "shared-memory plan exceeds 227 KB");
 };
 
-struct TmaMaps {
-    CUtensorMap psi_c, psi_z, psi_y, psi_x;  // boxes: interior, z-face, y-face, x-face (12 components)
-    CUtensorMap u_c, u_z, u_y, u_x;          // same shapes, 9 components (one link)
-    CUtensorMap s_c;                         // interior box, 9 components (half of a 6x6 block)
-};
-
-struct TmaParams {
-    double2 *out;
-    long long V, Vs;     // sites, component stride
-    int n[4];
-    int ntx, nty, ntz;   // tiles per direction
-    int py, pz;          // rasterisation panel (in tiles); py | nty, pz | ntz
-    int tchunk, ntc;     // T steps per work item, items per tile
-    int nrhs, rb;        // right-hand sides in this launch; RHS per block of the item order
-    int chunk0;          // first T chunk of this launch (0 unless a T range was asked for)
-    int nitems;          // ntx*nty*ntz*(chunks of this launch)*nrhs
-    double mass;
-    int flags;           // WD_TMA_FLAGS (experiments; 0 = production): 1 S evict_normal instead of evict_first,
-                         // 2 U evict_first, 4 psi evict_last, 16 static round-robin items
-    unsigned int *sched; // [0] next item, [1] CTAs finished (dynamic work distribution; both 0 between launches)
-    unsigned long long *trace;  // diagnostics (WD_TMA_TRACE): [cta][kTraceLen] globaltimer per step, or null
-};
-constexpr int kTraceLen = 1024;
-
-struct Item {
-    int x0, y0, z0, t0, rhs;
-};
-
-// Item order (slowest to fastest): T chunk, block of up to `rb` right-hand sides, tile (panel
-// order), right-hand side within the block.  The CTAs in flight therefore work on the same few
-// tiles for rb right-hand sides at once: the links and S of a tile are fetched from HBM by the
-// first of them and are L2 hits for the others (a8: +384 B per extra RHS instead of +1536 B).
-template <class P> __device__ __forceinline__ Item decode_item(const TmaParams &prm, int item) {
-    const int ntiles = prm.ntx * prm.nty * prm.ntz;
-    const int per_chunk = ntiles * prm.nrhs;
-    const int chunk_rel = item / per_chunk;
-    const int chunk = chunk_rel + prm.chunk0;
-    int rem = item - chunk_rel * per_chunk;
-    const int blk = rem / (ntiles * prm.rb);
-    rem -= blk * ntiles * prm.rb;
-    const int rb_here = min(prm.rb, prm.nrhs - blk * prm.rb);
-    const int tile = rem / rb_here;
-    const int rhs = blk * prm.rb + (rem - tile * rb_here);
-    const int tpp = prm.ntx * prm.py * prm.pz;  // tiles per rasterisation panel
-    const int panel = tile / tpp;
-    int r = tile - panel * tpp;
-    const int tx = r % prm.ntx;
-    r /= prm.ntx;
-    const int tyi = r % prm.py, tzi = r / prm.py;
-    const int npy = prm.nty / prm.py;
-    Item it;
-    it.x0 = tx * P::BX;
-    it.y0 = ((panel % npy) * prm.py + tyi) * P::BY;
-    it.z0 = ((panel / npy) * prm.pz + tzi) * P::BZ;
-    it.t0 = chunk * prm.tchunk;
-    it.rhs = rhs;
-    return it;
-}
-
 // ---------------------------------------------------------------- the producer (one thread)
 // A resumable state machine: advance() performs the next load of the fixed sequence if the buffer it
 // targets has been released, else returns false.  Sequence per work item:
@@ -143,9 +82,9 @@ template <class P> struct Producer {
         tma_prefetch_desc(&maps.psi_x); tma_prefetch_desc(&maps.u_c);   tma_prefetch_desc(&maps.u_z);
         tma_prefetch_desc(&maps.u_y);   tma_prefetch_desc(&maps.u_x);   tma_prefetch_desc(&maps.s_c);
         pol_n = l2_policy_evict_normal();
-        pol_s = (prm.flags & 1) ? pol_n : l2_policy_evict_first();  // S is used exactly once
-        pol_u = (prm.flags & 2) ? l2_policy_evict_first() : pol_n;
-        pol_p = (prm.flags & 4) ? l2_policy_evict_last() : pol_n;
+        pol_s = WD_FLAG(prm, 1) ? pol_n : l2_policy_evict_first();  // S is used exactly once
+        pol_u = WD_FLAG(prm, 2) ? l2_policy_evict_first() : pol_n;
+        pol_p = WD_FLAG(prm, 4) ? l2_policy_evict_last() : pol_n;
         nC = nR = nF = seq = 0;
         stage = ST_FETCH;
         j = t = 0;
@@ -181,28 +120,21 @@ template <class P> struct Producer {
         const uint32_t pe = (nF & 1) ^ 1;
         switch (stage) {
         case ST_FETCH: {
-            // next work item: atomic queue (fast SMs take more items; measured SM-to-SM spread of the
-            // streaming rate is ~20 %), handed to the consumers through a two-slot mailbox
+            // next work item from the atomic queue, handed to the consumers through a two-slot mailbox
             const uint32_t slot = seq & 1, mpar = (seq >> 1) & 1;
             if (!mbar_try_wait(bar_empty + 8 * (OB_ITEM0 + slot), mpar ^ 1)) return false;
-            const bool dynamic = !(prm.flags & 16);
-            int item = dynamic ? (int)atomicAdd(prm.sched, 1u) : (int)(blockIdx.x + seq * gridDim.x);
-            if (item >= prm.nitems) item = -1;
+            const int item = fetch_item(prm, seq);
             reinterpret_cast<volatile int *>(smem + P::OFF_MAIL)[slot] = item;
             mbar_arrive(bar_full + 8 * (OB_ITEM0 + slot));
             seq++;
             if (item < 0) {
-                if (dynamic && atomicAdd(prm.sched + 1, 1u) == gridDim.x - 1) {  // last CTA out re-arms the queue
-                    prm.sched[0] = 0;
-                    prm.sched[1] = 0;
-                }
                 done = true;
                 return false;
             }
             const Item it = decode_item<P>(prm, item);
             const int Z = prm.n[1], Y = prm.n[2], X = prm.n[3];
             cx = 2 * it.x0, y0 = it.y0, z0 = it.z0;  // dim-0 coordinates count doubles
-            pc = 12 * it.rhs;                        // first component of this right-hand side
+            pc = 12 * it.rhs0;                       // first component of this right-hand side
             zlo = (z0 == 0) ? Z - 1 : z0 - 1, zhi = (z0 + BZ == Z) ? 0 : z0 + BZ;
             ylo = (y0 == 0) ? Y - 1 : y0 - 1, yhi = (y0 + BY == Y) ? 0 : y0 + BY;
             cxlo = 2 * ((it.x0 == 0) ? X - 1 : it.x0 - 1), cxhi = 2 * ((it.x0 + BX == X) ? 0 : it.x0 + BX);
@@ -343,7 +275,9 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
     const long long V = prm.Vs;  // component stride
     const long long strideT = (long long)Z * Y * X;
     uint32_t nC = 0, nR = 0, nF = 0;  // fills consumed so far: C buffers, ring slots, per-step objects
+#ifdef WD_EXPERIMENTS
     int ntrace = 0;
+#endif
     cd acc[12];
 
     // own-site psi of C fill n, rows r0..r0+5 scaled by s
@@ -377,7 +311,7 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
         if (item < 0) break;
         const Item it = decode_item<P>(prm, item);
         const long long site0 = ((long long)(it.z0 + lz) * Y + (it.y0 + ly)) * X + (it.x0 + lx);
-        cd *__restrict__ out = prm.out + (long long)it.rhs * 12 * V;
+        cd *__restrict__ out = prm.out + (long long)it.rhs0 * 12 * V;
         int t = it.t0;
         {   // prologue: acc = backward-T hop of slice t0, (1 + gamma_T) U_T(t0-1)^H psi(t0-1)
             const uint32_t cb = (nC & 1) ? P::SZ_C : 0, slot = nR & 3;
@@ -425,11 +359,13 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
                 const uint32_t cn = cb ^ P::SZ_C, slot = nR & 3;  // psi(t+1) is in the other C buffer
                 wait_full(OB_C + ((nC + 1) & 1), ((nC + 1) >> 1) & 1);
                 wait_full(OB_R + slot, (nR >> 2) & 1);
+#ifdef WD_EXPERIMENTS
                 if (prm.trace && tid == 0 && ntrace < kTraceLen) {
                     unsigned long long now;
                     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
                     prm.trace[(size_t)blockIdx.x * kTraceLen + ntrace++] = now;
                 }
+#endif
                 cd u[9], p[12];
 #pragma unroll
                 for (int k = 0; k < 9; k++) u[k] = lds(smem, P::OFF_R + slot * P::SZ_U + own + k * NS);
@@ -470,119 +406,12 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
 }
 
 // ---------------------------------------------------------------- host side
-static int sm_count() {  // of the current device
-    int dev = 0, n = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1)
-        n = 148;
-    return n;
-}
-
-// Work decomposition.  An item = (tile, T chunk); a CTA marches one item at a time and takes the
-// next from an atomic queue.  tchunk trades the tail (the last items finish unevenly) against the
-// per-item prologue/epilogue (one extra psi slice in, one extra psi + U_T slice at the end).
-// The panel (py x pz tiles, all of X) is the set of tiles in flight together: as cubic as possible, at most one wave, so that most face
-// re-reads are L2 hits on data a neighbouring CTA is streaming at the same time.
-template <class P> static void plan_items(const KParams &p, TmaParams &prm) {
-    const int nsm = sm_count();
-    prm.ntx = p.n[3] / P::BX;
-    prm.nty = p.n[2] / P::BY;
-    prm.ntz = p.n[1] / P::BZ;
-    const int ntiles = prm.ntx * prm.nty * prm.ntz, T = p.n[0];
-    int best_tc = T;
-    if (p.opt_tchunk > 0 && T % p.opt_tchunk == 0) {
-        best_tc = p.opt_tchunk;
-    } else {
-        // Short chunks keep the CTAs of a panel within a few steps of each other (each item starts at a chunk
-        // boundary), which is what makes the face re-reads L2 hits; the price is one extra psi and U_T slice per
-        // item.  Measured at 64^4: tchunk 8 and 16 beat 32 and 64 by 3-7 %.  Largest divisor of T up to 16.
-        best_tc = 1;
-        for (int tc = 1; tc <= T && tc <= 16; tc++)
-            if (T % tc == 0) best_tc = tc;
-        if (best_tc < 4 && T > 16) best_tc = T;  // T without a small divisor: one chunk
-    }
-    prm.tchunk = best_tc;
-    prm.ntc = T / best_tc;
-    prm.nrhs = p.nrhs;
-    prm.rb = (p.nrhs < 4) ? p.nrhs : 4;  // RHS sharing the links of a tile through L2 (WD_TMA_RB: experiments)
-    if (const char *e = getenv("WD_TMA_RB")) {
-        const int v = atoi(e);
-        if (v >= 1) prm.rb = (v < p.nrhs) ? v : p.nrhs;
-    }
-    prm.chunk0 = (p.tc_count > 0) ? p.tc_begin : 0;
-    prm.nitems = ntiles * ((p.tc_count > 0) ? p.tc_count : prm.ntc) * p.nrhs;
-    const int wave = (nsm / prm.rb > 0) ? nsm / prm.rb : 1;  // tiles in flight together
-    int bpy = 1, bpz = 1;
-    double bscore = 1e300;
-    for (int py = 1; py <= prm.nty; py++) {
-        if (prm.nty % py) continue;
-        for (int pz = 1; pz <= prm.ntz; pz++) {
-            if (prm.ntz % pz) continue;
-            if (p.opt_zgroup > 0 && pz != p.opt_zgroup && prm.ntz % p.opt_zgroup == 0) continue;
-            const int tiles = prm.ntx * py * pz;
-            double score = 1.0 / (py * P::BY) + 1.0 / (pz * P::BZ);
-            if (tiles > wave) score += 10.0 * tiles / wave;  // over one wave: only if nothing smaller exists
-            if (score < bscore) bscore = score, bpy = py, bpz = pz;
-        }
-    }
-    prm.py = bpy;
-    prm.pz = bpz;
-}
-
+// Short chunks keep the CTAs of a panel within a few steps of each other (each item starts at a chunk boundary),
+// which is what makes the face re-reads L2 hits; the price is one extra psi and U_T slice per item.  Measured at
+// 64^4: tchunk 8 and 16 beat 32 and 64 by 3-7 % (CHUNK_SHORT).
 template <int BZ, int BY, int BX, int SELF> static cudaError_t launch_tma_self(const KParams &p, cudaStream_t st) {
     using P = Plan<BZ, BY, BX, SELF>;
-    static bool attr_done[64] = {};  // per device: the attribute belongs to the device's copy of the kernel
-    int dev_id = 0;
-    cudaGetDevice(&dev_id);
-    if (dev_id < 0 || dev_id >= 64 || !attr_done[dev_id]) {
-        cudaError_t e0 = cudaFuncSetAttribute(k_tma<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::SMEM);
-        if (e0 != cudaSuccess) return e0;
-        if (dev_id >= 0 && dev_id < 64) attr_done[dev_id] = true;
-    }
-    TmaMaps maps;
-    cudaError_t e;
-#define WD_ENC(m, base, nc, bx, by, bz, bc)                                      \
-    if ((e = encode_field_map(&maps.m, base, p.n, p.Vs, nc, bx, by, bz, bc)) != cudaSuccess) return e;
-    WD_ENC(psi_c, p.psi, 12 * p.nrhs, BX, BY, BZ, 12)
-    WD_ENC(psi_z, p.psi, 12 * p.nrhs, BX, BY, 1, 12)
-    WD_ENC(psi_y, p.psi, 12 * p.nrhs, BX, 1, BZ, 12)
-    WD_ENC(psi_x, p.psi, 12 * p.nrhs, 1, BY, BZ, 12)
-    WD_ENC(u_c, p.U, 36, BX, BY, BZ, 9)
-    WD_ENC(u_z, p.U, 36, BX, BY, 1, 9)
-    WD_ENC(u_y, p.U, 36, BX, 1, BZ, 9)
-    WD_ENC(u_x, p.U, 36, 1, BY, BZ, 9)
-    WD_ENC(s_c, (SELF == SELF_CLOVER) ? p.S : p.U, 36, BX, BY, BZ, 9)
-#undef WD_ENC
-    TmaParams prm;
-    prm.out = p.out;
-    prm.V = p.V;
-    prm.Vs = p.Vs;
-    for (int a = 0; a < 4; a++) prm.n[a] = p.n[a];
-    prm.mass = p.mass;
-    plan_items<P>(p, prm);
-    const int grid = (prm.nitems < sm_count()) ? prm.nitems : sm_count();
-    prm.trace = nullptr;
-    prm.sched = p.sched;
-    prm.flags = getenv("WD_TMA_FLAGS") ? atoi(getenv("WD_TMA_FLAGS")) : 0;
-    const char *trace_path = getenv("WD_TMA_TRACE");
-    if (trace_path) {
-        if ((e = cudaMalloc((void **)&prm.trace, (size_t)grid * kTraceLen * 8)) != cudaSuccess) return e;
-        cudaMemsetAsync(prm.trace, 0, (size_t)grid * kTraceLen * 8, st);
-    }
-    k_tma<P><<<grid, P::NTHREADS, P::SMEM, st>>>(maps, prm);
-    e = cudaGetLastError();
-    if (trace_path && e == cudaSuccess) {  // diagnostics only: synchronous dump of the last launch's step times
-        std::vector<unsigned long long> host((size_t)grid * kTraceLen);
-        cudaStreamSynchronize(st);
-        cudaMemcpy(host.data(), prm.trace, host.size() * 8, cudaMemcpyDeviceToHost);
-        if (FILE *f = fopen(trace_path, "wb")) {
-            const int hdr[4] = {grid, kTraceLen, prm.tchunk, prm.nitems};
-            fwrite(hdr, sizeof(int), 4, f);
-            fwrite(host.data(), 8, host.size(), f);
-            fclose(f);
-        }
-    }
-    if (prm.trace) cudaFree(prm.trace);
-    return e;
+    return launch_tma_kernel<P>(k_tma<P>, p, st, /*ucomp*/ 9, /*scomp*/ 9, CHUNK_SHORT, /*rb*/ 4);
 }
 
 template <int BZ, int BY, int BX> static cudaError_t launch_tma(const KParams &p, int self, cudaStream_t st) {
@@ -590,10 +419,9 @@ template <int BZ, int BY, int BX> static cudaError_t launch_tma(const KParams &p
     if (self == SELF_MASS) return launch_tma_self<BZ, BY, BX, SELF_MASS>(p, st);
     return launch_tma_self<BZ, BY, BX, SELF_NONE>(p, st);
 }
-
-// Tiles of 128 sites whose shared-memory plan fits 227 KB (2x4x16 is 816 B too large)
 }  // namespace tmb
 
+// Tiles of 128 sites whose shared-memory plan fits 227 KB (2x4x16 is 816 B too large)
 cudaError_t launch_tmb_4x4x8(const KParams &p, int self, cudaStream_t st) { return tmb::launch_tma<4, 4, 8>(p, self, st); }
 cudaError_t launch_tmb_2x8x8(const KParams &p, int self, cudaStream_t st) { return tmb::launch_tma<2, 8, 8>(p, self, st); }
 }  // namespace wd

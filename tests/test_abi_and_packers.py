@@ -14,10 +14,26 @@ import wdinputs
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def declared_functions():
-    text = open(os.path.join(ROOT, "include", "wd.h")).read()
+def declared_functions(header="wd.h", prefix="wd_"):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(wd_[a-z_0-9]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(" + prefix + r"[a-z_0-9]+)\s*\(", text)))
+
+
+def test_every_header_under_include_is_covered():
+    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["wd.h", "wd_bench.h"]
+
+
+def test_bench_library_exports_every_declared_symbol_and_is_not_the_product():
+    from paper_2407_00041_b200 import benchlib
+
+    names = declared_functions("wd_bench.h", "wdb_")
+    assert names == sorted(benchlib.SIGNATURES) and len(names) >= 2
+    B = ctypes.CDLL(benchlib.LIB_PATH)
+    L = ctypes.CDLL(wd.LIB_PATH)
+    for n in names:
+        assert hasattr(B, n), f"libwdbench.so does not export {n}"
+        assert not hasattr(L, n), f"libwd.so must not export the bench helper {n}"
 
 
 def test_library_exports_every_declared_symbol():

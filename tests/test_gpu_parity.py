@@ -124,7 +124,7 @@ def test_every_kernel_geometry_and_variant(torch, dims):
     ref_c = oracle.apply(dims, m0, U, C, psi)
     ref_w = oracle.apply(dims, m0, U, None, psi)
     kids = kernels_fitting(dims)
-    assert len(kids) >= 6
+    assert len(kids) >= 5
     for kid in kids:
         for variant in (0, 1):
             with Op(torch, dims, m0, csw, U, C, kernel=kid, variant=variant) as op:
@@ -143,7 +143,7 @@ def test_tiled_rasterisation_parameters(torch, tchunk, zgroup):
     psi = wdinputs.spinor(dims, 312)
     C = oracle.build_clover(dims, m0, 1.0, U)
     ref = oracle.apply(dims, m0, U, C, psi)
-    for name in ("tile_1x4x4x16", "tile_2x4x4x8", "tile_1x4x4x8"):
+    for name in ("tile_1x4x4x16", "tile_2x4x4x4"):
         if tchunk == 1 and name.startswith("tile_2"):
             continue
         with Op(torch, dims, m0, 1.0, U, C, kernel=wd.kernel_id(name), tchunk=tchunk, zgroup=zgroup) as op:
@@ -164,7 +164,7 @@ def test_ragged_and_degenerate_extents(torch, dims):
         assert wd.wd_kernel_name(wd.wd_kernel_in_use(op.h)).startswith("linear") or all(
             n % 4 == 0 for n in dims)
         assert rel_l2(op.apply(psi), ref) <= TOL
-    with Op(torch, dims, m0, 0.0, U, kernel=1) as op:
+    with Op(torch, dims, m0, 0.0, U, kernel=0) as op:
         assert rel_l2(op.apply(psi), oracle.apply(dims, m0, U, None, psi)) <= TOL
 
 
@@ -303,69 +303,137 @@ def test_cfg3_32x32x32x32_first_apply_and_repeatability(torch):
             assert rel_l2(op.apply(psi), ref) <= TOL, wd.wd_kernel_name(kid)
 
 
+# ---------------------------------------------------------------- R11, state handling
+def gauge_gaussian(dims, seed):
+    """General 3x3 complex links, NOT unitary (R11; as tests/test_oracle_pins.py P2): Re, Im ~ N(0, 1/2)."""
+    V = wdinputs.volume(dims)
+    return (wdinputs.gaussian(V * 72, seed) * 0.5).reshape(V, 4, 3, 3, 2)
+
+
+@pytest.mark.parametrize("dims", [(4, 4, 8, 16), (3, 5, 6, 7)])
+def test_non_unitary_links(torch, dims):
+    """wd.h promises "general 3x3 complex" links (U and U^H are used, never U^-1): every kernel that fits, clover built
+    on the device from those links and by the oracle, one and several right-hand sides."""
+    m0, csw, nrhs = -0.4, 1.0, 3
+    U = gauge_gaussian(dims, 381)
+    psi = wdinputs.spinor(dims, 382, nrhs=nrhs)
+    C = oracle.build_clover(dims, m0, csw, U)
+    ref_c = oracle.apply(dims, m0, U, C, psi)
+    ref_w = oracle.apply(dims, m0, U, None, psi)
+    for kid in kernels_fitting(dims):
+        with Op(torch, dims, m0, csw, U, build_clover=True, kernel=kid) as op:
+            Cdev = np.empty_like(C)
+            wd.wd_get_clover(op.h, Cdev)
+            assert rel_l2(Cdev, C) <= TOL
+            assert rel_l2(op.apply(psi, nrhs), ref_c) <= TOL, wd.wd_kernel_name(kid)
+        with Op(torch, dims, m0, 0.0, U, kernel=kid) as op:
+            assert rel_l2(op.apply(psi, nrhs), ref_w) <= TOL, wd.wd_kernel_name(kid)
+
+
+def test_load_clover_on_a_csw0_handle(torch):
+    """wd.h: wd_load_clover is allowed with csw == 0; the loaded S then replaces (m0+4) I."""
+    dims, m0 = (4, 4, 8, 16), -0.4
+    U = wdinputs.gauge_haar(dims, 385)
+    psi = wdinputs.spinor(dims, 386)
+    C = wdinputs.selfcoupling_random(dims, 387)
+    with Op(torch, dims, m0, 0.0, U) as op:
+        assert rel_l2(op.apply(psi), oracle.apply(dims, m0, U, None, psi)) <= TOL
+        wd.wd_load_clover(op.h, C)
+        assert rel_l2(op.apply(psi), oracle.apply(dims, m0, U, C, psi)) <= TOL
+        assert rel_l2(op.apply(np.concatenate([psi, psi]), 2)[1], oracle.apply(dims, m0, U, C, psi)[0]) <= TOL
+
+
+def test_reloading_the_gauge_field_invalidates_a_built_clover(torch):
+    """A second wd_load_gauge must not leave S built from the previous links in use."""
+    dims, m0, csw = (4, 4, 8, 16), -0.4, 1.0
+    U1, U2 = wdinputs.gauge_haar(dims, 391), wdinputs.gauge_haar(dims, 392)
+    psi = wdinputs.spinor(dims, 393)
+    with Op(torch, dims, m0, csw, U1, build_clover=True) as op:
+        ref1 = oracle.apply(dims, m0, U1, oracle.build_clover(dims, m0, csw, U1), psi)
+        assert rel_l2(op.apply(psi), ref1) <= TOL
+        wd.wd_load_gauge(op.h, U2)
+        with pytest.raises(wd.WDError) as e:
+            op.apply(psi)
+        assert e.value.code == wd.WD_ESTATE
+        wd.wd_build_clover(op.h)
+        C2 = oracle.build_clover(dims, m0, csw, U2)
+        assert rel_l2(op.apply(psi), oracle.apply(dims, m0, U2, C2, psi)) <= TOL
+        # a field the caller supplied is the caller's: it survives a new gauge field
+        wd.wd_load_clover(op.h, C2)
+        wd.wd_load_gauge(op.h, U1)
+        assert rel_l2(op.apply(psi), oracle.apply(dims, m0, U1, C2, psi)) <= TOL
+
+
 # ---------------------------------------------------------------- full size, bench configuration
-def _full_size_dims():
+def _require_memory(torch, host_gb, dev_gb, what):
+    """The full-size tests never shrink silently: WD_TEST_SMALL=1 asks for the reduced size explicitly (and the
+    test says so in its output); otherwise too little memory is a FAILURE, not a fallback."""
     import psutil
 
-    free_host = psutil.virtual_memory().available
-    return (64, 64, 64, 64) if free_host > 40e9 and not os.environ.get("WD_TEST_SMALL") else (32, 32, 32, 64)
+    if os.environ.get("WD_TEST_SMALL"):
+        return False
+    free_host, free_dev = psutil.virtual_memory().available, torch.cuda.mem_get_info()[0]
+    if free_host < host_gb * 1e9 or free_dev < dev_gb * 1e9:
+        pytest.fail(f"{what}: needs {host_gb} GB of host and {dev_gb} GB of device memory, found "
+                    f"{free_host / 1e9:.0f} / {free_dev / 1e9:.0f} GB (set WD_TEST_SMALL=1 to run the reduced size)")
+    return True
 
 
-def test_cfg4_full_size_sampled_outputs(torch):
-    """64^4 Wilson-clover in the launch configuration bench.py times (automatic kernel, S built on
-    the device), checked on sampled sites the oracle computes one by one from (U, psi) alone."""
+def _report(capsys, text):
+    with capsys.disabled():
+        print("\n[full-size parity] " + text, flush=True)
+
+
+def test_cfg4_full_size_whole_lattice(torch, capsys):
+    """64^4 Wilson-clover in the launch configuration bench.py times (automatic kernel, S built on the device,
+    device-side pack), compared with the oracle on EVERY site: rel. L2 and the worst component."""
     cfg = wdinputs.CONFIGS[4]
-    dims = _full_size_dims()
-    if torch.cuda.mem_get_info()[0] < 40e9:
-        dims = (32, 32, 32, 64)
-    V = wdinputs.volume(dims)
-    U = wdinputs.gauge_haar(dims, cfg["gauge"][1])
+    full = _require_memory(torch, 45, 40, "cfg 4 (64^4)")
+    dims = cfg["dims"] if full else (32, 32, 32, 64)
+    U = wdinputs.config_gauge(cfg, dims)
     psi = wdinputs.spinor(dims, cfg["spinor_seed"])
-    rng = np.random.default_rng(4)
-    T, Z, Y, X = dims
-    corners = [0, V - 1, X - 1, X, Y * X - 1, Z * Y * X - 1, Z * Y * X, (T - 1) * Z * Y * X, V - X, V // 2, V // 2 + X - 1]
-    sites = np.unique(np.concatenate([np.array(corners), rng.integers(0, V, size=4000)])).astype(np.int64)
-    ref = oracle.apply_sites(dims, cfg["m0"], cfg["csw"], U, psi[0], sites)
     with Op(torch, dims, cfg["m0"], cfg["csw"], U, build_clover=True, device_pack=1) as op:
-        del U
-        out = op.apply(psi)[0]
-        assert np.isfinite(out).all()
-        assert rel_l2(out[sites], ref) <= TOL
-        worst = np.abs(out[sites] - ref).max() / np.abs(ref).max()
-        assert worst <= 1e-13
+        kname = wd.wd_kernel_name(wd.wd_kernel_in_use(op.h))
+        out = op.apply(psi)
+    C = oracle.build_clover(dims, cfg["m0"], cfg["csw"], U)
+    ref = oracle.apply(dims, cfg["m0"], U, C, psi)
+    del U, C
+    assert np.isfinite(out).all()
+    err = rel_l2(out, ref)
+    worst = float(np.abs(out - ref).max() / np.abs(ref).max())
+    _report(capsys, f"lattice {'x'.join(map(str, dims))} nrhs 1 kernel {kname}: {out.size // 24} sites compared, "
+                    f"rel_l2 {err:.3e}, worst component {worst:.3e}" + ("" if full else "  (WD_TEST_SMALL)"))
+    assert err <= TOL and worst <= 1e-13
 
 
-def test_cfg5_full_size_multi_rhs_sampled_outputs(torch):
-    """48^3 x 96 Wilson-clover with 12 right-hand sides in ONE wd_apply (the launch configuration bench.py
-    --config 5 times: automatic kernel, RHS-blocked item order, S built on the device), checked on sampled
-    sites of every right-hand side that the oracle computes one by one from (U, psi_r) alone.  The host
-    streams one RHS at a time through the oracle."""
-    import psutil
-
+def test_cfg5_full_size_multi_rhs_whole_lattice(torch, capsys):
+    """48^3 x 96 Wilson-clover with 12 right-hand sides in ONE wd_apply (the launch configuration bench.py --config 5
+    times: automatic kernel, S built on the device), EVERY right-hand side compared with the oracle on EVERY site.
+    The host streams one right-hand side at a time through the oracle."""
     cfg = wdinputs.CONFIGS[5]
-    dims, nrhs = cfg["dims"], cfg["nrhs"]
-    if psutil.virtual_memory().available < 80e9 or torch.cuda.mem_get_info()[0] < 80e9 or os.environ.get("WD_TEST_SMALL"):
-        dims, nrhs = (24, 16, 16, 48), 5
+    full = _require_memory(torch, 30, 80, "cfg 5 (48^3 x 96, 12 RHS)")
+    dims, nrhs = (cfg["dims"], cfg["nrhs"]) if full else ((24, 16, 16, 48), 5)
     V = wdinputs.volume(dims)
-    T, Z, Y, X = dims
-    U = wdinputs.gauge_haar(dims, cfg["gauge"][1])
-    rng = np.random.default_rng(5)
-    corners = [0, V - 1, X - 1, X, Y * X - 1, Z * Y * X - 1, Z * Y * X, (T - 1) * Z * Y * X, V - X, V // 2]
-    sites = np.unique(np.concatenate([np.array(corners), rng.integers(0, V, size=600)])).astype(np.int64)
+    U = wdinputs.config_gauge(cfg, dims)
     with Op(torch, dims, cfg["m0"], cfg["csw"], U, build_clover=True, device_pack=1) as op:
+        kname = wd.wd_kernel_name(wd.wd_kernel_for(op.h, nrhs))
         Vs = wd.wd_component_stride(op.h)
         din, dout = op.dev_spinor(nrhs), op.dev_spinor(nrhs)
         dout.fill_(float("nan"))
-        refs = []
-        for r in range(nrhs):  # one RHS at a time: generate, pack into its slot, keep only the sampled reference
-            psi_r = wdinputs.spinor(dims, cfg["spinor_seed"] + r)
-            wd.wd_pack_spinor(op.h, din[r * 24 * Vs:(r + 1) * 24 * Vs], psi_r, 1)
-            refs.append(oracle.apply_sites(dims, cfg["m0"], cfg["csw"], U, psi_r[0], sites))
-            del psi_r
+        for r in range(nrhs):  # one RHS at a time: generate, pack into its slot
+            wd.wd_pack_spinor(op.h, din[r * 24 * Vs:(r + 1) * 24 * Vs], wdinputs.spinor(dims, cfg["spinor_seed"] + r), 1)
         wd.wd_apply(op.h, dout, din, nrhs)
         wd.wd_synchronize(op.h)
+        C = oracle.build_clover(dims, cfg["m0"], cfg["csw"], U)
         out_r = np.empty((1, V, 12, 2))
+        errs, worsts = [], []
         for r in range(nrhs):
+            psi_r = wdinputs.spinor(dims, cfg["spinor_seed"] + r)
+            ref = oracle.apply(dims, cfg["m0"], U, C, psi_r)
             wd.wd_unpack_spinor(op.h, out_r, dout[r * 24 * Vs:(r + 1) * 24 * Vs], 1)
             assert np.isfinite(out_r).all(), r
-            assert rel_l2(out_r[0][sites], refs[r]) <= TOL, r
+            errs.append(rel_l2(out_r, ref))
+            worsts.append(float(np.abs(out_r - ref).max() / np.abs(ref).max()))
+    _report(capsys, f"lattice {'x'.join(map(str, dims))} x{nrhs} kernel {kname}: {nrhs} x {V} sites compared, "
+                    f"max rel_l2 {max(errs):.3e}, worst component {max(worsts):.3e}" + ("" if full else "  (WD_TEST_SMALL)"))
+    assert max(errs) <= TOL and max(worsts) <= 1e-13

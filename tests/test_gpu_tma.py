@@ -23,7 +23,7 @@ def tma_kernels(dims):
     out = []
     for k in range(wd.wd_kernel_count()):
         name = wd.wd_kernel_name(k)
-        if name.startswith(("tma_", "tmb_", "tmr")):
+        if name.startswith(("tma_", "tmb_", "tmc_")):
             b = [int(v) for v in name.split("_")[1].split("x")]
             if all(n % t == 0 for n, t in zip(dims[-3:], b)):
                 out.append(k)
@@ -80,17 +80,17 @@ def test_tma_many_items_per_cta_and_multi_rhs(torch):
             assert rel_l2(op.apply(psi, nrhs), ref) <= TOL, wd.wd_kernel_name(kid)
 
 
-@pytest.mark.parametrize("nrhs", [2, 5, 7])
-def test_multi_rhs_groups_share_links(torch, nrhs):
-    """tmr kernels: G right-hand sides of a tile are processed by G thread groups that share U and S in shared
-    memory; nrhs that is not a multiple of G leaves groups without a right-hand side in the last block."""
-    dims, m0, csw = (6, 4, 8, 16), -0.4, 1.0
+@pytest.mark.parametrize("nrhs", [1, 2, 5, 7])
+def test_multi_rhs_two_per_thread(torch, nrhs):
+    """tmc kernels: every thread handles two right-hand sides with the links and S in registers; an odd nrhs leaves
+    the last unit with one right-hand side (computed twice, stored once)."""
+    dims, m0, csw = (6, 4, 8, 32), -0.4, 1.0
     U = wdinputs.gauge_haar(dims, 431)
     psi = wdinputs.spinor(dims, 432, nrhs=nrhs)
     C = wdinputs.selfcoupling_random(dims, 433)
     ref_c = oracle.apply(dims, m0, U, C, psi)
     ref_w = oracle.apply(dims, m0, U, None, psi)
-    kids = [k for k in tma_kernels(dims) if wd.wd_kernel_name(k).startswith("tmr")]
+    kids = [k for k in tma_kernels(dims) if wd.wd_kernel_name(k).startswith("tmc")]
     assert kids
     for kid in kids:
         for tchunk in (0, 2):
@@ -106,8 +106,6 @@ def test_multi_rhs_groups_share_links(torch, nrhs):
 def test_apply_host_pipelined_over_t_chunks(torch, dims, csw):
     """wd_apply_host with a TMA kernel cuts the lattice into T chunks and overlaps upload, compute and download;
     each chunk is a launch restricted to a T range.  Against the oracle, and bit for bit against the serial path."""
-    import os
-
     m0, nrhs = -0.4, 2
     U = wdinputs.gauge_haar(dims, 441)
     psi = wdinputs.spinor(dims, 442, nrhs=nrhs)
@@ -122,12 +120,10 @@ def test_apply_host_pipelined_over_t_chunks(torch, dims, csw):
         pin_out = torch.empty_like(pin_in).pin_memory()
         wd.wd_apply_host(op.h, pin_out, pin_in, nrhs)
         assert np.array_equal(pin_out.numpy(), out)
-        os.environ["WD_HOST_SERIAL"] = "1"
-        try:
-            ser = np.empty_like(psi)
-            wd.wd_apply_host(op.h, ser, psi, nrhs)
-        finally:
-            del os.environ["WD_HOST_SERIAL"]
+        wd.wd_set_option(op.h, wd.WD_OPT_HOST_PIPELINE, 0)
+        ser = np.empty_like(psi)
+        wd.wd_apply_host(op.h, ser, psi, nrhs)
+        wd.wd_set_option(op.h, wd.WD_OPT_HOST_PIPELINE, 1)
         assert np.array_equal(ser, out)
         # the device path is untouched by the extra streams
         assert rel_l2(op.apply(psi, nrhs), ref) <= TOL
