@@ -51,6 +51,11 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-ceilings", action="store_true", help="skip the streaming / FP64 ceiling microbenchmarks")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--parallel", default="dd", choices=["dd", "replicas"],
+                    help="N > 1: dd = ONE lattice cut over the ranks, half-spinor faces exchanged with NCCL send/recv "
+                         "(strong scaling, default); replicas = N independent copies (weak)")
+    ap.add_argument("--gmres", type=int, default=0, metavar="M",
+                    help="also run restarted GMRES(M) on the device (wd_gmres) and report its timing")
     ap.add_argument("--graph", action="store_true",
                     help="also time the K steps captured as ONE CUDA graph (cfg 3: 100 back-to-back applies)")
     return ap.parse_args()
@@ -266,6 +271,90 @@ def reduce_over_ranks(total_ms, units, dist=None, device="cpu"):
     return float(t.item()), int(u.item())
 
 
+def run_dd(args, torch, dist, world, rank, local):
+    """N > 1, --parallel dd: ONE lattice of the configured size cut into `world` sub-lattices (T first, then Z:
+    decomp.default_grid), one per rank.  A step = one application of D to the global field: pack the half-spinor
+    faces, exchange them with NCCL point-to-point on a communication stream while the fused kernel computes the
+    interior, add the exterior terms.  value = global sites x steps / max-over-ranks device time (strong scaling)."""
+    import numpy as np
+
+    import paper_2407_00041_b200 as wd
+    import wdinputs
+    from paper_2407_00041_b200 import dd as wdd
+    from paper_2407_00041_b200.decomp import Decomposition, default_grid
+
+    cfg = workload(args)
+    dims, nrhs = tuple(cfg["dims"]), cfg["nrhs"]
+    V = wdinputs.volume(dims)
+    clover = cfg["csw"] != 0.0
+    flop = FLOP_WILSON + (FLOP_CLOVER if clover else 0)
+    d = Decomposition(dims, default_grid(world, dims))
+    # ---- setup (untimed).  Every rank draws the global fields from the counter-based generators and keeps its part.
+    U = wdinputs.config_gauge(cfg)
+    Ul = d.extract(U, rank)
+    Cl = wdd.local_clover(d, rank, cfg["m0"], cfg["csw"], d.extract(U, rank, halo=1)) if clover else None
+    del U
+    lo = wdd.LocalOperator(torch, d, rank, cfg["m0"], cfg["csw"], Ul, Cl)
+    del Ul, Cl
+    op = wdd.DistributedOperator(torch, dist, lo)
+    ins = [lo.spinor(nrhs) for _ in range(3)]
+    outs = [lo.spinor(nrhs) for _ in range(2)]
+    for k in range(3):
+        psi = np.stack([d.extract(wdinputs.spinor(dims, cfg["spinor_seed"] + 100 * k + r)[0], rank) for r in range(nrhs)])
+        wd.wd_pack_spinor(lo.h, ins[k], psi, nrhs)
+    del psi
+    torch.cuda.synchronize()
+    kname = wd.wd_kernel_name(wd.wd_kernel_for(lo.h, nrhs))
+
+    def step(k):
+        op.apply(outs[k % 2], ins[k % 3], nrhs)
+
+    for k in range(args.warmup):
+        step(k)
+    torch.cuda.synchronize()
+    dist.barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = wd.wd_launch_count(lo.h)
+    torch.cuda.synchronize()
+    e0.record(lo.stream)
+    for k in range(args.steps):
+        step(k)
+    e1.record(lo.stream)
+    torch.cuda.synchronize()
+    launches = wd.wd_launch_count(lo.h) - launches0
+    sampler.stop_flag = True
+    sampler.join()
+    total_ms, _ = reduce_over_ranks(e0.elapsed_time(e1), 0, dist, "cuda")
+    units = V * nrhs * args.steps  # the GLOBAL lattice, once per step
+    site_rhs_per_s = units / (total_ms * 1e-3)
+    peak, peak_src = peak_hbm()
+    alg_bytes_step = V * (576 + (576 if clover else 0) + 384 * nrhs)
+    face_bytes = sum(2 * wd.wd_dd_face_bytes(lo.h, mu, nrhs) for mu in d.decomposed)
+    achieved = alg_bytes_step / world / (total_ms / args.steps * 1e-3) / 1e9  # per GPU
+    line = {
+        "metric": METRIC, "value": site_rhs_per_s * flop / 1e9, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "strong",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "sites_per_s": site_rhs_per_s,
+        "config": {"workload": cfg["name"], "lattice": list(dims), "m0": cfg["m0"], "csw": cfg["csw"], "nrhs": nrhs,
+                   "kernel": kname, "variant": "fused", "parallelism": f"dd grid {d.grid} local {d.local_dims}",
+                   "exchange": "half-spinor faces (96 B per face site and direction), NCCL send/recv on a side stream",
+                   "l2": f"inputs larger than L2 ({alg_bytes_step / world / 1e9:.2f} GB touched per GPU and step)"},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": None, "peak_source": peak_src, "kernel": kname + "/fused+dd",
+                     "algorithmic_bytes_per_launch": alg_bytes_step / world,
+                     "nvlink_bytes_sent_per_gpu_and_step": face_bytes,
+                     "note": "per GPU: its share of the algorithmic bytes / time of the whole step (pack, interior, exterior)"},
+        "gpu_launches": launches, "clocks": sampler.summary(),
+    }
+    lo.close()
+    dist.barrier()
+    dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -284,6 +373,8 @@ def run_ours(args):
         import torch.distributed as dist
 
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if args.parallel == "dd":
+            return run_dd(args, torch, dist, world, rank, local)
 
     cfg = workload(args)
     dims, nrhs = cfg["dims"], cfg["nrhs"]
@@ -403,6 +494,33 @@ def run_ours(args):
                        "ms_per_step": ms, "steps": args.e2e_steps,
                        "api": "wd_apply_host (pinned host buffers, canonical layout)"}
         del hin, hout
+    # ---- restarted GMRES(M) on the device around the operator: the consumer of the applies
+    if args.gmres and rank == 0 and nrhs == 1:
+        gs = torch.cuda.Stream()
+        wd.wd_set_stream(h, gs.cuda_stream)
+        M, cycles_max = args.gmres, 10
+        res = {}
+        with torch.cuda.stream(gs):
+            for label, graph in (("graph", 1), ("eager", 0)):
+                wd.wd_set_option(h, wd.WD_OPT_GMRES_GRAPH, graph)
+                hist = np.zeros(cycles_max + 1)
+                for rep in range(2):  # first repetition: work-space allocation, graph capture
+                    outs[0].zero_()
+                    g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    l0 = wd.wd_launch_count(h)
+                    g0.record(gs)
+                    cyc = wd.wd_gmres(h, outs[0], ins[0], M, cycles_max, 1e-30, hist)  # tol unreachable: all cycles run
+                    g1.record(gs)
+                    gs.synchronize()
+                ms = g0.elapsed_time(g1)
+                res[label] = {"ms_per_cycle": ms / max(cyc, 1), "cycles": cyc, "launches": wd.wd_launch_count(h) - l0,
+                              "applies": cyc * (M + 1) + 1, "resid_drop": float(hist[cyc] / hist[0]) if hist[0] else None}
+        apply_ms = ms_per_step * (M + 1)
+        line["gmres"] = {"m": M, **res, "apply_ms_per_cycle": apply_ms,
+                         "operator_share_of_cycle": apply_ms / res["graph"]["ms_per_cycle"],
+                         "note": "one cycle = M + 1 operator applications + modified Gram-Schmidt (fused axpy+dot kernels), "
+                                 "least squares and update on the device; graph = cycles 2.. replayed as one CUDA graph"}
+        wd.wd_set_stream(h, stream.cuda_stream)
     # ---- the K steps as ONE CUDA graph (cfg 3: "100 back-to-back applies ... also as one CUDA graph")
     if args.graph and rank == 0:
         gs = torch.cuda.Stream()

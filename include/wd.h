@@ -128,6 +128,42 @@ int wd_gmres(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_cycles
  * breakdown rule ended it); *lsq_resid (may be NULL) = min_y ||beta e_1 - H y||, the recurrence residual. */
 int wd_gmres_last_hessenberg(wd_handle *h, double *host_H, int *kdim, double *lsq_resid);
 
+/* ---- domain decomposition (Algorithm 3; local lattices, eqs. 2.1-2.4) ----
+ * A handle for ONE hyper-rectangular sub-lattice of a global periodic lattice: local extents = global_dims / proc_grid
+ * (int[4] each, order T,Z,Y,X; proc_coords = position of this sub-lattice in the grid).  In a direction with
+ * proc_grid[mu] > 1 ("decomposed") the local lattice does not wrap: wd_apply on such a handle computes everything that
+ * needs no neighbour — the hops across the two faces of that direction are left out — and wd_dd_exterior adds them from
+ * the half-spinors the neighbours packed with wd_dd_pack.  Gauge field: the forward links of the LOCAL sites only
+ * (wd_load_gauge, local canonical layout); no ghost links exist.  Self-coupling: wd_load_clover (S of the local sites,
+ * computed from the global field); wd_build_clover returns WD_ESTATE on a decomposed handle (plaquettes cross the seam).
+ * One application:   wd_dd_pack (every decomposed mu)  ->  exchange of the buffers by the caller (NCCL / peer / device
+ * copies), overlapping with  wd_apply  ->  wd_dd_exterior (every decomposed mu), all on the handle's stream. */
+int wd_create_local(wd_handle **h, const int *global_dims, const int *proc_grid, const int *proc_coords, double m0,
+                    double csw);
+
+/* Bit mu set: direction mu is decomposed on this handle (0 for a handle made by wd_create). */
+int wd_dd_open_mask(const wd_handle *h);
+
+/* Sites of one face of direction mu (V / n_mu) and bytes of one face buffer, nrhs * 6 * face_sites * 16; 0 if mu is not
+ * decomposed.  Face sites are enumerated in canonical order of the three remaining coordinates (X fastest), the same
+ * on both sides of a seam; a buffer is complex double [nrhs][6][face_sites]. */
+long long wd_dd_face_sites(const wd_handle *h, int mu);
+size_t wd_dd_face_bytes(const wd_handle *h, int mu, int nrhs);
+
+/* Alg. 3 lines 1-16 for direction mu.  dev_in: DEVICE spinor(s) in device layout.  Writes (DEVICE buffers of
+ * wd_dd_face_bytes each, caller-allocated):
+ *   dev_send_minus: lambda_mu(x) = rows 0,1 of (I4 - gamma_mu) psi(x), x on the low face — goes to the -mu neighbour,
+ *                   which passes it to wd_dd_exterior as dev_recv_from_plus;
+ *   dev_send_plus:  rows 0,1 of (I4 + gamma_mu) (x) U_mu(x)^H psi(x), x on the high face — goes to the +mu neighbour
+ *                   as its dev_recv_from_minus.   (The factor 1/2 of Alg. 3 is applied in wd_dd_exterior.) */
+int wd_dd_pack(wd_handle *h, const void *dev_in, int nrhs, int mu, void *dev_send_minus, void *dev_send_plus);
+
+/* Alg. 3 lines 17-31 for direction mu: dev_out (the result of wd_apply on this handle, same stream) receives
+ * -1/2 (I4 - gamma_mu) (x) U_mu(x) lambda on the high face and -1/2 times the (I4 + gamma_mu)-reconstruction of chi on
+ * the low face. */
+int wd_dd_exterior(wd_handle *h, void *dev_out, int nrhs, int mu, const void *dev_recv_from_plus,
+                   const void *dev_recv_from_minus);
+
 /* Same operation on HOST arrays in canonical spinor layout: host->device copy, on-device
  * repack, operator, repack, device->host copy, all inside the call; returns after the result is
  * in host_out.  With a TMA kernel the lattice is cut into up to 16 chunks along T and upload,

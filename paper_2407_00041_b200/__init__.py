@@ -32,6 +32,12 @@ SIGNATURES = {
     "wd_get_clover": (_i, [_vp, _vp]),
     "wd_apply": (_i, [_vp, _vp, _vp, _i]),
     "wd_apply_host": (_i, [_vp, _vp, _vp, _i]),
+    "wd_create_local": (_i, [ctypes.POINTER(_vp), ctypes.POINTER(_i), ctypes.POINTER(_i), ctypes.POINTER(_i), _d, _d]),
+    "wd_dd_open_mask": (_i, [_vp]),
+    "wd_dd_face_sites": (ctypes.c_longlong, [_vp, _i]),
+    "wd_dd_face_bytes": (_sz, [_vp, _i, _i]),
+    "wd_dd_pack": (_i, [_vp, _vp, _i, _i, _vp, _vp]),
+    "wd_dd_exterior": (_i, [_vp, _vp, _i, _i, _vp, _vp]),
     "wd_gmres": (_i, [_vp, _vp, _vp, _i, _i, _d, ctypes.POINTER(_i), _vp]),
     "wd_gmres_last_hessenberg": (_i, [_vp, _vp, ctypes.POINTER(_i), ctypes.POINTER(_d)]),
     "wd_spinor_bytes": (_sz, [_vp, _i]),
@@ -101,6 +107,34 @@ def wd_create(T: int, Z: int, Y: int, X: int, m0: float, csw: float) -> int:
     rc = lib().wd_create(ctypes.byref(h), T, Z, Y, X, m0, csw)
     _check(None, rc)
     return h.value
+
+
+def wd_create_local(global_dims, proc_grid, proc_coords, m0: float, csw: float) -> int:
+    h = _vp()
+    a = [(_i * 4)(*[int(v) for v in x]) for x in (global_dims, proc_grid, proc_coords)]
+    rc = lib().wd_create_local(ctypes.byref(h), a[0], a[1], a[2], m0, csw)
+    _check(None, rc)
+    return h.value
+
+
+def wd_dd_open_mask(h) -> int:
+    return int(lib().wd_dd_open_mask(h))
+
+
+def wd_dd_face_sites(h, mu: int) -> int:
+    return int(lib().wd_dd_face_sites(h, mu))
+
+
+def wd_dd_face_bytes(h, mu: int, nrhs: int = 1) -> int:
+    return int(lib().wd_dd_face_bytes(h, mu, nrhs))
+
+
+def wd_dd_pack(h, dev_in, nrhs: int, mu: int, dev_send_minus, dev_send_plus) -> None:
+    _check(h, lib().wd_dd_pack(h, _ptr(dev_in), nrhs, mu, _ptr(dev_send_minus), _ptr(dev_send_plus)))
+
+
+def wd_dd_exterior(h, dev_out, nrhs: int, mu: int, dev_recv_from_plus, dev_recv_from_minus) -> None:
+    _check(h, lib().wd_dd_exterior(h, _ptr(dev_out), nrhs, mu, _ptr(dev_recv_from_plus), _ptr(dev_recv_from_minus)))
 
 
 def wd_destroy(h) -> None:

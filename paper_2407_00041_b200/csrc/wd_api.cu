@@ -282,6 +282,8 @@ int wd_load_clover(wd_handle *h, const double *host_C) {
 int wd_build_clover(wd_handle *h) {
     WD_ENTER(h);
     if (!h->has_gauge) return fail(h, WD_ESTATE, "wd_build_clover: no gauge field loaded");
+    if (dd_open_mask(h))
+        return fail(h, WD_ESTATE, "wd_build_clover: plaquettes cross the seams of a decomposed handle; load S with wd_load_clover");
     int rc = ensure_clover_storage(h);
     if (rc) return rc;
     WD_CUDA(h, launch_build_clover(h->dS, h->dU, h->n, h->V, h->Vs, h->m0 + 4.0, h->csw, h->stream));
@@ -385,6 +387,7 @@ int wd_layout_unpack_host(int field, long long nsites, const double *packed, dou
 
 // ---- kernel selection -----------------------------------------------------------------------------
 static bool geometry_fits(const wd_handle *h, const KernelInfo &k) {
+    if (dd_open_mask(h) && !strncmp(k.name, "tmc", 3)) return false;  // no open-boundary mode in wd_tmc.cu
     if (k.bx == 0) return true;
     return h->n[0] % k.bt == 0 && h->n[1] % k.bz == 0 && h->n[2] % k.by == 0 && h->n[3] % k.bx == 0;
 }
@@ -428,7 +431,7 @@ int wd_set_option(wd_handle *h, int option, long value) {
     case WD_OPT_KERNEL:
         if (value < -1 || value >= kernel_count()) return fail(h, WD_EINVAL, "WD_OPT_KERNEL: id out of range");
         if (value >= 0 && !geometry_fits(h, kernel_info((int)value)))
-            return fail(h, WD_EINVAL, std::string("WD_OPT_KERNEL: tile of ") + kernel_info((int)value).name + " does not divide the lattice");
+            return fail(h, WD_EINVAL, std::string("WD_OPT_KERNEL: ") + kernel_info((int)value).name + " does not fit this handle (tile does not divide the lattice, or no open-boundary mode)");
         h->kernel_opt = value;
         return WD_OK;
     case WD_OPT_TCHUNK:
@@ -489,7 +492,7 @@ int wd::fill_params(wd_handle *h, KParams &p, const KernelInfo &k) {
     p.nsm = h->nsm;
     p.device = h->device;
     p.maps = h->maps;
-    p.open_mask = 0;
+    p.open_mask = dd_open_mask(h);
     p.gauge_rows = 3;
     if (k.bx) {
         p.ntx = h->n[3] / k.bx;
@@ -679,5 +682,3 @@ int wd_apply_host(wd_handle *h, double *host_out, const double *host_in, int nrh
 }
 
 }  // extern "C"
-
-void wd::dd_free(wd_handle *) {}

@@ -39,6 +39,7 @@ struct Scalars {          // device-resident scalars of the iteration
     double beta, inv;     // ||r||, and the reciprocal the next scaling uses (1/beta or 1/h_{j+1,j})
     double lsq_resid;     // |g_{kdim+1}|: the recurrence residual of the cycle
     int active, kdim;     // Arnoldi still running; Krylov dimension of this cycle
+    int kdim_done;        // Krylov dimension of the cycle that was completed last (kdim is re-armed for the next one)
     unsigned int ticket;  // last-block detection of the reductions (zero between kernels)
 };
 }  // namespace
@@ -186,6 +187,7 @@ __global__ void __launch_bounds__(kThreads) k_scale(double2 *__restrict__ dst, c
 __global__ void k_lsq(Scalars *sc, int m) {
     if (threadIdx.x || blockIdx.x) return;
     const int kd = sc->kdim, ld = m + 1;
+    sc->kdim_done = kd;
     double2 g[kMaxM + 1];
     double2 *H = sc->H;
     for (int k = 0; k <= kd; k++) g[k] = make_double2(0.0, 0.0);
@@ -361,13 +363,13 @@ int wd_gmres(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_cycles
     Cycle cyc{h, g, m, tol / 10.0};
     double2 *x = (double2 *)dev_x;
     const double2 *b = (const double2 *)dev_b;
-    struct { double beta, inv, lsq; int active, kdim; } hs;
+    struct { double beta, inv, lsq; int active, kdim, kdim_done; unsigned int ticket; } hs;
     auto read_scalars = [&]() -> int {
         WD_CUDA(h, cudaMemcpyAsync(&hs, &g->sc->beta, sizeof(hs), cudaMemcpyDeviceToHost, h->stream));
         WD_CUDA(h, cudaStreamSynchronize(h->stream));
         return WD_OK;
     };
-    static_assert(offsetof(Scalars, kdim) - offsetof(Scalars, beta) == 3 * sizeof(double) + sizeof(int), "layout of Scalars");
+    static_assert(offsetof(Scalars, ticket) - offsetof(Scalars, beta) == 3 * sizeof(double) + 3 * sizeof(int) && sizeof(hs) == 40, "layout of Scalars");
     // lines 4-5 for x_0
     if ((rc = cyc.residual(x, b))) return rc;
     h->launches += cyc.launches;
@@ -412,7 +414,7 @@ int wd_gmres(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_cycles
     }
     if (cycles_done) *cycles_done = k;
     g->last_m = m;
-    g->last_kdim = (k > 0) ? hs.kdim : 0;
+    g->last_kdim = (k > 0) ? hs.kdim_done : 0;
     return WD_OK;
 }
 

@@ -79,5 +79,6 @@ int fill_params(wd_handle *h, KParams &p, const KernelInfo &k);
 int launch_op(wd_handle *h, const KernelInfo &k, const KParams &p, int self);
 void gmres_free(wd_handle *h);  // wd_gmres.cu
 void dd_free(wd_handle *h);     // wd_dd.cu
+int dd_open_mask(const wd_handle *h);  // bit mu: direction mu does not wrap on this handle (wd_create_local)
 
 }  // namespace wd

@@ -20,22 +20,26 @@ namespace wd {
 
 __device__ __forceinline__ cd ldg(const cd *p) { return __ldg(p); }
 
+// fwd / bwd = false: the hop crosses an open boundary of a domain-decomposed sub-lattice (KParams::open_mask) and is
+// left to the exterior kernel of wd_dd.cu.
 template <int MU>
 __device__ __forceinline__ void hop_direction(cd acc[12], const cd *__restrict__ psi, const cd *__restrict__ U,
-                                              long long V, long long i, long long ip, long long im) {
+                                              long long V, long long i, long long ip, long long im, bool fwd, bool bwd) {
     cd p[12], u[9];
-    // forward: (1 - gamma_mu) (x) U_mu(x) psi(x+mu)
+    if (fwd) {  // forward: (1 - gamma_mu) (x) U_mu(x) psi(x+mu)
 #pragma unroll
-    for (int k = 0; k < 9; k++) u[k] = ldg(U + (long long)(MU * 9 + k) * V + i);
+        for (int k = 0; k < 9; k++) u[k] = ldg(U + (long long)(MU * 9 + k) * V + i);
 #pragma unroll
-    for (int c = 0; c < 12; c++) p[c] = ldg(psi + (long long)c * V + ip);
-    hop_term<MU, -1>(acc, p, u);
-    // backward: (1 + gamma_mu) (x) U_mu(x-mu)^H psi(x-mu)
+        for (int c = 0; c < 12; c++) p[c] = ldg(psi + (long long)c * V + ip);
+        hop_term<MU, -1>(acc, p, u);
+    }
+    if (bwd) {  // backward: (1 + gamma_mu) (x) U_mu(x-mu)^H psi(x-mu)
 #pragma unroll
-    for (int k = 0; k < 9; k++) u[k] = ldg(U + (long long)(MU * 9 + k) * V + im);
+        for (int k = 0; k < 9; k++) u[k] = ldg(U + (long long)(MU * 9 + k) * V + im);
 #pragma unroll
-    for (int c = 0; c < 12; c++) p[c] = ldg(psi + (long long)c * V + im);
-    hop_term<MU, +1>(acc, p, u);
+        for (int c = 0; c < 12; c++) p[c] = ldg(psi + (long long)c * V + im);
+        hop_term<MU, +1>(acc, p, u);
+    }
 }
 
 template <int SELF>
@@ -43,6 +47,7 @@ __device__ __forceinline__ void site_apply(const KParams &p, long long i, int t,
     const cd *__restrict__ psi = p.psi;
     const cd *__restrict__ U = p.U;
     const long long V = p.Vs;  // component stride
+    const int open = p.open_mask;
     cd acc[12];
 #pragma unroll
     for (int c = 0; c < 12; c++) acc[c] = make_double2(0.0, 0.0);
@@ -51,24 +56,24 @@ __device__ __forceinline__ void site_apply(const KParams &p, long long i, int t,
         const long long s = p.stride[0];
         const long long ip = (t + 1 < p.n[0]) ? i + s : i - (long long)(p.n[0] - 1) * s;
         const long long im = (t > 0) ? i - s : i + (long long)(p.n[0] - 1) * s;
-        hop_direction<0>(acc, psi, U, V, i, ip, im);
+        hop_direction<0>(acc, psi, U, V, i, ip, im, !(open & 1) || t + 1 < p.n[0], !(open & 1) || t > 0);
     }
     {
         const long long s = p.stride[1];
         const long long ip = (z + 1 < p.n[1]) ? i + s : i - (long long)(p.n[1] - 1) * s;
         const long long im = (z > 0) ? i - s : i + (long long)(p.n[1] - 1) * s;
-        hop_direction<1>(acc, psi, U, V, i, ip, im);
+        hop_direction<1>(acc, psi, U, V, i, ip, im, !(open & 2) || z + 1 < p.n[1], !(open & 2) || z > 0);
     }
     {
         const long long s = p.stride[2];
         const long long ip = (y + 1 < p.n[2]) ? i + s : i - (long long)(p.n[2] - 1) * s;
         const long long im = (y > 0) ? i - s : i + (long long)(p.n[2] - 1) * s;
-        hop_direction<2>(acc, psi, U, V, i, ip, im);
+        hop_direction<2>(acc, psi, U, V, i, ip, im, !(open & 4) || y + 1 < p.n[2], !(open & 4) || y > 0);
     }
     {
         const long long ip = (x + 1 < p.n[3]) ? i + 1 : i - (long long)(p.n[3] - 1);
         const long long im = (x > 0) ? i - 1 : i + (long long)(p.n[3] - 1);
-        hop_direction<3>(acc, psi, U, V, i, ip, im);
+        hop_direction<3>(acc, psi, U, V, i, ip, im, !(open & 8) || x + 1 < p.n[3], !(open & 8) || x > 0);
     }
 
     cd *__restrict__ out = p.out;

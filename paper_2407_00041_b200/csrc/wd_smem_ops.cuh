@@ -16,21 +16,27 @@ __device__ __forceinline__ cd lds(const unsigned char *smem, uint32_t off) {
 // One direction MU != T of the stencil for the thread's site: both hops, operands from shared
 // memory.  (base, stride) pairs select interior or face storage per thread (no divergence: both
 // are shared-memory addresses).
+// fwd / bwd = false: that hop crosses an open boundary of a domain-decomposed sub-lattice and is left out here (the
+// exterior kernel of wd_dd.cu adds it from the neighbour's half-spinor); always true on a periodic lattice.
 template <int MU>
 __device__ __forceinline__ void hop_pair_smem(cd acc[12], const unsigned char *smem, uint32_t u_own, uint32_t u_own_stride,
                                               uint32_t pf, uint32_t pf_stride, uint32_t ub, uint32_t ub_stride,
-                                              uint32_t pb, uint32_t pb_stride) {
+                                              uint32_t pb, uint32_t pb_stride, bool fwd = true, bool bwd = true) {
     cd p[12], u[9];
+    if (fwd) {
 #pragma unroll
-    for (int k = 0; k < 9; k++) u[k] = lds(smem, u_own + k * u_own_stride);
+        for (int k = 0; k < 9; k++) u[k] = lds(smem, u_own + k * u_own_stride);
 #pragma unroll
-    for (int c = 0; c < 12; c++) p[c] = lds(smem, pf + c * pf_stride);
-    hop_term<MU, -1>(acc, p, u);
+        for (int c = 0; c < 12; c++) p[c] = lds(smem, pf + c * pf_stride);
+        hop_term<MU, -1>(acc, p, u);
+    }
+    if (bwd) {
 #pragma unroll
-    for (int k = 0; k < 9; k++) u[k] = lds(smem, ub + k * ub_stride);
+        for (int k = 0; k < 9; k++) u[k] = lds(smem, ub + k * ub_stride);
 #pragma unroll
-    for (int c = 0; c < 12; c++) p[c] = lds(smem, pb + c * pb_stride);
-    hop_term<MU, +1>(acc, p, u);
+        for (int c = 0; c < 12; c++) p[c] = lds(smem, pb + c * pb_stride);
+        hop_term<MU, +1>(acc, p, u);
+    }
 }
 
 // acc[0..5] += (part of B) q for one 6x6 Hermitian block B.  H = 0: the 6 real diagonal entries (slots

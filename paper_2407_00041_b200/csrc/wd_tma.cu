@@ -260,6 +260,11 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
         const Item it = decode_item<P>(prm, item);
         const long long site0 = ((long long)(it.z0 + lz) * Y + (it.y0 + ly)) * X + (it.x0 + lx);
         cd *__restrict__ out = prm.out + (long long)it.rhs0 * 12 * V;
+        // open boundaries of a domain-decomposed sub-lattice: hops that would cross them are left out
+        const int open = prm.open_mask;
+        const bool zf_on = !((open & 2) && it.z0 + lz == Z - 1), zb_on = !((open & 2) && it.z0 + lz == 0);
+        const bool yf_on = !((open & 4) && it.y0 + ly == Y - 1), yb_on = !((open & 4) && it.y0 + ly == 0);
+        const bool xf_on = !((open & 8) && it.x0 + lx == X - 1), xb_on = !((open & 8) && it.x0 + lx == 0);
         int t = (it.t0 == 0) ? T - 1 : it.t0 - 1;
         {   // prologue: seed the carried half-spinor from psi(t0-1)
             cd p[12];
@@ -267,6 +272,10 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
 #pragma unroll
             for (int c = 0; c < 12; c++) p[c] = lds(smem, P::OFF_C + own + c * NS);
             project<0, +1>(hprev, p);
+            if ((open & 1) && it.t0 == 0) {
+#pragma unroll
+                for (int c = 0; c < 6; c++) hprev[c] = make_double2(0.0, 0.0);
+            }
             release(OB_C);
             nC++;
         }
@@ -293,7 +302,7 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
                     cd f[12];
 #pragma unroll
                     for (int c = 0; c < 12; c++) f[c] = make_double2(0.0, 0.0);
-                    hop_term<0, -1>(f, p, u);  // (1 - gamma_T) U_T(t-1) psi(t)
+                    if (!((open & 1) && tprev == T - 1)) hop_term<0, -1>(f, p, u);  // (1 - gamma_T) U_T(t-1) psi(t)
                     const long long ip = (long long)tprev * strideT + site0;
 #pragma unroll
                     for (int c = 0; c < 12; c++)
@@ -318,13 +327,13 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
             }
             const uint32_t pf = nF & 1;
             mbar_wait(bar_full + 8 * OB_Z, pf);
-            hop_pair_smem<1>(acc, smem, P::OFF_Z + own, NS, z_pf, z_pf_s, z_ub, z_b_s, z_pb, z_b_s);
+            hop_pair_smem<1>(acc, smem, P::OFF_Z + own, NS, z_pf, z_pf_s, z_ub, z_b_s, z_pb, z_b_s, zf_on, zb_on);
             release(OB_Z);
             mbar_wait(bar_full + 8 * OB_Y, pf);
-            hop_pair_smem<2>(acc, smem, P::OFF_Y + own, NS, y_pf, y_pf_s, y_ub, y_b_s, y_pb, y_b_s);
+            hop_pair_smem<2>(acc, smem, P::OFF_Y + own, NS, y_pf, y_pf_s, y_ub, y_b_s, y_pb, y_b_s, yf_on, yb_on);
             release(OB_Y);
             mbar_wait(bar_full + 8 * OB_X, pf);
-            hop_pair_smem<3>(acc, smem, P::OFF_X + own, NS, x_pf, x_pf_s, x_ub, x_b_s, x_pb, x_b_s);
+            hop_pair_smem<3>(acc, smem, P::OFF_X + own, NS, x_pf, x_pf_s, x_ub, x_b_s, x_pb, x_b_s, xf_on, xb_on);
             release(OB_X);
             release(OB_C);
             nC++;

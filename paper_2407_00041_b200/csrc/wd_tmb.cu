@@ -312,6 +312,11 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
         const Item it = decode_item<P>(prm, item);
         const long long site0 = ((long long)(it.z0 + lz) * Y + (it.y0 + ly)) * X + (it.x0 + lx);
         cd *__restrict__ out = prm.out + (long long)it.rhs0 * 12 * V;
+        // open boundaries of a domain-decomposed sub-lattice: hops that would cross them are left out
+        const int open = prm.open_mask;
+        const bool zf_on = !((open & 2) && it.z0 + lz == Z - 1), zb_on = !((open & 2) && it.z0 + lz == 0);
+        const bool yf_on = !((open & 4) && it.y0 + ly == Y - 1), yb_on = !((open & 4) && it.y0 + ly == 0);
+        const bool xf_on = !((open & 8) && it.x0 + lx == X - 1), xb_on = !((open & 8) && it.x0 + lx == 0);
         int t = it.t0;
         {   // prologue: acc = backward-T hop of slice t0, (1 + gamma_T) U_T(t0-1)^H psi(t0-1)
             const uint32_t cb = (nC & 1) ? P::SZ_C : 0, slot = nR & 3;
@@ -330,7 +335,7 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
             su3_mul<true>(g, u, h);
 #pragma unroll
             for (int c = 0; c < 12; c++) acc[c] = make_double2(0.0, 0.0);
-            reconstruct_add<0, +1>(acc, g);
+            if (!((open & 1) && it.t0 == 0)) reconstruct_add<0, +1>(acc, g);
         }
         for (int j = 1; j <= prm.tchunk; j++) {
             const bool last = (j == prm.tchunk);
@@ -339,11 +344,11 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
             const uint32_t pf = nF & 1;
             wait_full(OB_Z, pf);
             hop_pair_smem<1>(acc, smem, P::OFF_Z + own, NS, z_pf + (zf_in ? cb : 0), z_pf_s, z_ub, z_b_s,
-                             z_pb + (zb_in ? cb : 0), z_b_s);
+                             z_pb + (zb_in ? cb : 0), z_b_s, zf_on, zb_on);
             release(OB_Z);
             wait_full(OB_Y, pf);
             hop_pair_smem<2>(acc, smem, P::OFF_Y + own, NS, y_pf + (yf_in ? cb : 0), y_pf_s, y_ub, y_b_s,
-                             y_pb + (yb_in ? cb : 0), y_b_s);
+                             y_pb + (yb_in ? cb : 0), y_b_s, yf_on, yb_on);
             release(OB_Y);
             if (CLOVER) {  // between the Y and X hops, so that neither S4 nor the next U_T waits on a just-freed slot
                 s_phase(cb, 0);
@@ -351,7 +356,7 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
             }
             wait_full(OB_X, pf);
             hop_pair_smem<3>(acc, smem, P::OFF_X + own, NS, x_pf + (xf_in ? cb : 0), x_pf_s, x_ub, x_b_s,
-                             x_pb + (xb_in ? cb : 0), x_b_s);
+                             x_pb + (xb_in ? cb : 0), x_b_s, xf_on, xb_on);
             release(OB_X);
             nF++;
             {   // T phase: forward hop (1 - gamma_T) U_T(t) psi(t+1) completes out(t); the backward hop of slice
@@ -371,7 +376,7 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
                 for (int k = 0; k < 9; k++) u[k] = lds(smem, P::OFF_R + slot * P::SZ_U + own + k * NS);
 #pragma unroll
                 for (int c = 0; c < 12; c++) p[c] = lds(smem, P::OFF_C + cn + own + c * NS);
-                hop_term<0, -1>(acc, p, u);
+                if (!((open & 1) && t == T - 1)) hop_term<0, -1>(acc, p, u);
                 if (P::SELF == SELF_MASS || !last) {
 #pragma unroll
                     for (int c = 0; c < 12; c++) p[c] = lds(smem, P::OFF_C + cb + own + c * NS);  // psi(t)

@@ -381,6 +381,7 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tmc(const __grid_constant__ 
 // ---------------------------------------------------------------- host side
 template <int BZ, int BY, int BX, int SELF> static cudaError_t launch_self(const KParams &p, cudaStream_t st) {
     using P = Plan<BZ, BY, BX, SELF>;
+    if (p.open_mask) return cudaErrorNotSupported;  // sub-lattices of a domain decomposition: wd_tma.cu / wd_tmb.cu
     // units of two right-hand sides that share a tile's U and S through L2: three (six right-hand sides in flight per tile)
     return launch_tma_kernel<P>(k_tmc<P>, p, st, /*ucomp*/ 9, /*scomp*/ 9, CHUNK_SHORT, /*rb*/ 3);
 }
