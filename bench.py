@@ -51,6 +51,9 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-ceilings", action="store_true", help="skip the streaming / FP64 ceiling microbenchmarks")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--gauge-rows", type=int, default=3, choices=[2, 3],
+                    help="2 = opt-in two-row link storage (SU(3) links only): 1344 instead of 1536 algorithmic B/site")
+    ap.add_argument("--f32", action="store_true", help="also time the FP32 variant (wd_apply_f32) on the same workload")
     ap.add_argument("--parallel", default="dd", choices=["dd", "replicas"],
                     help="N > 1: dd = ONE lattice cut over the ranks, half-spinor faces exchanged with NCCL send/recv "
                          "(strong scaling, default); replicas = N independent copies (weak)")
@@ -397,6 +400,11 @@ def run_ours(args):
         wd.wd_set_option(h, wd.WD_OPT_TCHUNK, args.tchunk)
     if args.zgroup:
         wd.wd_set_option(h, wd.WD_OPT_ZGROUP, args.zgroup)
+    if args.gauge_rows == 2:
+        wd.wd_set_option(h, wd.WD_OPT_GAUGE_ROWS, 2)
+        gauge_b = 384  # rows 0 and 1 only: the roofline is reported against the reduced byte count
+        alg_bytes_site_rhs = (gauge_b + self_b) / nrhs + 384
+        alg_bytes_step = V * (gauge_b + self_b + 384 * nrhs)
     U = wdinputs.config_gauge(cfg)
     wd.wd_load_gauge(h, U)
     del U
@@ -468,7 +476,7 @@ def run_ours(args):
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "sites_per_s": site_rhs_per_s, "hbm_gbs_algorithmic": site_rhs_per_s * alg_bytes_site_rhs / 1e9,
         "config": {"workload": cfg["name"], "lattice": list(dims), "m0": cfg["m0"], "csw": cfg["csw"],
-                   "nrhs": nrhs, "kernel": kname, "variant": "fused" if args.variant == 0 else "unfused",
+                   "nrhs": nrhs, "kernel": kname, "variant": "fused" if args.variant == 0 else "unfused", "gauge_rows": args.gauge_rows,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": f"inputs larger than L2 ({alg_bytes_step / 1e9:.2f} GB touched per step); "
                          "3 inputs / 2 outputs rotate"},
@@ -494,6 +502,29 @@ def run_ours(args):
                        "ms_per_step": ms, "steps": args.e2e_steps,
                        "api": "wd_apply_host (pinned host buffers, canonical layout)"}
         del hin, hout
+    # ---- the FP32 variant on the same workload: 768 instead of 1536 algorithmic B/site
+    if args.f32 and rank == 0:
+        wd.wd_enable_f32(h)
+        n32 = wd.wd_spinor_bytes_f32(h, nrhs) // 4
+        fin = [torch.empty(n32, dtype=torch.float32, device="cuda") for _ in range(3)]
+        fout = [torch.empty(n32, dtype=torch.float32, device="cuda") for _ in range(2)]
+        for k in range(3):
+            wd.wd_convert_spinor(h, fin[k], ins[k], nrhs, True)
+        for k in range(5):
+            wd.wd_apply_f32(h, fout[k % 2], fin[k % 3], nrhs)
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        nst = max(10, args.steps // 4)
+        f0.record(stream)
+        for k in range(nst):
+            wd.wd_apply_f32(h, fout[k % 2], fin[k % 3], nrhs)
+        f1.record(stream)
+        torch.cuda.synchronize()
+        fms = f0.elapsed_time(f1) / nst
+        line["f32"] = {"ms_per_step": fms, "steps": nst, "value": V * nrhs * flop / (fms * 1e-3) / 1e9, "unit": "GFLOP/s",
+                       "dtype": "f32", "algorithmic_gbs": alg_bytes_step / 2 / (fms * 1e-3) / 1e9,
+                       "frac_of_measured_peak": alg_bytes_step / 2 / (fms * 1e-3) / 1e9 / peak,
+                       "kernel": "tile_1x4x4x16<float2> / linear256<float2> (one-thread-per-site LDG kernels)"}
+        del fin, fout
     # ---- restarted GMRES(M) on the device around the operator: the consumer of the applies
     if args.gmres and rank == 0 and nrhs == 1:
         gs = torch.cuda.Stream()

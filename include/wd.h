@@ -68,7 +68,12 @@ enum {
     WD_OPT_ZGROUP = 4,    /* number of Z-tiles per rasterisation group in tiled geometries; 0 = automatic         */
     WD_OPT_DEVICE_PACK = 5,/* 1 = wd_load_* / wd_pack_* transpose on the device instead of on the host (default 0) */
     WD_OPT_HOST_PIPELINE = 6,/* wd_apply_host: 1 = overlap upload, compute and download over T chunks (default), 0 = serial */
-    WD_OPT_GMRES_GRAPH = 7 /* wd_gmres: 1 = replay restart cycles as one CUDA graph (default; needs a non-default stream), 0 = launch by launch */
+    WD_OPT_GMRES_GRAPH = 7,/* wd_gmres: 1 = replay restart cycles as one CUDA graph (default; needs a non-default stream), 0 = launch by launch */
+    WD_OPT_GAUGE_ROWS = 8  /* 3 = links stored as 9 complex numbers (default).  2 = two-row storage for SU(3) links: the
+                              fused TMA kernel of one right-hand side reads rows 0, 1 (384 instead of 576 B per site) and
+                              rebuilds row 2 = conj(row 0 x row 1) in registers.  EXACT ONLY FOR SU(3) LINKS: with 2 the
+                              "general 3x3 complex" promise of wd_load_gauge (R11) does not hold.  Costs a second,
+                              two-row copy of the gauge field on the device. */
 };
 
 /* Create an operator for a T x Z x Y x X periodic lattice.  Every extent >= 1 (n = 2, where
@@ -163,6 +168,19 @@ int wd_dd_pack(wd_handle *h, const void *dev_in, int nrhs, int mu, void *dev_sen
  * the low face. */
 int wd_dd_exterior(wd_handle *h, void *dev_out, int nrhs, int mu, const void *dev_recv_from_plus,
                    const void *dev_recv_from_minus);
+
+/* ---- FP32 variant (the paper's PRECISION templating) ----
+ * wd_enable_f32: makes single-precision copies of the loaded links and of S on the device (call again after the FP64
+ * fields change).  A single-precision device spinor is the device layout with 8-byte elements: wd_spinor_bytes_f32
+ * bytes, 8-byte aligned; it is produced from / turned into an FP64 device spinor by wd_convert_spinor (to_f32 = 1:
+ * dst float <- src double; 0: dst double <- src float; both DEVICE pointers).  wd_apply_f32: out = D in with every load,
+ * store and arithmetic operation in FP32 (one fused pass per right-hand side); the error against the FP64 operator is
+ * bounded in DESIGN.md ("Tolerance of the FP32 variant": relative L2 <= 1e-6).  Asynchronous on the handle's stream.
+ * Errors: WD_ESTATE (fields missing / wd_enable_f32 not called), WD_EINVAL, WD_ENOMEM, WD_ECUDA. */
+int wd_enable_f32(wd_handle *h);
+size_t wd_spinor_bytes_f32(const wd_handle *h, int nrhs);
+int wd_convert_spinor(wd_handle *h, void *dev_dst, const void *dev_src, int nrhs, int to_f32);
+int wd_apply_f32(wd_handle *h, void *dev_out, const void *dev_in, int nrhs);
 
 /* Same operation on HOST arrays in canonical spinor layout: host->device copy, on-device
  * repack, operator, repack, device->host copy, all inside the call; returns after the result is

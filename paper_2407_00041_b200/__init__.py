@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libwd.so")
 WD_OK, WD_EINVAL, WD_ENOMEM, WD_ESTATE, WD_ECUDA = 0, -1, -2, -3, -4
 WD_FIELD_SPINOR, WD_FIELD_GAUGE, WD_FIELD_CLOVER = 0, 1, 2
 WD_OPT_VARIANT, WD_OPT_KERNEL, WD_OPT_TCHUNK, WD_OPT_ZGROUP, WD_OPT_DEVICE_PACK, WD_OPT_HOST_PIPELINE = 1, 2, 3, 4, 5, 6
-WD_OPT_GMRES_GRAPH = 7
+WD_OPT_GMRES_GRAPH, WD_OPT_GAUGE_ROWS = 7, 8
 
 # name -> (restype, argtypes); mirrors include/wd.h declaration by declaration
 _vp, _i, _d, _l, _sz, _cp = (ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_long,
@@ -32,6 +32,10 @@ SIGNATURES = {
     "wd_get_clover": (_i, [_vp, _vp]),
     "wd_apply": (_i, [_vp, _vp, _vp, _i]),
     "wd_apply_host": (_i, [_vp, _vp, _vp, _i]),
+    "wd_enable_f32": (_i, [_vp]),
+    "wd_spinor_bytes_f32": (_sz, [_vp, _i]),
+    "wd_convert_spinor": (_i, [_vp, _vp, _vp, _i, _i]),
+    "wd_apply_f32": (_i, [_vp, _vp, _vp, _i]),
     "wd_create_local": (_i, [ctypes.POINTER(_vp), ctypes.POINTER(_i), ctypes.POINTER(_i), ctypes.POINTER(_i), _d, _d]),
     "wd_dd_open_mask": (_i, [_vp]),
     "wd_dd_face_sites": (ctypes.c_longlong, [_vp, _i]),
@@ -135,6 +139,22 @@ def wd_dd_pack(h, dev_in, nrhs: int, mu: int, dev_send_minus, dev_send_plus) -> 
 
 def wd_dd_exterior(h, dev_out, nrhs: int, mu: int, dev_recv_from_plus, dev_recv_from_minus) -> None:
     _check(h, lib().wd_dd_exterior(h, _ptr(dev_out), nrhs, mu, _ptr(dev_recv_from_plus), _ptr(dev_recv_from_minus)))
+
+
+def wd_enable_f32(h) -> None:
+    _check(h, lib().wd_enable_f32(h))
+
+
+def wd_spinor_bytes_f32(h, nrhs: int = 1) -> int:
+    return int(lib().wd_spinor_bytes_f32(h, nrhs))
+
+
+def wd_convert_spinor(h, dev_dst, dev_src, nrhs: int, to_f32: bool) -> None:
+    _check(h, lib().wd_convert_spinor(h, _ptr(dev_dst), _ptr(dev_src), nrhs, 1 if to_f32 else 0))
+
+
+def wd_apply_f32(h, dev_out, dev_in, nrhs: int = 1) -> None:
+    _check(h, lib().wd_apply_f32(h, _ptr(dev_out), _ptr(dev_in), nrhs))
 
 
 def wd_destroy(h) -> None:

@@ -63,6 +63,16 @@ static void release_dstage(wd_handle *h) {
     h->dstage_bytes = 0;
 }
 
+// (re)build the two-row copy of the links when two-row storage is selected and a gauge field is present
+static int refresh_two_row_copy(wd_handle *h) {
+    if (h->gauge_rows != 2 || !h->has_gauge) return WD_OK;
+    if (!h->dU2) WD_CUDA(h, cudaMalloc((void **)&h->dU2, (size_t)h->Vs * 24 * sizeof(double2)));
+    WD_CUDA(h, launch_compress_gauge(h->dU2, h->dU, h->V, h->Vs, h->stream));
+    h->launches++;
+    map_cache_clear(h->maps);
+    return WD_OK;
+}
+
 extern "C" {
 
 const char *wd_version(void) { return "wd-b200 0.1 (sm_100a, FP64)"; }
@@ -88,7 +98,7 @@ int wd_create(wd_handle **out, int T, int Z, int Y, int X, double m0, double csw
     h->csw = csw;
     h->device = dev;
     h->stream = nullptr;
-    h->dU = h->dS = nullptr;
+    h->dU = h->dS = h->dU2 = nullptr;
     h->dsched = nullptr;
     h->sched_dirty = false;
     h->has_gauge = h->has_clover = h->clover_built = false;
@@ -97,6 +107,7 @@ int wd_create(wd_handle **out, int T, int Z, int Y, int X, double m0, double csw
     h->maps = map_cache_new();
     h->host_pipeline = 1;
     h->gmres_graph = 1;
+    h->gauge_rows = 3;
     h->variant = 0;
     h->kernel_opt = -1;
     h->tchunk_opt = 0;
@@ -114,6 +125,7 @@ int wd_create(wd_handle **out, int T, int Z, int Y, int X, double m0, double csw
     h->launches = 0;
     h->gmres = nullptr;
     h->dd = nullptr;
+    h->f32 = nullptr;
     e = cudaMalloc((void **)&h->dU, (size_t)h->Vs * kGaugeComps * sizeof(double2));
     if (e == cudaSuccess) e = cudaMalloc((void **)&h->dsched, 2 * sizeof(unsigned int));
     if (e == cudaSuccess) e = cudaMemset(h->dsched, 0, 2 * sizeof(unsigned int));
@@ -135,9 +147,11 @@ int wd_destroy(wd_handle *h) {
     cudaStreamSynchronize(h->stream);
     gmres_free(h);
     dd_free(h);
+    f32_free(h);
     map_cache_delete(h->maps);
     if (h->dU) cudaFree(h->dU);
     if (h->dS) cudaFree(h->dS);
+    if (h->dU2) cudaFree(h->dU2);
     if (h->dsched) cudaFree(h->dsched);
     if (h->dstage) cudaFree(h->dstage);
     if (h->work_in) cudaFree(h->work_in);
@@ -248,7 +262,7 @@ int wd_load_gauge(wd_handle *h, const double *host_U) {
         if (rc) return rc;
     }
     h->has_gauge = true;
-    return WD_OK;
+    return refresh_two_row_copy(h);
 }
 
 static int ensure_clover_storage(wd_handle *h) {
@@ -451,6 +465,12 @@ int wd_set_option(wd_handle *h, int option, long value) {
     case WD_OPT_GMRES_GRAPH:
         h->gmres_graph = value ? 1 : 0;
         return WD_OK;
+    case WD_OPT_GAUGE_ROWS: {
+        if (value != 2 && value != 3) return fail(h, WD_EINVAL, "WD_OPT_GAUGE_ROWS: 3 (all nine entries, default) or 2 (two-row storage)");
+        DeviceGuard guard(h->device);
+        h->gauge_rows = value;
+        return refresh_two_row_copy(h);
+    }
     default:
         return fail(h, WD_EINVAL, "wd_set_option: unknown option");
     }
@@ -466,6 +486,7 @@ int wd_get_option(const wd_handle *h, int option, long *value) {
     case WD_OPT_DEVICE_PACK: *value = h->device_pack; return WD_OK;
     case WD_OPT_HOST_PIPELINE: *value = h->host_pipeline; return WD_OK;
     case WD_OPT_GMRES_GRAPH: *value = h->gmres_graph; return WD_OK;
+    case WD_OPT_GAUGE_ROWS: *value = h->gauge_rows; return WD_OK;
     default: return WD_EINVAL;
     }
 }
@@ -475,6 +496,7 @@ int wd_get_option(const wd_handle *h, int option, long *value) {
 
 int wd::fill_params(wd_handle *h, KParams &p, const KernelInfo &k) {
     p.U = h->dU;
+    p.U2 = (h->gauge_rows == 2) ? h->dU2 : nullptr;
     p.S = h->dS;
     p.V = h->V;
     p.Vs = h->Vs;
@@ -493,7 +515,7 @@ int wd::fill_params(wd_handle *h, KParams &p, const KernelInfo &k) {
     p.device = h->device;
     p.maps = h->maps;
     p.open_mask = dd_open_mask(h);
-    p.gauge_rows = 3;
+    p.gauge_rows = (h->gauge_rows == 2 && h->dU2) ? 2 : 3;
     if (k.bx) {
         p.ntx = h->n[3] / k.bx;
         p.nty = h->n[2] / k.by;

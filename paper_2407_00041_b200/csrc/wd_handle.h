@@ -11,6 +11,7 @@ static const int kMaxPipeChunks = 16;  // T chunks of the pipelined wd_apply_hos
 using wd::MapCache;
 struct wd_gmres_state;  // wd_gmres.cu
 struct wd_dd_state;     // wd_dd.cu
+struct wd_f32_state;    // wd_f32.cu
 
 struct wd_handle {
     int n[4];
@@ -19,6 +20,7 @@ struct wd_handle {
     int device;
     cudaStream_t stream;
     double2 *dU, *dS;
+    double2 *dU2;          // two-row copy of the links (WD_OPT_GAUGE_ROWS = 2), or null
     unsigned int *dsched;  // work-queue words of the TMA kernels
     bool sched_dirty;      // a launch failed or the stream changed with work pending: re-zero the queue words first
     bool has_gauge, has_clover;
@@ -26,7 +28,7 @@ struct wd_handle {
     int nsm;               // SMs of the handle's device
     MapCache *maps;        // tensor maps of the TMA kernels, keyed by (buffers, nrhs, tile)
     // options
-    long variant, kernel_opt, tchunk_opt, zgroup_opt, device_pack, host_pipeline, gmres_graph;
+    long variant, kernel_opt, tchunk_opt, zgroup_opt, device_pack, host_pipeline, gmres_graph, gauge_rows;
     // staging
     double2 *pinned[2];
     size_t pinned_bytes;
@@ -42,6 +44,7 @@ struct wd_handle {
     std::string err;
     wd_gmres_state *gmres;  // workspace of wd_gmres (Krylov basis, Hessenberg matrix, CUDA graph), or null
     wd_dd_state *dd;        // sub-lattice state of a domain-decomposed operator (wd_create_local), or null
+    wd_f32_state *f32;      // single-precision copies of the links and of S (wd_enable_f32), or null
 };
 
 
@@ -79,6 +82,7 @@ int fill_params(wd_handle *h, KParams &p, const KernelInfo &k);
 int launch_op(wd_handle *h, const KernelInfo &k, const KParams &p, int self);
 void gmres_free(wd_handle *h);  // wd_gmres.cu
 void dd_free(wd_handle *h);     // wd_dd.cu
+void f32_free(wd_handle *h);    // wd_f32.cu
 int dd_open_mask(const wd_handle *h);  // bit mu: direction mu does not wrap on this handle (wd_create_local)
 
 }  // namespace wd

@@ -41,6 +41,7 @@ struct KParams {
     const double2 *psi;  // right-hand side 0; RHS r at + r * 12 * Vs (same for out)
     int nrhs;            // right-hand sides of this launch (> 1 only for kernels with multi_rhs)
     const double2 *U;
+    const double2 *U2;   // two-row copy of the links, double2 [4][6][Vs] (rows 0 and 1), or null
     const double2 *S;
     double2 *out;
     long long V;    // sites
@@ -97,6 +98,9 @@ void host_pack_aos_to_soa(double2 *dst, const double2 *src_aos, long long i0, lo
 void host_unpack_soa_to_aos(double2 *dst_aos, const double2 *src, long long i0, long long cnt, int ncomp);
 void host_pack_clover(double2 *dst, const double2 *src42, long long i0, long long cnt);
 void host_unpack_clover(double2 *dst42, const double2 *src, long long i0, long long cnt);
+
+// two-row copy of the gauge field (wd_pack.cu): U2[mu][k] = U[mu][k], k = 0..5
+cudaError_t launch_compress_gauge(double2 *U2, const double2 *U, long long V, long long Vs, cudaStream_t st);
 
 // device clover construction (wd_clover.cu): S slots from the device gauge field
 cudaError_t launch_build_clover(double2 *S_slots, const double2 *U, const int n[4], long long V, long long Vs,

@@ -10,6 +10,19 @@
 namespace wd {
 
 typedef double2 cd;  // complex double: x = re, y = im (one 16-byte LDG.128 / STG.128)
+typedef float2 cf;   // complex float (the FP32 variant): one 8-byte LDG.64 / STG.64
+
+// Everything below is a template on the complex type C (double2 or float2); R<C> is its real type.
+template <class C> struct RealOf;
+template <> struct RealOf<double2> { typedef double type; };
+template <> struct RealOf<float2> { typedef float type; };
+template <class C> using R = typename RealOf<C>::type;
+template <class C> __host__ __device__ __forceinline__ C mk(R<C> x, R<C> y) {
+    C c;
+    c.x = x;
+    c.y = y;
+    return c;
+}
 
 // gamma_mu, mu = 0..3 = T,Z,Y,X (R1): (gamma_mu psi)_s = i^GK[mu][s] * psi_{GC[mu][s]}.
 //   gamma_T: 0->(2,1)  1->(3,1)  2->(0,1)  3->(1,1)
@@ -26,37 +39,37 @@ WD_GAM(3, 0, 3, 1) WD_GAM(3, 1, 2, 1) WD_GAM(3, 2, 1, 3) WD_GAM(3, 3, 0, 3)
 #undef WD_GAM
 
 // a + i^K b
-template <int K> __device__ __forceinline__ cd add_ik(cd a, cd b) {
+template <int K, class C> __device__ __forceinline__ C add_ik(C a, C b) {
     constexpr int k = K & 3;
-    if (k == 0) return make_double2(a.x + b.x, a.y + b.y);
-    if (k == 1) return make_double2(a.x - b.y, a.y + b.x);
-    if (k == 2) return make_double2(a.x - b.x, a.y - b.y);
-    return make_double2(a.x + b.y, a.y - b.x);
+    if (k == 0) return mk<C>(a.x + b.x, a.y + b.y);
+    if (k == 1) return mk<C>(a.x - b.y, a.y + b.x);
+    if (k == 2) return mk<C>(a.x - b.x, a.y - b.y);
+    return mk<C>(a.x + b.y, a.y - b.x);
 }
 
 // r += a * b
-__device__ __forceinline__ void cfma(cd &r, cd a, cd b) {
+template <class C> __device__ __forceinline__ void cfma(C &r, C a, C b) {
     r.x = fma(a.x, b.x, r.x);
     r.y = fma(a.x, b.y, r.y);
     r.x = fma(-a.y, b.y, r.x);
     r.y = fma(a.y, b.x, r.y);
 }
 // r += conj(a) * b
-__device__ __forceinline__ void cfma_conj(cd &r, cd a, cd b) {
+template <class C> __device__ __forceinline__ void cfma_conj(C &r, C a, C b) {
     r.x = fma(a.x, b.x, r.x);
     r.y = fma(a.x, b.y, r.y);
     r.x = fma(a.y, b.y, r.x);
     r.y = fma(-a.y, b.x, r.y);
 }
-__device__ __forceinline__ cd cmul(cd a, cd b) {
-    return make_double2(fma(a.x, b.x, -a.y * b.y), fma(a.x, b.y, a.y * b.x));
+template <class C> __device__ __forceinline__ C cmul(C a, C b) {
+    return mk<C>(fma(a.x, b.x, -a.y * b.y), fma(a.x, b.y, a.y * b.x));
 }
-__device__ __forceinline__ cd cmul_conj(cd a, cd b) {  // conj(a) * b
-    return make_double2(fma(a.x, b.x, a.y * b.y), fma(a.x, b.y, -a.y * b.x));
+template <class C> __device__ __forceinline__ C cmul_conj(C a, C b) {  // conj(a) * b
+    return mk<C>(fma(a.x, b.x, a.y * b.y), fma(a.x, b.y, -a.y * b.x));
 }
 
 // a2: half-spinor h = rows 0,1 of (I4 + SIGN*gamma_MU) psi   (6 of 12 entries)
-template <int MU, int SIGN> __device__ __forceinline__ void project(cd h[6], const cd psi[12]) {
+template <int MU, int SIGN, class C> __device__ __forceinline__ void project(C h[6], const C psi[12]) {
     constexpr int KS = (SIGN < 0) ? 2 : 0;
 #pragma unroll
     for (int c = 0; c < 3; c++) {
@@ -66,12 +79,12 @@ template <int MU, int SIGN> __device__ __forceinline__ void project(cd h[6], con
 }
 
 // a3: g = U h (DAG = false) or g = U^H h (DAG = true) on both colour vectors; u row-major 3x3.
-template <bool DAG> __device__ __forceinline__ void su3_mul(cd g[6], const cd u[9], const cd h[6]) {
+template <bool DAG, class C> __device__ __forceinline__ void su3_mul(C g[6], const C u[9], const C h[6]) {
 #pragma unroll
     for (int s = 0; s < 2; s++)
 #pragma unroll
         for (int c = 0; c < 3; c++) {
-            cd r;
+            C r;
             if (!DAG) {
                 r = cmul(u[3 * c], h[3 * s]);
                 cfma(r, u[3 * c + 1], h[3 * s + 1]);
@@ -87,7 +100,7 @@ template <bool DAG> __device__ __forceinline__ void su3_mul(cd g[6], const cd u[
 
 // a4: acc += (I4 + SIGN*gamma_MU)-reconstruction of g.  With phi = (1 + SIGN*gamma) psi one has
 // gamma phi = SIGN*phi, hence phi_s = SIGN * i^k_s * phi_{col(s)} for the lower rows s = 2,3.
-template <int MU, int SIGN> __device__ __forceinline__ void reconstruct_add(cd acc[12], const cd g[6]) {
+template <int MU, int SIGN, class C> __device__ __forceinline__ void reconstruct_add(C acc[12], const C g[6]) {
     constexpr int KS = (SIGN < 0) ? 2 : 0;
 #pragma unroll
     for (int c = 0; c < 3; c++) {
@@ -100,8 +113,8 @@ template <int MU, int SIGN> __device__ __forceinline__ void reconstruct_add(cd a
 
 // One hopping term: acc += [(I4 + SIGN*gamma_MU) (x) W] psi,  W = U (SIGN = -1, forward
 // neighbour) or U^H (SIGN = +1, backward neighbour)   — eq. 1.13 lines 2 and 3 without the -1/2.
-template <int MU, int SIGN> __device__ __forceinline__ void hop_term(cd acc[12], const cd psi[12], const cd u[9]) {
-    cd h[6], g[6];
+template <int MU, int SIGN, class C> __device__ __forceinline__ void hop_term(C acc[12], const C psi[12], const C u[9]) {
+    C h[6], g[6];
     project<MU, SIGN>(h, psi);
     su3_mul<(SIGN > 0)>(g, u, h);
     reconstruct_add<MU, SIGN>(acc, g);
@@ -109,9 +122,9 @@ template <int MU, int SIGN> __device__ __forceinline__ void hop_term(cd acc[12],
 
 // a5: r = B p for one 6x6 Hermitian block: d = 6 real diagonal entries, a = 15 strict-upper
 // entries row-major (R6).  2*(6 real x cplx + 30 cmul) per site = 504 flop.
-__device__ __forceinline__ void herm6_mul(cd r[6], const double d[6], const cd a[15], const cd p[6]) {
+template <class C> __device__ __forceinline__ void herm6_mul(C r[6], const R<C> d[6], const C a[15], const C p[6]) {
 #pragma unroll
-    for (int i = 0; i < 6; i++) r[i] = make_double2(d[i] * p[i].x, d[i] * p[i].y);
+    for (int i = 0; i < 6; i++) r[i] = mk<C>(d[i] * p[i].x, d[i] * p[i].y);
     int k = 0;
 #pragma unroll
     for (int i = 0; i < 6; i++)

@@ -150,4 +150,17 @@ cudaError_t launch_clover_dev_to_canon(double2 *dst42, const double2 *src_slots,
     return cudaGetLastError();
 }
 
+// two-row copy of the gauge field: rows 0 and 1 of every link, double2 [4][6][Vs]
+__global__ void __launch_bounds__(256) k_compress_gauge(double2 *__restrict__ U2, const double2 *__restrict__ U, long long V, long long Vs) {
+    const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
+    if (i >= V) return;
+    const int mu = blockIdx.y / 6, k = blockIdx.y % 6;
+    U2[(long long)(6 * mu + k) * Vs + i] = U[(long long)(9 * mu + k) * Vs + i];
+}
+
+cudaError_t launch_compress_gauge(double2 *U2, const double2 *U, long long V, long long Vs, cudaStream_t st) {
+    k_compress_gauge<<<dim3((unsigned)((V + 255) / 256), 24), 256, 0, st>>>(U2, U, V, Vs);
+    return cudaGetLastError();
+}
+
 }  // namespace wd

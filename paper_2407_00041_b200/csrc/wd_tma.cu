@@ -83,26 +83,28 @@ void map_cache_clear(MapCache *c) {
 //   SA, SB  the two 6x6 blocks of S(t)                    [18][N] each
 enum { OB_C = 0, OB_T, OB_Z, OB_Y, OB_X, OB_SA, OB_SB, OB_ITEM0, OB_ITEM1, OB_COUNT };  // ITEM: work-item mailbox
 
-template <int BZ_, int BY_, int BX_, int SELF_> struct Plan {
-    static constexpr int BZ = BZ_, BY = BY_, BX = BX_, SELF = SELF_;
+// UC = complex numbers stored per link: 9, or 6 with two-row storage (WD_OPT_GAUGE_ROWS = 2: the third row of an SU(3)
+// link is the conjugate cross product of the first two and is rebuilt in registers, wd_smem_ops.cuh)
+template <int BZ_, int BY_, int BX_, int SELF_, int UC_ = 9> struct Plan {
+    static constexpr int BZ = BZ_, BY = BY_, BX = BX_, SELF = SELF_, UC = UC_;
     static constexpr int G = 1;             // right-hand sides per work item
     static constexpr int N = BZ * BY * BX;  // sites per tile = compute threads
     static constexpr int NW = N / 32;       // compute warps
     static constexpr int NTHREADS = N + 32; // + the producer warp
     static constexpr int FZ = BY * BX, FY = BZ * BX, FX = BZ * BY;  // sites per face
     static constexpr uint32_t E = 16;                               // bytes per element
-    static constexpr uint32_t SZ_C = 12 * N * E, SZ_U = 9 * N * E, SZ_S = 18 * N * E;
+    static constexpr uint32_t SZ_C = 12 * N * E, SZ_U = UC * N * E, SZ_S = 18 * N * E;
     static constexpr uint32_t OFF_C = 0;
     static constexpr uint32_t OFF_T = OFF_C + SZ_C;
     static constexpr uint32_t OFF_Z = OFF_T + SZ_U;
-    static constexpr uint32_t OFF_ZUF = OFF_Z + SZ_U, OFF_ZLO = OFF_ZUF + 9 * FZ * E, OFF_ZHI = OFF_ZLO + 12 * FZ * E;
-    static constexpr uint32_t SZ_Z = SZ_U + (9 + 24) * FZ * E;
+    static constexpr uint32_t OFF_ZUF = OFF_Z + SZ_U, OFF_ZLO = OFF_ZUF + UC * FZ * E, OFF_ZHI = OFF_ZLO + 12 * FZ * E;
+    static constexpr uint32_t SZ_Z = SZ_U + (UC + 24) * FZ * E;
     static constexpr uint32_t OFF_Y = OFF_Z + SZ_Z;
-    static constexpr uint32_t OFF_YUF = OFF_Y + SZ_U, OFF_YLO = OFF_YUF + 9 * FY * E, OFF_YHI = OFF_YLO + 12 * FY * E;
-    static constexpr uint32_t SZ_Y = SZ_U + (9 + 24) * FY * E;
+    static constexpr uint32_t OFF_YUF = OFF_Y + SZ_U, OFF_YLO = OFF_YUF + UC * FY * E, OFF_YHI = OFF_YLO + 12 * FY * E;
+    static constexpr uint32_t SZ_Y = SZ_U + (UC + 24) * FY * E;
     static constexpr uint32_t OFF_X = OFF_Y + SZ_Y;
-    static constexpr uint32_t OFF_XUF = OFF_X + SZ_U, OFF_XLO = OFF_XUF + 9 * FX * E, OFF_XHI = OFF_XLO + 12 * FX * E;
-    static constexpr uint32_t SZ_X = SZ_U + (9 + 24) * FX * E;
+    static constexpr uint32_t OFF_XUF = OFF_X + SZ_U, OFF_XLO = OFF_XUF + UC * FX * E, OFF_XHI = OFF_XLO + 12 * FX * E;
+    static constexpr uint32_t SZ_X = SZ_U + (UC + 24) * FX * E;
     static constexpr uint32_t OFF_SA = OFF_X + SZ_X;
     static constexpr uint32_t OFF_SB = OFF_SA + SZ_S;
     static constexpr uint32_t OFF_BAR = (SELF == SELF_CLOVER) ? OFF_SB + SZ_S : OFF_SA;
@@ -179,20 +181,20 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
                     const uint32_t pe = (nF & 1) ^ 1;
                     mbar_wait(bar_empty + 8 * OB_Z, pe);
                     mbar_arrive_expect_tx(bar_full + 8 * OB_Z, P::SZ_Z);
-                    tma_load_5d_hint(sbase + P::OFF_Z, &maps.u_c, bar_full + 8 * OB_Z, cx, y0, z0, t, 9, pol_u);
-                    tma_load_5d_hint(sbase + P::OFF_ZUF, &maps.u_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, 9, pol_u);
+                    tma_load_5d_hint(sbase + P::OFF_Z, &maps.u_c, bar_full + 8 * OB_Z, cx, y0, z0, t, P::UC, pol_u);
+                    tma_load_5d_hint(sbase + P::OFF_ZUF, &maps.u_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, P::UC, pol_u);
                     tma_load_5d_hint(sbase + P::OFF_ZLO, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, pc, pol_p);
                     tma_load_5d_hint(sbase + P::OFF_ZHI, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zhi, t, pc, pol_p);
                     mbar_wait(bar_empty + 8 * OB_Y, pe);
                     mbar_arrive_expect_tx(bar_full + 8 * OB_Y, P::SZ_Y);
-                    tma_load_5d_hint(sbase + P::OFF_Y, &maps.u_c, bar_full + 8 * OB_Y, cx, y0, z0, t, 18, pol_u);
-                    tma_load_5d_hint(sbase + P::OFF_YUF, &maps.u_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, 18, pol_u);
+                    tma_load_5d_hint(sbase + P::OFF_Y, &maps.u_c, bar_full + 8 * OB_Y, cx, y0, z0, t, 2 * P::UC, pol_u);
+                    tma_load_5d_hint(sbase + P::OFF_YUF, &maps.u_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, 2 * P::UC, pol_u);
                     tma_load_5d_hint(sbase + P::OFF_YLO, &maps.psi_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, pc, pol_p);
                     tma_load_5d_hint(sbase + P::OFF_YHI, &maps.psi_y, bar_full + 8 * OB_Y, cx, yhi, z0, t, pc, pol_p);
                     mbar_wait(bar_empty + 8 * OB_X, pe);
                     mbar_arrive_expect_tx(bar_full + 8 * OB_X, P::SZ_X);
-                    tma_load_5d_hint(sbase + P::OFF_X, &maps.u_c, bar_full + 8 * OB_X, cx, y0, z0, t, 27, pol_u);
-                    tma_load_5d_hint(sbase + P::OFF_XUF, &maps.u_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, 27, pol_u);
+                    tma_load_5d_hint(sbase + P::OFF_X, &maps.u_c, bar_full + 8 * OB_X, cx, y0, z0, t, 3 * P::UC, pol_u);
+                    tma_load_5d_hint(sbase + P::OFF_XUF, &maps.u_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, 3 * P::UC, pol_u);
                     tma_load_5d_hint(sbase + P::OFF_XLO, &maps.psi_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, pc, pol_p);
                     tma_load_5d_hint(sbase + P::OFF_XHI, &maps.psi_x, bar_full + 8 * OB_X, cxhi, y0, z0, t, pc, pol_p);
                 }
@@ -294,8 +296,7 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
                     prm.trace[(size_t)blockIdx.x * kTraceLen + ntrace++] = now;
                 }
 #endif
-#pragma unroll
-                for (int k = 0; k < 9; k++) u[k] = lds(smem, P::OFF_T + own + k * NS);
+                load_link<P::UC>(u, smem, P::OFF_T + own, NS);
 #pragma unroll
                 for (int c = 0; c < 12; c++) p[c] = lds(smem, P::OFF_C + own + c * NS);
                 if (j > 1) {
@@ -327,13 +328,13 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
             }
             const uint32_t pf = nF & 1;
             mbar_wait(bar_full + 8 * OB_Z, pf);
-            hop_pair_smem<1>(acc, smem, P::OFF_Z + own, NS, z_pf, z_pf_s, z_ub, z_b_s, z_pb, z_b_s, zf_on, zb_on);
+            hop_pair_smem<1, P::UC>(acc, smem, P::OFF_Z + own, NS, z_pf, z_pf_s, z_ub, z_b_s, z_pb, z_b_s, zf_on, zb_on);
             release(OB_Z);
             mbar_wait(bar_full + 8 * OB_Y, pf);
-            hop_pair_smem<2>(acc, smem, P::OFF_Y + own, NS, y_pf, y_pf_s, y_ub, y_b_s, y_pb, y_b_s, yf_on, yb_on);
+            hop_pair_smem<2, P::UC>(acc, smem, P::OFF_Y + own, NS, y_pf, y_pf_s, y_ub, y_b_s, y_pb, y_b_s, yf_on, yb_on);
             release(OB_Y);
             mbar_wait(bar_full + 8 * OB_X, pf);
-            hop_pair_smem<3>(acc, smem, P::OFF_X + own, NS, x_pf, x_pf_s, x_ub, x_b_s, x_pb, x_b_s, xf_on, xb_on);
+            hop_pair_smem<3, P::UC>(acc, smem, P::OFF_X + own, NS, x_pf, x_pf_s, x_ub, x_b_s, x_pb, x_b_s, xf_on, xb_on);
             release(OB_X);
             release(OB_C);
             nC++;
@@ -374,6 +375,12 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
 
 // ---------------------------------------------------------------- host side
 template <int BZ, int BY, int BX, int SELF> static cudaError_t launch_tma_self(const KParams &p, cudaStream_t st) {
+    if (p.gauge_rows == 2) {  // two-row link storage: boxes of 6 components from the compressed gauge array
+        using P = Plan<BZ, BY, BX, SELF, 6>;
+        KParams q = p;
+        q.U = p.U2;
+        return launch_tma_kernel<P>(k_tma<P>, q, st, /*ucomp*/ 6, /*scomp*/ 18, CHUNK_COST_MODEL, /*rb*/ 4);
+    }
     using P = Plan<BZ, BY, BX, SELF>;
     return launch_tma_kernel<P>(k_tma<P>, p, st, /*ucomp*/ 9, /*scomp*/ 18, CHUNK_COST_MODEL, /*rb*/ 4);
 }

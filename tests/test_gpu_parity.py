@@ -437,3 +437,29 @@ def test_cfg5_full_size_multi_rhs_whole_lattice(torch, capsys):
     _report(capsys, f"lattice {'x'.join(map(str, dims))} x{nrhs} kernel {kname}: {nrhs} x {V} sites compared, "
                     f"max rel_l2 {max(errs):.3e}, worst component {max(worsts):.3e}" + ("" if full else "  (WD_TEST_SMALL)"))
     assert max(errs) <= TOL and max(worsts) <= 1e-13
+
+
+# ---------------------------------------------------------------- two-row gauge storage (opt-in)
+@pytest.mark.parametrize("dims", [(8, 8, 8, 16), (6, 4, 12, 32)])
+def test_two_row_gauge_storage_on_su3_links(torch, dims):
+    """WD_OPT_GAUGE_ROWS = 2: the fused TMA kernel reads rows 0, 1 of every link and rebuilds row 2 as the conjugate
+    cross product — exact for SU(3) links up to rounding, so the 1e-13 bar holds on Haar and exp(i eps H) links; set
+    before or after the gauge field is loaded; switching back restores the nine-entry path bit for bit."""
+    m0, csw = -0.4, 1.0
+    for U in (wdinputs.gauge_haar(dims, 901), wdinputs.gauge_exp(dims, 902, 0.5)):
+        psi = wdinputs.spinor(dims, 903, nrhs=2)
+        C = oracle.build_clover(dims, m0, csw, U)
+        ref = oracle.apply(dims, m0, U, C, psi)
+        with Op(torch, dims, m0, csw, U, C, kernel=wd.kernel_id("tma_2x4x16")) as op:
+            full = op.apply(psi, 2)
+            wd.wd_set_option(op.h, wd.WD_OPT_GAUGE_ROWS, 2)  # after the load
+            two = op.apply(psi, 2)
+            assert rel_l2(two, ref) <= TOL and not np.array_equal(two, full)
+            wd.wd_set_option(op.h, wd.WD_OPT_GAUGE_ROWS, 3)
+            assert np.array_equal(op.apply(psi, 2), full)
+        with Op(torch, dims, m0, 0.0, gauge_rows=2, kernel=wd.kernel_id("tma_2x4x16")) as op:  # before the load, pure Wilson
+            wd.wd_load_gauge(op.h, U)
+            assert rel_l2(op.apply(psi, 2), oracle.apply(dims, m0, U, None, psi)) <= TOL
+    with Op(torch, dims, m0, 0.0) as op:
+        with pytest.raises(wd.WDError):
+            wd.wd_set_option(op.h, wd.WD_OPT_GAUGE_ROWS, 1)
