@@ -459,6 +459,7 @@ def run_ours(args):
     alg_bytes_launch = alg_bytes_step / launches_per_step  # tma_*: one launch per step, all RHS
     achieved = alg_bytes_launch / (avg_launch_ms * 1e-3) / 1e9
     traffic, traffic_src = (ncu_traffic(kname + ("/clover" if clover else "/wilson") + ("" if nrhs == 1 else f"/x{nrhs}")
+                                        + ("/rows2" if args.gauge_rows == 2 else "")
                                         + "@" + "x".join(map(str, dims))))
     roofline = {
         "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
@@ -523,7 +524,7 @@ def run_ours(args):
         line["f32"] = {"ms_per_step": fms, "steps": nst, "value": V * nrhs * flop / (fms * 1e-3) / 1e9, "unit": "GFLOP/s",
                        "dtype": "f32", "algorithmic_gbs": alg_bytes_step / 2 / (fms * 1e-3) / 1e9,
                        "frac_of_measured_peak": alg_bytes_step / 2 / (fms * 1e-3) / 1e9 / peak,
-                       "kernel": "tile_1x4x4x16<float2> / linear256<float2> (one-thread-per-site LDG kernels)"}
+                       "kernel": "tma_2x4x16<float2>: the TMA kernel on 8-byte elements, two persistent CTAs per SM"}
         del fin, fout
     # ---- restarted GMRES(M) on the device around the operator: the consumer of the applies
     if args.gmres and rank == 0 and nrhs == 1:

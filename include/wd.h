@@ -74,6 +74,8 @@ enum {
                               rebuilds row 2 = conj(row 0 x row 1) in registers.  EXACT ONLY FOR SU(3) LINKS: with 2 the
                               "general 3x3 complex" promise of wd_load_gauge (R11) does not hold.  Costs a second,
                               two-row copy of the gauge field on the device. */
+    ,WD_OPT_F32_KERNEL = 9 /* wd_apply_f32: 0 = automatic (the TMA kernel where its 2x4x16 tile divides the lattice), 1 = always
+                              the one-thread-per-site kernels */
 };
 
 /* Create an operator for a T x Z x Y x X periodic lattice.  Every extent >= 1 (n = 2, where

@@ -108,6 +108,7 @@ int wd_create(wd_handle **out, int T, int Z, int Y, int X, double m0, double csw
     h->host_pipeline = 1;
     h->gmres_graph = 1;
     h->gauge_rows = 3;
+    h->f32_kernel = 0;
     h->variant = 0;
     h->kernel_opt = -1;
     h->tchunk_opt = 0;
@@ -465,6 +466,10 @@ int wd_set_option(wd_handle *h, int option, long value) {
     case WD_OPT_GMRES_GRAPH:
         h->gmres_graph = value ? 1 : 0;
         return WD_OK;
+    case WD_OPT_F32_KERNEL:
+        if (value != 0 && value != 1) return fail(h, WD_EINVAL, "WD_OPT_F32_KERNEL: 0 (automatic) or 1 (one-thread-per-site kernels)");
+        h->f32_kernel = value;
+        return WD_OK;
     case WD_OPT_GAUGE_ROWS: {
         if (value != 2 && value != 3) return fail(h, WD_EINVAL, "WD_OPT_GAUGE_ROWS: 3 (all nine entries, default) or 2 (two-row storage)");
         DeviceGuard guard(h->device);
@@ -487,6 +492,7 @@ int wd_get_option(const wd_handle *h, int option, long *value) {
     case WD_OPT_HOST_PIPELINE: *value = h->host_pipeline; return WD_OK;
     case WD_OPT_GMRES_GRAPH: *value = h->gmres_graph; return WD_OK;
     case WD_OPT_GAUGE_ROWS: *value = h->gauge_rows; return WD_OK;
+    case WD_OPT_F32_KERNEL: *value = h->f32_kernel; return WD_OK;
     default: return WD_EINVAL;
     }
 }
@@ -515,6 +521,7 @@ int wd::fill_params(wd_handle *h, KParams &p, const KernelInfo &k) {
     p.device = h->device;
     p.maps = h->maps;
     p.open_mask = dd_open_mask(h);
+    p.esize = 16;
     p.gauge_rows = (h->gauge_rows == 2 && h->dU2) ? 2 : 3;
     if (k.bx) {
         p.ntx = h->n[3] / k.bx;

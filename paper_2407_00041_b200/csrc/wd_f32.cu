@@ -1,6 +1,7 @@
 // wd_f32.cu — the FP32 variant of the operator (the paper's PRECISION templating):
-// the same one-pass kernels (wd_ldg_kernels.cuh) instantiated on float2, on single-precision copies of the links and of
-// S that live beside the FP64 fields.  Halves every byte of the path (768 instead of 1536 algorithmic B/site); all
+// the same kernels instantiated on float2 — the TMA-staged T-marching kernel of wd_tma.cu on 8-byte elements where its
+// tile divides the lattice, the one-thread-per-site kernels of wd_ldg_kernels.cuh otherwise — on single-precision copies
+// of the links and of S that live beside the FP64 fields.  Halves every byte of the path (768 instead of 1536 algorithmic B/site); all
 // arithmetic, including the accumulation over the eight hops, is FP32 — the error budget is derived in DESIGN.md
 // ("Tolerance of the FP32 variant").  Device layout: the FP64 layout with 8-byte elements, float2 [nrhs][12][Vs].
 #include <cstring>
@@ -92,15 +93,28 @@ int wd_apply_f32(wd_handle *h, void *dev_out, const void *dev_in, int nrhs) {
     if (o < i + bytes && i < o + bytes) return fail(h, WD_EINVAL, "wd_apply_f32: out overlaps in");
     if (!h->f32 || !h->f32->dU) return fail(h, WD_ESTATE, "wd_apply_f32: call wd_enable_f32 after loading the fields");
     if (h->csw != 0.0 && !h->f32->has_clover) return fail(h, WD_ESTATE, "wd_apply_f32: no FP32 self-coupling field (wd_enable_f32)");
-    // geometry: the 1x4x4x16 tile kernel where it divides the lattice, else the linear kernel
+    const int self = h->f32->has_clover ? SELF_CLOVER : SELF_MASS;
+    // geometry: the TMA kernel (the FP64 skeleton on 8-byte elements) where its 2x4x16 tile divides the lattice, else
+    // the one-thread-per-site kernels: 1x4x4x16 tiles, or the linear kernel for any extents
+    const bool tma = h->f32_kernel != 1 && h->n[1] % 2 == 0 && h->n[2] % 4 == 0 && h->n[3] % 16 == 0;
     const bool tiled = h->n[1] % 4 == 0 && h->n[2] % 4 == 0 && h->n[3] % 16 == 0;
     const KernelInfo *ki = nullptr;
     for (int id = 0; id < kernel_count(); id++)
-        if (!strcmp(kernel_info(id).name, tiled ? "tile_1x4x4x16" : "linear256")) ki = &kernel_info(id);
+        if (!strcmp(kernel_info(id).name, tma ? "tma_2x4x16" : tiled ? "tile_1x4x4x16" : "linear256")) ki = &kernel_info(id);
     KParams p;
     int rc = fill_params(h, p, *ki);
     if (rc) return rc;
-    const int self = h->f32->has_clover ? SELF_CLOVER : SELF_MASS;
+    if (tma) {  // one launch for all right-hand sides; the field pointers of p are float2 arrays (p.esize = 8)
+        p.psi = (const double2 *)dev_in;
+        p.out = (double2 *)dev_out;
+        p.U = (const double2 *)h->f32->dU;
+        p.S = (const double2 *)h->f32->dS;
+        p.U2 = nullptr;
+        p.gauge_rows = 3;
+        p.esize = 8;
+        p.nrhs = nrhs;
+        return launch_op(h, *ki, p, self);
+    }
     const size_t per = (size_t)h->Vs * kSpinorComps;
     for (int r = 0; r < nrhs; r++) {
         const KP<cf> q = make_kp<cf>(p, (const cf *)dev_in + r * per, h->f32->dU, h->f32->dS, (cf *)dev_out + r * per);

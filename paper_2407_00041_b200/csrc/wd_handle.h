@@ -28,7 +28,7 @@ struct wd_handle {
     int nsm;               // SMs of the handle's device
     MapCache *maps;        // tensor maps of the TMA kernels, keyed by (buffers, nrhs, tile)
     // options
-    long variant, kernel_opt, tchunk_opt, zgroup_opt, device_pack, host_pipeline, gmres_graph, gauge_rows;
+    long variant, kernel_opt, tchunk_opt, zgroup_opt, device_pack, host_pipeline, gmres_graph, gauge_rows, f32_kernel;
     // staging
     double2 *pinned[2];
     size_t pinned_bytes;

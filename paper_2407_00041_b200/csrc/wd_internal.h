@@ -60,6 +60,7 @@ struct KParams {
     int nsm, device;             // SM count and ordinal of the handle's device (read once in wd_create)
     MapCache *maps;              // tensor-map cache of the handle (may be null: encode per launch)
     int open_mask;               // bit mu: direction mu does not wrap (sub-lattice of a domain decomposition, wd_dd.cu)
+    int esize;                   // bytes per complex element of the fields: 16 (FP64), 8 (FP32 variant: the pointers above are float2)
     int gauge_rows;              // 3: links stored as 9 complex; 2: two-row storage, third row rebuilt in the kernel
 };
 

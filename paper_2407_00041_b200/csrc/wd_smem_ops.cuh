@@ -9,8 +9,8 @@
 namespace wd {
 
 // ---------------------------------------------------------------- shared-memory operand fetch
-__device__ __forceinline__ cd lds(const unsigned char *smem, uint32_t off) {
-    return *reinterpret_cast<const cd *>(smem + off);
+template <class C = cd> __device__ __forceinline__ C lds(const unsigned char *smem, uint32_t off) {
+    return *reinterpret_cast<const C *>(smem + off);
 }
 
 // One direction MU != T of the stencil for the thread's site: both hops, operands from shared
@@ -18,37 +18,37 @@ __device__ __forceinline__ cd lds(const unsigned char *smem, uint32_t off) {
 // are shared-memory addresses).
 // One link from a shared-memory SoA box into registers.  UC = 9: all nine entries.  UC = 6 (two-row storage): rows 0
 // and 1 are loaded, row 2 = conj(row 0 x row 1), which holds for every SU(3) matrix (unitary, determinant 1).
-template <int UC> __device__ __forceinline__ void load_link(cd u[9], const unsigned char *smem, uint32_t off, uint32_t stride) {
+template <int UC, class C = cd> __device__ __forceinline__ void load_link(C u[9], const unsigned char *smem, uint32_t off, uint32_t stride) {
 #pragma unroll
-    for (int k = 0; k < UC; k++) u[k] = lds(smem, off + k * stride);
+    for (int k = 0; k < UC; k++) u[k] = lds<C>(smem, off + k * stride);
     if (UC == 6) {
 #pragma unroll
         for (int k = 0; k < 3; k++) {
-            const cd a = u[(k + 1) % 3], b = u[3 + (k + 2) % 3], c = u[(k + 2) % 3], d = u[3 + (k + 1) % 3];
+            const C a = u[(k + 1) % 3], b = u[3 + (k + 2) % 3], c = u[(k + 2) % 3], d = u[3 + (k + 1) % 3];
             // conj(a b - c d)
-            u[6 + k] = make_double2(fma(a.x, b.x, -a.y * b.y) - fma(c.x, d.x, -c.y * d.y),
-                                    -(fma(a.x, b.y, a.y * b.x) - fma(c.x, d.y, c.y * d.x)));
+            u[6 + k] = mk<C>(fma(a.x, b.x, -a.y * b.y) - fma(c.x, d.x, -c.y * d.y),
+                             -(fma(a.x, b.y, a.y * b.x) - fma(c.x, d.y, c.y * d.x)));
         }
     }
 }
 
 // fwd / bwd = false: that hop crosses an open boundary of a domain-decomposed sub-lattice and is left out here (the
 // exterior kernel of wd_dd.cu adds it from the neighbour's half-spinor); always true on a periodic lattice.
-template <int MU, int UC = 9>
-__device__ __forceinline__ void hop_pair_smem(cd acc[12], const unsigned char *smem, uint32_t u_own, uint32_t u_own_stride,
+template <int MU, int UC = 9, class C = cd>
+__device__ __forceinline__ void hop_pair_smem(C acc[12], const unsigned char *smem, uint32_t u_own, uint32_t u_own_stride,
                                               uint32_t pf, uint32_t pf_stride, uint32_t ub, uint32_t ub_stride,
                                               uint32_t pb, uint32_t pb_stride, bool fwd = true, bool bwd = true) {
-    cd p[12], u[9];
+    C p[12], u[9];
     if (fwd) {
-        load_link<UC>(u, smem, u_own, u_own_stride);
+        load_link<UC, C>(u, smem, u_own, u_own_stride);
 #pragma unroll
-        for (int c = 0; c < 12; c++) p[c] = lds(smem, pf + c * pf_stride);
+        for (int c = 0; c < 12; c++) p[c] = lds<C>(smem, pf + c * pf_stride);
         hop_term<MU, -1>(acc, p, u);
     }
     if (bwd) {
-        load_link<UC>(u, smem, ub, ub_stride);
+        load_link<UC, C>(u, smem, ub, ub_stride);
 #pragma unroll
-        for (int c = 0; c < 12; c++) p[c] = lds(smem, pb + c * pb_stride);
+        for (int c = 0; c < 12; c++) p[c] = lds<C>(smem, pb + c * pb_stride);
         hop_term<MU, +1>(acc, p, u);
     }
 }

@@ -51,18 +51,19 @@ static EncodeTiledFn encode_fn() {
 }
 
 cudaError_t encode_field_map(CUtensorMap *map, const void *base, const int n[4], long long Vs, int ncomp, int bx,
-                             int by, int bz, int bc) {
+                             int by, int bz, int bc, int esize) {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return cudaErrorNotSupported;
     const cuuint64_t T = n[0], Z = n[1], Y = n[2], X = n[3];
     const cuuint64_t dims[5] = {2 * X, Y, Z, T, (cuuint64_t)ncomp};
-    const cuuint64_t strides[4] = {X * 16, X * Y * 16, X * Y * Z * 16, (cuuint64_t)Vs * 16};  // bytes, dims 1..4
+    const cuuint64_t es = (cuuint64_t)esize;  // bytes per complex element: 16 (FP64) or 8 (FP32)
+    const cuuint64_t strides[4] = {X * es, X * Y * es, X * Y * Z * es, (cuuint64_t)Vs * es};  // bytes, dims 1..4
     const cuuint32_t box[5] = {(cuuint32_t)(2 * bx), (cuuint32_t)by, (cuuint32_t)bz, 1u, (cuuint32_t)bc};
     const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
-    const CUtensorMapL2promotion promo = (bx * 16 >= 256)   ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B
-                                         : (bx * 16 >= 128) ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B
+    const CUtensorMapL2promotion promo = (bx * es >= 256)   ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B
+                                         : (bx * es >= 128) ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B
                                                             : CU_TENSOR_MAP_L2_PROMOTION_NONE;
-    const CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, const_cast<void *>(base), dims, strides, box, estr,
+    const CUresult r = fn(map, (esize == 8) ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, const_cast<void *>(base), dims, strides, box, estr,
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, promo,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return (r == CUDA_SUCCESS) ? cudaSuccess : cudaErrorInvalidValue;
@@ -81,48 +82,74 @@ void map_cache_clear(MapCache *c) {
 //   Z  U_Z(t) interior | U_Z face z0-1 | psi faces z0-1, z0+BZ      [9][N] [9][FZ] [12][FZ] [12][FZ]
 //   Y  same for Y;  X  same for X
 //   SA, SB  the two 6x6 blocks of S(t)                    [18][N] each
-enum { OB_C = 0, OB_T, OB_Z, OB_Y, OB_X, OB_SA, OB_SB, OB_ITEM0, OB_ITEM1, OB_COUNT };  // ITEM: work-item mailbox
+enum { OB_C = 0, OB_T, OB_Z, OB_Y, OB_X, OB_SA };  // then OB_SB, OB_ITEM0, OB_ITEM1 (work-item mailbox): see Plan
 
 // UC = complex numbers stored per link: 9, or 6 with two-row storage (WD_OPT_GAUGE_ROWS = 2: the third row of an SU(3)
 // link is the conjugate cross product of the first two and is rebuilt in registers, wd_smem_ops.cuh)
-template <int BZ_, int BY_, int BX_, int SELF_, int UC_ = 9> struct Plan {
+// C = complex element type: double2 (FP64) or float2 (the FP32 variant, wd_f32.cu).  Sub-objects are padded to 128
+// bytes, the alignment TMA needs for a shared-memory destination (only the 8-byte X link face is not a multiple already).
+constexpr uint32_t al128(uint32_t x) { return (x + 127u) & ~127u; }
+template <int BZ_, int BY_, int BX_, int SELF_, int UC_ = 9, class C_ = cd> struct Plan {
+    typedef C_ C;
     static constexpr int BZ = BZ_, BY = BY_, BX = BX_, SELF = SELF_, UC = UC_;
     static constexpr int G = 1;             // right-hand sides per work item
     static constexpr int N = BZ * BY * BX;  // sites per tile = compute threads
     static constexpr int NW = N / 32;       // compute warps
     static constexpr int NTHREADS = N + 32; // + the producer warp
-    static constexpr int FZ = BY * BX, FY = BZ * BX, FX = BZ * BY;  // sites per face
-    static constexpr uint32_t E = 16;                               // bytes per element
+    static constexpr uint32_t E = sizeof(C);                        // bytes per element
+    // A TMA box must be a multiple of 16 bytes wide: the X faces of 8-byte elements are fetched two sites wide (the
+    // neighbour column and the one beyond it), of which the consumers read one.
+    static constexpr int XW = (E == 8) ? 2 : 1;
+
+    static constexpr int FZ = BY * BX, FY = BZ * BX, FX = BZ * BY * XW;  // sites stored per face
     static constexpr uint32_t SZ_C = 12 * N * E, SZ_U = UC * N * E, SZ_S = 18 * N * E;
     static constexpr uint32_t OFF_C = 0;
     static constexpr uint32_t OFF_T = OFF_C + SZ_C;
     static constexpr uint32_t OFF_Z = OFF_T + SZ_U;
-    static constexpr uint32_t OFF_ZUF = OFF_Z + SZ_U, OFF_ZLO = OFF_ZUF + UC * FZ * E, OFF_ZHI = OFF_ZLO + 12 * FZ * E;
-    static constexpr uint32_t SZ_Z = SZ_U + (UC + 24) * FZ * E;
-    static constexpr uint32_t OFF_Y = OFF_Z + SZ_Z;
-    static constexpr uint32_t OFF_YUF = OFF_Y + SZ_U, OFF_YLO = OFF_YUF + UC * FY * E, OFF_YHI = OFF_YLO + 12 * FY * E;
-    static constexpr uint32_t SZ_Y = SZ_U + (UC + 24) * FY * E;
-    static constexpr uint32_t OFF_X = OFF_Y + SZ_Y;
-    static constexpr uint32_t OFF_XUF = OFF_X + SZ_U, OFF_XLO = OFF_XUF + UC * FX * E, OFF_XHI = OFF_XLO + 12 * FX * E;
-    static constexpr uint32_t SZ_X = SZ_U + (UC + 24) * FX * E;
-    static constexpr uint32_t OFF_SA = OFF_X + SZ_X;
+    static constexpr uint32_t OFF_ZUF = OFF_Z + SZ_U, OFF_ZLO = OFF_ZUF + al128(UC * FZ * E), OFF_ZHI = OFF_ZLO + 12 * FZ * E;
+    static constexpr uint32_t SZ_Z = SZ_U + (UC + 24) * FZ * E;  // bytes the TMA delivers
+    static constexpr uint32_t SP_Z = SZ_U + al128(UC * FZ * E) + 24 * FZ * E;  // bytes it occupies
+    static constexpr uint32_t OFF_Y = OFF_Z + SP_Z;
+    static constexpr uint32_t OFF_YUF = OFF_Y + SZ_U, OFF_YLO = OFF_YUF + al128(UC * FY * E), OFF_YHI = OFF_YLO + 12 * FY * E;
+    static constexpr uint32_t SZ_Y = SZ_U + (UC + 24) * FY * E;  // bytes the TMA delivers
+    static constexpr uint32_t SP_Y = SZ_U + al128(UC * FY * E) + 24 * FY * E;  // bytes it occupies
+    static constexpr uint32_t OFF_X = OFF_Y + SP_Y;
+    static constexpr uint32_t OFF_XUF = OFF_X + SZ_U, OFF_XLO = OFF_XUF + al128(UC * FX * E), OFF_XHI = OFF_XLO + 12 * FX * E;
+    static constexpr uint32_t SZ_X = SZ_U + (UC + 24) * FX * E;  // bytes the TMA delivers
+    static constexpr uint32_t SP_X = SZ_U + al128(UC * FX * E) + 24 * FX * E;  // bytes it occupies
+    static constexpr uint32_t OFF_SA = OFF_X + SP_X;
     static constexpr uint32_t OFF_SB = OFF_SA + SZ_S;
     static constexpr uint32_t OFF_BAR = (SELF == SELF_CLOVER) ? OFF_SB + SZ_S : OFF_SA;
-    static constexpr uint32_t OFF_MAIL = OFF_BAR + 2 * OB_COUNT * 8;  // int[2]: item index per mailbox slot
-    static constexpr uint32_t SMEM = OFF_MAIL + 16;
-    static_assert(N % 32 == 0 && FZ % 8 == 0 && FY % 8 == 0 && FX % 8 == 0, "tile faces must keep 128-byte alignment");
+    // COMPACT (8-byte elements with S): the two blocks of S share one barrier pair and the mailbox has one slot, which
+    // brings the plan to 115 704 B — two CTAs (8 compute warps) per SM; measured on the FP32 Wilson kernel: 2.45 -> 1.93 ms
+    static constexpr bool COMPACT = (E == 8) && (SELF == SELF_CLOVER);
+    static constexpr int OB_SB = COMPACT ? OB_SA : OB_SA + 1;
+    static constexpr int OB_ITEM0 = OB_SB + 1, OB_ITEM1 = COMPACT ? OB_ITEM0 : OB_ITEM0 + 1;
+    static constexpr int OB_COUNT = OB_ITEM1 + 1;
+    static constexpr uint32_t OFF_MAIL = OFF_BAR + 2 * OB_COUNT * 8;  // int per mailbox slot: item index
+    static constexpr uint32_t SMEM = OFF_MAIL + (COMPACT ? 8 : 16);
+    // persistent CTAs per SM: two (8 compute warps) where two plans plus the 1 KB the system reserves per CTA fit the
+    // 228 KB of an SM — the plans of 8-byte elements without S buffers
+    static constexpr int CTAS_PER_SM = (2 * (SMEM + 1024) <= 233472) ? 2 : 1;
+    static_assert(N % 32 == 0 && (12 * FZ * E) % 128 == 0 && (12 * FY * E) % 128 == 0 && (12 * FX * E) % 128 == 0 && SZ_U % 128 == 0,
+                  "tile faces must keep 128-byte alignment");
     static_assert(SMEM <= 232448, "shared-memory plan exceeds 227 KB");
 };
 
 // ---------------------------------------------------------------- the kernel
-template <class P>
-__global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ TmaMaps maps, const TmaParams prm) {
+// OPEN = false: a periodic lattice — the open-boundary predicates fold away (they cost 9 % more instructions)
+template <class P, bool OPEN>
+__global__ void __launch_bounds__(P::NTHREADS, P::CTAS_PER_SM) k_tma(const __grid_constant__ TmaMaps maps, const TmaParams prm) {
     extern __shared__ __align__(128) unsigned char smem[];
     const uint32_t sbase = smem_u32(smem);
+    constexpr int OB_SB = P::OB_SB, OB_ITEM0 = P::OB_ITEM0, OB_COUNT = P::OB_COUNT;
     const uint32_t bar_full = sbase + P::OFF_BAR, bar_empty = bar_full + OB_COUNT * 8;
     const int tid = threadIdx.x;
+    typedef typename P::C C;
+    typedef R<C> Real;
     constexpr int BZ = P::BZ, BY = P::BY, BX = P::BX, N = P::N;
     constexpr bool CLOVER = (P::SELF == SELF_CLOVER);
+    const Real half = (Real)0.5, mass = (Real)prm.mass;
 
     if (tid == 0) {
         if (sbase & 127u) __trap();  // TMA destinations need 128-byte alignment
@@ -151,17 +178,17 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
         for (uint32_t seq = 0;; seq++) {
             // next work item from the atomic queue, handed to the consumers through a two-slot mailbox
             const int item = fetch_item(prm, seq);
-            const uint32_t slot = seq & 1, mpar = (seq >> 1) & 1;
+            const uint32_t slot = P::COMPACT ? 0 : (seq & 1), mpar = P::COMPACT ? (seq & 1) : ((seq >> 1) & 1);
             mbar_wait(bar_empty + 8 * (OB_ITEM0 + slot), mpar ^ 1);
             mail[slot] = item;
             mbar_arrive(bar_full + 8 * (OB_ITEM0 + slot));
             if (item < 0) break;
             const Item it = decode_item<P>(prm, item);
-            const int cx = 2 * it.x0, y0 = it.y0, z0 = it.z0;  // dim-0 coordinates count doubles
+            const int cx = 2 * it.x0, y0 = it.y0, z0 = it.z0;  // dim-0 coordinates count real numbers
             const int pc = 12 * it.rhs0;                       // first component of this right-hand side
             const int zlo = (z0 == 0) ? Z - 1 : z0 - 1, zhi = (z0 + BZ == Z) ? 0 : z0 + BZ;
             const int ylo = (y0 == 0) ? Y - 1 : y0 - 1, yhi = (y0 + BY == Y) ? 0 : y0 + BY;
-            const int cxlo = 2 * ((it.x0 == 0) ? X - 1 : it.x0 - 1), cxhi = 2 * ((it.x0 + BX == X) ? 0 : it.x0 + BX);
+            const int cxlo = 2 * ((it.x0 == 0) ? X - P::XW : it.x0 - P::XW), cxhi = 2 * ((it.x0 + BX == X) ? 0 : it.x0 + BX);
             int t = (it.t0 == 0) ? T - 1 : it.t0 - 1;
             // prologue: psi(t0-1), only to seed the carried half-spinor
             mbar_wait(bar_empty + 8 * OB_C, (nC & 1) ^ 1);
@@ -209,10 +236,12 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
                 if (full && CLOVER) {
                     const uint32_t pe = (nF & 1) ^ 1;
                     mbar_wait(bar_empty + 8 * OB_SA, pe);
-                    mbar_arrive_expect_tx(bar_full + 8 * OB_SA, P::SZ_S);
+                    mbar_arrive_expect_tx(bar_full + 8 * OB_SA, P::COMPACT ? 2 * P::SZ_S : P::SZ_S);
                     tma_load_5d_hint(sbase + P::OFF_SA, &maps.s_c, bar_full + 8 * OB_SA, cx, y0, z0, t, 0, pol_s);
-                    mbar_wait(bar_empty + 8 * OB_SB, pe);
-                    mbar_arrive_expect_tx(bar_full + 8 * OB_SB, P::SZ_S);
+                    if (!P::COMPACT) {
+                        mbar_wait(bar_empty + 8 * OB_SB, pe);
+                        mbar_arrive_expect_tx(bar_full + 8 * OB_SB, P::SZ_S);
+                    }
                     tma_load_5d_hint(sbase + P::OFF_SB, &maps.s_c, bar_full + 8 * OB_SB, cx, y0, z0, t, 18, pol_s);
                 }
                 if (full) nF++;
@@ -226,7 +255,9 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
     constexpr uint32_t E = P::E, NS = N * E;
     const uint32_t own = tid * E;
     // operand addresses (bytes from the start of shared memory): interior or face storage
-    const uint32_t fz = (ly * BX + lx) * E, fy = (lz * BX + lx) * E, fx = (lz * BY + ly) * E;
+    const uint32_t fz = (ly * BX + lx) * E, fy = (lz * BX + lx) * E;
+    // X faces: XW sites per (z, y) row; the neighbour column is the last one of the low face, the first of the high face
+    const uint32_t fxl = ((lz * BY + ly) * P::XW + (P::XW - 1)) * E, fxh = ((lz * BY + ly) * P::XW) * E;
     const bool zf_in = lz < BZ - 1, zb_in = lz > 0, yf_in = ly < BY - 1, yb_in = ly > 0, xf_in = lx < BX - 1, xb_in = lx > 0;
     const uint32_t z_pf = zf_in ? P::OFF_C + own + P::FZ * E : P::OFF_ZHI + fz, z_pf_s = zf_in ? NS : P::FZ * E;
     const uint32_t z_pb = zb_in ? P::OFF_C + own - P::FZ * E : P::OFF_ZLO + fz, z_b_s = zb_in ? NS : P::FZ * E;
@@ -234,9 +265,9 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
     const uint32_t y_pf = yf_in ? P::OFF_C + own + BX * E : P::OFF_YHI + fy, y_pf_s = yf_in ? NS : P::FY * E;
     const uint32_t y_pb = yb_in ? P::OFF_C + own - BX * E : P::OFF_YLO + fy, y_b_s = yb_in ? NS : P::FY * E;
     const uint32_t y_ub = yb_in ? P::OFF_Y + own - BX * E : P::OFF_YUF + fy;
-    const uint32_t x_pf = xf_in ? P::OFF_C + own + E : P::OFF_XHI + fx, x_pf_s = xf_in ? NS : P::FX * E;
-    const uint32_t x_pb = xb_in ? P::OFF_C + own - E : P::OFF_XLO + fx, x_b_s = xb_in ? NS : P::FX * E;
-    const uint32_t x_ub = xb_in ? P::OFF_X + own - E : P::OFF_XUF + fx;
+    const uint32_t x_pf = xf_in ? P::OFF_C + own + E : P::OFF_XHI + fxh, x_pf_s = xf_in ? NS : P::FX * E;
+    const uint32_t x_pb = xb_in ? P::OFF_C + own - E : P::OFF_XLO + fxl, x_b_s = xb_in ? NS : P::FX * E;
+    const uint32_t x_ub = xb_in ? P::OFF_X + own - E : P::OFF_XUF + fxl;
 
     auto release = [&](int ob) {
         __syncwarp();
@@ -249,34 +280,34 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
 #ifdef WD_EXPERIMENTS
     int ntrace = 0;
 #endif
-    cd hprev[6];                      // rows 0,1 of (1 + gamma_T) psi(t-1)
-    cd outp[12];                      // out(t-1) still missing its forward-T hop
+    C hprev[6];                      // rows 0,1 of (1 + gamma_T) psi(t-1)
+    C outp[12];                      // out(t-1) still missing its forward-T hop
 
     const volatile int *mail = reinterpret_cast<const volatile int *>(smem + P::OFF_MAIL);
     for (uint32_t seq = 0;; seq++) {
-        const uint32_t slot = seq & 1, mpar = (seq >> 1) & 1;
+        const uint32_t slot = P::COMPACT ? 0 : (seq & 1), mpar = P::COMPACT ? (seq & 1) : ((seq >> 1) & 1);
         mbar_wait(bar_full + 8 * (OB_ITEM0 + slot), mpar);
         const int item = mail[slot];
         release(OB_ITEM0 + slot);
         if (item < 0) break;
         const Item it = decode_item<P>(prm, item);
         const long long site0 = ((long long)(it.z0 + lz) * Y + (it.y0 + ly)) * X + (it.x0 + lx);
-        cd *__restrict__ out = prm.out + (long long)it.rhs0 * 12 * V;
+        C *__restrict__ out = reinterpret_cast<C *>(prm.out) + (long long)it.rhs0 * 12 * V;
         // open boundaries of a domain-decomposed sub-lattice: hops that would cross them are left out
-        const int open = prm.open_mask;
+        const int open = OPEN ? prm.open_mask : 0;
         const bool zf_on = !((open & 2) && it.z0 + lz == Z - 1), zb_on = !((open & 2) && it.z0 + lz == 0);
         const bool yf_on = !((open & 4) && it.y0 + ly == Y - 1), yb_on = !((open & 4) && it.y0 + ly == 0);
         const bool xf_on = !((open & 8) && it.x0 + lx == X - 1), xb_on = !((open & 8) && it.x0 + lx == 0);
         int t = (it.t0 == 0) ? T - 1 : it.t0 - 1;
         {   // prologue: seed the carried half-spinor from psi(t0-1)
-            cd p[12];
+            C p[12];
             mbar_wait(bar_full + 8 * OB_C, nC & 1);
 #pragma unroll
-            for (int c = 0; c < 12; c++) p[c] = lds(smem, P::OFF_C + own + c * NS);
+            for (int c = 0; c < 12; c++) p[c] = lds<C>(smem, P::OFF_C + own + c * NS);
             project<0, +1>(hprev, p);
             if ((open & 1) && it.t0 == 0) {
 #pragma unroll
-                for (int c = 0; c < 6; c++) hprev[c] = make_double2(0.0, 0.0);
+                for (int c = 0; c < 6; c++) hprev[c] = mk<C>(0, 0);
             }
             release(OB_C);
             nC++;
@@ -284,9 +315,9 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
         for (int j = 1; j <= prm.tchunk + 1; j++) {
             const int tprev = t;
             t = (t + 1 == T) ? 0 : t + 1;
-            cd p[12], acc[12];
+            C p[12], acc[12];
             {   // T phase: finish out(t-1) with its forward hop, start out(t) with its backward hop
-                cd u[9];
+                C u[9];
                 mbar_wait(bar_full + 8 * OB_T, nT & 1);
                 mbar_wait(bar_full + 8 * OB_C, nC & 1);
 #ifdef WD_EXPERIMENTS
@@ -296,19 +327,19 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
                     prm.trace[(size_t)blockIdx.x * kTraceLen + ntrace++] = now;
                 }
 #endif
-                load_link<P::UC>(u, smem, P::OFF_T + own, NS);
+                load_link<P::UC, C>(u, smem, P::OFF_T + own, NS);
 #pragma unroll
-                for (int c = 0; c < 12; c++) p[c] = lds(smem, P::OFF_C + own + c * NS);
+                for (int c = 0; c < 12; c++) p[c] = lds<C>(smem, P::OFF_C + own + c * NS);
                 if (j > 1) {
-                    cd f[12];
+                    C f[12];
 #pragma unroll
-                    for (int c = 0; c < 12; c++) f[c] = make_double2(0.0, 0.0);
+                    for (int c = 0; c < 12; c++) f[c] = mk<C>(0, 0);
                     if (!((open & 1) && tprev == T - 1)) hop_term<0, -1>(f, p, u);  // (1 - gamma_T) U_T(t-1) psi(t)
                     const long long ip = (long long)tprev * strideT + site0;
 #pragma unroll
                     for (int c = 0; c < 12; c++)
                         __stcs(out + (long long)c * V + ip,
-                               make_double2(fma(-0.5, f[c].x, outp[c].x), fma(-0.5, f[c].y, outp[c].y)));
+                               mk<C>(fma(-half, f[c].x, outp[c].x), fma(-half, f[c].y, outp[c].y)));
                 }
                 if (j == prm.tchunk + 1) {  // epilogue step: nothing else to do for slice t
                     release(OB_T);
@@ -317,10 +348,10 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
                     nC++;
                     break;
                 }
-                cd g[6];
+                C g[6];
                 su3_mul<true>(g, u, hprev);  // U_T(t-1)^H (1 + gamma_T) psi(t-1)
 #pragma unroll
-                for (int c = 0; c < 12; c++) acc[c] = make_double2(0.0, 0.0);
+                for (int c = 0; c < 12; c++) acc[c] = mk<C>(0, 0);
                 reconstruct_add<0, +1>(acc, g);
                 project<0, +1>(hprev, p);
                 release(OB_T);
@@ -328,13 +359,13 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
             }
             const uint32_t pf = nF & 1;
             mbar_wait(bar_full + 8 * OB_Z, pf);
-            hop_pair_smem<1, P::UC>(acc, smem, P::OFF_Z + own, NS, z_pf, z_pf_s, z_ub, z_b_s, z_pb, z_b_s, zf_on, zb_on);
+            hop_pair_smem<1, P::UC, C>(acc, smem, P::OFF_Z + own, NS, z_pf, z_pf_s, z_ub, z_b_s, z_pb, z_b_s, zf_on, zb_on);
             release(OB_Z);
             mbar_wait(bar_full + 8 * OB_Y, pf);
-            hop_pair_smem<2, P::UC>(acc, smem, P::OFF_Y + own, NS, y_pf, y_pf_s, y_ub, y_b_s, y_pb, y_b_s, yf_on, yb_on);
+            hop_pair_smem<2, P::UC, C>(acc, smem, P::OFF_Y + own, NS, y_pf, y_pf_s, y_ub, y_b_s, y_pb, y_b_s, yf_on, yb_on);
             release(OB_Y);
             mbar_wait(bar_full + 8 * OB_X, pf);
-            hop_pair_smem<3, P::UC>(acc, smem, P::OFF_X + own, NS, x_pf, x_pf_s, x_ub, x_b_s, x_pb, x_b_s, xf_on, xb_on);
+            hop_pair_smem<3, P::UC, C>(acc, smem, P::OFF_X + own, NS, x_pf, x_pf_s, x_ub, x_b_s, x_pb, x_b_s, xf_on, xb_on);
             release(OB_X);
             release(OB_C);
             nC++;
@@ -343,30 +374,30 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
 #pragma unroll
                 for (int b = 0; b < 2; b++) {
                     const uint32_t so = (b == 0 ? P::OFF_SA : P::OFF_SB) + own;
-                    mbar_wait(bar_full + 8 * (OB_SA + b), pf);
-                    double d[6];
-                    cd a[15], r[6];
+                    if (!P::COMPACT || b == 0) mbar_wait(bar_full + 8 * (b == 0 ? OB_SA : OB_SB), pf);
+                    Real d[6];
+                    C a[15], r[6];
 #pragma unroll
                     for (int q = 0; q < 3; q++) {
-                        const cd dd = lds(smem, so + q * NS);
+                        const C dd = lds<C>(smem, so + q * NS);
                         d[2 * q] = dd.x;
                         d[2 * q + 1] = dd.y;
                     }
 #pragma unroll
-                    for (int k = 0; k < 15; k++) a[k] = lds(smem, so + (3 + k) * NS);
-                    release(OB_SA + b);
+                    for (int k = 0; k < 15; k++) a[k] = lds<C>(smem, so + (3 + k) * NS);
+                    if (!P::COMPACT || b == 1) release(b == 0 ? OB_SA : OB_SB);
                     herm6_mul(r, d, a, p + 6 * b);
 #pragma unroll
                     for (int c = 0; c < 6; c++)
-                        outp[6 * b + c] = make_double2(fma(-0.5, acc[6 * b + c].x, r[c].x), fma(-0.5, acc[6 * b + c].y, r[c].y));
+                        outp[6 * b + c] = mk<C>(fma(-half, acc[6 * b + c].x, r[c].x), fma(-half, acc[6 * b + c].y, r[c].y));
                 }
             } else if (P::SELF == SELF_MASS) {
 #pragma unroll
                 for (int c = 0; c < 12; c++)
-                    outp[c] = make_double2(fma(prm.mass, p[c].x, -0.5 * acc[c].x), fma(prm.mass, p[c].y, -0.5 * acc[c].y));
+                    outp[c] = mk<C>(fma(mass, p[c].x, -half * acc[c].x), fma(mass, p[c].y, -half * acc[c].y));
             } else {
 #pragma unroll
-                for (int c = 0; c < 12; c++) outp[c] = make_double2(-0.5 * acc[c].x, -0.5 * acc[c].y);
+                for (int c = 0; c < 12; c++) outp[c] = mk<C>(-half * acc[c].x, -half * acc[c].y);
             }
             nF++;
         }
@@ -375,14 +406,18 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
 
 // ---------------------------------------------------------------- host side
 template <int BZ, int BY, int BX, int SELF> static cudaError_t launch_tma_self(const KParams &p, cudaStream_t st) {
+    if (p.esize == 8) {  // FP32 variant: the same kernel on 8-byte elements (pointers of p are float2 fields)
+        using P = Plan<BZ, BY, BX, SELF, 9, cf>;
+        return p.open_mask ? launch_tma_kernel<P>(k_tma<P, true>, p, st, /*ucomp*/ 9, /*scomp*/ 18, CHUNK_COST_MODEL, /*rb*/ 4) : launch_tma_kernel<P>(k_tma<P, false>, p, st, /*ucomp*/ 9, /*scomp*/ 18, CHUNK_COST_MODEL, /*rb*/ 4);
+    }
     if (p.gauge_rows == 2) {  // two-row link storage: boxes of 6 components from the compressed gauge array
         using P = Plan<BZ, BY, BX, SELF, 6>;
         KParams q = p;
         q.U = p.U2;
-        return launch_tma_kernel<P>(k_tma<P>, q, st, /*ucomp*/ 6, /*scomp*/ 18, CHUNK_COST_MODEL, /*rb*/ 4);
+        return q.open_mask ? launch_tma_kernel<P>(k_tma<P, true>, q, st, /*ucomp*/ 6, /*scomp*/ 18, CHUNK_COST_MODEL, /*rb*/ 4) : launch_tma_kernel<P>(k_tma<P, false>, q, st, /*ucomp*/ 6, /*scomp*/ 18, CHUNK_COST_MODEL, /*rb*/ 4);
     }
     using P = Plan<BZ, BY, BX, SELF>;
-    return launch_tma_kernel<P>(k_tma<P>, p, st, /*ucomp*/ 9, /*scomp*/ 18, CHUNK_COST_MODEL, /*rb*/ 4);
+    return p.open_mask ? launch_tma_kernel<P>(k_tma<P, true>, p, st, /*ucomp*/ 9, /*scomp*/ 18, CHUNK_COST_MODEL, /*rb*/ 4) : launch_tma_kernel<P>(k_tma<P, false>, p, st, /*ucomp*/ 9, /*scomp*/ 18, CHUNK_COST_MODEL, /*rb*/ 4);
 }
 
 template <int BZ, int BY, int BX> static cudaError_t launch_tma(const KParams &p, int self, cudaStream_t st) {

@@ -94,10 +94,10 @@ __device__ __forceinline__ uint64_t l2_policy_evict_last() {
 }
 
 // ---------------------------------------------------------------- host side
-// A field of double2 [ncomp][Vs] (Vs >= T*Z*Y*X, site index X fastest) seen as a 5-D FP64 tensor
+// A field of double2 (esize 16) or float2 (esize 8) [ncomp][Vs] (Vs >= T*Z*Y*X, site index X fastest) seen as a 5-D FP64 tensor
 // (2X, Y, Z, T, ncomp); a box is (2*bx, by, bz, 1, bc) and lands in shared memory densely as
 // double2 [bc][bz][by][bx].
 cudaError_t encode_field_map(CUtensorMap *map, const void *base, const int n[4], long long Vs, int ncomp, int bx,
-                             int by, int bz, int bc);
+                             int by, int bz, int bc, int esize = 16);
 
 }  // namespace wd

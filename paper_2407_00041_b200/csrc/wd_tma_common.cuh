@@ -22,7 +22,7 @@ struct TmaMaps {
 };
 
 struct TmaParams {
-    double2 *out;
+    void *out;              // double2 (or float2, FP32 variant) [nrhs][12][Vs]
     const double2 *psi, *U, *S;  // for kernels that read psi(t0-1) / links / S with LDG (wd_tmc.cu)
     long long V, Vs;       // sites, component stride
     int n[4];
@@ -136,7 +136,7 @@ enum ChunkPolicy {
 // tiles, all of X) is the set of tiles in flight together: as cubic as possible, at most one wave, so that
 // most face re-reads are L2 hits on data a neighbouring CTA is streaming at the same time.
 template <class P> static void plan_items(const KParams &p, TmaParams &prm, ChunkPolicy policy, int rb_units) {
-    const int nsm = p.nsm;
+    const int nsm = p.nsm * P::CTAS_PER_SM;  // persistent CTAs in flight
     prm.ntx = p.n[3] / P::BX;
     prm.nty = p.n[2] / P::BY;
     prm.ntz = p.n[1] / P::BZ;
@@ -193,7 +193,7 @@ template <class P> static void plan_items(const KParams &p, TmaParams &prm, Chun
 // (9, or 6 with two-row storage), scomp = components per S box (18 or 9).
 template <class P> static cudaError_t get_maps(const KParams &p, int ucomp, int scomp, const TmaMaps **out, TmaMaps *scratch) {
     constexpr int BZ = P::BZ, BY = P::BY, BX = P::BX;
-    const int tag = (((ucomp * 32 + scomp) * 64 + BZ) * 64 + BY) * 64 + BX;  // everything a box shape depends on
+    const int tag = ((((ucomp * 32 + scomp) * 64 + BZ) * 64 + BY) * 64 + BX) * 2 + (p.esize == 8);  // everything a box depends on
     const void *Sbase = (P::SELF == SELF_CLOVER) ? (const void *)p.S : (const void *)p.U;
     if (p.maps) {
         if (const TmaMaps *m = p.maps->find(tag, p.psi, p.U, Sbase, p.nrhs)) {
@@ -206,18 +206,18 @@ template <class P> static cudaError_t get_maps(const KParams &p, int ucomp, int 
     const int nucomp = 4 * ucomp, nscomp = (P::SELF == SELF_CLOVER) ? 36 : nucomp;
     const int sc = (scomp <= nscomp) ? scomp : nscomp;
 #define WD_ENC(m, base, nc, bx, by, bz, bc)                                                  \
-    if ((e = encode_field_map(&maps->m, base, p.n, p.Vs, nc, bx, by, bz, bc)) != cudaSuccess) { \
+    if ((e = encode_field_map(&maps->m, base, p.n, p.Vs, nc, bx, by, bz, bc, p.esize)) != cudaSuccess) { \
         if (p.maps) p.maps->clear();                                                         \
         return e;                                                                            \
     }
     WD_ENC(psi_c, p.psi, 12 * p.nrhs, BX, BY, BZ, 12)
     WD_ENC(psi_z, p.psi, 12 * p.nrhs, BX, BY, 1, 12)
     WD_ENC(psi_y, p.psi, 12 * p.nrhs, BX, 1, BZ, 12)
-    WD_ENC(psi_x, p.psi, 12 * p.nrhs, 1, BY, BZ, 12)
+    WD_ENC(psi_x, p.psi, 12 * p.nrhs, P::XW, BY, BZ, 12)
     WD_ENC(u_c, p.U, nucomp, BX, BY, BZ, ucomp)
     WD_ENC(u_z, p.U, nucomp, BX, BY, 1, ucomp)
     WD_ENC(u_y, p.U, nucomp, BX, 1, BZ, ucomp)
-    WD_ENC(u_x, p.U, nucomp, 1, BY, BZ, ucomp)
+    WD_ENC(u_x, p.U, nucomp, P::XW, BY, BZ, ucomp)
     WD_ENC(s_c, Sbase, nscomp, BX, BY, BZ, sc)
 #undef WD_ENC
     *out = maps;
@@ -262,7 +262,8 @@ static cudaError_t launch_tma_kernel(K kernel, const KParams &p, cudaStream_t st
     prm.mass = p.mass;
     prm.open_mask = p.open_mask;
     plan_items<P>(p, prm, policy, rb_units);
-    const int grid = (prm.nitems < p.nsm) ? prm.nitems : p.nsm;
+    const int ctas = p.nsm * P::CTAS_PER_SM;
+    const int grid = (prm.nitems < ctas) ? prm.nitems : ctas;
     if (grid < 1) return cudaSuccess;
     prm.sched = p.sched;
 #ifdef WD_EXPERIMENTS

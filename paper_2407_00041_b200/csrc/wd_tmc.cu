@@ -42,6 +42,8 @@ template <int BZ_, int BY_, int BX_, int SELF_> struct Plan {
     static constexpr int BZ = BZ_, BY = BY_, BX = BX_, SELF = SELF_;
     static constexpr int G = 2;              // right-hand sides per work item = per thread
     static constexpr int N = BZ * BY * BX;   // sites per tile = compute threads
+    static constexpr int CTAS_PER_SM = 1;
+    static constexpr int XW = 1;             // sites per row of an X-face box (wd_tma.cu: 2 for 8-byte elements)
     static constexpr int NW = N / 32;
     static constexpr int NTHREADS = N + 32;  // + the producer warp
     static constexpr int FZ = BY * BX, FY = BZ * BX, FX = BZ * BY;
@@ -346,7 +348,7 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tmc(const __grid_constant__ 
                 for (int g = 0; g < G; g++) {
                     const uint32_t pown = P::OFF_C + cb + g * P::SZ_C1 + own;  // psi_g(t) of the own site
                     if (g < it.ng) {
-                        cd *__restrict__ out = prm.out + (long long)(it.rhs0 + g) * 12 * Vs + i;
+                        cd *__restrict__ out = reinterpret_cast<cd *>(prm.out) + (long long)(it.rhs0 + g) * 12 * Vs + i;
 #pragma unroll
                         for (int c = 0; c < 12; c++) {
                             cd o = make_double2(-0.5 * acc[g][c].x, -0.5 * acc[g][c].y);

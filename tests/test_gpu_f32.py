@@ -40,9 +40,11 @@ def apply_f32(torch, op, psi, nrhs):
     return out
 
 
-@pytest.mark.parametrize("dims", [(8, 8, 8, 16), (4, 4, 8, 32), (3, 5, 6, 7), (2, 2, 2, 2)])
-def test_fp32_operator_matches_the_oracle_on_rounded_inputs(torch, dims):
-    m0, csw, nrhs = -0.4, 1.0, 2
+@pytest.mark.parametrize("f32_kernel", [0, 1])
+@pytest.mark.parametrize("dims", [(8, 8, 8, 16), (4, 4, 8, 32), (5, 2, 4, 16), (3, 5, 6, 7), (2, 2, 2, 2)])
+def test_fp32_operator_matches_the_oracle_on_rounded_inputs(torch, dims, f32_kernel):
+    """f32_kernel 0: automatic (the TMA kernel on 8-byte elements where its tile fits, else the LDG kernels); 1: LDG."""
+    m0, csw, nrhs = -0.4, 1.0, 3
     U = wdinputs.gauge_exp(dims, 911, 0.5)
     psi = wdinputs.spinor(dims, 912, nrhs=nrhs)
     C = oracle.build_clover(dims, m0, csw, U)
@@ -54,6 +56,7 @@ def test_fp32_operator_matches_the_oracle_on_rounded_inputs(torch, dims):
             wd.wd_apply_f32(op.h, a, b, 1)
         assert e.value.code == wd.WD_ESTATE
         wd.wd_enable_f32(op.h)
+        wd.wd_set_option(op.h, wd.WD_OPT_F32_KERNEL, f32_kernel)
         out = apply_f32(torch, op, psi, nrhs)
         assert np.isfinite(out).all()
         assert rel_l2(out, ref_c) <= TOL32
@@ -62,7 +65,7 @@ def test_fp32_operator_matches_the_oracle_on_rounded_inputs(torch, dims):
         assert rel_l2(out, ref_c) > 1e-9
         with pytest.raises(wd.WDError):
             wd.wd_apply_f32(op.h, a, a, 1)
-    with Op(torch, dims, m0, 0.0, U) as op:
+    with Op(torch, dims, m0, 0.0, U, f32_kernel=f32_kernel) as op:
         wd.wd_enable_f32(op.h)
         out = apply_f32(torch, op, psi, nrhs)
         assert rel_l2(out, ref_w) <= TOL32 and np.abs(out - ref_w).max() <= WORST32 * np.abs(ref_w).max()
