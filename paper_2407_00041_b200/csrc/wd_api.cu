@@ -402,22 +402,22 @@ int wd_layout_unpack_host(int field, long long nsites, const double *packed, dou
 
 // ---- kernel selection -----------------------------------------------------------------------------
 static bool geometry_fits(const wd_handle *h, const KernelInfo &k) {
-    if (dd_open_mask(h) && !strncmp(k.name, "tmc", 3)) return false;  // no open-boundary mode in wd_tmc.cu
     if (k.bx == 0) return true;
     return h->n[0] % k.bt == 0 && h->n[1] % k.bz == 0 && h->n[2] % k.by == 0 && h->n[3] % k.bx == 0;
 }
 
 static int auto_kernel(const wd_handle *h, int nrhs) {
-    // Preference order: one right-hand side with a clover term, fused: the first-generation
-    // TMA kernel (64^4: 4.17 ms vs 4.36 ms); the hopping term alone (csw = 0, or the unfused variant): the second
-    // generation (3.66 ms vs 2.96 ms); several right-hand sides in one call: wd_tmc.cu (two per thread, links in
-    // registers).  linear256 always fits.
-    static const char *pref_clover[] = {"tma_2x4x16", "tmb_4x4x8", "tmb_2x8x8", "tile_1x4x4x16", "tile_2x4x4x4"};
-    static const char *pref_hop[] = {"tmb_4x4x8", "tmb_2x8x8", "tma_2x4x16", "tile_1x4x4x16", "tile_2x4x4x4"};
-    static const char *pref_multi[] = {"tmb_4x4x8", "tmb_2x8x8", "tmc_2x4x16", "tile_1x4x4x16", "tile_2x4x4x4"};
+    // Preference order.  One right-hand side with a clover term, fused: the warpgroup-split
+    // kernel (64^4: 4.13 ms burst / 4.30 ms sustained against 4.15 / 4.35 ms of the first generation, which stays the
+    // choice with two-row links).  The hopping term alone (csw = 0, or the unfused variant) and several right-hand
+    // sides in one call: the second generation (pure Wilson 2.90 ms vs 3.06 / 3.66 ms; cfg 5 25.6 ms vs 27.4 / 28.5 ms).
+    // linear256 always fits.
+    static const char *pref_clover[] = {"tmw_2x4x16", "tma_2x4x16", "tmb_4x4x8", "tmb_2x8x8", "tile_1x4x4x16", "tile_2x4x4x4"};
+    static const char *pref_tworow[] = {"tma_2x4x16", "tmw_2x4x16", "tmb_4x4x8", "tmb_2x8x8", "tile_1x4x4x16", "tile_2x4x4x4"};
+    static const char *pref_hop[] = {"tmb_4x4x8", "tmb_2x8x8", "tmw_2x4x16", "tma_2x4x16", "tile_1x4x4x16", "tile_2x4x4x4"};
     const bool clover_fused = (h->csw != 0.0 || h->has_clover) && h->variant == 0;
-    const char **pref = (nrhs > 1 && h->variant == 0) ? pref_multi : clover_fused ? pref_clover : pref_hop;
-    for (int i = 0; i < 5; i++)
+    const char **pref = (nrhs > 1 && h->variant == 0) ? pref_hop : !clover_fused ? pref_hop : (h->gauge_rows == 2) ? pref_tworow : pref_clover;
+    for (int i = 0; i < 6; i++)
         for (int id = 0; id < kernel_count(); id++)
             if (!strcmp(kernel_info(id).name, pref[i]) && geometry_fits(h, kernel_info(id))) return id;
     return 0;
@@ -446,7 +446,7 @@ int wd_set_option(wd_handle *h, int option, long value) {
     case WD_OPT_KERNEL:
         if (value < -1 || value >= kernel_count()) return fail(h, WD_EINVAL, "WD_OPT_KERNEL: id out of range");
         if (value >= 0 && !geometry_fits(h, kernel_info((int)value)))
-            return fail(h, WD_EINVAL, std::string("WD_OPT_KERNEL: ") + kernel_info((int)value).name + " does not fit this handle (tile does not divide the lattice, or no open-boundary mode)");
+            return fail(h, WD_EINVAL, std::string("WD_OPT_KERNEL: ") + kernel_info((int)value).name + " does not fit this handle (its tile does not divide the lattice)");
         h->kernel_opt = value;
         return WD_OK;
     case WD_OPT_TCHUNK:

@@ -79,8 +79,8 @@ const KernelInfo &kernel_info(int id);
 cudaError_t launch_tma_2x4x16(const KParams &p, int self, cudaStream_t st);
 cudaError_t launch_tmb_4x4x8(const KParams &p, int self, cudaStream_t st);
 cudaError_t launch_tmb_2x8x8(const KParams &p, int self, cudaStream_t st);
-// multi-RHS kernel: two right-hand sides per thread, links and S by LDG into registers (wd_tmc.cu)
-cudaError_t launch_tmc_2x4x16(const KParams &p, int self, cudaStream_t st);
+// first generation with two compute warpgroups per tile (wd_tmw.cu)
+cudaError_t launch_tmw_2x4x16(const KParams &p, int self, cudaStream_t st);
 MapCache *map_cache_new();
 void map_cache_delete(MapCache *c);
 void map_cache_clear(MapCache *c);

@@ -63,7 +63,7 @@ cudaError_t launch_selfcoupling(const KParams &p, int self, cudaStream_t st) {
 }
 
 // ---- registry -------------------------------------------------------------------------------
-// linear: any lattice.  tile_*: LDG kernels for lattices no TMA tile divides (cfg 1: 4^4).  tma/tmb/tmc: the TMA kernels.
+// linear: any lattice.  tile_*: LDG kernels for lattices no TMA tile divides (cfg 1: 4^4).  tma/tmb: the TMA kernels.
 static const KernelInfo kKernels[] = {
     {"linear256", 0, 0, 0, 0, 256, false, launch_linear<256>},
     {"tile_1x4x4x16", 1, 4, 4, 16, 256, false, launch_tiled<1, 4, 4, 16>},
@@ -71,7 +71,7 @@ static const KernelInfo kKernels[] = {
     {"tma_2x4x16", 1, 2, 4, 16, 160, true, launch_tma_2x4x16},
     {"tmb_4x4x8", 1, 4, 4, 8, 160, true, launch_tmb_4x4x8},
     {"tmb_2x8x8", 1, 2, 8, 8, 160, true, launch_tmb_2x8x8},
-    {"tmc_2x4x16", 1, 2, 4, 16, 160, true, launch_tmc_2x4x16},
+    {"tmw_2x4x16", 1, 2, 4, 16, 384, true, launch_tmw_2x4x16},
 };
 
 int kernel_count() { return (int)(sizeof(kKernels) / sizeof(kKernels[0])); }

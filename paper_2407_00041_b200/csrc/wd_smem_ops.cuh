@@ -84,83 +84,4 @@ __device__ __forceinline__ void herm6_half_add(cd acc[6], const unsigned char *s
         }
 }
 
-
-// ---------------------------------------------------------------- register-operand variants (wd_tmc.cu)
-// One spin row S (0 or 1) of one hopping term with the link in registers and psi in shared memory:
-//   h = rows S of (I4 + SIGN*gamma_MU) psi   (3 complex: psi row S combined with its partner row, a2)
-//   g = U h  (SIGN < 0, forward neighbour)  or  U^H h  (SIGN > 0, backward neighbour)            (a3)
-//   acc[row S] += g,  acc[the lower row that gamma_MU couples to S] += (+-1, +-i) g               (a4)
-// Six LDS.128 instead of twelve at a time keep the operand footprint at 24 registers.
-template <int MU, int SIGN, int S>
-__device__ __forceinline__ void hop_row(cd acc[12], const cd u[9], const cd pa[3], const cd pb[3]) {
-    constexpr int KS = (SIGN < 0) ? 2 : 0;
-    constexpr int R = (Gam<MU, 2>::col == S) ? 2 : 3;             // lower row that receives from S
-    constexpr int KR = (R == 2) ? Gam<MU, 2>::k : Gam<MU, 3>::k;  // with coefficient i^KR (times SIGN)
-    cd h[3];
-#pragma unroll
-    for (int c = 0; c < 3; c++) h[c] = add_ik<Gam<MU, S>::k + KS>(pa[c], pb[c]);
-#pragma unroll
-    for (int c = 0; c < 3; c++) {
-        cd r;
-        if (SIGN < 0) {
-            r = cmul(u[3 * c], h[0]);
-            cfma(r, u[3 * c + 1], h[1]);
-            cfma(r, u[3 * c + 2], h[2]);
-        } else {
-            r = cmul_conj(u[c], h[0]);
-            cfma_conj(r, u[3 + c], h[1]);
-            cfma_conj(r, u[6 + c], h[2]);
-        }
-        acc[3 * S + c] = add_ik<0>(acc[3 * S + c], r);
-        acc[3 * R + c] = add_ik<KR + KS>(acc[3 * R + c], r);
-    }
-}
-// psi row S (pa) and its partner row Gam<MU,S>::col (pb) from shared memory / from global memory
-template <int MU, int SIGN, int S>
-__device__ __forceinline__ void hop_row_smem(cd acc[12], const unsigned char *smem, uint32_t p, uint32_t stride, const cd u[9]) {
-    constexpr int col = Gam<MU, S>::col;
-    cd pa[3], pb[3];
-#pragma unroll
-    for (int c = 0; c < 3; c++) {
-        pa[c] = lds(smem, p + (3 * S + c) * stride);
-        pb[c] = lds(smem, p + (3 * col + c) * stride);
-    }
-    hop_row<MU, SIGN, S>(acc, u, pa, pb);
-}
-template <int MU, int SIGN, int S>
-__device__ __forceinline__ void hop_row_ldg(cd acc[12], const cd *__restrict__ p, long long stride, const cd u[9]) {
-    constexpr int col = Gam<MU, S>::col;
-    cd pa[3], pb[3];
-#pragma unroll
-    for (int c = 0; c < 3; c++) {
-        pa[c] = __ldg(p + (long long)(3 * S + c) * stride);
-        pb[c] = __ldg(p + (long long)(3 * col + c) * stride);
-    }
-    hop_row<MU, SIGN, S>(acc, u, pa, pb);
-}
-
-// acc[0..5] += (part of B) q, as herm6_half_add, with the nine slots of S in registers
-template <int H> __device__ __forceinline__ void herm6_half_add_reg(cd acc[6], const cd a[9], const cd q[6]) {
-    if (H == 0) {
-#pragma unroll
-        for (int i = 0; i < 3; i++) {
-            acc[2 * i].x = fma(a[i].x, q[2 * i].x, acc[2 * i].x);
-            acc[2 * i].y = fma(a[i].x, q[2 * i].y, acc[2 * i].y);
-            acc[2 * i + 1].x = fma(a[i].y, q[2 * i + 1].x, acc[2 * i + 1].x);
-            acc[2 * i + 1].y = fma(a[i].y, q[2 * i + 1].y, acc[2 * i + 1].y);
-        }
-    }
-    int k = 0;
-#pragma unroll
-    for (int i = 0; i < 6; i++)
-#pragma unroll
-        for (int j = i + 1; j < 6; j++, k++) {
-            const int slot = (H == 0) ? k + 3 : k - 6;
-            if ((H == 0 && k < 6) || (H == 1 && k >= 6)) {
-                cfma(acc[i], a[slot], q[j]);
-                cfma_conj(acc[j], a[slot], q[i]);
-            }
-        }
-}
-
 }  // namespace wd

@@ -1,5 +1,4 @@
-// wd_tma_common.cuh — the ONE skeleton shared by the TMA-staged T-marching kernels (wd_tma.cu, wd_tmb.cu,
-// wd_tmc.cu): tensor maps and their per-handle cache, launch parameters, the work-item order, the work
+// wd_tma_common.cuh — the ONE skeleton shared by the TMA-staged T-marching kernels (wd_tma.cu, wd_tmb.cu): tensor maps and their per-handle cache, launch parameters, the work-item order, the work
 // decomposition (T chunk, rasterisation panel) and the launch wrapper.  A kernel file only adds its
 // shared-memory plan, its producer and its consumer code.
 //
@@ -23,7 +22,7 @@ struct TmaMaps {
 
 struct TmaParams {
     void *out;              // double2 (or float2, FP32 variant) [nrhs][12][Vs]
-    const double2 *psi, *U, *S;  // for kernels that read psi(t0-1) / links / S with LDG (wd_tmc.cu)
+    const double2 *psi, *U, *S;  // the fields themselves (kernels that read operands with LDG)
     long long V, Vs;       // sites, component stride
     int n[4];
     int ntx, nty, ntz;     // tiles per direction

@@ -23,7 +23,7 @@ def tma_kernels(dims):
     out = []
     for k in range(wd.wd_kernel_count()):
         name = wd.wd_kernel_name(k)
-        if name.startswith(("tma_", "tmb_", "tmc_")):
+        if name.startswith(("tma_", "tmb_", "tmw_")):
             b = [int(v) for v in name.split("_")[1].split("x")]
             if all(n % t == 0 for n, t in zip(dims[-3:], b)):
                 out.append(k)
@@ -80,28 +80,6 @@ def test_tma_many_items_per_cta_and_multi_rhs(torch):
             assert rel_l2(op.apply(psi, nrhs), ref) <= TOL, wd.wd_kernel_name(kid)
 
 
-@pytest.mark.parametrize("nrhs", [1, 2, 5, 7])
-def test_multi_rhs_two_per_thread(torch, nrhs):
-    """tmc kernels: every thread handles two right-hand sides with the links and S in registers; an odd nrhs leaves
-    the last unit with one right-hand side (computed twice, stored once)."""
-    dims, m0, csw = (6, 4, 8, 32), -0.4, 1.0
-    U = wdinputs.gauge_haar(dims, 431)
-    psi = wdinputs.spinor(dims, 432, nrhs=nrhs)
-    C = wdinputs.selfcoupling_random(dims, 433)
-    ref_c = oracle.apply(dims, m0, U, C, psi)
-    ref_w = oracle.apply(dims, m0, U, None, psi)
-    kids = [k for k in tma_kernels(dims) if wd.wd_kernel_name(k).startswith("tmc")]
-    assert kids
-    for kid in kids:
-        for tchunk in (0, 2):
-            with Op(torch, dims, m0, csw, U, C, kernel=kid, tchunk=tchunk) as op:
-                out = op.apply(psi, nrhs)
-                for r in range(nrhs):
-                    assert rel_l2(out[r], ref_c[r]) <= TOL, (wd.wd_kernel_name(kid), r)
-        with Op(torch, dims, m0, 0.0, U, None, kernel=kid) as op:
-            assert rel_l2(op.apply(psi, nrhs), ref_w) <= TOL, wd.wd_kernel_name(kid)
-
-
 @pytest.mark.parametrize("dims,csw", [((8, 4, 8, 16), 1.0), ((8, 4, 8, 16), 0.0), ((12, 8, 8, 32), 1.0), ((5, 4, 8, 16), 1.0)])
 def test_apply_host_pipelined_over_t_chunks(torch, dims, csw):
     """wd_apply_host with a TMA kernel cuts the lattice into T chunks and overlaps upload, compute and download;
@@ -112,7 +90,7 @@ def test_apply_host_pipelined_over_t_chunks(torch, dims, csw):
     C = oracle.build_clover(dims, m0, csw, U) if csw else None
     ref = oracle.apply(dims, m0, U, C, psi)
     with Op(torch, dims, m0, csw, U, C) as op:
-        assert wd.wd_kernel_name(wd.wd_kernel_in_use(op.h)).startswith(("tma_", "tmb_"))
+        assert wd.wd_kernel_name(wd.wd_kernel_in_use(op.h)).startswith(("tma_", "tmb_", "tmw_"))
         out = np.empty_like(psi)
         wd.wd_apply_host(op.h, out, psi, nrhs)
         assert rel_l2(out, ref) <= TOL
