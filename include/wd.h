@@ -186,7 +186,7 @@ int wd_apply_f32(wd_handle *h, void *dev_out, const void *dev_in, int nrhs);
 
 /* Same operation on HOST arrays in canonical spinor layout: host->device copy, on-device
  * repack, operator, repack, device->host copy, all inside the call; returns after the result is
- * in host_out.  With a TMA kernel the lattice is cut into up to 16 chunks along T and upload,
+ * in host_out.  With a TMA kernel the lattice is cut into up to 32 chunks along T and upload,
  * compute and download of different chunks overlap on three streams (the library's own two plus
  * the handle's); otherwise the steps run one after the other on the handle's stream.  Pinned
  * host memory lets the copies overlap and is faster, but is not required.  Result identical bit

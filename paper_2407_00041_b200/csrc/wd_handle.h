@@ -6,7 +6,7 @@
 #include "../../include/wd.h"
 #include "wd_internal.h"
 
-static const int kMaxPipeChunks = 16;  // T chunks of the pipelined wd_apply_host
+static const int kMaxPipeChunks = 32;  // T chunks of the pipelined wd_apply_host (more chunks: shorter fill and drain)
 
 using wd::MapCache;
 struct wd_gmres_state;  // wd_gmres.cu
