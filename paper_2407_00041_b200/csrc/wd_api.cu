@@ -409,14 +409,16 @@ static bool geometry_fits(const wd_handle *h, const KernelInfo &k) {
 static int auto_kernel(const wd_handle *h, int nrhs) {
     // Preference order.  One right-hand side with a clover term, fused: the warpgroup-split
     // kernel (64^4: 4.13 ms burst / 4.30 ms sustained against 4.15 / 4.35 ms of the first generation, which stays the
-    // choice with two-row links).  The hopping term alone (csw = 0, or the unfused variant) and several right-hand
-    // sides in one call: the second generation (pure Wilson 2.90 ms vs 3.06 / 3.66 ms; cfg 5 25.6 ms vs 27.4 / 28.5 ms).
-    // linear256 always fits.
+    // choice with two-row links).  The hopping term alone (csw = 0, or the unfused variant): the second generation on
+    // the 2x4x16 tile (pure Wilson 2.80 ms; 4x4x8 tile 2.88, tmw 3.06, tma 3.66 ms).  Several right-hand sides in one
+    // call: the second generation on the 4x4x8 tile with its four-slot ring (cfg 5: 25.8 ms; 2x4x16 with three slots
+    // 28.3, tmw 27.4, tma 28.5 ms).  linear256 always fits.
     static const char *pref_clover[] = {"tmw_2x4x16", "tma_2x4x16", "tmb_4x4x8", "tmb_2x8x8", "tile_1x4x4x16", "tile_2x4x4x4"};
     static const char *pref_tworow[] = {"tma_2x4x16", "tmw_2x4x16", "tmb_4x4x8", "tmb_2x8x8", "tile_1x4x4x16", "tile_2x4x4x4"};
-    static const char *pref_hop[] = {"tmb_4x4x8", "tmb_2x8x8", "tmw_2x4x16", "tma_2x4x16", "tile_1x4x4x16", "tile_2x4x4x4"};
+    static const char *pref_hop[] = {"tmb_2x4x16", "tmb_4x4x8", "tmb_2x8x8", "tmw_2x4x16", "tile_1x4x4x16", "tile_2x4x4x4"};
+    static const char *pref_multi[] = {"tmb_4x4x8", "tmb_2x8x8", "tmb_2x4x16", "tmw_2x4x16", "tile_1x4x4x16", "tile_2x4x4x4"};
     const bool clover_fused = (h->csw != 0.0 || h->has_clover) && h->variant == 0;
-    const char **pref = (nrhs > 1 && h->variant == 0) ? pref_hop : !clover_fused ? pref_hop : (h->gauge_rows == 2) ? pref_tworow : pref_clover;
+    const char **pref = (nrhs > 1 && h->variant == 0) ? pref_multi : !clover_fused ? pref_hop : (h->gauge_rows == 2) ? pref_tworow : pref_clover;
     for (int i = 0; i < 6; i++)
         for (int id = 0; id < kernel_count(); id++)
             if (!strcmp(kernel_info(id).name, pref[i]) && geometry_fits(h, kernel_info(id))) return id;

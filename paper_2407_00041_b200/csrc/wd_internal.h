@@ -79,6 +79,7 @@ const KernelInfo &kernel_info(int id);
 cudaError_t launch_tma_2x4x16(const KParams &p, int self, cudaStream_t st);
 cudaError_t launch_tmb_4x4x8(const KParams &p, int self, cudaStream_t st);
 cudaError_t launch_tmb_2x8x8(const KParams &p, int self, cudaStream_t st);
+cudaError_t launch_tmb_2x4x16(const KParams &p, int self, cudaStream_t st);  // three ring slots
 // first generation with two compute warpgroups per tile (wd_tmw.cu)
 cudaError_t launch_tmw_2x4x16(const KParams &p, int self, cudaStream_t st);
 MapCache *map_cache_new();

@@ -71,6 +71,7 @@ static const KernelInfo kKernels[] = {
     {"tma_2x4x16", 1, 2, 4, 16, 160, true, launch_tma_2x4x16},
     {"tmb_4x4x8", 1, 4, 4, 8, 160, true, launch_tmb_4x4x8},
     {"tmb_2x8x8", 1, 2, 8, 8, 160, true, launch_tmb_2x8x8},
+    {"tmb_2x4x16", 1, 2, 4, 16, 160, true, launch_tmb_2x4x16},
     {"tmw_2x4x16", 1, 2, 4, 16, 384, true, launch_tmw_2x4x16},
 };
 

@@ -35,8 +35,9 @@ namespace tmb {
 //       (consumed between the Y and X hops, and at the end of the step)
 enum { OB_C = 0, OB_C1, OB_Z, OB_Y, OB_X, OB_R, OB_R1, OB_R2, OB_R3, OB_ITEM0, OB_ITEM1, OB_COUNT };
 
-template <int BZ_, int BY_, int BX_, int SELF_> struct Plan {
-    static constexpr int BZ = BZ_, BY = BY_, BX = BX_, SELF = SELF_;
+// KR = slots of the ring (4; 3 lets the 2x4x16 tile fit)
+template <int BZ_, int BY_, int BX_, int SELF_, int KR_ = 4> struct Plan {
+    static constexpr int BZ = BZ_, BY = BY_, BX = BX_, SELF = SELF_, KR = KR_;
     static constexpr int G = 1;              // right-hand sides per work item
     static constexpr int N = BZ * BY * BX;   // sites per tile = compute threads
     static constexpr int CTAS_PER_SM = 1;
@@ -57,7 +58,7 @@ template <int BZ_, int BY_, int BX_, int SELF_> struct Plan {
     static constexpr uint32_t OFF_XUF = OFF_X + SZ_U, OFF_XLO = OFF_XUF + 9 * FX * E, OFF_XHI = OFF_XLO + 12 * FX * E;
     static constexpr uint32_t SZ_X = SZ_U + (9 + 24) * FX * E;
     static constexpr uint32_t OFF_R = OFF_X + SZ_X;
-    static constexpr uint32_t OFF_BAR = OFF_R + 4 * SZ_U;
+    static constexpr uint32_t OFF_BAR = OFF_R + KR * SZ_U;
     static constexpr uint32_t OFF_MAIL = OFF_BAR + 2 * OB_COUNT * 8;  // int[2]: item index per mailbox slot
     static constexpr uint32_t SMEM = OFF_MAIL + 16;
     static constexpr int RING_PER_STEP = (SELF == SELF_CLOVER) ? 5 : 1;  // S1..S4 and T, or T alone
@@ -102,11 +103,11 @@ template <class P> struct Producer {
         nC++;
         return true;
     }
-    // nine components of U or S into ring slot nR & 3 (its previous content was fill nR - 4)
+    // nine components of U or S into ring slot nR % P::KR (its previous content was fill nR - 4)
     __device__ __forceinline__ bool load_ring(const CUtensorMap *map, uint32_t sbase, uint32_t bar_full, uint32_t bar_empty,
                                               int tt, int comp, uint64_t pol) {
-        const uint32_t b = nR & 3, ob = OB_R + b;
-        if (!mbar_try_wait(bar_empty + 8 * ob, ((nR >> 2) & 1) ^ 1)) return false;
+        const uint32_t b = nR % P::KR, ob = OB_R + b;
+        if (!mbar_try_wait(bar_empty + 8 * ob, ((nR / P::KR) & 1) ^ 1)) return false;
         mbar_arrive_expect_tx(bar_full + 8 * ob, P::SZ_U);
         tma_load_5d_hint(sbase + P::OFF_R + b * P::SZ_U, map, bar_full + 8 * ob, cx, y0, z0, tt, comp, pol);
         nR++;
@@ -293,12 +294,12 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
     };
     // one 6x6 block of S (two consecutive ring objects): acc[6b..6b+5] += B_b * (-2 psi)
     auto s_phase = [&](uint32_t cb, int b) {
-        const uint32_t s0 = nR & 3, s1 = (nR + 1) & 3;
+        const uint32_t s0 = nR % P::KR, s1 = (nR + 1) % P::KR;
         cd q[6];
         load_half(q, cb, 6 * b, -2.0);
-        wait_full(OB_R + s0, (nR >> 2) & 1);
+        wait_full(OB_R + s0, (nR / P::KR) & 1);
         herm6_half_add<0>(acc + 6 * b, smem, P::OFF_R + s0 * P::SZ_U + own, NS, q);
-        wait_full(OB_R + s1, ((nR + 1) >> 2) & 1);
+        wait_full(OB_R + s1, ((nR + 1) / P::KR) & 1);
         herm6_half_add<1>(acc + 6 * b, smem, P::OFF_R + s1 * P::SZ_U + own, NS, q);
         release(OB_R + s0);
         release(OB_R + s1);
@@ -322,9 +323,9 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
         const bool xf_on = !((open & 8) && it.x0 + lx == X - 1), xb_on = !((open & 8) && it.x0 + lx == 0);
         int t = it.t0;
         {   // prologue: acc = backward-T hop of slice t0, (1 + gamma_T) U_T(t0-1)^H psi(t0-1)
-            const uint32_t cb = (nC & 1) ? P::SZ_C : 0, slot = nR & 3;
+            const uint32_t cb = (nC & 1) ? P::SZ_C : 0, slot = nR % P::KR;
             wait_full(OB_C + (nC & 1), (nC >> 1) & 1);
-            wait_full(OB_R + slot, (nR >> 2) & 1);
+            wait_full(OB_R + slot, (nR / P::KR) & 1);
             cd p[12], u[9], h[6], g[6];
 #pragma unroll
             for (int k = 0; k < 9; k++) u[k] = lds(smem, P::OFF_R + slot * P::SZ_U + own + k * NS);
@@ -364,9 +365,9 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
             nF++;
             {   // T phase: forward hop (1 - gamma_T) U_T(t) psi(t+1) completes out(t); the backward hop of slice
                 // t+1, (1 + gamma_T) U_T(t)^H psi(t), starts the next accumulator
-                const uint32_t cn = cb ^ P::SZ_C, slot = nR & 3;  // psi(t+1) is in the other C buffer
+                const uint32_t cn = cb ^ P::SZ_C, slot = nR % P::KR;  // psi(t+1) is in the other C buffer
                 wait_full(OB_C + ((nC + 1) & 1), ((nC + 1) >> 1) & 1);
-                wait_full(OB_R + slot, (nR >> 2) & 1);
+                wait_full(OB_R + slot, (nR / P::KR) & 1);
 #ifdef WD_EXPERIMENTS
                 if (prm.trace && tid == 0 && ntrace < kTraceLen) {
                     unsigned long long now;
@@ -417,19 +418,20 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
 // Short chunks keep the CTAs of a panel within a few steps of each other (each item starts at a chunk boundary),
 // which is what makes the face re-reads L2 hits; the price is one extra psi and U_T slice per item.  Measured at
 // 64^4: tchunk 8 and 16 beat 32 and 64 by 3-7 % (CHUNK_SHORT).
-template <int BZ, int BY, int BX, int SELF> static cudaError_t launch_tma_self(const KParams &p, cudaStream_t st) {
-    using P = Plan<BZ, BY, BX, SELF>;
+template <int BZ, int BY, int BX, int SELF, int KR> static cudaError_t launch_tma_self(const KParams &p, cudaStream_t st) {
+    using P = Plan<BZ, BY, BX, SELF, KR>;
     return p.open_mask ? launch_tma_kernel<P>(k_tma<P, true>, p, st, /*ucomp*/ 9, /*scomp*/ 9, CHUNK_SHORT, /*rb*/ 4) : launch_tma_kernel<P>(k_tma<P, false>, p, st, /*ucomp*/ 9, /*scomp*/ 9, CHUNK_SHORT, /*rb*/ 4);
 }
 
-template <int BZ, int BY, int BX> static cudaError_t launch_tma(const KParams &p, int self, cudaStream_t st) {
-    if (self == SELF_CLOVER) return launch_tma_self<BZ, BY, BX, SELF_CLOVER>(p, st);
-    if (self == SELF_MASS) return launch_tma_self<BZ, BY, BX, SELF_MASS>(p, st);
-    return launch_tma_self<BZ, BY, BX, SELF_NONE>(p, st);
+template <int BZ, int BY, int BX, int KR = 4> static cudaError_t launch_tma(const KParams &p, int self, cudaStream_t st) {
+    if (self == SELF_CLOVER) return launch_tma_self<BZ, BY, BX, SELF_CLOVER, KR>(p, st);
+    if (self == SELF_MASS) return launch_tma_self<BZ, BY, BX, SELF_MASS, KR>(p, st);
+    return launch_tma_self<BZ, BY, BX, SELF_NONE, KR>(p, st);
 }
 }  // namespace tmb
 
 // Tiles of 128 sites whose shared-memory plan fits 227 KB (2x4x16 is 816 B too large)
 cudaError_t launch_tmb_4x4x8(const KParams &p, int self, cudaStream_t st) { return tmb::launch_tma<4, 4, 8>(p, self, st); }
 cudaError_t launch_tmb_2x8x8(const KParams &p, int self, cudaStream_t st) { return tmb::launch_tma<2, 8, 8>(p, self, st); }
+cudaError_t launch_tmb_2x4x16(const KParams &p, int self, cudaStream_t st) { return tmb::launch_tma<2, 4, 16, 3>(p, self, st); }
 }  // namespace wd
