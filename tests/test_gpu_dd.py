@@ -104,3 +104,115 @@ def test_decomposed_bench_size_slab(torch, capsys):
     with capsys.disabled():
         print(f"\n[decomposed parity] global {'x'.join(map(str, gdims))} grid {grid} kernel {kname}: rel_l2 {err:.3e}", flush=True)
     assert err <= TOL
+
+
+class _InProcessDist:
+    """Stand-in for torch.distributed point-to-point between `world` ranks that are THREADS of this process sharing one
+    GPU: a send records an event on the sender's stream and leaves (tensor, event) in a mailbox; a receive blocks the
+    receiving host thread until the message is there, makes its stream wait for the event and copies.  Only
+    stream-ordered dependencies exist on the device (no kernel waits for another), so this is safe on one GPU."""
+
+    class P2POp:
+        def __init__(self, fn, tensor, peer, tag=0):
+            self.fn, self.tensor, self.peer, self.tag = fn, tensor, peer, tag
+
+    class _Work:
+        def __init__(self, fn):
+            self._fn = fn
+
+        def wait(self):
+            self._fn()
+
+    def __init__(self, torch, world):
+        import collections
+        import threading
+
+        self.torch, self.world = torch, world
+        self.box = collections.defaultdict(list)
+        self.cv = threading.Condition()
+        self.local = threading.local()
+
+    def isend(self, *a, **k):  # markers only: batch_isend_irecv looks at op.fn
+        raise NotImplementedError
+
+    def irecv(self, *a, **k):
+        raise NotImplementedError
+
+    def batch_isend_irecv(self, ops):
+        torch, me = self.torch, self.local.rank
+        works = []
+        for op in ops:
+            if op.fn == self.isend:
+                ev = torch.cuda.Event()
+                ev.record(torch.cuda.current_stream())
+                with self.cv:
+                    self.box[(me, op.peer, op.tag)].append((op.tensor, ev))
+                    self.cv.notify_all()
+                works.append(self._Work(lambda: None))
+            else:
+                stream = torch.cuda.current_stream()
+
+                def recv(op=op, stream=stream):
+                    with self.cv:
+                        self.cv.wait_for(lambda: self.box[(op.peer, me, op.tag)], timeout=60)
+                        src, ev = self.box[(op.peer, me, op.tag)].pop(0)
+                    with torch.cuda.stream(stream):
+                        stream.wait_event(ev)
+                        op.tensor.copy_(src)
+
+                works.append(self._Work(recv))
+        return works
+
+
+@pytest.mark.parametrize("gdims,grid", [((8, 8, 8, 16), (2, 1, 1, 1)), ((8, 8, 8, 16), (2, 2, 1, 1))])
+def test_distributed_operator_with_in_process_ranks(torch, gdims, grid):
+    """dd.DistributedOperator — the class bench.py --gpus N drives — with its ranks as threads of one process and
+    torch.distributed replaced by `_InProcessDist`: pack, exchange on the side stream, interior, exterior, three
+    applications in a row (buffers are reused), against the oracle on the global lattice."""
+    import threading
+
+    from paper_2407_00041_b200 import dd as wdd
+    from paper_2407_00041_b200.decomp import Decomposition
+
+    m0, csw = -0.4, 1.0
+    d = Decomposition(gdims, grid)
+    U = wdinputs.gauge_haar(gdims, 841)
+    C = oracle.build_clover(gdims, m0, csw, U)
+    psis = [wdinputs.spinor(gdims, 842 + k) for k in range(3)]
+    refs = [oracle.apply(gdims, m0, U, C, p) for p in psis]
+    fake = _InProcessDist(torch, d.world_size)
+    outs = [[None] * d.world_size for _ in psis]
+    errors = []
+
+    def rank_main(r):
+        try:
+            fake.local.rank = r
+            torch.cuda.set_device(0)
+            with torch.cuda.stream(torch.cuda.Stream()):
+                lo = wdd.LocalOperator(torch, d, r, m0, csw, d.extract(U, r), d.extract(C, r))
+                op = wdd.DistributedOperator(torch, fake, lo)
+                fake.P2POp  # noqa: B018  (the plan builder uses dist.P2POp / dist.isend / dist.irecv)
+                for k, psi in enumerate(psis):
+                    din, dout = lo.spinor(), lo.spinor()
+                    dout.fill_(float("nan"))
+                    wd.wd_pack_spinor(lo.h, din, np.ascontiguousarray(d.extract(psi[0], r)[None]), 1)
+                    op.apply(dout, din, 1)
+                    wd.wd_synchronize(lo.h)
+                    loc = np.empty((1, int(np.prod(d.local_dims)), 12, 2))
+                    wd.wd_unpack_spinor(lo.h, loc, dout, 1)
+                    outs[k][r] = loc[0]
+                lo.close()
+        except Exception as exc:  # surfaced in the main thread
+            errors.append((r, repr(exc)))
+
+    threads = [threading.Thread(target=rank_main, args=(r,)) for r in range(d.world_size)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(timeout=180)
+    assert not errors, errors
+    for k, ref in enumerate(refs):
+        out = np.empty_like(ref)
+        for r in range(d.world_size):
+            d.insert(out[0], r, outs[k][r])
+        assert rel_l2(out, ref) <= TOL, k
