@@ -470,6 +470,9 @@ def run_ours(args):
         "best_launch_ms": min(per_step) / launches_per_step,
         "frac_of_8000_spec": achieved / 8000.0,
     }
+    if traffic:  # the two ways SURVEY.md section 8(d) asks for: algorithmic GB/s and the DRAM bytes ncu counted / time
+        roofline["traffic_gbs"] = traffic / (avg_launch_ms * 1e-3) / 1e9
+        roofline["reuse_efficiency"] = alg_bytes_launch / traffic  # 1.0 = every byte fetched once
 
     line = {
         "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,

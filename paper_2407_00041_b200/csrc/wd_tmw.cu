@@ -20,46 +20,22 @@
 #include <cstdio>
 #include <cstdlib>
 
-#include "wd_tma_common.cuh"
-#include "wd_smem_ops.cuh"
+#include "wd_tma_plan.cuh"
 
 namespace wd {
 namespace tmw {
 
-enum { OB_C = 0, OB_T, OB_Z, OB_Y, OB_X, OB_SA, OB_SB, OB_ITEM0, OB_ITEM1, OB_COUNT };
+using namespace gen1;  // OB_C .. OB_SA, the plan and the producer of the first generation (wd_tma_plan.cuh)
+enum { OB_SB = OB_SA + 1, OB_ITEM0, OB_ITEM1, OB_COUNT };
 
-template <int BZ_, int BY_, int BX_, int SELF_> struct Plan {
-    typedef cd C;
-    static constexpr int BZ = BZ_, BY = BY_, BX = BX_, SELF = SELF_, UC = 9;
-    static constexpr int G = 1;
-    static constexpr int N = BZ * BY * BX;    // sites per tile = threads per compute warpgroup
-    static constexpr int NW = N / 32;         // warps per warpgroup
-    static constexpr int NTHREADS = 3 * N;    // warpgroups A, B and the producer's
+// The first generation's plan (FP64, nine-entry links) with three warpgroups of N threads
+template <int BZ_, int BY_, int BX_, int SELF_> struct Plan : gen1::Plan<BZ_, BY_, BX_, SELF_, 9, cd> {
+    typedef gen1::Plan<BZ_, BY_, BX_, SELF_, 9, cd> Base;
+    static constexpr int NTHREADS = 3 * Base::N;  // warpgroups A, B and the producer's
     static constexpr int CTAS_PER_SM = 1;
-    static constexpr int XW = 1;
-    static constexpr int FZ = BY * BX, FY = BZ * BX, FX = BZ * BY;
-    static constexpr uint32_t E = 16;
-    static constexpr uint32_t SZ_C = 12 * N * E, SZ_U = 9 * N * E, SZ_S = 18 * N * E;
-    static constexpr uint32_t OFF_C = 0;
-    static constexpr uint32_t OFF_T = OFF_C + SZ_C;
-    static constexpr uint32_t OFF_Z = OFF_T + SZ_U;
-    static constexpr uint32_t OFF_ZUF = OFF_Z + SZ_U, OFF_ZLO = OFF_ZUF + 9 * FZ * E, OFF_ZHI = OFF_ZLO + 12 * FZ * E;
-    static constexpr uint32_t SZ_Z = SZ_U + (9 + 24) * FZ * E;
-    static constexpr uint32_t OFF_Y = OFF_Z + SZ_Z;
-    static constexpr uint32_t OFF_YUF = OFF_Y + SZ_U, OFF_YLO = OFF_YUF + 9 * FY * E, OFF_YHI = OFF_YLO + 12 * FY * E;
-    static constexpr uint32_t SZ_Y = SZ_U + (9 + 24) * FY * E;
-    static constexpr uint32_t OFF_X = OFF_Y + SZ_Y;
-    static constexpr uint32_t OFF_XUF = OFF_X + SZ_U, OFF_XLO = OFF_XUF + 9 * FX * E, OFF_XHI = OFF_XLO + 12 * FX * E;
-    static constexpr uint32_t SZ_X = SZ_U + (9 + 24) * FX * E;
-    static constexpr uint32_t OFF_SA = OFF_X + SZ_X;
-    static constexpr uint32_t OFF_SB = OFF_SA + SZ_S;
-    static constexpr uint32_t OFF_BAR = (SELF == SELF_CLOVER) ? OFF_SB + SZ_S : OFF_SA;
-    static constexpr uint32_t OFF_MAIL = OFF_BAR + 2 * OB_COUNT * 8;
-    static constexpr uint32_t SMEM = OFF_MAIL + 16;
-    static_assert(N == 128, "a compute warpgroup is 128 threads");
-    static_assert(SZ_Y >= 12 * N * E, "the Y object doubles as the hand-over buffer of warpgroup B");
-    static_assert(FZ % 8 == 0 && FY % 8 == 0 && FX % 8 == 0, "tile faces must keep 128-byte alignment");
-    static_assert(SMEM <= 232448, "shared-memory plan exceeds 227 KB");
+    static_assert(Base::N == 128, "a compute warpgroup is 128 threads");
+    static_assert(Base::SZ_Y >= 12 * Base::N * Base::E, "the Y object doubles as the hand-over buffer of warpgroup B");
+    static_assert(!Base::COMPACT && Base::OB_SB == OB_SB && Base::OB_ITEM0 == OB_ITEM0 && Base::OB_COUNT == OB_COUNT, "barrier layout");
 };
 
 template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
@@ -97,81 +73,7 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tmw(const __grid_constant__ 
     if (wg == 2) {
         // ======================= producer warpgroup: one thread issues every TMA =======================
         reg_dec<40>();
-        if (tid != 2 * N) return;
-        tma_prefetch_desc(&maps.psi_c); tma_prefetch_desc(&maps.psi_z); tma_prefetch_desc(&maps.psi_y);
-        tma_prefetch_desc(&maps.psi_x); tma_prefetch_desc(&maps.u_c);   tma_prefetch_desc(&maps.u_z);
-        tma_prefetch_desc(&maps.u_y);   tma_prefetch_desc(&maps.u_x);   tma_prefetch_desc(&maps.s_c);
-        const uint64_t pol_n = l2_policy_evict_normal();
-        const uint64_t pol_s = l2_policy_evict_first();  // S is used exactly once
-        uint32_t nC = 0, nT = 0, nF = 0;
-        volatile int *mail = reinterpret_cast<volatile int *>(smem + P::OFF_MAIL);
-        for (uint32_t seq = 0;; seq++) {
-            const int item = fetch_item(prm, seq);
-            const uint32_t slot = seq & 1, mpar = (seq >> 1) & 1;
-            mbar_wait(bar_empty + 8 * (OB_ITEM0 + slot), mpar ^ 1);
-            mail[slot] = item;
-            mbar_arrive(bar_full + 8 * (OB_ITEM0 + slot));
-            if (item < 0) break;
-            const Item it = decode_item<P>(prm, item);
-            const int cx = 2 * it.x0, y0 = it.y0, z0 = it.z0;
-            const int pc = 12 * it.rhs0;
-            const int zlo = (z0 == 0) ? Z - 1 : z0 - 1, zhi = (z0 + BZ == Z) ? 0 : z0 + BZ;
-            const int ylo = (y0 == 0) ? Y - 1 : y0 - 1, yhi = (y0 + BY == Y) ? 0 : y0 + BY;
-            const int cxlo = 2 * ((it.x0 == 0) ? X - 1 : it.x0 - 1), cxhi = 2 * ((it.x0 + BX == X) ? 0 : it.x0 + BX);
-            int t = (it.t0 == 0) ? T - 1 : it.t0 - 1;
-            // prologue: psi(t0-1), only to seed the carried half-spinor
-            mbar_wait(bar_empty + 8 * OB_C, (nC & 1) ^ 1);
-            mbar_arrive_expect_tx(bar_full + 8 * OB_C, P::SZ_C);
-            tma_load_5d_hint(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cx, y0, z0, t, pc, pol_n);
-            nC++;
-            for (int j = 1; j <= prm.tchunk + 1; j++) {
-                const int tprev = t;
-                t = (t + 1 == T) ? 0 : t + 1;
-                const bool full = (j <= prm.tchunk);
-                const uint32_t pe = (nF & 1) ^ 1;
-                // T object: U_T(t-1)
-                mbar_wait(bar_empty + 8 * OB_T, (nT & 1) ^ 1);
-                mbar_arrive_expect_tx(bar_full + 8 * OB_T, P::SZ_U);
-                tma_load_5d_hint(sbase + P::OFF_T, &maps.u_c, bar_full + 8 * OB_T, cx, y0, z0, tprev, 0, pol_n);
-                nT++;
-                if (full) {
-                    mbar_wait(bar_empty + 8 * OB_Z, pe);
-                    mbar_arrive_expect_tx(bar_full + 8 * OB_Z, P::SZ_Z);
-                    tma_load_5d_hint(sbase + P::OFF_Z, &maps.u_c, bar_full + 8 * OB_Z, cx, y0, z0, t, 9, pol_n);
-                    tma_load_5d_hint(sbase + P::OFF_ZUF, &maps.u_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, 9, pol_n);
-                    tma_load_5d_hint(sbase + P::OFF_ZLO, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, pc, pol_n);
-                    tma_load_5d_hint(sbase + P::OFF_ZHI, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zhi, t, pc, pol_n);
-                    mbar_wait(bar_empty + 8 * OB_X, pe);
-                    mbar_arrive_expect_tx(bar_full + 8 * OB_X, P::SZ_X);
-                    tma_load_5d_hint(sbase + P::OFF_X, &maps.u_c, bar_full + 8 * OB_X, cx, y0, z0, t, 27, pol_n);
-                    tma_load_5d_hint(sbase + P::OFF_XUF, &maps.u_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, 27, pol_n);
-                    tma_load_5d_hint(sbase + P::OFF_XLO, &maps.psi_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, pc, pol_n);
-                    tma_load_5d_hint(sbase + P::OFF_XHI, &maps.psi_x, bar_full + 8 * OB_X, cxhi, y0, z0, t, pc, pol_n);
-                }
-                // psi(t): both warpgroups have released the buffer once they hold what they need of psi(t-1)
-                mbar_wait(bar_empty + 8 * OB_C, (nC & 1) ^ 1);
-                mbar_arrive_expect_tx(bar_full + 8 * OB_C, P::SZ_C);
-                tma_load_5d_hint(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cx, y0, z0, t, pc, pol_n);
-                nC++;
-                if (full && CLOVER) {
-                    mbar_wait(bar_empty + 8 * OB_SA, pe);
-                    mbar_arrive_expect_tx(bar_full + 8 * OB_SA, P::SZ_S);
-                    tma_load_5d_hint(sbase + P::OFF_SA, &maps.s_c, bar_full + 8 * OB_SA, cx, y0, z0, t, 0, pol_s);
-                    mbar_wait(bar_empty + 8 * OB_SB, pe);
-                    mbar_arrive_expect_tx(bar_full + 8 * OB_SB, P::SZ_S);
-                    tma_load_5d_hint(sbase + P::OFF_SB, &maps.s_c, bar_full + 8 * OB_SB, cx, y0, z0, t, 18, pol_s);
-                }
-                if (full) {  // Y last: its buffer comes back only after the hand-over of the previous step
-                    mbar_wait(bar_empty + 8 * OB_Y, pe);
-                    mbar_arrive_expect_tx(bar_full + 8 * OB_Y, P::SZ_Y);
-                    tma_load_5d_hint(sbase + P::OFF_Y, &maps.u_c, bar_full + 8 * OB_Y, cx, y0, z0, t, 18, pol_n);
-                    tma_load_5d_hint(sbase + P::OFF_YUF, &maps.u_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, 18, pol_n);
-                    tma_load_5d_hint(sbase + P::OFF_YLO, &maps.psi_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, pc, pol_n);
-                    tma_load_5d_hint(sbase + P::OFF_YHI, &maps.psi_y, bar_full + 8 * OB_Y, cx, yhi, z0, t, pc, pol_n);
-                    nF++;
-                }
-            }
-        }
+        if (tid == 2 * N) producer<P, true>(maps, prm, smem, sbase, bar_full, bar_empty);
         return;
     }
     // ======================= compute warpgroups: thread = site =======================
