@@ -75,7 +75,7 @@ static int refresh_two_row_copy(wd_handle *h) {
 
 extern "C" {
 
-const char *wd_version(void) { return "wd-b200 0.1 (sm_100a, FP64)"; }
+const char *wd_version(void) { return "wd-b200 0.2 (sm_100a; FP64, FP32 variant)"; }
 
 const char *wd_last_error(const wd_handle *h) { return h ? h->err.c_str() : g_create_err.c_str(); }
 

@@ -420,7 +420,9 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
 // 64^4: tchunk 8 and 16 beat 32 and 64 by 3-7 % (CHUNK_SHORT).
 template <int BZ, int BY, int BX, int SELF, int KR> static cudaError_t launch_tma_self(const KParams &p, cudaStream_t st) {
     using P = Plan<BZ, BY, BX, SELF, KR>;
-    return p.open_mask ? launch_tma_kernel<P>(k_tma<P, true>, p, st, /*ucomp*/ 9, /*scomp*/ 9, CHUNK_SHORT, /*rb*/ 4) : launch_tma_kernel<P>(k_tma<P, false>, p, st, /*ucomp*/ 9, /*scomp*/ 9, CHUNK_SHORT, /*rb*/ 4);
+    // 8-site rows (4x4x8, 2x8x8): short chunks; the 2x4x16 tile does better with the cost model (64^4 Wilson: 2.83 vs 2.87 ms)
+    const ChunkPolicy pol = (BX >= 16) ? CHUNK_COST_MODEL : CHUNK_SHORT;
+    return p.open_mask ? launch_tma_kernel<P>(k_tma<P, true>, p, st, /*ucomp*/ 9, /*scomp*/ 9, pol, /*rb*/ 4) : launch_tma_kernel<P>(k_tma<P, false>, p, st, /*ucomp*/ 9, /*scomp*/ 9, pol, /*rb*/ 4);
 }
 
 template <int BZ, int BY, int BX, int KR = 4> static cudaError_t launch_tma(const KParams &p, int self, cudaStream_t st) {
