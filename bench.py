@@ -386,6 +386,9 @@ def run_ours(args):
     if world > 1:
         import torch.distributed as dist
 
+        # NCCL logging stays on (stderr; the JSON line is the only thing on stdout): which transport each pair got
+        os.environ.setdefault("NCCL_DEBUG", "INFO")
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT,P2P")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
         if args.parallel == "dd":
             return run_dd(args, torch, dist, world, rank, local)
