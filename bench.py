@@ -45,6 +45,8 @@ def parse_args():
     ap.add_argument("--nrhs", type=int, default=0, help="override the number of right-hand sides")
     ap.add_argument("--kernel", type=str, default="", help="kernel geometry name (default automatic)")
     ap.add_argument("--variant", type=int, default=0, help="0 fused, 1 unfused")
+    ap.add_argument("--rhs-block", type=int, default=1, choices=[1, 4],
+                    help="device layout of multi-RHS spinors (WD_OPT_RHS_BLOCK): 1 plain [nrhs][12][Vs], 4 blocked [unit][12][Vs][4]")
     ap.add_argument("--tchunk", type=int, default=0)
     ap.add_argument("--zgroup", type=int, default=0)
     ap.add_argument("--no-e2e", action="store_true")
@@ -408,6 +410,8 @@ def run_ours(args):
     wd.wd_set_stream(h, stream.cuda_stream)
     wd.wd_set_option(h, wd.WD_OPT_DEVICE_PACK, 1)
     wd.wd_set_option(h, wd.WD_OPT_VARIANT, args.variant)
+    if args.rhs_block != 1:
+        wd.wd_set_option(h, wd.WD_OPT_RHS_BLOCK, args.rhs_block)
     if args.kernel:
         wd.wd_set_option(h, wd.WD_OPT_KERNEL, wd.kernel_id(args.kernel))
     if args.tchunk:
@@ -495,6 +499,7 @@ def run_ours(args):
         "sites_per_s": site_rhs_per_s, "hbm_gbs_algorithmic": site_rhs_per_s * alg_bytes_site_rhs / 1e9,
         "config": {"workload": cfg["name"], "lattice": list(dims), "m0": cfg["m0"], "csw": cfg["csw"],
                    "nrhs": nrhs, "kernel": kname, "variant": "fused" if args.variant == 0 else "unfused", "gauge_rows": args.gauge_rows,
+                   "rhs_layout": "plain [nrhs][12][Vs]" if args.rhs_block == 1 else f"blocked [unit][12][Vs][{args.rhs_block}]",
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": f"inputs larger than L2 ({alg_bytes_step / 1e9:.2f} GB touched per step); "
                          "3 inputs / 2 outputs rotate"},
@@ -502,6 +507,8 @@ def run_ours(args):
     }
 
     # ---- end to end through the C-ABI with HOST buffers (pinned), copies inside the timed region
+    if args.rhs_block != 1:  # the host-to-host path, the FP32 variant and GMRES below use the plain device layout
+        wd.wd_set_option(h, wd.WD_OPT_RHS_BLOCK, 1)
     if not args.no_e2e and rank == 0:
         hin = torch.from_numpy(psi_host).pin_memory()
         hout = torch.empty_like(hin).pin_memory()

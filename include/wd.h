@@ -76,6 +76,15 @@ enum {
                               two-row copy of the gauge field on the device. */
     ,WD_OPT_F32_KERNEL = 9 /* wd_apply_f32: 0 = automatic (the TMA kernel where its 2x4x16 tile divides the lattice), 1 = always
                               the one-thread-per-site kernels */
+    ,WD_OPT_RHS_BLOCK = 10 /* Device layout of spinor buffers that hold SEVERAL right-hand sides ("multi-tuple" storage, cf.
+                              PAPER.md:15, :1037).  1 (default): plain, double2 [nrhs][12][Vs].  4: BLOCKED, double2
+                              [ceil(nrhs/4)][12][Vs][4] — the right-hand sides of a unit of four interleaved per site, the last
+                              unit padded to four — the layout of the fastest multi-RHS kernel (tmqb_*: every spinor access of
+                              a warp is 512 consecutive bytes, the links and S of a site are read once for its four right-hand
+                              sides).  Changes what wd_spinor_bytes / wd_pack_spinor / wd_unpack_spinor / wd_apply mean by a
+                              device spinor buffer, for every nrhs; set it before allocating buffers.  Needs a lattice the
+                              2x4x8 tile divides (else WD_EINVAL).  While it is 4, wd_apply_host, wd_gmres, the wd_dd_* and the
+                              *_f32 calls and the unfused variant return WD_ESTATE (they use the plain layout). */
 };
 
 /* Create an operator for a T x Z x Y x X periodic lattice.  Every extent >= 1 (n = 2, where

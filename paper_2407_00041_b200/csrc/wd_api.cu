@@ -109,6 +109,7 @@ int wd_create(wd_handle **out, int T, int Z, int Y, int X, double m0, double csw
     h->gmres_graph = 1;
     h->gauge_rows = 3;
     h->f32_kernel = 0;
+    h->rhs_block = 1;
     h->variant = 0;
     h->kernel_opt = -1;
     h->tchunk_opt = 0;
@@ -318,7 +319,61 @@ int wd_get_clover(wd_handle *h, double *host_C) {
 // ---- spinors ------------------------------------------------------------------------------------
 size_t wd_spinor_bytes(const wd_handle *h, int nrhs) {
     if (!h || nrhs < 1) return 0;
-    return (size_t)nrhs * (size_t)h->Vs * kSpinorComps * sizeof(double2);
+    const size_t slots = (h->rhs_block > 1) ? (size_t)((nrhs + h->rhs_block - 1) / h->rhs_block * h->rhs_block) : (size_t)nrhs;
+    return slots * (size_t)h->Vs * kSpinorComps * sizeof(double2);
+}
+
+// Blocked multi-RHS layout (WD_OPT_RHS_BLOCK = B): unit u = right-hand sides uB .. uB+B-1 is double2 [12][Vs][B].  Seen as
+// a field of 12 components whose "sites" are B elements wide, a chunk of sites is one strided 2-D copy like the plain layout.
+// Staging [12][cnt][B]; right-hand sides past the last one are zero.
+static int pack_spinor_blocked(wd_handle *h, double2 *dev, const double2 *host, int nrhs) {
+    const long long V = h->V, B = h->rhs_block;
+    const long long chunk = (V < (long long)kStageSites) ? V : (long long)kStageSites;
+    int rc = ensure_pinned(h, (size_t)chunk * kSpinorComps * B * sizeof(double2));
+    if (rc) return rc;
+    const size_t per = (size_t)V * kSpinorComps, uper = (size_t)h->Vs * kSpinorComps * B;
+    int b = 0;
+    for (int u = 0; u * B < nrhs; u++)
+        for (long long i0 = 0; i0 < V; i0 += chunk, b ^= 1) {
+            const long long cnt = (V - i0 < chunk) ? V - i0 : chunk;
+            WD_CUDA(h, cudaEventSynchronize(h->pinned_ev[b]));
+            double2 *st = h->pinned[b];
+#pragma omp parallel for schedule(static)
+            for (long long j = 0; j < cnt; j++)
+                for (int r = 0; r < B; r++) {
+                    const bool live = u * B + r < nrhs;
+                    const double2 *src = host + (size_t)(u * B + r) * per + (size_t)(i0 + j) * kSpinorComps;
+                    for (int c = 0; c < kSpinorComps; c++) st[((long long)c * cnt + j) * B + r] = live ? src[c] : make_double2(0.0, 0.0);
+                }
+            WD_CUDA(h, cudaMemcpy2DAsync(dev + u * uper + i0 * B, (size_t)h->Vs * B * sizeof(double2), st, (size_t)cnt * B * sizeof(double2),
+                                         (size_t)cnt * B * sizeof(double2), kSpinorComps, cudaMemcpyHostToDevice, h->stream));
+            WD_CUDA(h, cudaEventRecord(h->pinned_ev[b], h->stream));
+        }
+    WD_CUDA(h, cudaStreamSynchronize(h->stream));
+    return WD_OK;
+}
+
+static int unpack_spinor_blocked(wd_handle *h, double2 *host, const double2 *dev, int nrhs) {
+    const long long V = h->V, B = h->rhs_block;
+    const long long chunk = (V < (long long)kStageSites) ? V : (long long)kStageSites;
+    int rc = ensure_pinned(h, (size_t)chunk * kSpinorComps * B * sizeof(double2));
+    if (rc) return rc;
+    const size_t per = (size_t)V * kSpinorComps, uper = (size_t)h->Vs * kSpinorComps * B;
+    for (int u = 0; u * B < nrhs; u++)
+        for (long long i0 = 0; i0 < V; i0 += chunk) {
+            const long long cnt = (V - i0 < chunk) ? V - i0 : chunk;
+            double2 *st = h->pinned[0];
+            WD_CUDA(h, cudaMemcpy2DAsync(st, (size_t)cnt * B * sizeof(double2), dev + u * uper + i0 * B, (size_t)h->Vs * B * sizeof(double2),
+                                         (size_t)cnt * B * sizeof(double2), kSpinorComps, cudaMemcpyDeviceToHost, h->stream));
+            WD_CUDA(h, cudaStreamSynchronize(h->stream));
+#pragma omp parallel for schedule(static)
+            for (long long j = 0; j < cnt; j++)
+                for (int r = 0; r < B && u * B + r < nrhs; r++) {
+                    double2 *dst = host + (size_t)(u * B + r) * per + (size_t)(i0 + j) * kSpinorComps;
+                    for (int c = 0; c < kSpinorComps; c++) dst[c] = st[((long long)c * cnt + j) * B + r];
+                }
+        }
+    return WD_OK;
 }
 
 long long wd_component_stride(const wd_handle *h) { return h ? h->Vs : 0; }
@@ -328,6 +383,7 @@ static bool misaligned(const void *p) { return ((size_t)p & 15) != 0; }
 int wd_pack_spinor(wd_handle *h, void *dev_dst, const double *host_src, int nrhs) {
     WD_ENTER(h);
     if (!dev_dst || !host_src || nrhs < 1 || misaligned(dev_dst)) return fail(h, WD_EINVAL, "wd_pack_spinor: bad argument");
+    if (h->rhs_block > 1) return pack_spinor_blocked(h, (double2 *)dev_dst, (const double2 *)host_src, nrhs);
     const size_t per = (size_t)h->V * kSpinorComps, dper = (size_t)h->Vs * kSpinorComps;
     for (int r = 0; r < nrhs; r++) {
         double2 *dst = (double2 *)dev_dst + r * dper;
@@ -350,6 +406,7 @@ int wd_pack_spinor(wd_handle *h, void *dev_dst, const double *host_src, int nrhs
 int wd_unpack_spinor(wd_handle *h, double *host_dst, const void *dev_src, int nrhs) {
     WD_ENTER(h);
     if (!host_dst || !dev_src || nrhs < 1 || misaligned(dev_src)) return fail(h, WD_EINVAL, "wd_unpack_spinor: bad argument");
+    if (h->rhs_block > 1) return unpack_spinor_blocked(h, (double2 *)host_dst, (const double2 *)dev_src, nrhs);
     const size_t per = (size_t)h->V * kSpinorComps, dper = (size_t)h->Vs * kSpinorComps;
     for (int r = 0; r < nrhs; r++) {
         double2 *dst = (double2 *)host_dst + r * per;
@@ -417,6 +474,16 @@ static int auto_kernel(const wd_handle *h, int nrhs) {
     static const char *pref_tworow[] = {"tma_2x4x16", "tmw_2x4x16", "tmb_4x4x8", "tmb_2x8x8", "tile_1x4x4x16", "tile_2x4x4x4"};
     static const char *pref_hop[] = {"tmb_2x4x16", "tmb_4x4x8", "tmb_2x8x8", "tmw_2x4x16", "tile_1x4x4x16", "tile_2x4x4x4"};
     static const char *pref_multi[] = {"tmb_4x4x8", "tmb_2x8x8", "tmb_2x4x16", "tmw_2x4x16", "tile_1x4x4x16", "tile_2x4x4x4"};
+    if (h->rhs_block > 1) {  // blocked multi-RHS layout: the kernels written for it
+        for (int id = 0; id < kernel_count(); id++)
+            if (kernel_info(id).rhs_block == h->rhs_block && geometry_fits(h, kernel_info(id))) return id;
+        return 0;
+    }
+    // several right-hand sides on the plain layout: the quad kernel when its units of four are well filled (cfg 5: 21.7 ms
+    // against 26.4 ms of tmb_4x4x8; a unit costs the same however many of its four right-hand sides exist)
+    if (nrhs > 1 && h->variant == 0 && 20 * nrhs >= 17 * 4 * ((nrhs + 3) / 4))
+        for (int id = 0; id < kernel_count(); id++)
+            if (!strcmp(kernel_info(id).name, "tmq_2x4x8") && geometry_fits(h, kernel_info(id))) return id;
     const bool clover_fused = (h->csw != 0.0 || h->has_clover) && h->variant == 0;
     const char **pref = (nrhs > 1 && h->variant == 0) ? pref_multi : !clover_fused ? pref_hop : (h->gauge_rows == 2) ? pref_tworow : pref_clover;
     for (int i = 0; i < 6; i++)
@@ -447,6 +514,8 @@ int wd_set_option(wd_handle *h, int option, long value) {
         return WD_OK;
     case WD_OPT_KERNEL:
         if (value < -1 || value >= kernel_count()) return fail(h, WD_EINVAL, "WD_OPT_KERNEL: id out of range");
+        if (value >= 0 && kernel_info((int)value).rhs_block != h->rhs_block)
+            return fail(h, WD_EINVAL, std::string("WD_OPT_KERNEL: ") + kernel_info((int)value).name + " is written for WD_OPT_RHS_BLOCK = " + std::to_string(kernel_info((int)value).rhs_block));
         if (value >= 0 && !geometry_fits(h, kernel_info((int)value)))
             return fail(h, WD_EINVAL, std::string("WD_OPT_KERNEL: ") + kernel_info((int)value).name + " does not fit this handle (its tile does not divide the lattice)");
         h->kernel_opt = value;
@@ -472,6 +541,18 @@ int wd_set_option(wd_handle *h, int option, long value) {
         if (value != 0 && value != 1) return fail(h, WD_EINVAL, "WD_OPT_F32_KERNEL: 0 (automatic) or 1 (one-thread-per-site kernels)");
         h->f32_kernel = value;
         return WD_OK;
+    case WD_OPT_RHS_BLOCK: {
+        if (value != 1 && value != 4) return fail(h, WD_EINVAL, "WD_OPT_RHS_BLOCK: 1 (plain layout, default) or 4 (blocked)");
+        if (value == 4) {
+            bool fits = false;
+            for (int id = 0; id < kernel_count(); id++) fits = fits || (kernel_info(id).rhs_block == 4 && geometry_fits(h, kernel_info(id)));
+            if (!fits) return fail(h, WD_EINVAL, "WD_OPT_RHS_BLOCK = 4: the 2x4x8 tile of the blocked kernel does not divide this lattice");
+            if (h->dd) return fail(h, WD_EINVAL, "WD_OPT_RHS_BLOCK = 4: not available on a decomposed handle (wd_create_local)");
+        }
+        if (value != h->rhs_block) h->kernel_opt = -1;  // a kernel chosen by hand belongs to the other layout
+        h->rhs_block = value;
+        return WD_OK;
+    }
     case WD_OPT_GAUGE_ROWS: {
         if (value != 2 && value != 3) return fail(h, WD_EINVAL, "WD_OPT_GAUGE_ROWS: 3 (all nine entries, default) or 2 (two-row storage)");
         DeviceGuard guard(h->device);
@@ -495,6 +576,7 @@ int wd_get_option(const wd_handle *h, int option, long *value) {
     case WD_OPT_GMRES_GRAPH: *value = h->gmres_graph; return WD_OK;
     case WD_OPT_GAUGE_ROWS: *value = h->gauge_rows; return WD_OK;
     case WD_OPT_F32_KERNEL: *value = h->f32_kernel; return WD_OK;
+    case WD_OPT_RHS_BLOCK: *value = h->rhs_block; return WD_OK;
     default: return WD_EINVAL;
     }
 }
@@ -577,6 +659,8 @@ int wd_apply(wd_handle *h, void *dev_out, const void *dev_in, int nrhs) {
         return fail(h, WD_ESTATE, "wd_apply: csw != 0 but no self-coupling field (wd_load_clover / wd_build_clover)");
     const int kid = wd_kernel_for(h, nrhs);
     const KernelInfo &k = kernel_info(kid);
+    if (k.rhs_block != h->rhs_block) return fail(h, WD_ESTATE, "wd_apply: no kernel for this spinor layout on this lattice");
+    if (h->rhs_block > 1 && h->variant != 0) return fail(h, WD_ESTATE, "wd_apply: the unfused variant reads the plain layout (WD_OPT_RHS_BLOCK = 1)");
     KParams p;
     int rc = fill_params(h, p, k);
     if (rc) return rc;
@@ -681,6 +765,7 @@ static int apply_host_pipelined(wd_handle *h, double *host_out, const double *ho
 int wd_apply_host(wd_handle *h, double *host_out, const double *host_in, int nrhs) {
     WD_ENTER(h);
     if (!host_out || !host_in || nrhs < 1) return fail(h, WD_EINVAL, "wd_apply_host: null pointer or nrhs < 1");
+    WD_PLAIN_ONLY(h, "wd_apply_host");
     if (!h->has_gauge) return fail(h, WD_ESTATE, "wd_apply_host: no gauge field loaded");
     if (h->csw != 0.0 && !h->has_clover)
         return fail(h, WD_ESTATE, "wd_apply_host: csw != 0 but no self-coupling field (wd_load_clover / wd_build_clover)");

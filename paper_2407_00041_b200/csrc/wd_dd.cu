@@ -178,6 +178,7 @@ size_t wd_dd_face_bytes(const wd_handle *h, int mu, int nrhs) {
 
 int wd_dd_pack(wd_handle *h, const void *dev_in, int nrhs, int mu, void *dev_send_minus, void *dev_send_plus) {
     WD_ENTER(h);
+    WD_PLAIN_ONLY(h, "wd_dd_pack");
     if (!dev_in || !dev_send_minus || !dev_send_plus || nrhs < 1) return fail(h, WD_EINVAL, "wd_dd_pack: null pointer or nrhs < 1");
     if (!decomposed(h, mu)) return fail(h, WD_EINVAL, "wd_dd_pack: direction is not decomposed on this handle");
     if (!h->has_gauge) return fail(h, WD_ESTATE, "wd_dd_pack: no gauge field loaded");
@@ -198,6 +199,7 @@ int wd_dd_pack(wd_handle *h, const void *dev_in, int nrhs, int mu, void *dev_sen
 
 int wd_dd_exterior(wd_handle *h, void *dev_out, int nrhs, int mu, const void *dev_recv_from_plus, const void *dev_recv_from_minus) {
     WD_ENTER(h);
+    WD_PLAIN_ONLY(h, "wd_dd_exterior");
     if (!dev_out || !dev_recv_from_plus || !dev_recv_from_minus || nrhs < 1)
         return fail(h, WD_EINVAL, "wd_dd_exterior: null pointer or nrhs < 1");
     if (!decomposed(h, mu)) return fail(h, WD_EINVAL, "wd_dd_exterior: direction is not decomposed on this handle");

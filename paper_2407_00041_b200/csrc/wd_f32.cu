@@ -76,6 +76,7 @@ size_t wd_spinor_bytes_f32(const wd_handle *h, int nrhs) {
 
 int wd_convert_spinor(wd_handle *h, void *dev_dst, const void *dev_src, int nrhs, int to_f32) {
     WD_ENTER(h);
+    WD_PLAIN_ONLY(h, "wd_convert_spinor");
     if (!dev_dst || !dev_src || nrhs < 1) return fail(h, WD_EINVAL, "wd_convert_spinor: null pointer or nrhs < 1");
     const long long n = (long long)nrhs * h->Vs * kSpinorComps;
     if (to_f32) WD_CUDA(h, convert((float2 *)dev_dst, (const double2 *)dev_src, n, h->nsm, h->stream));
@@ -86,6 +87,7 @@ int wd_convert_spinor(wd_handle *h, void *dev_dst, const void *dev_src, int nrhs
 
 int wd_apply_f32(wd_handle *h, void *dev_out, const void *dev_in, int nrhs) {
     WD_ENTER(h);
+    WD_PLAIN_ONLY(h, "wd_apply_f32");
     if (!dev_out || !dev_in || nrhs < 1) return fail(h, WD_EINVAL, "wd_apply_f32: null pointer or nrhs < 1");
     if (((size_t)dev_out | (size_t)dev_in) & 7) return fail(h, WD_EINVAL, "wd_apply_f32: spinor buffers must be 8-byte aligned");
     const size_t bytes = wd_spinor_bytes_f32(h, nrhs);

@@ -352,6 +352,7 @@ extern "C" {
 int wd_gmres(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_cycles, double tol, int *cycles_done,
              double *host_resid) {
     WD_ENTER(h);
+    WD_PLAIN_ONLY(h, "wd_gmres");
     if (!dev_x || !dev_b || m < 1 || m > kMaxM || max_cycles < 0 || !(tol > 0.0))
         return fail(h, WD_EINVAL, "wd_gmres: null pointer, m outside 1..64, max_cycles < 0 or tol <= 0");
     if (((size_t)dev_x | (size_t)dev_b) & 15) return fail(h, WD_EINVAL, "wd_gmres: spinor buffers must be 16-byte aligned");

@@ -29,6 +29,7 @@ struct wd_handle {
     MapCache *maps;        // tensor maps of the TMA kernels, keyed by (buffers, nrhs, tile)
     // options
     long variant, kernel_opt, tchunk_opt, zgroup_opt, device_pack, host_pipeline, gmres_graph, gauge_rows, f32_kernel;
+    long rhs_block;  // WD_OPT_RHS_BLOCK: 1 = plain multi-RHS device layout, 4 = blocked (units of four interleaved per site)
     // staging
     double2 *pinned[2];
     size_t pinned_bytes;
@@ -67,6 +68,10 @@ struct DeviceGuard {
     if (!(h)) return WD_EINVAL; \
     wd::DeviceGuard guard_((h)->device)
 
+
+// entry points that work on the plain device layout only
+#define WD_PLAIN_ONLY(h, what) \
+    if ((h)->rhs_block != 1) return wd::fail(h, WD_ESTATE, what ": not available while WD_OPT_RHS_BLOCK = 4 (blocked spinor layout)")
 
 #define WD_CUDA(h, call)                                                                          \
     do {                                                                                          \

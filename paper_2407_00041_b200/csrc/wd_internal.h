@@ -69,6 +69,7 @@ struct KernelInfo {
     int bt, bz, by, bx;  // tile extents (all 0: linear geometry, any lattice)
     int threads;
     bool multi_rhs;      // one launch applies the operator to all p.nrhs right-hand sides
+    int rhs_block;       // device layout of the spinors it reads and writes: 1 plain, 4 blocked (WD_OPT_RHS_BLOCK)
     cudaError_t (*launch)(const KParams &p, int self, cudaStream_t st);
 };
 
@@ -77,6 +78,8 @@ const KernelInfo &kernel_info(int id);
 
 // TMA-staged T-marching kernels: first generation (wd_tma.cu), second generation (wd_tmb.cu)
 cudaError_t launch_tma_2x4x16(const KParams &p, int self, cudaStream_t st);
+cudaError_t launch_tmq_2x4x8(const KParams &p, int self, cudaStream_t st);   // four right-hand sides per work item
+cudaError_t launch_tmqb_2x4x8(const KParams &p, int self, cudaStream_t st);  // the same on the blocked multi-RHS layout
 cudaError_t launch_tmb_4x4x8(const KParams &p, int self, cudaStream_t st);
 cudaError_t launch_tmb_2x8x8(const KParams &p, int self, cudaStream_t st);
 cudaError_t launch_tmb_2x4x16(const KParams &p, int self, cudaStream_t st);  // three ring slots

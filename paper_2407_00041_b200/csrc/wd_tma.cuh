@@ -93,11 +93,18 @@ __device__ __forceinline__ uint64_t l2_policy_evict_last() {
     return p;
 }
 
+// register budget of a warpgroup (all four warps execute it): kernels with a producer warpgroup start every warpgroup at
+// the launch bound and move the producer's share to the compute warpgroups
+template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+
 // ---------------------------------------------------------------- host side
 // A field of double2 (esize 16) or float2 (esize 8) [ncomp][Vs] (Vs >= T*Z*Y*X, site index X fastest) seen as a 5-D FP64 tensor
 // (2X, Y, Z, T, ncomp); a box is (2*bx, by, bz, 1, bc) and lands in shared memory densely as
 // double2 [bc][bz][by][bx].
+// rb > 1: a blocked multi-RHS spinor field [ncomp][Vs][rb] (rb right-hand sides interleaved per site): dimension 0 and
+// the box are rb times as wide, the box lands as [bc][bz][by][bx][rb].
 cudaError_t encode_field_map(CUtensorMap *map, const void *base, const int n[4], long long Vs, int ncomp, int bx,
-                             int by, int bz, int bc, int esize = 16);
+                             int by, int bz, int bc, int esize = 16, int rb = 1);
 
 }  // namespace wd

@@ -192,7 +192,8 @@ template <class P> static void plan_items(const KParams &p, TmaParams &prm, Chun
 // (9, or 6 with two-row storage), scomp = components per S box (18 or 9).
 template <class P> static cudaError_t get_maps(const KParams &p, int ucomp, int scomp, const TmaMaps **out, TmaMaps *scratch) {
     constexpr int BZ = P::BZ, BY = P::BY, BX = P::BX;
-    const int tag = ((((ucomp * 32 + scomp) * 64 + BZ) * 64 + BY) * 64 + BX) * 2 + (p.esize == 8);  // everything a box depends on
+    static_assert(BZ < 16 && BY < 32 && BX < 64 && P::G < 16, "tag fields");
+    const int tag = ((((((ucomp * 32 + scomp) * 16 + BZ) * 32 + BY) * 64 + BX) * 16 + P::G) * 2 + (p.esize == 8)) * 2 + P::BLK;  // everything a box depends on
     const void *Sbase = (P::SELF == SELF_CLOVER) ? (const void *)p.S : (const void *)p.U;
     if (p.maps) {
         if (const TmaMaps *m = p.maps->find(tag, p.psi, p.U, Sbase, p.nrhs)) {
@@ -204,21 +205,26 @@ template <class P> static cudaError_t get_maps(const KParams &p, int ucomp, int 
     cudaError_t e;
     const int nucomp = 4 * ucomp, nscomp = (P::SELF == SELF_CLOVER) ? 36 : nucomp;
     const int sc = (scomp <= nscomp) ? scomp : nscomp;
-#define WD_ENC(m, base, nc, bx, by, bz, bc)                                                  \
-    if ((e = encode_field_map(&maps->m, base, p.n, p.Vs, nc, bx, by, bz, bc, p.esize)) != cudaSuccess) { \
+#define WD_ENC(m, base, nc, bx, by, bz, bc) WD_ENCR(m, base, nc, bx, by, bz, bc, 1)
+#define WD_ENCR(m, base, nc, bx, by, bz, bc, rb)                                             \
+    if ((e = encode_field_map(&maps->m, base, p.n, p.Vs, nc, bx, by, bz, bc, p.esize, rb)) != cudaSuccess) { \
         if (p.maps) p.maps->clear();                                                         \
         return e;                                                                            \
     }
-    WD_ENC(psi_c, p.psi, 12 * p.nrhs, BX, BY, BZ, 12)
-    WD_ENC(psi_z, p.psi, 12 * p.nrhs, BX, BY, 1, 12)
-    WD_ENC(psi_y, p.psi, 12 * p.nrhs, BX, 1, BZ, 12)
-    WD_ENC(psi_x, p.psi, 12 * p.nrhs, P::XW, BY, BZ, 12)
+    // spinor boxes: the G right-hand sides of a unit — 12 G consecutive components of the plain layout, or 12 components of
+    // G-interleaved sites in the blocked layout (whose units are padded to G right-hand sides)
+    const int pcomp = P::BLK ? 12 * ((p.nrhs + P::G - 1) / P::G) : 12 * p.nrhs, pbox = P::BLK ? 12 : 12 * P::G;
+    WD_ENCR(psi_c, p.psi, pcomp, BX, BY, BZ, pbox, P::RBK)
+    WD_ENCR(psi_z, p.psi, pcomp, BX, BY, 1, pbox, P::RBK)
+    WD_ENCR(psi_y, p.psi, pcomp, BX, 1, BZ, pbox, P::RBK)
+    WD_ENCR(psi_x, p.psi, pcomp, P::XW, BY, BZ, pbox, P::RBK)
     WD_ENC(u_c, p.U, nucomp, BX, BY, BZ, ucomp)
     WD_ENC(u_z, p.U, nucomp, BX, BY, 1, ucomp)
     WD_ENC(u_y, p.U, nucomp, BX, 1, BZ, ucomp)
     WD_ENC(u_x, p.U, nucomp, P::XW, BY, BZ, ucomp)
     WD_ENC(s_c, Sbase, nscomp, BX, BY, BZ, sc)
 #undef WD_ENC
+#undef WD_ENCR
     *out = maps;
     return cudaSuccess;
 }

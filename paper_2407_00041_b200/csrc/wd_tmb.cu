@@ -39,6 +39,8 @@ enum { OB_C = 0, OB_C1, OB_Z, OB_Y, OB_X, OB_R, OB_R1, OB_R2, OB_R3, OB_ITEM0, O
 template <int BZ_, int BY_, int BX_, int SELF_, int KR_ = 4> struct Plan {
     static constexpr int BZ = BZ_, BY = BY_, BX = BX_, SELF = SELF_, KR = KR_;
     static constexpr int G = 1;              // right-hand sides per work item
+    static constexpr bool BLK = false;       // plain multi-RHS layout only
+    static constexpr int RBK = 1;
     static constexpr int N = BZ * BY * BX;   // sites per tile = compute threads
     static constexpr int CTAS_PER_SM = 1;
     static constexpr int XW = 1;             // sites per row of an X-face box (wd_tma.cu: 2 for 8-byte elements)

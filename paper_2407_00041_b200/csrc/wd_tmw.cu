@@ -38,8 +38,6 @@ template <int BZ_, int BY_, int BX_, int SELF_> struct Plan : gen1::Plan<BZ_, BY
     static_assert(!Base::COMPACT && Base::OB_SB == OB_SB && Base::OB_ITEM0 == OB_ITEM0 && Base::OB_COUNT == OB_COUNT, "barrier layout");
 };
 
-template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
-template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 // named barrier 1: warpgroup B arrives when its partial sums are in shared memory, warpgroup A waits for them
 __device__ __forceinline__ void handover_arrive() { asm volatile("bar.arrive 1, 256;" ::: "memory"); }
 __device__ __forceinline__ void handover_wait() { asm volatile("bar.sync 1, 256;" ::: "memory"); }

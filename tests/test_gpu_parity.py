@@ -46,7 +46,8 @@ class Op:
 
     def dev_spinor(self, nrhs=1):
         n = wd.wd_spinor_bytes(self.h, nrhs) // 8
-        assert n == nrhs * wd.wd_component_stride(self.h) * 24 and wd.wd_component_stride(self.h) >= self.V
+        blk = wd.wd_get_option(self.h, wd.WD_OPT_RHS_BLOCK)  # blocked layout: units padded to blk right-hand sides
+        assert n == -(-nrhs // blk) * blk * wd.wd_component_stride(self.h) * 24 and wd.wd_component_stride(self.h) >= self.V
         return self.torch.empty(n, dtype=self.torch.float64, device="cuda")
 
     def apply(self, psi, nrhs=1):
@@ -79,6 +80,8 @@ def kernels_fitting(dims):
         name = wd.wd_kernel_name(k)
         if name.startswith("linear"):
             out.append(k)
+            continue
+        if name.startswith("tmqb_"):  # written for the blocked multi-RHS layout (WD_OPT_RHS_BLOCK = 4): test_gpu_tma.py
             continue
         b = [int(v) for v in name.split("_")[1].split("x")]  # tile_TxZxYxX or tma_ZxYxX
         if all(n % t == 0 for n, t in zip(dims[-len(b):], b)):

@@ -23,7 +23,7 @@ def tma_kernels(dims):
     out = []
     for k in range(wd.wd_kernel_count()):
         name = wd.wd_kernel_name(k)
-        if name.startswith(("tma_", "tmb_", "tmw_")):
+        if name.startswith(("tma_", "tmb_", "tmw_", "tmq_")):
             b = [int(v) for v in name.split("_")[1].split("x")]
             if all(n % t == 0 for n, t in zip(dims[-3:], b)):
                 out.append(k)
@@ -78,6 +78,82 @@ def test_tma_many_items_per_cta_and_multi_rhs(torch):
     for kid in tma_kernels(dims):
         with Op(torch, dims, m0, csw, U, C, kernel=kid, tchunk=1) as op:
             assert rel_l2(op.apply(psi, nrhs), ref) <= TOL, wd.wd_kernel_name(kid)
+
+
+@pytest.mark.parametrize("nrhs", [2, 4, 5, 12])
+def test_quad_kernel_units_of_four_right_hand_sides(torch, nrhs):
+    """tmq_*: one compute thread per (site, right-hand side), four right-hand sides per work item.  Full units, a partial
+    last unit (its TMA boxes reach past the last right-hand side and are zero-filled; its threads must not store), every
+    self-coupling mode, every right-hand side different."""
+    dims, m0, csw = (6, 4, 8, 16), -0.4, 1.0
+    U = wdinputs.gauge_haar(dims, 431)
+    psi = wdinputs.spinor(dims, 432, nrhs=nrhs)
+    C = wdinputs.selfcoupling_random(dims, 433)
+    ref_c = oracle.apply(dims, m0, U, C, psi)
+    ref_w = oracle.apply(dims, m0, U, None, psi)
+    kids = [k for k in tma_kernels(dims) if wd.wd_kernel_name(k).startswith("tmq_")]
+    assert kids
+    for kid in kids:
+        for tchunk in (0, 1, 3):
+            with Op(torch, dims, m0, csw, U, C, kernel=kid, tchunk=tchunk) as op:
+                out = op.apply(psi, nrhs)
+                for r in range(nrhs):
+                    assert rel_l2(out[r], ref_c[r]) <= TOL, (wd.wd_kernel_name(kid), "clover", tchunk, r)
+        with Op(torch, dims, m0, 0.0, U, None, kernel=kid) as op:
+            assert rel_l2(op.apply(psi, nrhs), ref_w) <= TOL, (wd.wd_kernel_name(kid), "mass")
+
+
+@pytest.mark.parametrize("nrhs", [1, 3, 4, 9, 12])
+@pytest.mark.parametrize("dims", [(6, 4, 8, 16), (3, 2, 4, 8), (4, 6, 12, 24)])
+def test_blocked_multi_rhs_layout(torch, dims, nrhs):
+    """WD_OPT_RHS_BLOCK = 4: device spinors are double2 [unit][12][Vs][4]; pack / apply (tmqb_*) / unpack against the
+    oracle for full and padded units, on lattices of one tile (every face wraps onto the tile itself) and of several,
+    with clover term, mass term, T chunks of 1; every right-hand side different; bit-repeatable."""
+    m0, csw = -0.4, 1.0
+    U = wdinputs.gauge_haar(dims, 451)
+    psi = wdinputs.spinor(dims, 452, nrhs=nrhs).reshape(nrhs, -1, 12, 2)
+    C = wdinputs.selfcoupling_random(dims, 453)
+    ref_c = oracle.apply(dims, m0, U, C, psi).reshape(psi.shape)
+    ref_w = oracle.apply(dims, m0, U, None, psi).reshape(psi.shape)
+    for tchunk in (0, 1):
+        with Op(torch, dims, m0, csw, U, C, rhs_block=4, tchunk=tchunk) as op:
+            assert wd.wd_kernel_name(wd.wd_kernel_for(op.h, nrhs)).startswith("tmqb_")
+            out = op.apply(psi, nrhs)
+            for r in range(nrhs):
+                assert rel_l2(out[r], ref_c[r]) <= TOL, ("clover", tchunk, r)
+            assert np.array_equal(op.apply(psi, nrhs), out)
+    with Op(torch, dims, m0, 0.0, U, None, rhs_block=4) as op:
+        assert rel_l2(op.apply(psi, nrhs), ref_w) <= TOL, "mass"
+        # the round trip through the blocked layout alone is exact
+        d = op.dev_spinor(nrhs)
+        wd.wd_pack_spinor(op.h, d, psi, nrhs)
+        back = np.empty_like(psi)
+        wd.wd_unpack_spinor(op.h, back, d, nrhs)
+        assert np.array_equal(back, psi)
+
+
+def test_blocked_layout_rules(torch):
+    """What WD_OPT_RHS_BLOCK = 4 refuses: lattices its tile does not divide, kernels of the other layout, and the entry
+    points that work on the plain layout."""
+    with Op(torch, (4, 4, 4, 4), -0.4, 0.0) as op:
+        with pytest.raises(wd.WDError):
+            wd.wd_set_option(op.h, wd.WD_OPT_RHS_BLOCK, 4)
+        assert wd.wd_get_option(op.h, wd.WD_OPT_RHS_BLOCK) == 1
+    dims = (4, 2, 4, 8)
+    U = wdinputs.gauge_haar(dims, 461)
+    with Op(torch, dims, -0.4, 0.0, U) as op:
+        with pytest.raises(wd.WDError):
+            wd.wd_set_option(op.h, wd.WD_OPT_KERNEL, wd.kernel_id("tmqb_2x4x8"))  # plain handle, blocked kernel
+        wd.wd_set_option(op.h, wd.WD_OPT_RHS_BLOCK, 4)
+        with pytest.raises(wd.WDError):
+            wd.wd_set_option(op.h, wd.WD_OPT_KERNEL, wd.kernel_id("tmb_4x4x8"))   # blocked handle, plain kernel
+        psi = wdinputs.spinor(dims, 462)
+        with pytest.raises(wd.WDError):
+            wd.wd_apply_host(op.h, np.empty_like(psi), psi, 1)
+        wd.wd_set_option(op.h, wd.WD_OPT_RHS_BLOCK, 1)
+        out = np.empty_like(psi)
+        wd.wd_apply_host(op.h, out, psi, 1)
+        assert rel_l2(out, oracle.apply(dims, -0.4, U, None, psi)) <= TOL
 
 
 @pytest.mark.parametrize("dims,csw", [((8, 4, 8, 16), 1.0), ((8, 4, 8, 16), 0.0), ((12, 8, 8, 32), 1.0), ((5, 4, 8, 16), 1.0)])
