@@ -14,7 +14,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJDIR = os.path.join(HERE, "build")
 SO = os.path.join(HERE, "libwd.so")
 BENCH_SO = os.path.join(HERE, "libwdbench.so")  # measurement helpers of bench.py (include/wd_bench.h), not the product
-SOURCES = ["wd_api.cu", "wd_kernels.cu", "wd_tma.cu", "wd_tmb.cu", "wd_tmw.cu", "wd_pack.cu", "wd_clover.cu", "wd_gmres.cu", "wd_dd.cu", "wd_f32.cu"]
+SOURCES = ["wd_api.cu", "wd_kernels.cu", "wd_tma.cu", "wd_tmb.cu", "wd_tmw.cu", "wd_tmq.cu", "wd_pack.cu", "wd_clover.cu", "wd_gmres.cu", "wd_dd.cu", "wd_f32.cu"]
 BENCH_SOURCES = [os.path.join("bench", "wd_peaks.cu")]
 HEADERS = ["wd_internal.h", "wd_handle.h", "wd_math.cuh", "wd_tma.cuh", "wd_tma_common.cuh", "wd_tma_plan.cuh", "wd_smem_ops.cuh", "wd_ldg_kernels.cuh",
            os.path.join("..", "..", "include", "wd.h"), os.path.join("..", "..", "include", "wd_bench.h")]

@@ -103,45 +103,29 @@ __global__ void __launch_bounds__(P::NTHREADS, P::CTAS_PER_SM) k_tma(const __gri
 
     const int T = prm.n[0], Z = prm.n[1], Y = prm.n[2], X = prm.n[3];
 
-    if (tid >= P::NC) {
+    if (tid >= N) {
         // ======================= producer: one thread issues every TMA (wd_tma_plan.cuh) =======================
-        if (P::PRODUCER_WG) reg_dec<40>();
-        if (tid == P::NC) producer<P, false>(maps, prm, smem, sbase, bar_full, bar_empty);
+        if (tid == N) producer<P, false>(maps, prm, smem, sbase, bar_full, bar_empty);
         return;
     }
-    if (P::PRODUCER_WG) reg_inc<232>();
-    // ======================= consumers: one thread per (site of the tile, right-hand side of the unit) =======================
-    // G > 1: a warp holds SPW = 32 / G consecutive sites of the tile for the G right-hand sides of the unit.  Plain
-    // multi-RHS layout: lane = r * SPW + site, psi boxes [r][component][site].  Blocked layout (P::BLK): lane = site * G + r,
-    // psi boxes [component][site][r] — a warp reads 512 consecutive bytes per psi component, and the links and S of a site,
-    // the same for its G right-hand sides, are one address per G adjacent lanes (wd_tma_plan.cuh).
+    // ======================= consumers: one thread per site of the tile =======================
     const int lane = tid & 31;
-    constexpr int G = P::G, SPW = 32 / G;
-    constexpr bool BLK = P::BLK;
-    const int r = (G == 1) ? 0 : BLK ? lane % G : lane / SPW;                                   // right-hand side within the unit
-    const int sid = (G == 1) ? tid : (tid >> 5) * SPW + (BLK ? lane / G : lane % SPW);          // site within the tile
-    const int lx = sid % BX, ly = (sid / BX) % BY, lz = sid / (BX * BY);
+    const int lx = tid % BX, ly = (tid / BX) % BY, lz = tid / (BX * BY);
     constexpr uint32_t E = P::E, NS = N * E;
-    constexpr uint32_t EP = E * P::RBK, NSP = N * EP;  // psi boxes: bytes per site, component stride of the interior
-    const uint32_t own = sid * E;                                            // links, S
-    const uint32_t ownp = BLK ? sid * EP + r * E : own + r * 12 * NS;        // psi interior of right-hand side r
+    const uint32_t own = tid * E;
     // operand addresses (bytes from the start of shared memory): interior or face storage
     const uint32_t fz = (ly * BX + lx) * E, fy = (lz * BX + lx) * E;
-    // psi faces: site offset and right-hand side r
-    const uint32_t fzp = (ly * BX + lx) * EP + (BLK ? r * E : r * 12 * P::FZ * E), fyp = (lz * BX + lx) * EP + (BLK ? r * E : r * 12 * P::FY * E);
     // X faces: XW sites per (z, y) row; the neighbour column is the last one of the low face, the first of the high face
-    const uint32_t fxl = ((lz * BY + ly) * P::XW + (P::XW - 1)) * E;
-    const uint32_t rxp = BLK ? r * E : r * 12 * P::FX * E;
-    const uint32_t fxlp = ((lz * BY + ly) * P::XW + (P::XW - 1)) * EP + rxp, fxhp = ((lz * BY + ly) * P::XW) * EP + rxp;
+    const uint32_t fxl = ((lz * BY + ly) * P::XW + (P::XW - 1)) * E, fxh = ((lz * BY + ly) * P::XW) * E;
     const bool zf_in = lz < BZ - 1, zb_in = lz > 0, yf_in = ly < BY - 1, yb_in = ly > 0, xf_in = lx < BX - 1, xb_in = lx > 0;
-    const uint32_t z_pf = zf_in ? P::OFF_C + ownp + P::FZ * EP : P::OFF_ZHI + fzp, z_pf_s = zf_in ? NSP : P::FZ * EP;
-    const uint32_t z_pb = zb_in ? P::OFF_C + ownp - P::FZ * EP : P::OFF_ZLO + fzp, z_pb_s = zb_in ? NSP : P::FZ * EP, z_b_s = zb_in ? NS : P::FZ * E;
+    const uint32_t z_pf = zf_in ? P::OFF_C + own + P::FZ * E : P::OFF_ZHI + fz, z_pf_s = zf_in ? NS : P::FZ * E;
+    const uint32_t z_pb = zb_in ? P::OFF_C + own - P::FZ * E : P::OFF_ZLO + fz, z_b_s = zb_in ? NS : P::FZ * E;
     const uint32_t z_ub = zb_in ? P::OFF_Z + own - P::FZ * E : P::OFF_ZUF + fz;
-    const uint32_t y_pf = yf_in ? P::OFF_C + ownp + BX * EP : P::OFF_YHI + fyp, y_pf_s = yf_in ? NSP : P::FY * EP;
-    const uint32_t y_pb = yb_in ? P::OFF_C + ownp - BX * EP : P::OFF_YLO + fyp, y_pb_s = yb_in ? NSP : P::FY * EP, y_b_s = yb_in ? NS : P::FY * E;
+    const uint32_t y_pf = yf_in ? P::OFF_C + own + BX * E : P::OFF_YHI + fy, y_pf_s = yf_in ? NS : P::FY * E;
+    const uint32_t y_pb = yb_in ? P::OFF_C + own - BX * E : P::OFF_YLO + fy, y_b_s = yb_in ? NS : P::FY * E;
     const uint32_t y_ub = yb_in ? P::OFF_Y + own - BX * E : P::OFF_YUF + fy;
-    const uint32_t x_pf = xf_in ? P::OFF_C + ownp + EP : P::OFF_XHI + fxhp, x_pf_s = xf_in ? NSP : P::FX * EP;
-    const uint32_t x_pb = xb_in ? P::OFF_C + ownp - EP : P::OFF_XLO + fxlp, x_pb_s = xb_in ? NSP : P::FX * EP, x_b_s = xb_in ? NS : P::FX * E;
+    const uint32_t x_pf = xf_in ? P::OFF_C + own + E : P::OFF_XHI + fxh, x_pf_s = xf_in ? NS : P::FX * E;
+    const uint32_t x_pb = xb_in ? P::OFF_C + own - E : P::OFF_XLO + fxl, x_b_s = xb_in ? NS : P::FX * E;
     const uint32_t x_ub = xb_in ? P::OFF_X + own - E : P::OFF_XUF + fxl;
 
     auto release = [&](int ob) {
@@ -167,11 +151,7 @@ __global__ void __launch_bounds__(P::NTHREADS, P::CTAS_PER_SM) k_tma(const __gri
         if (item < 0) break;
         const Item it = decode_item<P>(prm, item);
         const long long site0 = ((long long)(it.z0 + lz) * Y + (it.y0 + ly)) * X + (it.x0 + lx);
-        // blocked layout: unit u at u * 12 * Vs * G elements, element (c, site, r) at (c * Vs + site) * G + r; its units are
-        // padded to G right-hand sides, so every thread stores.  Plain layout: the last unit may hold fewer than G right-hand
-        // sides (its boxes reach past the last one and are zero-filled); those threads do not store.
-        C *__restrict__ out = reinterpret_cast<C *>(prm.out) + (BLK ? (long long)it.rhs0 * 12 * V + r : (long long)(it.rhs0 + r) * 12 * V);
-        const bool live = (G == 1) || BLK || r < it.ng;
+        C *__restrict__ out = reinterpret_cast<C *>(prm.out) + (long long)it.rhs0 * 12 * V;
         // open boundaries of a domain-decomposed sub-lattice: hops that would cross them are left out
         const int open = OPEN ? prm.open_mask : 0;
         const bool zf_on = !((open & 2) && it.z0 + lz == Z - 1), zb_on = !((open & 2) && it.z0 + lz == 0);
@@ -182,7 +162,7 @@ __global__ void __launch_bounds__(P::NTHREADS, P::CTAS_PER_SM) k_tma(const __gri
             C p[12];
             mbar_wait(bar_full + 8 * OB_C, nC & 1);
 #pragma unroll
-            for (int c = 0; c < 12; c++) p[c] = lds<C>(smem, P::OFF_C + ownp + c * NSP);
+            for (int c = 0; c < 12; c++) p[c] = lds<C>(smem, P::OFF_C + own + c * NS);
             project<0, +1>(hprev, p);
             if ((open & 1) && it.t0 == 0) {
 #pragma unroll
@@ -208,7 +188,7 @@ __global__ void __launch_bounds__(P::NTHREADS, P::CTAS_PER_SM) k_tma(const __gri
 #endif
                 load_link<P::UC, C>(u, smem, P::OFF_T + own, NS);
 #pragma unroll
-                for (int c = 0; c < 12; c++) p[c] = lds<C>(smem, P::OFF_C + ownp + c * NSP);
+                for (int c = 0; c < 12; c++) p[c] = lds<C>(smem, P::OFF_C + own + c * NS);
                 if (j > 1) {
                     C f[12];
 #pragma unroll
@@ -217,7 +197,7 @@ __global__ void __launch_bounds__(P::NTHREADS, P::CTAS_PER_SM) k_tma(const __gri
                     const long long ip = (long long)tprev * strideT + site0;
 #pragma unroll
                     for (int c = 0; c < 12; c++)
-                        if (live) __stcs(out + ((long long)c * V + ip) * P::RBK,
+                        __stcs(out + (long long)c * V + ip,
                                mk<C>(fma(-half, f[c].x, outp[c].x), fma(-half, f[c].y, outp[c].y)));
                 }
                 if (j == prm.tchunk + 1) {  // epilogue step: nothing else to do for slice t
@@ -238,13 +218,13 @@ __global__ void __launch_bounds__(P::NTHREADS, P::CTAS_PER_SM) k_tma(const __gri
             }
             const uint32_t pf = nF & 1;
             mbar_wait(bar_full + 8 * OB_Z, pf);
-            hop_pair_smem<1, P::UC, C>(acc, smem, P::OFF_Z + own, NS, z_pf, z_pf_s, z_ub, z_b_s, z_pb, z_pb_s, zf_on, zb_on);
+            hop_pair_smem<1, P::UC, C>(acc, smem, P::OFF_Z + own, NS, z_pf, z_pf_s, z_ub, z_b_s, z_pb, z_b_s, zf_on, zb_on);
             release(OB_Z);
             mbar_wait(bar_full + 8 * OB_Y, pf);
-            hop_pair_smem<2, P::UC, C>(acc, smem, P::OFF_Y + own, NS, y_pf, y_pf_s, y_ub, y_b_s, y_pb, y_pb_s, yf_on, yb_on);
+            hop_pair_smem<2, P::UC, C>(acc, smem, P::OFF_Y + own, NS, y_pf, y_pf_s, y_ub, y_b_s, y_pb, y_b_s, yf_on, yb_on);
             release(OB_Y);
             mbar_wait(bar_full + 8 * OB_X, pf);
-            hop_pair_smem<3, P::UC, C>(acc, smem, P::OFF_X + own, NS, x_pf, x_pf_s, x_ub, x_b_s, x_pb, x_pb_s, xf_on, xb_on);
+            hop_pair_smem<3, P::UC, C>(acc, smem, P::OFF_X + own, NS, x_pf, x_pf_s, x_ub, x_b_s, x_pb, x_b_s, xf_on, xb_on);
             release(OB_X);
             release(OB_C);
             nC++;
@@ -306,25 +286,4 @@ template <int BZ, int BY, int BX> static cudaError_t launch_tma(const KParams &p
 }
 
 cudaError_t launch_tma_2x4x16(const KParams &p, int self, cudaStream_t st) { return launch_tma<2, 4, 16>(p, self, st); }
-
-// The "quad" instance for several right-hand sides in one call (a8): a 64-site tile, four right-hand sides per work item,
-// 256 compute threads (site, r).  FP64, nine-entry links.
-template <int BZ, int BY, int BX, int G, bool BLK, int SELF> static cudaError_t launch_tmq_self(const KParams &p, cudaStream_t st) {
-    using P = Plan<BZ, BY, BX, SELF, 9, cd, G, BLK>;
-    return p.open_mask ? launch_tma_kernel<P>(k_tma<P, true>, p, st, /*ucomp*/ 9, /*scomp*/ 18, CHUNK_COST_MODEL, /*rb*/ 4)
-                       : launch_tma_kernel<P>(k_tma<P, false>, p, st, /*ucomp*/ 9, /*scomp*/ 18, CHUNK_COST_MODEL, /*rb*/ 4);
-}
-cudaError_t launch_tmq_2x4x8(const KParams &p, int self, cudaStream_t st) {
-    if (p.esize != 16) return cudaErrorNotSupported;  // FP64 only (two-row storage is ignored: nine-entry links are read)
-    if (self == SELF_CLOVER) return launch_tmq_self<2, 4, 8, 4, false, SELF_CLOVER>(p, st);
-    if (self == SELF_MASS) return launch_tmq_self<2, 4, 8, 4, false, SELF_MASS>(p, st);
-    return launch_tmq_self<2, 4, 8, 4, false, SELF_NONE>(p, st);
-}
-// ... and on the blocked multi-RHS layout (WD_OPT_RHS_BLOCK = 4): p.psi / p.out are double2 [unit][12][Vs][4]
-cudaError_t launch_tmqb_2x4x8(const KParams &p, int self, cudaStream_t st) {
-    if (p.esize != 16) return cudaErrorNotSupported;
-    if (self == SELF_CLOVER) return launch_tmq_self<2, 4, 8, 4, true, SELF_CLOVER>(p, st);
-    if (self == SELF_MASS) return launch_tmq_self<2, 4, 8, 4, true, SELF_MASS>(p, st);
-    return launch_tmq_self<2, 4, 8, 4, true, SELF_NONE>(p, st);
-}
 }  // namespace wd

@@ -21,52 +21,36 @@ enum { OB_C = 0, OB_T, OB_Z, OB_Y, OB_X, OB_SA };  // then OB_SB, OB_ITEM0, OB_I
 // C = complex element type: double2 (FP64) or float2 (the FP32 variant, wd_f32.cu).  Sub-objects are padded to 128
 // bytes, the alignment TMA needs for a shared-memory destination (only the 8-byte X link face is not a multiple already).
 constexpr uint32_t al128(uint32_t x) { return (x + 127u) & ~127u; }
-// G = right-hand sides per work item (the "quad" kernel tmq_*: G = 4).  One compute thread per (site, right-hand side);
-// a warp holds 32 / G consecutive sites of the tile for all G right-hand sides, lane = r * (32 / G) + site, so that the
-// links and S of a site — the same for every right-hand side — are one shared-memory wavefront per LDS.128 instead of
-// four, and come from L2 / HBM once per G right-hand sides.
-// BLK (with G > 1): the spinors are in the BLOCKED multi-RHS device layout (WD_OPT_RHS_BLOCK, wd.h) — double2
-// [unit][12][Vs][G], the G right-hand sides of a unit interleaved per site.  A psi box then lands in shared memory as
-// [component][site][r]; with lane = site * G + r a warp reads 512 consecutive bytes per psi component (four conflict-free
-// wavefronts), and the links and S — one address per group of G adjacent lanes — cost two wavefronts per LDS.128 instead of
-// four (measured: the shared-memory pipe merges quarter-warps only when their banks are disjoint, so lane = r * SPW + site
-// on the plain layout pays four).
-template <int BZ_, int BY_, int BX_, int SELF_, int UC_ = 9, class C_ = cd, int G_ = 1, bool BLK_ = false> struct Plan {
+template <int BZ_, int BY_, int BX_, int SELF_, int UC_ = 9, class C_ = cd> struct Plan {
     typedef C_ C;
     static constexpr int BZ = BZ_, BY = BY_, BX = BX_, SELF = SELF_, UC = UC_;
-    static constexpr int G = G_;            // right-hand sides per work item
-    static constexpr bool BLK = BLK_;
-    static constexpr int RBK = BLK ? G : 1;  // right-hand sides interleaved per site in the spinor fields
-    static_assert(!BLK || G > 1, "blocked layout needs G > 1");
-    static constexpr int N = BZ * BY * BX;  // sites per tile
-    static constexpr int NC = N * G;        // compute threads
-    static constexpr int NW = NC / 32;      // compute warps
-    // + the producer: one warp; with 8 compute warps (G > 1) a whole warpgroup, so that setmaxnreg can hand its registers
-    // to the compute warpgroups (a ninth warp alone would cap everyone at 168 registers: three warps on one scheduler)
-    static constexpr bool PRODUCER_WG = (NC == 256);
-    static constexpr int NTHREADS = NC + (PRODUCER_WG ? 128 : 32);
-    static constexpr int PC = 12 * G;       // spinor components per box: the G right-hand sides of a unit are contiguous
+    static constexpr int G = 1;             // right-hand sides per work item
+    static constexpr bool BLK = false;      // plain multi-RHS layout only (the quad kernels of wd_tmq.cu read the blocked one)
+    static constexpr int RBK = 1;
+    static constexpr int N = BZ * BY * BX;  // sites per tile = compute threads
+    static constexpr int NW = N / 32;       // compute warps
+    static constexpr int NTHREADS = N + 32; // + the producer warp
     static constexpr uint32_t E = sizeof(C);                        // bytes per element
     // A TMA box must be a multiple of 16 bytes wide: the X faces of 8-byte elements are fetched two sites wide (the
     // neighbour column and the one beyond it), of which the consumers read one.
     static constexpr int XW = (E == 8) ? 2 : 1;
 
     static constexpr int FZ = BY * BX, FY = BZ * BX, FX = BZ * BY * XW;  // sites stored per face
-    static constexpr uint32_t SZ_C = PC * N * E, SZ_U = UC * N * E, SZ_S = 18 * N * E;
+    static constexpr uint32_t SZ_C = 12 * N * E, SZ_U = UC * N * E, SZ_S = 18 * N * E;
     static constexpr uint32_t OFF_C = 0;
     static constexpr uint32_t OFF_T = OFF_C + SZ_C;
     static constexpr uint32_t OFF_Z = OFF_T + SZ_U;
-    static constexpr uint32_t OFF_ZUF = OFF_Z + SZ_U, OFF_ZLO = OFF_ZUF + al128(UC * FZ * E), OFF_ZHI = OFF_ZLO + PC * FZ * E;
-    static constexpr uint32_t SZ_Z = SZ_U + (UC + 2 * PC) * FZ * E;  // bytes the TMA delivers
-    static constexpr uint32_t SP_Z = SZ_U + al128(UC * FZ * E) + 2 * PC * FZ * E;  // bytes it occupies
+    static constexpr uint32_t OFF_ZUF = OFF_Z + SZ_U, OFF_ZLO = OFF_ZUF + al128(UC * FZ * E), OFF_ZHI = OFF_ZLO + 12 * FZ * E;
+    static constexpr uint32_t SZ_Z = SZ_U + (UC + 24) * FZ * E;  // bytes the TMA delivers
+    static constexpr uint32_t SP_Z = SZ_U + al128(UC * FZ * E) + 24 * FZ * E;  // bytes it occupies
     static constexpr uint32_t OFF_Y = OFF_Z + SP_Z;
-    static constexpr uint32_t OFF_YUF = OFF_Y + SZ_U, OFF_YLO = OFF_YUF + al128(UC * FY * E), OFF_YHI = OFF_YLO + PC * FY * E;
-    static constexpr uint32_t SZ_Y = SZ_U + (UC + 2 * PC) * FY * E;  // bytes the TMA delivers
-    static constexpr uint32_t SP_Y = SZ_U + al128(UC * FY * E) + 2 * PC * FY * E;  // bytes it occupies
+    static constexpr uint32_t OFF_YUF = OFF_Y + SZ_U, OFF_YLO = OFF_YUF + al128(UC * FY * E), OFF_YHI = OFF_YLO + 12 * FY * E;
+    static constexpr uint32_t SZ_Y = SZ_U + (UC + 24) * FY * E;  // bytes the TMA delivers
+    static constexpr uint32_t SP_Y = SZ_U + al128(UC * FY * E) + 24 * FY * E;  // bytes it occupies
     static constexpr uint32_t OFF_X = OFF_Y + SP_Y;
-    static constexpr uint32_t OFF_XUF = OFF_X + SZ_U, OFF_XLO = OFF_XUF + al128(UC * FX * E), OFF_XHI = OFF_XLO + PC * FX * E;
-    static constexpr uint32_t SZ_X = SZ_U + (UC + 2 * PC) * FX * E;  // bytes the TMA delivers
-    static constexpr uint32_t SP_X = SZ_U + al128(UC * FX * E) + 2 * PC * FX * E;  // bytes it occupies
+    static constexpr uint32_t OFF_XUF = OFF_X + SZ_U, OFF_XLO = OFF_XUF + al128(UC * FX * E), OFF_XHI = OFF_XLO + 12 * FX * E;
+    static constexpr uint32_t SZ_X = SZ_U + (UC + 24) * FX * E;  // bytes the TMA delivers
+    static constexpr uint32_t SP_X = SZ_U + al128(UC * FX * E) + 24 * FX * E;  // bytes it occupies
     static constexpr uint32_t OFF_SA = OFF_X + SP_X;
     static constexpr uint32_t OFF_SB = OFF_SA + SZ_S;
     static constexpr uint32_t OFF_BAR = (SELF == SELF_CLOVER) ? OFF_SB + SZ_S : OFF_SA;
@@ -81,7 +65,7 @@ template <int BZ_, int BY_, int BX_, int SELF_, int UC_ = 9, class C_ = cd, int 
     // persistent CTAs per SM: two (8 compute warps) where two plans plus the 1 KB the system reserves per CTA fit the
     // 228 KB of an SM — the plans of 8-byte elements without S buffers
     static constexpr int CTAS_PER_SM = (2 * (SMEM + 1024) <= 233472) ? 2 : 1;
-    static_assert(NC % 32 == 0 && 32 % G == 0 && (12 * FZ * E) % 128 == 0 && (12 * FY * E) % 128 == 0 && (12 * FX * E) % 128 == 0 && SZ_U % 128 == 0,
+    static_assert(N % 32 == 0 && (12 * FZ * E) % 128 == 0 && (12 * FY * E) % 128 == 0 && (12 * FX * E) % 128 == 0 && SZ_U % 128 == 0,
                   "tile faces must keep 128-byte alignment");
     static_assert(SMEM <= 232448, "shared-memory plan exceeds 227 KB");
 };
@@ -116,19 +100,15 @@ __device__ __forceinline__ void producer(const TmaMaps &maps, const TmaParams &p
         if (item < 0) break;
         const Item it = decode_item<P>(prm, item);
         const int cx = 2 * it.x0, y0 = it.y0, z0 = it.z0;  // dim-0 coordinates count real numbers
-        // spinor boxes: first component of this unit, dim-0 coordinates (2 * RBK reals per site)
-        const int pc = P::BLK ? 12 * (it.rhs0 / P::G) : 12 * it.rhs0;
-        constexpr int RBK = P::RBK;
-        const int cxp = RBK * cx;
+        const int pc = 12 * it.rhs0;                       // first component of this right-hand side
         const int zlo = (z0 == 0) ? Z - 1 : z0 - 1, zhi = (z0 + BZ == Z) ? 0 : z0 + BZ;
         const int ylo = (y0 == 0) ? Y - 1 : y0 - 1, yhi = (y0 + BY == Y) ? 0 : y0 + BY;
         const int cxlo = 2 * ((it.x0 == 0) ? X - P::XW : it.x0 - P::XW), cxhi = 2 * ((it.x0 + BX == X) ? 0 : it.x0 + BX);
-        const int cxplo = RBK * cxlo, cxphi = RBK * cxhi;
         int t = (it.t0 == 0) ? T - 1 : it.t0 - 1;
         // prologue: psi(t0-1), only to seed the carried half-spinor
         mbar_wait(bar_empty + 8 * OB_C, (nC & 1) ^ 1);
         mbar_arrive_expect_tx(bar_full + 8 * OB_C, P::SZ_C);
-        tma_load_5d_hint(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cxp, y0, z0, t, pc, pol_p);
+        tma_load_5d_hint(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cx, y0, z0, t, pc, pol_p);
         nC++;
         for (int j = 1; j <= prm.tchunk + 1; j++) {
             const int tprev = t;
@@ -145,31 +125,31 @@ __device__ __forceinline__ void producer(const TmaMaps &maps, const TmaParams &p
                 mbar_arrive_expect_tx(bar_full + 8 * OB_Z, P::SZ_Z);
                 tma_load_5d_hint(sbase + P::OFF_Z, &maps.u_c, bar_full + 8 * OB_Z, cx, y0, z0, t, P::UC, pol_u);
                 tma_load_5d_hint(sbase + P::OFF_ZUF, &maps.u_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, P::UC, pol_u);
-                tma_load_5d_hint(sbase + P::OFF_ZLO, &maps.psi_z, bar_full + 8 * OB_Z, cxp, y0, zlo, t, pc, pol_p);
-                tma_load_5d_hint(sbase + P::OFF_ZHI, &maps.psi_z, bar_full + 8 * OB_Z, cxp, y0, zhi, t, pc, pol_p);
+                tma_load_5d_hint(sbase + P::OFF_ZLO, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zlo, t, pc, pol_p);
+                tma_load_5d_hint(sbase + P::OFF_ZHI, &maps.psi_z, bar_full + 8 * OB_Z, cx, y0, zhi, t, pc, pol_p);
                 if (!Y_LAST) {
                     mbar_wait(bar_empty + 8 * OB_Y, pe);
                     mbar_arrive_expect_tx(bar_full + 8 * OB_Y, P::SZ_Y);
                     tma_load_5d_hint(sbase + P::OFF_Y, &maps.u_c, bar_full + 8 * OB_Y, cx, y0, z0, t, 2 * P::UC, pol_u);
                     tma_load_5d_hint(sbase + P::OFF_YUF, &maps.u_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, 2 * P::UC, pol_u);
-                    tma_load_5d_hint(sbase + P::OFF_YLO, &maps.psi_y, bar_full + 8 * OB_Y, cxp, ylo, z0, t, pc, pol_p);
-                    tma_load_5d_hint(sbase + P::OFF_YHI, &maps.psi_y, bar_full + 8 * OB_Y, cxp, yhi, z0, t, pc, pol_p);
+                    tma_load_5d_hint(sbase + P::OFF_YLO, &maps.psi_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, pc, pol_p);
+                    tma_load_5d_hint(sbase + P::OFF_YHI, &maps.psi_y, bar_full + 8 * OB_Y, cx, yhi, z0, t, pc, pol_p);
                 }
                 mbar_wait(bar_empty + 8 * OB_X, pe);
                 mbar_arrive_expect_tx(bar_full + 8 * OB_X, P::SZ_X);
                 tma_load_5d_hint(sbase + P::OFF_X, &maps.u_c, bar_full + 8 * OB_X, cx, y0, z0, t, 3 * P::UC, pol_u);
                 tma_load_5d_hint(sbase + P::OFF_XUF, &maps.u_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, 3 * P::UC, pol_u);
-                tma_load_5d_hint(sbase + P::OFF_XLO, &maps.psi_x, bar_full + 8 * OB_X, cxplo, y0, z0, t, pc, pol_p);
-                tma_load_5d_hint(sbase + P::OFF_XHI, &maps.psi_x, bar_full + 8 * OB_X, cxphi, y0, z0, t, pc, pol_p);
+                tma_load_5d_hint(sbase + P::OFF_XLO, &maps.psi_x, bar_full + 8 * OB_X, cxlo, y0, z0, t, pc, pol_p);
+                tma_load_5d_hint(sbase + P::OFF_XHI, &maps.psi_x, bar_full + 8 * OB_X, cxhi, y0, z0, t, pc, pol_p);
             }
             // C object: psi(t).  Its buffer is released after the X phase of the previous step, so it
             // has only the S phases to land.  (Warming L2 one step ahead with a TMA prefetch was
             // measured to cost 20 % at 64^4 — flag 8, profiles/r1b — so it is off.)
             mbar_wait(bar_empty + 8 * OB_C, (nC & 1) ^ 1);
             mbar_arrive_expect_tx(bar_full + 8 * OB_C, P::SZ_C);
-            tma_load_5d_hint(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cxp, y0, z0, t, pc, pol_p);
+            tma_load_5d_hint(sbase + P::OFF_C, &maps.psi_c, bar_full + 8 * OB_C, cx, y0, z0, t, pc, pol_p);
             nC++;
-            if (full && WD_FLAG(prm, 8)) tma_prefetch_5d(&maps.psi_c, cxp, y0, z0, (t + 1 == T) ? 0 : t + 1, pc);
+            if (full && WD_FLAG(prm, 8)) tma_prefetch_5d(&maps.psi_c, cx, y0, z0, (t + 1 == T) ? 0 : t + 1, pc);
             if (full && CLOVER) {
                 const uint32_t pe = (nF & 1) ^ 1;
                 mbar_wait(bar_empty + 8 * OB_SA, pe);
@@ -187,8 +167,8 @@ __device__ __forceinline__ void producer(const TmaMaps &maps, const TmaParams &p
                 mbar_arrive_expect_tx(bar_full + 8 * OB_Y, P::SZ_Y);
                 tma_load_5d_hint(sbase + P::OFF_Y, &maps.u_c, bar_full + 8 * OB_Y, cx, y0, z0, t, 2 * P::UC, pol_u);
                 tma_load_5d_hint(sbase + P::OFF_YUF, &maps.u_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, 2 * P::UC, pol_u);
-                tma_load_5d_hint(sbase + P::OFF_YLO, &maps.psi_y, bar_full + 8 * OB_Y, cxp, ylo, z0, t, pc, pol_p);
-                tma_load_5d_hint(sbase + P::OFF_YHI, &maps.psi_y, bar_full + 8 * OB_Y, cxp, yhi, z0, t, pc, pol_p);
+                tma_load_5d_hint(sbase + P::OFF_YLO, &maps.psi_y, bar_full + 8 * OB_Y, cx, ylo, z0, t, pc, pol_p);
+                tma_load_5d_hint(sbase + P::OFF_YHI, &maps.psi_y, bar_full + 8 * OB_Y, cx, yhi, z0, t, pc, pol_p);
             }
             if (full) nF++;
         }
