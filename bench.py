@@ -45,8 +45,9 @@ def parse_args():
     ap.add_argument("--nrhs", type=int, default=0, help="override the number of right-hand sides")
     ap.add_argument("--kernel", type=str, default="", help="kernel geometry name (default automatic)")
     ap.add_argument("--variant", type=int, default=0, help="0 fused, 1 unfused")
-    ap.add_argument("--rhs-block", type=int, default=1, choices=[1, 4],
-                    help="device layout of multi-RHS spinors (WD_OPT_RHS_BLOCK): 1 plain [nrhs][12][Vs], 4 blocked [unit][12][Vs][4]")
+    ap.add_argument("--rhs-block", type=int, default=0, choices=[0, 1, 4],
+                    help="device layout of multi-RHS spinors (WD_OPT_RHS_BLOCK): 1 plain [nrhs][12][Vs], 4 blocked [unit][12][Vs][4]; "
+                         "0 (default) = blocked when the workload has at least four right-hand sides and the 2x4x8 tile divides the lattice")
     ap.add_argument("--tchunk", type=int, default=0)
     ap.add_argument("--zgroup", type=int, default=0)
     ap.add_argument("--no-e2e", action="store_true")
@@ -410,6 +411,9 @@ def run_ours(args):
     wd.wd_set_stream(h, stream.cuda_stream)
     wd.wd_set_option(h, wd.WD_OPT_DEVICE_PACK, 1)
     wd.wd_set_option(h, wd.WD_OPT_VARIANT, args.variant)
+    if args.rhs_block == 0:  # cfg 5 ("multi-tuple layout"): the blocked layout where it exists
+        fits = dims[1] % 2 == 0 and dims[2] % 4 == 0 and dims[3] % 8 == 0
+        args.rhs_block = 4 if (nrhs >= 4 and fits and args.variant == 0 and not args.kernel) else 1
     if args.rhs_block != 1:
         wd.wd_set_option(h, wd.WD_OPT_RHS_BLOCK, args.rhs_block)
     if args.kernel:

@@ -410,36 +410,49 @@ def test_cfg4_full_size_whole_lattice(torch, capsys):
 
 
 def test_cfg5_full_size_multi_rhs_whole_lattice(torch, capsys):
-    """48^3 x 96 Wilson-clover with 12 right-hand sides in ONE wd_apply (the launch configuration bench.py --config 5
-    times: automatic kernel, S built on the device), EVERY right-hand side compared with the oracle on EVERY site.
-    The host streams one right-hand side at a time through the oracle."""
+    """48^3 x 96 Wilson-clover with 12 right-hand sides in ONE wd_apply (the launch configurations bench.py --config 5
+    times: S built on the device; the blocked multi-RHS layout with its kernel, and the plain layout with the automatic
+    kernel), EVERY right-hand side compared with the oracle on EVERY site.  The host streams one unit of four right-hand
+    sides at a time through the oracle."""
     cfg = wdinputs.CONFIGS[5]
-    full = _require_memory(torch, 30, 80, "cfg 5 (48^3 x 96, 12 RHS)")
+    full = _require_memory(torch, 40, 100, "cfg 5 (48^3 x 96, 12 RHS)")
     dims, nrhs = (cfg["dims"], cfg["nrhs"]) if full else ((24, 16, 16, 48), 5)
     V = wdinputs.volume(dims)
     U = wdinputs.config_gauge(cfg, dims)
+    units = [list(range(u, min(u + 4, nrhs))) for u in range(0, nrhs, 4)]
     with Op(torch, dims, cfg["m0"], cfg["csw"], U, build_clover=True, device_pack=1) as op:
-        kname = wd.wd_kernel_name(wd.wd_kernel_for(op.h, nrhs))
         Vs = wd.wd_component_stride(op.h)
-        din, dout = op.dev_spinor(nrhs), op.dev_spinor(nrhs)
-        dout.fill_(float("nan"))
-        for r in range(nrhs):  # one RHS at a time: generate, pack into its slot
-            wd.wd_pack_spinor(op.h, din[r * 24 * Vs:(r + 1) * 24 * Vs], wdinputs.spinor(dims, cfg["spinor_seed"] + r), 1)
-        wd.wd_apply(op.h, dout, din, nrhs)
-        wd.wd_synchronize(op.h)
+        outs, knames = {}, {}
+        for layout in (1, 4):
+            wd.wd_set_option(op.h, wd.WD_OPT_RHS_BLOCK, layout)
+            knames[layout] = wd.wd_kernel_name(wd.wd_kernel_for(op.h, nrhs))
+            din, dout = op.dev_spinor(nrhs), op.dev_spinor(nrhs)
+            dout.fill_(float("nan"))
+            for rs in units:  # one unit at a time: generate, pack into its slots (a unit is contiguous in both layouts)
+                psi_u = np.concatenate([wdinputs.spinor(dims, cfg["spinor_seed"] + r) for r in rs])
+                wd.wd_pack_spinor(op.h, din[rs[0] * 24 * Vs:], psi_u, len(rs))
+            wd.wd_apply(op.h, dout, din, nrhs)
+            wd.wd_synchronize(op.h)
+            outs[layout] = dout
+            del din
+        assert knames[4].startswith("tmqb_")
         C = oracle.build_clover(dims, cfg["m0"], cfg["csw"], U)
-        out_r = np.empty((1, V, 12, 2))
-        errs, worsts = [], []
-        for r in range(nrhs):
-            psi_r = wdinputs.spinor(dims, cfg["spinor_seed"] + r)
-            ref = oracle.apply(dims, cfg["m0"], U, C, psi_r)
-            wd.wd_unpack_spinor(op.h, out_r, dout[r * 24 * Vs:(r + 1) * 24 * Vs], 1)
-            assert np.isfinite(out_r).all(), r
-            errs.append(rel_l2(out_r, ref))
-            worsts.append(float(np.abs(out_r - ref).max() / np.abs(ref).max()))
-    _report(capsys, f"lattice {'x'.join(map(str, dims))} x{nrhs} kernel {kname}: {nrhs} x {V} sites compared, "
-                    f"max rel_l2 {max(errs):.3e}, worst component {max(worsts):.3e}" + ("" if full else "  (WD_TEST_SMALL)"))
-    assert max(errs) <= TOL and max(worsts) <= 1e-13
+        errs, worsts = {1: [], 4: []}, {1: [], 4: []}
+        for rs in units:
+            ref = np.concatenate([oracle.apply(dims, cfg["m0"], U, C, wdinputs.spinor(dims, cfg["spinor_seed"] + r)) for r in rs])
+            out_u = np.empty_like(ref)
+            for layout in (1, 4):
+                wd.wd_set_option(op.h, wd.WD_OPT_RHS_BLOCK, layout)
+                wd.wd_unpack_spinor(op.h, out_u, outs[layout][rs[0] * 24 * Vs:], len(rs))
+                assert np.isfinite(out_u).all(), (layout, rs)
+                for k in range(len(rs)):
+                    errs[layout].append(rel_l2(out_u[k], ref[k]))
+                    worsts[layout].append(float(np.abs(out_u[k] - ref[k]).max() / np.abs(ref[k]).max()))
+    for layout in (1, 4):
+        _report(capsys, f"lattice {'x'.join(map(str, dims))} x{nrhs} kernel {knames[layout]} ({'blocked' if layout == 4 else 'plain'} layout): "
+                        f"{nrhs} x {V} sites compared, max rel_l2 {max(errs[layout]):.3e}, worst component {max(worsts[layout]):.3e}"
+                        + ("" if full else "  (WD_TEST_SMALL)"))
+        assert len(errs[layout]) == nrhs and max(errs[layout]) <= TOL and max(worsts[layout]) <= 1e-13
 
 
 # ---------------------------------------------------------------- two-row gauge storage (opt-in)
