@@ -530,6 +530,28 @@ def run_ours(args):
                        "h2d_bytes_per_step": V * nrhs * 192, "d2h_bytes_per_step": V * nrhs * 192,
                        "ms_per_step": ms, "steps": args.e2e_steps,
                        "api": "wd_apply_host (pinned host buffers, canonical layout)"}
+        # the bound of that path: one right-hand side up and one down AT THE SAME TIME, plain copies on two streams
+        one = hin.numel() // nrhs
+        dbuf = [torch.empty(one, dtype=torch.float64, device="cuda") for _ in range(2)]
+        s_up, s_dn = torch.cuda.Stream(), torch.cuda.Stream()
+        best = 1e30
+        for _ in range(3):
+            torch.cuda.synchronize()
+            e0.record(stream)
+            s_up.wait_stream(stream)
+            s_dn.wait_stream(stream)
+            with torch.cuda.stream(s_up):
+                dbuf[0].copy_(hin.view(-1)[:one], non_blocking=True)
+            with torch.cuda.stream(s_dn):
+                hout.view(-1)[:one].copy_(dbuf[1], non_blocking=True)
+            stream.wait_stream(s_up)
+            stream.wait_stream(s_dn)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        line["e2e"]["pcie_bidirectional_ms_per_rhs"] = best
+        line["e2e"]["frac_of_pcie_bound"] = best * nrhs / ms
+        del dbuf
         del hin, hout
     # ---- the FP32 variant on the same workload: 768 instead of 1536 algorithmic B/site
     if args.f32 and rank == 0:

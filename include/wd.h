@@ -203,7 +203,8 @@ int wd_apply_f32(wd_handle *h, void *dev_out, const void *dev_in, int nrhs);
 int wd_apply_host(wd_handle *h, double *host_out, const double *host_in, int nrhs);
 
 /* Size in bytes of a device spinor buffer for nrhs right-hand sides (0 on error).  It is
- * nrhs * 12 * wd_component_stride(h) * 16 — a little more than nrhs * V * 192, see below. */
+ * nrhs * 12 * wd_component_stride(h) * 16 — a little more than nrhs * V * 192, see below; with
+ * WD_OPT_RHS_BLOCK = 4, nrhs is rounded up to a multiple of four first. */
 size_t wd_spinor_bytes(const wd_handle *h, int nrhs);
 
 /* Component stride Vs of the device layout, in complex elements (0 on error): component c of
@@ -212,6 +213,10 @@ size_t wd_spinor_bytes(const wd_handle *h, int nrhs);
  * padding keeps the components of one site from aliasing onto one L2 slice when V*16 B is a
  * power of two. */
 long long wd_component_stride(const wd_handle *h);
+/* Blocked multi-RHS layout (WD_OPT_RHS_BLOCK = 4): right-hand sides 4u .. 4u+3 form unit u; element (c, site i, r) of
+ * unit u is at complex element ((12*u + c) * Vs + i) * 4 + r of the buffer.  A unit occupies the same 4 * 12 * Vs elements
+ * as four right-hand sides of the plain layout, so "right-hand sides 4u onwards" start at the same offset in both.  The
+ * slots of a last, partial unit are zero-filled by wd_pack_spinor and hold unspecified values after wd_apply. */
 
 /* HOST canonical [nrhs][V][12][2]  <->  DEVICE layout.  Synchronous. */
 int wd_pack_spinor(wd_handle *h, void *dev_dst, const double *host_src, int nrhs);
