@@ -122,6 +122,7 @@ int wd_create(wd_handle **out, int T, int Z, int Y, int X, double m0, double csw
     h->dstage_bytes = 0;
     h->work_in = h->work_out = nullptr;
     h->dstage_out = nullptr;
+    h->dstage_out_bytes = 0;
     h->s_up = h->s_dn = nullptr;
     h->pipe_ready = false;
     h->launches = 0;
@@ -708,7 +709,20 @@ static int apply_host_pipelined(wd_handle *h, double *host_out, const double *ho
         WD_CUDA(h, cudaEventCreateWithFlags(&h->ev_misc[1], cudaEventDisableTiming));
         h->pipe_ready = true;
     }
-    if (!h->dstage_out) WD_CUDA(h, cudaMalloc((void **)&h->dstage_out, per * sizeof(double2)));
+    // canonical-layout staging on the device: rings of kStageRing chunks (stream order makes a slot's next use wait for
+    // its previous one: upload and transpose of a chunk are both on s_up, transpose and download both on s_dn)
+    const int kStageRing = 4;
+    int rc0 = ensure_dstage(h, (size_t)kStageRing * cbytes);
+    if (rc0) return rc0;
+    if (h->dstage_out_bytes < (size_t)kStageRing * cbytes) {
+        if (h->dstage_out) cudaFree(h->dstage_out);
+        h->dstage_out = nullptr;
+        h->dstage_out_bytes = 0;
+        WD_CUDA(h, cudaMalloc((void **)&h->dstage_out, (size_t)kStageRing * cbytes));
+        h->dstage_out_bytes = (size_t)kStageRing * cbytes;
+    }
+    const size_t celems = (size_t)Vc * kSpinorComps;  // elements per chunk in canonical layout
+    long long nup = 0, ndn = 0;                       // chunks uploaded / downloaded so far (ring positions)
     const KernelInfo &kinfo = kernel_info(wd_kernel_in_use(h));
     KParams p;
     const long saved_tchunk = h->tchunk_opt;
@@ -735,8 +749,9 @@ static int apply_host_pipelined(wd_handle *h, double *host_out, const double *ho
         for (int i = 0; i < C; i++) {  // upload order: last chunk first (chunk 0 needs slice T-1), then 0, 1, ...
             const int k = (i == 0) ? C - 1 : i - 1;
             const long long s0 = (long long)k * Vc;
-            WD_CUDA(h, cudaMemcpyAsync(h->dstage + s0 * kSpinorComps, src + s0 * kSpinorComps, cbytes, cudaMemcpyHostToDevice, h->s_up));
-            WD_CUDA(h, launch_aos_to_soa(h->work_in + s0, h->dstage + s0 * kSpinorComps, Vc, h->Vs, kSpinorComps, h->s_up));
+            double2 *stage = h->dstage + (size_t)(nup++ % kStageRing) * celems;
+            WD_CUDA(h, cudaMemcpyAsync(stage, src + s0 * kSpinorComps, cbytes, cudaMemcpyHostToDevice, h->s_up));
+            WD_CUDA(h, launch_aos_to_soa(h->work_in + s0, stage, Vc, h->Vs, kSpinorComps, h->s_up));
             WD_CUDA(h, cudaEventRecord(h->ev_up[k], h->s_up));
             h->launches++;
         }
@@ -750,10 +765,11 @@ static int apply_host_pipelined(wd_handle *h, double *host_out, const double *ho
             WD_CUDA(h, cudaEventRecord(h->ev_cmp[k], h->stream));
             const long long s0 = (long long)k * Vc;
             WD_CUDA(h, cudaStreamWaitEvent(h->s_dn, h->ev_cmp[k], 0));
-            WD_CUDA(h, launch_soa_to_aos(h->dstage_out + s0 * kSpinorComps, h->work_out + s0, Vc, h->Vs, kSpinorComps, h->s_dn));
+            double2 *stage = h->dstage_out + (size_t)(ndn++ % kStageRing) * celems;
+            WD_CUDA(h, launch_soa_to_aos(stage, h->work_out + s0, Vc, h->Vs, kSpinorComps, h->s_dn));
             h->launches++;
             if (k == C - 1) WD_CUDA(h, cudaEventRecord(h->ev_misc[1], h->s_dn));
-            WD_CUDA(h, cudaMemcpyAsync(dst + s0 * kSpinorComps, h->dstage_out + s0 * kSpinorComps, cbytes, cudaMemcpyDeviceToHost, h->s_dn));
+            WD_CUDA(h, cudaMemcpyAsync(dst + s0 * kSpinorComps, stage, cbytes, cudaMemcpyDeviceToHost, h->s_dn));
         }
     }
     WD_CUDA(h, cudaStreamSynchronize(h->s_dn));
@@ -773,9 +789,7 @@ int wd_apply_host(wd_handle *h, double *host_out, const double *host_in, int nrh
     const size_t dbytes = wd_spinor_bytes(h, 1);
     if (!h->work_in) WD_CUDA(h, cudaMalloc((void **)&h->work_in, dbytes));
     if (!h->work_out) WD_CUDA(h, cudaMalloc((void **)&h->work_out, dbytes));
-    int rc = ensure_dstage(h, bytes);
-    if (rc) return rc;
-    // pipelined path (WD_OPT_HOST_PIPELINE, default on): a TMA kernel, fused variant, and T splits into 4..16 equal chunks
+    // pipelined path (WD_OPT_HOST_PIPELINE, default on): a TMA kernel, fused variant, and T splits into 4..32 equal chunks
     const KernelInfo &kinfo = kernel_info(wd_kernel_in_use(h));
     int C = 0;
     if (kinfo.multi_rhs && h->variant == 0 && h->host_pipeline) {
@@ -783,6 +797,8 @@ int wd_apply_host(wd_handle *h, double *host_out, const double *host_in, int nrh
             if (h->n[0] % c == 0) C = c;
     }
     if (C) return apply_host_pipelined(h, host_out, host_in, nrhs, C);
+    int rc = ensure_dstage(h, bytes);  // the serial path stages a whole right-hand side
+    if (rc) return rc;
     for (int r = 0; r < nrhs; r++) {
         WD_CUDA(h, cudaMemcpyAsync(h->dstage, (const double2 *)host_in + r * per, bytes, cudaMemcpyHostToDevice, h->stream));
         WD_CUDA(h, launch_aos_to_soa(h->work_in, h->dstage, h->V, h->Vs, kSpinorComps, h->stream));

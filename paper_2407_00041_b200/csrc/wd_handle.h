@@ -37,7 +37,8 @@ struct wd_handle {
     double2 *dstage;
     size_t dstage_bytes;
     double2 *work_in, *work_out;  // wd_apply_host
-    double2 *dstage_out;          // pipelined wd_apply_host: AoS staging of the result
+    double2 *dstage_out;          // pipelined wd_apply_host: AoS staging of the result (a ring of chunks)
+    size_t dstage_out_bytes;
     cudaStream_t s_up, s_dn;      // its upload and download streams
     cudaEvent_t ev_up[kMaxPipeChunks], ev_cmp[kMaxPipeChunks], ev_misc[2];
     bool pipe_ready;
