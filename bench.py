@@ -597,6 +597,21 @@ def run_ours(args):
                 ms = g0.elapsed_time(g1)
                 res[label] = {"ms_per_cycle": ms / max(cyc, 1), "cycles": cyc, "launches": wd.wd_launch_count(h) - l0,
                               "applies": cyc * (M + 1) + 1, "resid_drop": float(hist[cyc] / hist[0]) if hist[0] else None}
+            # the same cycles with single-precision Krylov vectors and operator applications (wd_gmres_mixed)
+            wd.wd_enable_f32(h)
+            hist = np.zeros(cycles_max + 1)
+            for rep in range(2):
+                outs[0].zero_()
+                g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                l0 = wd.wd_launch_count(h)
+                g0.record(gs)
+                cyc = wd.wd_gmres_mixed(h, outs[0], ins[0], M, cycles_max, 1e-30, hist)
+                g1.record(gs)
+                gs.synchronize()
+            ms = g0.elapsed_time(g1)
+            res["mixed"] = {"ms_per_cycle": ms / max(cyc, 1), "cycles": cyc, "launches": wd.wd_launch_count(h) - l0,
+                            "resid_drop": float(hist[cyc] / hist[0]) if hist[0] else None,
+                            "what": "Krylov vectors and M applications per cycle in FP32, residual and solution in FP64"}
         apply_ms = ms_per_step * (M + 1)
         line["gmres"] = {"m": M, **res, "apply_ms_per_cycle": apply_ms,
                          "operator_share_of_cycle": apply_ms / res["graph"]["ms_per_cycle"],

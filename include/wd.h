@@ -138,6 +138,18 @@ int wd_apply(wd_handle *h, void *dev_out, const void *dev_in, int nrhs);
 int wd_gmres(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_cycles, double tol, int *cycles_done,
              double *host_resid);
 
+/* The same algorithm in MIXED precision (SURVEY.md section 8(f)3 + 8(f)4; the paper's operator exists in both precisions,
+ * PAPER.md:642): the Krylov vectors v_1 .. v_{m+1}, the operator applications w = D v_j (wd_apply_f32) and the
+ * orthogonalisation run on single-precision vectors; the residual r = b - D x of line 4 (wd_apply), the solution x,
+ * every inner product, norm and entry of H are double.  Each restart cycle is thus a defect correction: it solves
+ * D e = r approximately in single precision and adds e to the double-precision x, so the iteration converges to the
+ * solution of the DOUBLE-precision system as long as a cycle reduces the residual at all (single precision limits the
+ * reduction per cycle to about 1e-6, not the final accuracy).  Arguments, termination and errors as wd_gmres; dev_x
+ * and dev_b are FP64 device spinors.  Needs wd_enable_f32 (WD_ESTATE otherwise).  The library owns (m + 2)
+ * single-precision work spinors and one double-precision one.  Cycles are launched kernel by kernel (no graph). */
+int wd_gmres_mixed(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_cycles, double tol, int *cycles_done,
+                   double *host_resid);
+
 /* The Hessenberg matrix of the LAST restart cycle of the last wd_gmres call as the Arnoldi process produced it:
  * host_H (HOST, may be NULL): (m+1) * m complex numbers, column-major with leading dimension m + 1
  * (host_H[2 * (i + (m+1) * j)] = Re h_{i+1,j+1}); *kdim (may be NULL) = Krylov dimension of that cycle (m unless the

@@ -43,6 +43,7 @@ SIGNATURES = {
     "wd_dd_pack": (_i, [_vp, _vp, _i, _i, _vp, _vp]),
     "wd_dd_exterior": (_i, [_vp, _vp, _i, _i, _vp, _vp]),
     "wd_gmres": (_i, [_vp, _vp, _vp, _i, _i, _d, ctypes.POINTER(_i), _vp]),
+    "wd_gmres_mixed": (_i, [_vp, _vp, _vp, _i, _i, _d, ctypes.POINTER(_i), _vp]),
     "wd_gmres_last_hessenberg": (_i, [_vp, _vp, ctypes.POINTER(_i), ctypes.POINTER(_d)]),
     "wd_spinor_bytes": (_sz, [_vp, _i]),
     "wd_component_stride": (ctypes.c_longlong, [_vp]),
@@ -189,6 +190,13 @@ def wd_gmres(h, dev_x, dev_b, m: int, max_cycles: int, tol: float, host_resid=No
     """Returns the number of restart cycles done; host_resid: float64 array of max_cycles + 1 entries, or None."""
     n = _i(0)
     _check(h, lib().wd_gmres(h, _ptr(dev_x), _ptr(dev_b), m, max_cycles, tol, ctypes.byref(n), _ptr(host_resid)))
+    return n.value
+
+
+def wd_gmres_mixed(h, dev_x, dev_b, m: int, max_cycles: int, tol: float, host_resid=None) -> int:
+    """wd_gmres with single-precision Krylov vectors and operator applications (needs wd_enable_f32)."""
+    n = _i(0)
+    _check(h, lib().wd_gmres_mixed(h, _ptr(dev_x), _ptr(dev_b), m, max_cycles, tol, ctypes.byref(n), _ptr(host_resid)))
     return n.value
 
 

@@ -47,6 +47,9 @@ struct Scalars {          // device-resident scalars of the iteration
 struct wd_gmres_state {
     int m;
     double2 *basis;       // (m + 2) device spinors: v_0 .. v_m, w
+    int m32;
+    float2 *basis32;      // wd_gmres_mixed: (m + 2) single-precision device spinors v_0 .. v_m, w
+    double2 *r64;         // wd_gmres_mixed: the FP64 residual b - A x
     Scalars *sc;          // device
     double2 *partials;    // per-block partial sums of the reductions
     int nbx;              // blocks per component
@@ -120,9 +123,17 @@ enum { OP_DOT = 0, OP_AXPY_DOT, OP_AXPY_NORM, OP_RESID_NORM };
 //   OP_AXPY_DOT   : w -= h_in * vp;  h_out = <w, vn>
 //   OP_AXPY_NORM  : w -= h_in * vp;  h_out = ||w|| (real), inv = 1 / h_out, breakdown rule
 //   OP_RESID_NORM : w = bvec - w;    beta = ||w||, inv = 1 / beta; starts a cycle (active = 1, kdim = m)
-template <int OP>
-__global__ void __launch_bounds__(kThreads) k_fused(double2 *__restrict__ w, const double2 *__restrict__ vp,
-                                                    const double2 *__restrict__ vn, long long V, long long Vs, Scalars *sc,
+// CV = element type of the vectors: double2, or float2 (wd_gmres_mixed: single-precision Krylov vectors; every product and
+// sum is still formed in double, only the stored vector is rounded)
+template <class CV> __device__ __forceinline__ double2 ldv(const CV *p, long long i) {
+    const CV v = p[i];
+    return make_double2((double)v.x, (double)v.y);
+}
+template <class CV> __device__ __forceinline__ void stv(CV *p, long long i, double2 v) { p[i] = mk<CV>((R<CV>)v.x, (R<CV>)v.y); }
+
+template <int OP, class CV>
+__global__ void __launch_bounds__(kThreads) k_fused(CV *__restrict__ w, const CV *__restrict__ vp,
+                                                    const CV *__restrict__ vn, long long V, long long Vs, Scalars *sc,
                                                     int h_in, int h_out, int j, int m, double tol10) {
     if (OP != OP_RESID_NORM && !sc->active) return;
     const long long base = (long long)blockIdx.y * Vs;
@@ -130,19 +141,20 @@ __global__ void __launch_bounds__(kThreads) k_fused(double2 *__restrict__ w, con
     if (OP == OP_AXPY_DOT || OP == OP_AXPY_NORM) h = sc->H[h_in];
     double2 acc = make_double2(0.0, 0.0);
     for (long long i = (long long)blockIdx.x * kThreads + threadIdx.x; i < V; i += (long long)gridDim.x * kThreads) {
-        double2 x = w[base + i];
+        double2 x = ldv(w, base + i);
         if (OP == OP_AXPY_DOT || OP == OP_AXPY_NORM) {
-            const double2 p = vp[base + i];
+            const double2 p = ldv(vp, base + i);
             x.x = fma(-h.x, p.x, fma(h.y, p.y, x.x));
             x.y = fma(-h.x, p.y, fma(-h.y, p.x, x.y));
-            w[base + i] = x;
+            stv(w, base + i, x);
+            if (sizeof(CV) == sizeof(float2)) x = ldv(w, base + i);  // the inner product sees the vector as stored
         } else if (OP == OP_RESID_NORM) {
-            const double2 b = vp[base + i];
+            const double2 b = ldv(vp, base + i);
             x = make_double2(b.x - x.x, b.y - x.y);
-            w[base + i] = x;
+            stv(w, base + i, x);
         }
         if (OP == OP_DOT || OP == OP_AXPY_DOT) {  // conj(vn) * x
-            const double2 q = vn[base + i];
+            const double2 q = ldv(vn, base + i);
             acc.x = fma(q.x, x.x, fma(q.y, x.y, acc.x));
             acc.y = fma(q.x, x.y, fma(-q.y, x.x, acc.y));
         } else {
@@ -171,14 +183,15 @@ __global__ void __launch_bounds__(kThreads) k_fused(double2 *__restrict__ w, con
 }
 
 // dst = inv * src (v_1 = r / beta, v_{j+1} = w / h_{j+1,j}); `always`: also when the Arnoldi loop has ended
-__global__ void __launch_bounds__(kThreads) k_scale(double2 *__restrict__ dst, const double2 *__restrict__ src, long long V,
+template <class CD, class CS>
+__global__ void __launch_bounds__(kThreads) k_scale(CD *__restrict__ dst, const CS *__restrict__ src, long long V,
                                                     long long Vs, const Scalars *sc, int always) {
     if (!always && !sc->active) return;
     const double s = sc->inv;
     const long long base = (long long)blockIdx.y * Vs;
     for (long long i = (long long)blockIdx.x * kThreads + threadIdx.x; i < V; i += (long long)gridDim.x * kThreads) {
-        const double2 x = src[base + i];
-        dst[base + i] = make_double2(s * x.x, s * x.y);
+        const double2 x = ldv(src, base + i);
+        stv(dst, base + i, make_double2(s * x.x, s * x.y));
     }
 }
 
@@ -231,14 +244,15 @@ __global__ void k_lsq(Scalars *sc, int m) {
 }
 
 // x += sum_i y_i v_i over the kdim basis vectors of this cycle, one pass (line 19)
-__global__ void __launch_bounds__(kThreads) k_update(double2 *__restrict__ x, const double2 *__restrict__ basis, long long V,
+template <class CV>
+__global__ void __launch_bounds__(kThreads) k_update(double2 *__restrict__ x, const CV *__restrict__ basis, long long V,
                                                      long long Vs, long long vec_stride, const Scalars *sc) {
     const int kd = sc->kdim;
     const long long base = (long long)blockIdx.y * Vs;
     for (long long i = (long long)blockIdx.x * kThreads + threadIdx.x; i < V; i += (long long)gridDim.x * kThreads) {
         double2 s = x[base + i];
         for (int k = 0; k < kd; k++) {
-            const double2 yk = sc->y[k], v = basis[(long long)k * vec_stride + base + i];
+            const double2 yk = sc->y[k], v = ldv(basis, (long long)k * vec_stride + base + i);
             s.x = fma(yk.x, v.x, fma(-yk.y, v.y, s.x));
             s.y = fma(yk.x, v.y, fma(yk.y, v.x, s.y));
         }
@@ -251,14 +265,36 @@ __global__ void k_copy_h(double2 *dst, const Scalars *sc, int n) {
     for (int k = threadIdx.x; k < n; k += blockDim.x) dst[k] = sc->H[k];
 }
 
-int ensure_workspace(wd_handle *h, int m) {
+// the state and the device scalars; then the Krylov vectors of the precision asked for
+int ensure_workspace(wd_handle *h, int m, bool mixed) {
     wd_gmres_state *g = h->gmres;
-    if (g && g->m >= m) return WD_OK;
-    gmres_free(h);
+    const size_t vec = (size_t)h->Vs * kSpinorComps * sizeof(double2);
+    if (g) {
+        if (!mixed && g->m < m) {
+            if (g->graph) cudaGraphExecDestroy(g->graph);
+            g->graph = nullptr;
+            if (g->basis) cudaFree(g->basis);
+            g->basis = nullptr;
+            g->m = 0;
+            WD_CUDA(h, cudaMalloc((void **)&g->basis, (size_t)(m + 2) * vec));
+            g->m = m;
+        }
+        if (mixed && g->m32 < m) {
+            if (g->basis32) cudaFree(g->basis32);
+            g->basis32 = nullptr;
+            g->m32 = 0;
+            WD_CUDA(h, cudaMalloc((void **)&g->basis32, (size_t)(m + 2) * vec / 2));
+            g->m32 = m;
+        }
+        if (mixed && !g->r64) WD_CUDA(h, cudaMalloc((void **)&g->r64, vec));
+        return WD_OK;
+    }
     g = new (std::nothrow) wd_gmres_state();
     if (!g) return fail(h, WD_ENOMEM, "wd_gmres: out of host memory");
-    g->m = m;
+    g->m = g->m32 = 0;
     g->basis = nullptr;
+    g->basis32 = nullptr;
+    g->r64 = nullptr;
     g->sc = nullptr;
     g->graph = nullptr;
     g->gx = g->gb = nullptr;
@@ -270,65 +306,77 @@ int ensure_workspace(wd_handle *h, int m) {
     if (nbx < 1) nbx = 1;
     g->nbx = (int)nbx;
     h->gmres = g;
-    const size_t vec = (size_t)h->Vs * kSpinorComps * sizeof(double2);
-    WD_CUDA(h, cudaMalloc((void **)&g->basis, (size_t)(m + 2) * vec));
     // the scalars, followed by the per-block partial sums and room for a copy of H
     const size_t extra = (size_t)g->nbx * 12 * sizeof(double2) + (size_t)(kMaxM + 1) * kMaxM * sizeof(double2);
     WD_CUDA(h, cudaMalloc((void **)&g->sc, sizeof(Scalars) + extra));
     WD_CUDA(h, cudaMemsetAsync(g->sc, 0, sizeof(Scalars) + extra, h->stream));
-    return WD_OK;
+    return ensure_workspace(h, m, mixed);
 }
 
-struct Cycle {  // issues the launches of the algorithm on the handle's stream; counts them
+// Issues the launches of the algorithm on the handle's stream and counts them.  CV = double2: wd_gmres.  CV = float2:
+// wd_gmres_mixed — Krylov vectors, operator applications and orthogonalisation in single precision, the residual
+// b - A x, the solution x and every scalar in double.
+template <class CV> struct Cycle {
+    static constexpr bool MIXED = sizeof(CV) == sizeof(float2);
     wd_handle *h;
     wd_gmres_state *g;
     int m;
     double tol10;
     long launches = 0;
-    double2 *vec(int k) const { return g->basis + (size_t)k * h->Vs * kSpinorComps; }
-    double2 *w() const { return vec(m + 1); }
+    CV *base() const {
+        if constexpr (MIXED) return g->basis32;
+        else return g->basis;
+    }
+    CV *vec(int k) const { return base() + (size_t)k * h->Vs * kSpinorComps; }
+    CV *w() const { return vec(m + 1); }
+    double2 *r() const {  // the FP64 residual vector: w itself, or its own buffer when w is single precision
+        if constexpr (MIXED) return g->r64;
+        else return w();
+    }
     dim3 grid() const { return dim3((unsigned)g->nbx, 12); }
-    template <int OP> int fused(double2 *wv, const double2 *vp, const double2 *vn, int h_in, int h_out, int j) {
-        k_fused<OP><<<grid(), kThreads, 0, h->stream>>>(wv, vp, vn, h->V, h->Vs, g->sc, h_in, h_out, j, m, tol10);
+    template <int OP, class T> int fused(T *wv, const T *vp, const T *vn, int h_in, int h_out, int j) {
+        k_fused<OP, T><<<grid(), kThreads, 0, h->stream>>>(wv, vp, vn, h->V, h->Vs, g->sc, h_in, h_out, j, m, tol10);
         WD_CUDA(h, cudaGetLastError());
         launches++;
         return WD_OK;
     }
-    int apply(double2 *out, const double2 *in) {
+    template <class T> int apply(T *out, const T *in) {
         const long before = h->launches;
-        const int rc = wd_apply(h, out, in, 1);
+        int rc;
+        if constexpr (sizeof(T) == sizeof(float2)) rc = wd_apply_f32(h, out, in, 1);
+        else rc = wd_apply(h, out, in, 1);
         launches += h->launches - before;
         h->launches = before;  // the caller adds `launches` once per executed cycle (graph replays included)
         return rc;
     }
-    // w = b - A x;  beta = ||w||
+    // r = b - A x;  beta = ||r||   (always FP64)
     int residual(const double2 *x, const double2 *b) {
-        int rc = apply(w(), x);
+        int rc = apply(r(), x);
         if (rc) return rc;
-        return fused<OP_RESID_NORM>(w(), b, nullptr, 0, 0, 0);
+        return fused<OP_RESID_NORM, double2>(r(), b, nullptr, 0, 0, 0);
     }
     // lines 6-20 of Algorithm 1, then line 4-5 for the new x
     int body(double2 *x, const double2 *b) {
         const int ld = m + 1;
         int rc;
-        k_scale<<<grid(), kThreads, 0, h->stream>>>(vec(0), w(), h->V, h->Vs, g->sc, 1);  // v_1 = r / beta
+        k_scale<CV, double2><<<grid(), kThreads, 0, h->stream>>>(vec(0), r(), h->V, h->Vs, g->sc, 1);  // v_1 = r / beta
         WD_CUDA(h, cudaGetLastError());
         launches++;
         WD_CUDA(h, cudaMemsetAsync(g->sc->H, 0, sizeof(double2) * (size_t)ld * m, h->stream));
         for (int j = 0; j < m; j++) {
-            if ((rc = apply(w(), vec(j)))) return rc;                                      // w = A v_j
-            if ((rc = fused<OP_DOT>(w(), nullptr, vec(0), 0, 0 + ld * j, j))) return rc;   // h_1j
-            for (int i = 1; i <= j; i++)                                                   // w -= h_{i-1,j} v_{i-1}; h_ij
-                if ((rc = fused<OP_AXPY_DOT>(w(), vec(i - 1), vec(i), (i - 1) + ld * j, i + ld * j, j))) return rc;
-            if ((rc = fused<OP_AXPY_NORM>(w(), vec(j), nullptr, j + ld * j, (j + 1) + ld * j, j))) return rc;
-            k_scale<<<grid(), kThreads, 0, h->stream>>>(vec(j + 1), w(), h->V, h->Vs, g->sc, 0);  // v_{j+1}
+            if ((rc = apply(w(), (const CV *)vec(j)))) return rc;                                        // w = A v_j
+            if ((rc = fused<OP_DOT, CV>(w(), nullptr, vec(0), 0, 0 + ld * j, j))) return rc;            // h_1j
+            for (int i = 1; i <= j; i++)                                                                // w -= h_{i-1,j} v_{i-1}; h_ij
+                if ((rc = fused<OP_AXPY_DOT, CV>(w(), vec(i - 1), vec(i), (i - 1) + ld * j, i + ld * j, j))) return rc;
+            if ((rc = fused<OP_AXPY_NORM, CV>(w(), vec(j), nullptr, j + ld * j, (j + 1) + ld * j, j))) return rc;
+            k_scale<CV, CV><<<grid(), kThreads, 0, h->stream>>>(vec(j + 1), w(), h->V, h->Vs, g->sc, 0);  // v_{j+1}
             WD_CUDA(h, cudaGetLastError());
             launches++;
         }
         double2 *Hcopy = reinterpret_cast<double2 *>(g->sc + 1) + (size_t)g->nbx * 12;
         k_copy_h<<<1, 256, 0, h->stream>>>(Hcopy, g->sc, ld * m);
         k_lsq<<<1, 32, 0, h->stream>>>(g->sc, m);
-        k_update<<<grid(), kThreads, 0, h->stream>>>(x, g->basis, h->V, h->Vs, h->Vs * kSpinorComps, g->sc);
+        k_update<CV><<<grid(), kThreads, 0, h->stream>>>(x, base(), h->V, h->Vs, h->Vs * kSpinorComps, g->sc);
         WD_CUDA(h, cudaGetLastError());
         launches += 3;
         return residual(x, b);
@@ -342,6 +390,8 @@ void wd::gmres_free(wd_handle *h) {
     if (!g) return;
     if (g->graph) cudaGraphExecDestroy(g->graph);
     if (g->basis) cudaFree(g->basis);
+    if (g->basis32) cudaFree(g->basis32);
+    if (g->r64) cudaFree(g->r64);
     if (g->sc) cudaFree(g->sc);
     delete g;
     h->gmres = nullptr;
@@ -358,10 +408,10 @@ int wd_gmres(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_cycles
     if (((size_t)dev_x | (size_t)dev_b) & 15) return fail(h, WD_EINVAL, "wd_gmres: spinor buffers must be 16-byte aligned");
     if (dev_x == dev_b) return fail(h, WD_EINVAL, "wd_gmres: x overlaps b");
     if (!h->has_gauge) return fail(h, WD_ESTATE, "wd_gmres: no gauge field loaded");
-    int rc = ensure_workspace(h, m);
+    int rc = ensure_workspace(h, m, false);
     if (rc) return rc;
     wd_gmres_state *g = h->gmres;
-    Cycle cyc{h, g, m, tol / 10.0};
+    Cycle<double2> cyc{h, g, m, tol / 10.0};
     double2 *x = (double2 *)dev_x;
     const double2 *b = (const double2 *)dev_b;
     struct { double beta, inv, lsq; int active, kdim, kdim_done; unsigned int ticket; } hs;
@@ -409,6 +459,48 @@ int wd_gmres(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_cycles
             if ((rc = cyc.body(x, b))) return rc;
             h->launches += cyc.launches;
         }
+        if ((rc = read_scalars())) return rc;
+        k++;
+        if (host_resid) host_resid[k] = hs.beta;
+    }
+    if (cycles_done) *cycles_done = k;
+    g->last_m = m;
+    g->last_kdim = (k > 0) ? hs.kdim_done : 0;
+    return WD_OK;
+}
+
+int wd_gmres_mixed(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_cycles, double tol, int *cycles_done,
+                   double *host_resid) {
+    WD_ENTER(h);
+    WD_PLAIN_ONLY(h, "wd_gmres_mixed");
+    if (!dev_x || !dev_b || m < 1 || m > kMaxM || max_cycles < 0 || !(tol > 0.0))
+        return fail(h, WD_EINVAL, "wd_gmres_mixed: null pointer, m outside 1..64, max_cycles < 0 or tol <= 0");
+    if (((size_t)dev_x | (size_t)dev_b) & 15) return fail(h, WD_EINVAL, "wd_gmres_mixed: spinor buffers must be 16-byte aligned");
+    if (dev_x == dev_b) return fail(h, WD_EINVAL, "wd_gmres_mixed: x overlaps b");
+    if (!h->has_gauge) return fail(h, WD_ESTATE, "wd_gmres_mixed: no gauge field loaded");
+    if (!h->f32) return fail(h, WD_ESTATE, "wd_gmres_mixed: call wd_enable_f32 after loading the fields (single-precision copies of U and S)");
+    int rc = ensure_workspace(h, m, true);
+    if (rc) return rc;
+    wd_gmres_state *g = h->gmres;
+    Cycle<float2> cyc{h, g, m, tol / 10.0};
+    double2 *x = (double2 *)dev_x;
+    const double2 *b = (const double2 *)dev_b;
+    struct { double beta, inv, lsq; int active, kdim, kdim_done; unsigned int ticket; } hs;
+    auto read_scalars = [&]() -> int {
+        WD_CUDA(h, cudaMemcpyAsync(&hs, &g->sc->beta, sizeof(hs), cudaMemcpyDeviceToHost, h->stream));
+        WD_CUDA(h, cudaStreamSynchronize(h->stream));
+        return WD_OK;
+    };
+    if ((rc = cyc.residual(x, b))) return rc;
+    h->launches += cyc.launches;
+    if ((rc = read_scalars())) return rc;
+    const double r0 = hs.beta;
+    if (host_resid) host_resid[0] = r0;
+    int k = 0;
+    while (!(hs.beta < tol * r0) && k < max_cycles && hs.beta != 0.0) {
+        cyc.launches = 0;
+        if ((rc = cyc.body(x, b))) return rc;
+        h->launches += cyc.launches;
         if ((rc = read_scalars())) return rc;
         k++;
         if (host_resid) host_resid[k] = hs.beta;

@@ -143,3 +143,44 @@ def test_cfg3_size_gmres_residual_against_the_oracle_operator(torch):
     r = b - oracle.apply(dims, m0, U, C, x)
     rn = float(np.linalg.norm(r.ravel()))
     assert abs(rn - hist[-1]) <= 1e-9 * hist[0] and rn < hist[0]
+
+
+def test_mixed_precision_gmres_solves_the_fp64_system(torch):
+    """wd_gmres_mixed: Krylov vectors and operator applications in single precision, residual and solution in double.
+    An iteration in two precisions has no step-by-step oracle; what it must deliver is checked instead, with the
+    ORACLE's FP64 operator: the returned x satisfies ||b - D x|| < tol ||b - D x_0|| in DOUBLE precision (tol = 1e-10,
+    four orders below what single precision resolves), the norm the device reports is that true residual, the history
+    decreases, the cycle count stays within a few cycles of the FP64 solver's, and x agrees with the FP64 oracle
+    solution to the accuracy the residuals allow."""
+    cfg = wdinputs.CONFIGS[2]
+    dims, m0, csw, m = cfg["dims"], 0.0, cfg["csw"], 8
+    U = wdinputs.config_gauge(cfg)
+    C = oracle.build_clover(dims, m0, csw, U)
+    b = wdinputs.spinor(dims, cfg["spinor_seed"])[0]
+    x0 = 0.1 * wdinputs.spinor(dims, 2102)[0]
+    tol, max_cycles = 1e-10, 60
+    A = wilson_operator(dims, m0, U, C)
+    xo, info = gmres(A, c(b), x0=c(x0), m=m, tol=tol, max_cycles=max_cycles)
+    with Op(torch, dims, m0, csw, U, build_clover=True) as op:
+        db, dx = op.dev_spinor(), op.dev_spinor()
+        wd.wd_pack_spinor(op.h, db, np.ascontiguousarray(b[None]), 1)
+        wd.wd_pack_spinor(op.h, dx, np.ascontiguousarray(x0[None]), 1)
+        with pytest.raises(wd.WDError) as e:  # the single-precision copies of U and S do not exist yet
+            wd.wd_gmres_mixed(op.h, dx, db, m, max_cycles, tol)
+        assert e.value.code == wd.WD_ESTATE
+        wd.wd_enable_f32(op.h)
+        hist = np.full(max_cycles + 1, np.nan)
+        cycles = wd.wd_gmres_mixed(op.h, dx, db, m, max_cycles, tol, hist)
+        x = np.empty((1,) + b.shape)
+        wd.wd_unpack_spinor(op.h, x, dx, 1)
+        hist = hist[: cycles + 1]
+        # the FP64 solver on the same handle afterwards: the two share scalars and must not disturb each other
+        x64, hist64, cycles64, *_ = device_gmres(torch, op, b, x0, m, max_cycles, tol)
+    assert info["cycles"] <= cycles <= info["cycles"] + 3 and cycles64 == info["cycles"]
+    assert hist[-1] < tol * hist[0] and (np.diff(hist) < 0).all()
+    r = c(b) - A(c(x[0]))
+    rn = float(np.linalg.norm(r.ravel()))
+    assert abs(rn - hist[-1]) <= 1e-9 * hist[0] and rn <= 1.01 * tol * hist[0]
+    assert abs(hist[0] - info["resid"][0]) <= 1e-12 * hist[0]
+    assert rel_l2(x[0], f(xo)) <= 1e-7     # both residuals are 1e-10 ||r_0||: the solutions differ by cond(D) times that
+    assert rel_l2(x64, f(xo)) <= TOL_X
