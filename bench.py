@@ -666,6 +666,9 @@ def run_ours(args):
             roofline["fp64_peak_clocks"] = fs.summary()
             roofline["fp64_peak_how"] = "best of 5, 1024 threads x 8 chains per SM, register-only DFMA"
             roofline["frac_of_fp64_peak"] = (value / 1e3) / fp64
+            if nrhs > 1:  # the measurement behind the lane mapping of the quad kernels
+                roofline["lds128_cycles_per_warp_instruction"] = {
+                    name: round(benchlib.wdb_measure_lds(k), 3) for k, name in enumerate(benchlib.LDS_PATTERNS)}
         except Exception as exc:  # the ceilings are context, never the reason a bench line is lost
             roofline["ceilings_error"] = repr(exc)
 

@@ -238,9 +238,10 @@ int wd_unpack_spinor(wd_handle *h, double *host_dst, const void *dev_src, int nr
  * layout of one field — exactly the bytes wd_load_gauge / wd_load_clover / wd_pack_spinor place
  * in device memory — and its inverse.  field: WD_FIELD_SPINOR (one RHS, canonical 12 complex per
  * site), WD_FIELD_GAUGE (36), WD_FIELD_CLOVER (canonical 42 complex -> 36 packed slots; unpacking
- * returns zero imaginary parts on the diagonal).  HOST pointers; nsites = V.
- * wd_layout_bytes: size of the packed image (0 on error). */
-enum { WD_FIELD_SPINOR = 0, WD_FIELD_GAUGE = 1, WD_FIELD_CLOVER = 2 };
+ * returns zero imaginary parts on the diagonal), WD_FIELD_SPINOR_BLOCK4 (one unit of the blocked multi-RHS layout:
+ * canonical [4][nsites][12] -> [12][nsites][4], the image wd_pack_spinor writes with WD_OPT_RHS_BLOCK = 4).  HOST
+ * pointers; nsites = V.  wd_layout_bytes: size of the packed image (0 on error). */
+enum { WD_FIELD_SPINOR = 0, WD_FIELD_GAUGE = 1, WD_FIELD_CLOVER = 2, WD_FIELD_SPINOR_BLOCK4 = 3 };
 size_t wd_layout_bytes(int field, long long nsites);
 int wd_layout_pack_host(int field, long long nsites, const double *canonical, double *packed);
 int wd_layout_unpack_host(int field, long long nsites, const double *packed, double *canonical);

@@ -25,6 +25,18 @@ int wdb_measure_fp64(int threads_per_sm, int ilp, int one_cta_per_sm, int distin
  * *gbs = bytes moved (reads + writes) / time. */
 int wdb_measure_stream(int mode, size_t bytes, int reps, double *gbs);
 
+/* What an LDS.128 costs for a given lane-to-address pattern: the measurement behind the lane mapping of the quad
+ * multi-RHS kernels (csrc/wd_tmq.cu).  One CTA of 256 threads per SM issues back-to-back
+ * LDS.128; *cycles = SM cycles per warp instruction (the pipe moves 128 B per cycle, so 4.0 = 512 distinct bytes).
+ * pattern 0: every lane its own 16 bytes (512 B per warp)
+ *         1: lane & 7   — the same 128 bytes in each quarter-warp   (lane = r * 8 + site: links of the plain layout)
+ *         2: lane >> 2  — one address per four ADJACENT lanes        (lane = site * 4 + r: links of the blocked layout)
+ *         3: all lanes one address
+ *         4: four 128-byte-aligned segments, segment = lane & 3       (psi with lane = site * 4 + r on the plain layout)
+ *         5: four segments, segment = lane >> 3                       (psi with lane = r * 8 + site)
+ *         6: lane >> 1  — one address per pair of adjacent lanes */
+int wdb_measure_lds(int pattern, double *cycles);
+
 #ifdef __cplusplus
 }
 #endif

@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libwd.so")
 
 WD_OK, WD_EINVAL, WD_ENOMEM, WD_ESTATE, WD_ECUDA = 0, -1, -2, -3, -4
-WD_FIELD_SPINOR, WD_FIELD_GAUGE, WD_FIELD_CLOVER = 0, 1, 2
+WD_FIELD_SPINOR, WD_FIELD_GAUGE, WD_FIELD_CLOVER, WD_FIELD_SPINOR_BLOCK4 = 0, 1, 2, 3
 WD_OPT_VARIANT, WD_OPT_KERNEL, WD_OPT_TCHUNK, WD_OPT_ZGROUP, WD_OPT_DEVICE_PACK, WD_OPT_HOST_PIPELINE = 1, 2, 3, 4, 5, 6
 WD_OPT_GMRES_GRAPH, WD_OPT_GAUGE_ROWS, WD_OPT_F32_KERNEL, WD_OPT_RHS_BLOCK = 7, 8, 9, 10
 

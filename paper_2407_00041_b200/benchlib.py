@@ -13,6 +13,7 @@ _i, _d, _sz = ctypes.c_int, ctypes.c_double, ctypes.c_size_t
 SIGNATURES = {
     "wdb_measure_fp64": (_i, [_i, _i, _i, _i, ctypes.POINTER(_d), ctypes.POINTER(_d)]),
     "wdb_measure_stream": (_i, [_i, _sz, _i, ctypes.POINTER(_d)]),
+    "wdb_measure_lds": (_i, [_i, ctypes.POINTER(_d)]),
 }
 _lib = None
 
@@ -47,3 +48,16 @@ def wdb_measure_stream(mode: int, nbytes: int, reps: int = 5) -> float:
     if rc != 0:
         raise RuntimeError(f"wdb_measure_stream failed: {rc}")
     return g.value
+
+
+LDS_PATTERNS = ["512 distinct bytes", "lane & 7 (same 128 B in each quarter-warp)", "lane >> 2 (one address per 4 adjacent lanes)",
+                "one address", "4 aligned segments by lane & 3", "4 aligned segments by lane >> 3", "lane >> 1 (pairs)"]
+
+
+def wdb_measure_lds(pattern: int) -> float:
+    """SM cycles per warp-level LDS.128 for a lane-to-address pattern (index into LDS_PATTERNS)."""
+    c = _d(0.0)
+    rc = lib().wdb_measure_lds(pattern, ctypes.byref(c))
+    if rc != 0:
+        raise RuntimeError(f"wdb_measure_lds failed: {rc}")
+    return c.value

@@ -164,3 +164,73 @@ extern "C" int wdb_measure_stream(int mode, size_t bytes, int reps, double *gbs)
     *gbs = moved / (best * 1e-3) / 1e9;
     return WD_OK;
 }
+
+// ---------------------------------------------------------------- LDS.128 lane-pattern probe (wd_bench.h)
+namespace {
+__device__ __forceinline__ void lds128(double &a, double &b, unsigned addr) {
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(a), "=d"(b) : "r"(addr) : "memory");
+}
+__global__ void k_lds_pattern(double *out, long long *cyc, int iters, int pattern) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int tid = threadIdx.x, lane = tid & 31;
+    for (int i = tid; i < 98304 / 8; i += blockDim.x) reinterpret_cast<double *>(smem)[i] = i;
+    __syncthreads();
+    const unsigned base = (unsigned)__cvta_generic_to_shared(smem);
+    unsigned off = 0;
+    switch (pattern) {
+    case 0: off = lane * 16; break;
+    case 1: off = (lane & 7) * 16; break;
+    case 2: off = (lane >> 2) * 16; break;
+    case 3: off = 0; break;
+    case 4: off = (lane & 3) * 12288 + (lane >> 2) * 16; break;
+    case 5: off = (lane >> 3) * 12288 + (lane & 7) * 16; break;
+    default: off = (lane >> 1) * 16; break;
+    }
+    double s0 = 0, s1 = 0;
+    const long long t0 = clock64();
+    for (int it = 0; it < iters; it++) {
+        const unsigned a = base + off + ((it & 3) * 512);
+#pragma unroll
+        for (int j = 0; j < 16; j++) {  // sixteen different addresses: nothing for the compiler to merge
+            double x, y;
+            lds128(x, y, a + j * 2048);
+            s0 += x;
+            s1 += y;
+        }
+    }
+    const long long t1 = clock64();
+    if (tid == 0) cyc[blockIdx.x] = t1 - t0;
+    out[blockIdx.x * blockDim.x + tid] = s0 + s1;
+}
+}  // namespace
+
+extern "C" int wdb_measure_lds(int pattern, double *cycles) {
+    if (!cycles || pattern < 0 || pattern > 6) return WD_EINVAL;
+    int dev = 0, nsm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return WD_ECUDA;
+    if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm < 1) return WD_ECUDA;
+    const int threads = 256, iters = 4096, smem = 98304;
+    double *out = nullptr;
+    long long *cyc = nullptr;
+    if (cudaMalloc((void **)&out, (size_t)nsm * threads * sizeof(double)) != cudaSuccess) return WD_ENOMEM;
+    if (cudaMalloc((void **)&cyc, (size_t)nsm * sizeof(long long)) != cudaSuccess) {
+        cudaFree(out);
+        return WD_ENOMEM;
+    }
+    cudaError_t e = cudaFuncSetAttribute(k_lds_pattern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    long long *host = new long long[nsm];
+    for (int rep = 0; rep < 2 && e == cudaSuccess; rep++) {
+        k_lds_pattern<<<nsm, threads, smem>>>(out, cyc, iters, pattern);
+        e = cudaDeviceSynchronize();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(host, cyc, (size_t)nsm * sizeof(long long), cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) {
+        double sum = 0.0;
+        for (int k = 0; k < nsm; k++) sum += (double)host[k];
+        *cycles = sum / nsm / ((double)iters * 16 * (threads / 32));
+    }
+    delete[] host;
+    cudaFree(out);
+    cudaFree(cyc);
+    return (e == cudaSuccess) ? WD_OK : WD_ECUDA;
+}

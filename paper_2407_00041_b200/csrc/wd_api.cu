@@ -339,13 +339,10 @@ static int pack_spinor_blocked(wd_handle *h, double2 *dev, const double2 *host, 
             const long long cnt = (V - i0 < chunk) ? V - i0 : chunk;
             WD_CUDA(h, cudaEventSynchronize(h->pinned_ev[b]));
             double2 *st = h->pinned[b];
-#pragma omp parallel for schedule(static)
-            for (long long j = 0; j < cnt; j++)
-                for (int r = 0; r < B; r++) {
-                    const bool live = u * B + r < nrhs;
-                    const double2 *src = host + (size_t)(u * B + r) * per + (size_t)(i0 + j) * kSpinorComps;
-                    for (int c = 0; c < kSpinorComps; c++) st[((long long)c * cnt + j) * B + r] = live ? src[c] : make_double2(0.0, 0.0);
-                }
+            const double2 *src[8];
+            const int nlive = (nrhs - u * B < B) ? (int)(nrhs - u * B) : (int)B;
+            for (int r = 0; r < B; r++) src[r] = host + (size_t)(u * B + (r < nlive ? r : 0)) * per;
+            host_pack_spinor_blocked(st, src, (int)B, nlive, i0, cnt);
             WD_CUDA(h, cudaMemcpy2DAsync(dev + u * uper + i0 * B, (size_t)h->Vs * B * sizeof(double2), st, (size_t)cnt * B * sizeof(double2),
                                          (size_t)cnt * B * sizeof(double2), kSpinorComps, cudaMemcpyHostToDevice, h->stream));
             WD_CUDA(h, cudaEventRecord(h->pinned_ev[b], h->stream));
@@ -367,12 +364,10 @@ static int unpack_spinor_blocked(wd_handle *h, double2 *host, const double2 *dev
             WD_CUDA(h, cudaMemcpy2DAsync(st, (size_t)cnt * B * sizeof(double2), dev + u * uper + i0 * B, (size_t)h->Vs * B * sizeof(double2),
                                          (size_t)cnt * B * sizeof(double2), kSpinorComps, cudaMemcpyDeviceToHost, h->stream));
             WD_CUDA(h, cudaStreamSynchronize(h->stream));
-#pragma omp parallel for schedule(static)
-            for (long long j = 0; j < cnt; j++)
-                for (int r = 0; r < B && u * B + r < nrhs; r++) {
-                    double2 *dst = host + (size_t)(u * B + r) * per + (size_t)(i0 + j) * kSpinorComps;
-                    for (int c = 0; c < kSpinorComps; c++) dst[c] = st[((long long)c * cnt + j) * B + r];
-                }
+            double2 *dst[8];
+            const int nlive = (nrhs - u * B < B) ? (int)(nrhs - u * B) : (int)B;
+            for (int r = 0; r < B; r++) dst[r] = host + (size_t)(u * B + (r < nlive ? r : 0)) * per;
+            host_unpack_spinor_blocked(dst, st, (int)B, nlive, i0, cnt);
         }
     return WD_OK;
 }
@@ -434,6 +429,7 @@ size_t wd_layout_bytes(int field, long long nsites) {
     case WD_FIELD_SPINOR: return (size_t)nsites * kSpinorComps * sizeof(double2);
     case WD_FIELD_GAUGE: return (size_t)nsites * kGaugeComps * sizeof(double2);
     case WD_FIELD_CLOVER: return (size_t)nsites * kCloverSlots * sizeof(double2);
+    case WD_FIELD_SPINOR_BLOCK4: return (size_t)nsites * kSpinorComps * 4 * sizeof(double2);
     default: return 0;
     }
 }
@@ -444,6 +440,12 @@ int wd_layout_pack_host(int field, long long nsites, const double *canonical, do
     case WD_FIELD_SPINOR: host_pack_aos_to_soa((double2 *)packed, (const double2 *)canonical, 0, nsites, kSpinorComps); return WD_OK;
     case WD_FIELD_GAUGE: host_pack_aos_to_soa((double2 *)packed, (const double2 *)canonical, 0, nsites, kGaugeComps); return WD_OK;
     case WD_FIELD_CLOVER: host_pack_clover((double2 *)packed, (const double2 *)canonical, 0, nsites); return WD_OK;
+    case WD_FIELD_SPINOR_BLOCK4: {
+        const double2 *src[4];
+        for (int r = 0; r < 4; r++) src[r] = (const double2 *)canonical + (size_t)r * nsites * kSpinorComps;
+        host_pack_spinor_blocked((double2 *)packed, src, 4, 4, 0, nsites);
+        return WD_OK;
+    }
     default: return WD_EINVAL;
     }
 }
@@ -454,6 +456,12 @@ int wd_layout_unpack_host(int field, long long nsites, const double *packed, dou
     case WD_FIELD_SPINOR: host_unpack_soa_to_aos((double2 *)canonical, (const double2 *)packed, 0, nsites, kSpinorComps); return WD_OK;
     case WD_FIELD_GAUGE: host_unpack_soa_to_aos((double2 *)canonical, (const double2 *)packed, 0, nsites, kGaugeComps); return WD_OK;
     case WD_FIELD_CLOVER: host_unpack_clover((double2 *)canonical, (const double2 *)packed, 0, nsites); return WD_OK;
+    case WD_FIELD_SPINOR_BLOCK4: {
+        double2 *dst[4];
+        for (int r = 0; r < 4; r++) dst[r] = (double2 *)canonical + (size_t)r * nsites * kSpinorComps;
+        host_unpack_spinor_blocked(dst, (const double2 *)packed, 4, 4, 0, nsites);
+        return WD_OK;
+    }
     default: return WD_EINVAL;
     }
 }

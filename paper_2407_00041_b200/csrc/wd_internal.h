@@ -103,6 +103,10 @@ void host_pack_aos_to_soa(double2 *dst, const double2 *src_aos, long long i0, lo
 void host_unpack_soa_to_aos(double2 *dst_aos, const double2 *src, long long i0, long long cnt, int ncomp);
 void host_pack_clover(double2 *dst, const double2 *src42, long long i0, long long cnt);
 void host_unpack_clover(double2 *dst42, const double2 *src, long long i0, long long cnt);
+// blocked multi-RHS layout, one unit of B right-hand sides: staging [12][cnt][B] <-> canonical spinors src[r] (each
+// [V][12]) rows i0 .. i0+cnt; right-hand sides r >= nlive are written as zeros / not read back
+void host_pack_spinor_blocked(double2 *dst, const double2 *const *src, int B, int nlive, long long i0, long long cnt);
+void host_unpack_spinor_blocked(double2 *const *dst, const double2 *src, int B, int nlive, long long i0, long long cnt);
 
 // two-row copy of the gauge field (wd_pack.cu): U2[mu][k] = U[mu][k], k = 0..5
 cudaError_t launch_compress_gauge(double2 *U2, const double2 *U, long long V, long long Vs, cudaStream_t st);

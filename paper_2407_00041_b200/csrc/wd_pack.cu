@@ -59,6 +59,21 @@ void host_unpack_clover(double2 *dst42, const double2 *src, long long i0, long l
     }
 }
 
+void host_pack_spinor_blocked(double2 *dst, const double2 *const *src, int B, int nlive, long long i0, long long cnt) {
+#pragma omp parallel for schedule(static)
+    for (long long j = 0; j < cnt; j++)
+        for (int r = 0; r < B; r++)
+            for (int c = 0; c < kSpinorComps; c++)
+                dst[((long long)c * cnt + j) * B + r] = (r < nlive) ? src[r][(i0 + j) * kSpinorComps + c] : make_double2(0.0, 0.0);
+}
+
+void host_unpack_spinor_blocked(double2 *const *dst, const double2 *src, int B, int nlive, long long i0, long long cnt) {
+#pragma omp parallel for schedule(static)
+    for (long long j = 0; j < cnt; j++)
+        for (int r = 0; r < nlive; r++)
+            for (int c = 0; c < kSpinorComps; c++) dst[r][(i0 + j) * kSpinorComps + c] = src[((long long)c * cnt + j) * B + r];
+}
+
 // ---------------------------------------------------------------- device side
 // A CTA moves TS sites x ncomp components through shared memory: the AoS side is accessed as one
 // contiguous run of TS*ncomp elements, the SoA side as ncomp runs of TS elements.

@@ -85,6 +85,15 @@ def test_host_packer_is_the_stated_permutation(V):
         back = np.empty_like(a)
         wd.wd_layout_unpack_host(field, V, packed, back)
         assert np.array_equal(back, a)
+    # one unit of the blocked multi-RHS layout (WD_OPT_RHS_BLOCK = 4): [4][V][12] -> [12][V][4]
+    a = rng.normal(size=(4, V, 12, 2))
+    packed = np.empty((12, V, 4, 2))
+    assert wd.wd_layout_bytes(wd.WD_FIELD_SPINOR_BLOCK4, V) == packed.nbytes == 4 * V * 192
+    wd.wd_layout_pack_host(wd.WD_FIELD_SPINOR_BLOCK4, V, a, packed)
+    assert np.array_equal(packed, a.transpose(2, 1, 0, 3))
+    back = np.empty_like(a)
+    wd.wd_layout_unpack_host(wd.WD_FIELD_SPINOR_BLOCK4, V, packed, back)
+    assert np.array_equal(back, a)
     # self-coupling: 42 canonical -> 36 slots, 18 per chirality block (3 real-diagonal pairs, then
     # the block's 15 strict-upper entries), block A first
     C = wdinputs.selfcoupling_random((1, 1, 1, V), 77)
