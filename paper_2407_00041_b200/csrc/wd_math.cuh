@@ -111,6 +111,49 @@ template <int MU, int SIGN, class C> __device__ __forceinline__ void reconstruct
     }
 }
 
+// The same without an accumulator to start from — a sum that begins with 0 + g costs a DADD per real number (0.0 + x is
+// not x in IEEE arithmetic, the compiler keeps it):
+//   i^K b
+template <int K, class C> __device__ __forceinline__ C mul_ik(C b) {
+    constexpr int k = K & 3;
+    if (k == 0) return b;
+    if (k == 1) return mk<C>(-b.y, b.x);
+    if (k == 2) return mk<C>(-b.x, -b.y);
+    return mk<C>(b.y, -b.x);
+}
+//   a + s i^K b, s real: the phase is folded into the sign of s and the choice of operand (no extra instruction)
+template <int K, class C> __device__ __forceinline__ C axpy_ik(C a, R<C> s, C b) {
+    constexpr int k = K & 3;
+    if (k == 0) return mk<C>(fma(s, b.x, a.x), fma(s, b.y, a.y));
+    if (k == 1) return mk<C>(fma(-s, b.y, a.x), fma(s, b.x, a.y));
+    if (k == 2) return mk<C>(fma(-s, b.x, a.x), fma(-s, b.y, a.y));
+    return mk<C>(fma(s, b.y, a.x), fma(-s, b.x, a.y));
+}
+// acc = (I4 + SIGN*gamma_MU)-reconstruction of g   (the first hop of a sum; bit-identical to 0 + reconstruct_add
+// except for the sign of a zero)
+template <int MU, int SIGN, class C> __device__ __forceinline__ void reconstruct_set(C acc[12], const C g[6]) {
+    constexpr int KS = (SIGN < 0) ? 2 : 0;
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        acc[c] = g[c];
+        acc[3 + c] = g[3 + c];
+        acc[6 + c] = mul_ik<Gam<MU, 2>::k + KS>(g[3 * Gam<MU, 2>::col + c]);
+        acc[9 + c] = mul_ik<Gam<MU, 3>::k + KS>(g[3 * Gam<MU, 3>::col + c]);
+    }
+}
+// out = base + s * (I4 + SIGN*gamma_MU)-reconstruction of g, s real   (the last hop of a sum, scaled: out = outp - 1/2 f)
+template <int MU, int SIGN, class C>
+__device__ __forceinline__ void reconstruct_axpy(C out[12], const C base[12], R<C> s, const C g[6]) {
+    constexpr int KS = (SIGN < 0) ? 2 : 0;
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        out[c] = axpy_ik<0>(base[c], s, g[c]);
+        out[3 + c] = axpy_ik<0>(base[3 + c], s, g[3 + c]);
+        out[6 + c] = axpy_ik<Gam<MU, 2>::k + KS>(base[6 + c], s, g[3 * Gam<MU, 2>::col + c]);
+        out[9 + c] = axpy_ik<Gam<MU, 3>::k + KS>(base[9 + c], s, g[3 * Gam<MU, 3>::col + c]);
+    }
+}
+
 // One hopping term: acc += [(I4 + SIGN*gamma_MU) (x) W] psi,  W = U (SIGN = -1, forward
 // neighbour) or U^H (SIGN = +1, backward neighbour)   — eq. 1.13 lines 2 and 3 without the -1/2.
 template <int MU, int SIGN, class C> __device__ __forceinline__ void hop_term(C acc[12], const C psi[12], const C u[9]) {

@@ -189,16 +189,14 @@ __global__ void __launch_bounds__(P::NTHREADS, P::CTAS_PER_SM) k_tma(const __gri
                 load_link<P::UC, C>(u, smem, P::OFF_T + own, NS);
 #pragma unroll
                 for (int c = 0; c < 12; c++) p[c] = lds<C>(smem, P::OFF_C + own + c * NS);
-                if (j > 1) {
-                    C f[12];
-#pragma unroll
-                    for (int c = 0; c < 12; c++) f[c] = mk<C>(0, 0);
-                    if (!((open & 1) && tprev == T - 1)) hop_term<0, -1>(f, p, u);  // (1 - gamma_T) U_T(t-1) psi(t)
+                if (j > 1) {  // out(t-1) = outp - 1/2 (1 - gamma_T) U_T(t-1) psi(t)
+                    C hf[6], gf[6], o[12];
+                    project<0, -1>(hf, p);
+                    su3_mul<false>(gf, u, hf);
+                    reconstruct_axpy<0, -1>(o, outp, ((open & 1) && tprev == T - 1) ? (Real)0 : -half, gf);
                     const long long ip = (long long)tprev * strideT + site0;
 #pragma unroll
-                    for (int c = 0; c < 12; c++)
-                        __stcs(out + (long long)c * V + ip,
-                               mk<C>(fma(-half, f[c].x, outp[c].x), fma(-half, f[c].y, outp[c].y)));
+                    for (int c = 0; c < 12; c++) __stcs(out + (long long)c * V + ip, o[c]);
                 }
                 if (j == prm.tchunk + 1) {  // epilogue step: nothing else to do for slice t
                     release(OB_T);
@@ -209,9 +207,7 @@ __global__ void __launch_bounds__(P::NTHREADS, P::CTAS_PER_SM) k_tma(const __gri
                 }
                 C g[6];
                 su3_mul<true>(g, u, hprev);  // U_T(t-1)^H (1 + gamma_T) psi(t-1)
-#pragma unroll
-                for (int c = 0; c < 12; c++) acc[c] = mk<C>(0, 0);
-                reconstruct_add<0, +1>(acc, g);
+                reconstruct_set<0, +1>(acc, g);
                 project<0, +1>(hprev, p);
                 release(OB_T);
                 nT++;

@@ -398,9 +398,7 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tma(const __grid_constant__ 
                     cd h[6], g[6];
                     project<0, +1>(h, p);
                     su3_mul<true>(g, u, h);
-#pragma unroll
-                    for (int c = 0; c < 12; c++) acc[c] = make_double2(0.0, 0.0);
-                    reconstruct_add<0, +1>(acc, g);
+                    reconstruct_set<0, +1>(acc, g);
                 }
                 release(OB_R + slot);
                 nR++;

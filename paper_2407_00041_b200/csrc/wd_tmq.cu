@@ -305,15 +305,15 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tmq(const __grid_constant__ 
                 load_link<9, C>(u, smem, P::OFF_T + own, NS);
 #pragma unroll
                 for (int c = 0; c < 12; c++) p[c] = lds<C>(smem, P::OFF_C + cb + ownp + c * NSP);
-                if (j > 1) {
-                    C f[12];
-#pragma unroll
-                    for (int c = 0; c < 12; c++) f[c] = mk<C>(0, 0);
-                    if (!((open & 1) && tprev == T - 1)) hop_term<0, -1>(f, p, u);  // (1 - gamma_T) U_T(t-1) psi(t)
+                if (j > 1) {  // out(t-1) = outp - 1/2 (1 - gamma_T) U_T(t-1) psi(t)
+                    C hf[6], gf[6], o[12];
+                    project<0, -1>(hf, p);
+                    su3_mul<false>(gf, u, hf);
+                    reconstruct_axpy<0, -1>(o, outp, ((open & 1) && tprev == T - 1) ? 0.0 : -0.5, gf);
                     const long long ip = (long long)tprev * strideT + site0;
 #pragma unroll
                     for (int c = 0; c < 12; c++)
-                        if (live) __stcs(out + ((long long)c * V + ip) * P::RBK, mk<C>(fma(-0.5, f[c].x, outp[c].x), fma(-0.5, f[c].y, outp[c].y)));
+                        if (live) __stcs(out + ((long long)c * V + ip) * P::RBK, o[c]);
                 }
                 if (j == prm.tchunk + 1) {  // epilogue step: nothing else to do for slice t
                     release(OB_T);
@@ -324,9 +324,7 @@ __global__ void __launch_bounds__(P::NTHREADS, 1) k_tmq(const __grid_constant__ 
                 }
                 C g[6];
                 su3_mul<true>(g, u, hprev);  // U_T(t-1)^H (1 + gamma_T) psi(t-1)
-#pragma unroll
-                for (int c = 0; c < 12; c++) acc[c] = mk<C>(0, 0);
-                reconstruct_add<0, +1>(acc, g);
+                reconstruct_set<0, +1>(acc, g);
                 project<0, +1>(hprev, p);
                 release(OB_T);
                 nT++;
