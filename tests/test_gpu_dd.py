@@ -60,6 +60,25 @@ def test_every_kernel_family_supports_open_boundaries(torch, kernel):
         em.close()
 
 
+def test_quad_kernel_on_sub_lattices_with_several_right_hand_sides(torch):
+    """tmq_2x4x8 (one thread per site and right-hand side) with open boundaries in T, Z and X, five right-hand sides (a full
+    unit of four and a partial one) through pack / exchange / interior / exterior."""
+    gdims, grid, m0, csw, nrhs = (8, 8, 16, 32), (2, 2, 1, 2), -0.4, 1.0, 5
+    U = wdinputs.gauge_exp(gdims, 831, 0.5)
+    psi = wdinputs.spinor(gdims, 832, nrhs=nrhs)
+    C = wdinputs.selfcoupling_random(gdims, 833)
+    ref = oracle.apply(gdims, m0, U, C, psi)
+    em = EmulatedDecomposition(torch, gdims, grid, m0, csw, U, C)
+    try:
+        for op in em.ops:
+            wd.wd_set_option(op.h, wd.WD_OPT_KERNEL, wd.kernel_id("tmq_2x4x8"))
+        out = em.apply(psi, nrhs)
+        for r in range(nrhs):
+            assert rel_l2(out[r], ref[r]) <= TOL, r
+    finally:
+        em.close()
+
+
 def test_local_clover_from_extended_links_and_state_rules(torch):
     """S of a sub-lattice built on the device from the links of the local lattice extended by one site, against the
     oracle's S of the global lattice; wd_build_clover is refused on a decomposed handle."""
