@@ -146,7 +146,7 @@ int wd_gmres(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_cycles
  * solution of the DOUBLE-precision system as long as a cycle reduces the residual at all (single precision limits the
  * reduction per cycle to about 1e-6, not the final accuracy).  Arguments, termination and errors as wd_gmres; dev_x
  * and dev_b are FP64 device spinors.  Needs wd_enable_f32 (WD_ESTATE otherwise).  The library owns (m + 2)
- * single-precision work spinors and one double-precision one.  Cycles are launched kernel by kernel (no graph). */
+ * single-precision work spinors and one double-precision one.  CUDA graph as wd_gmres. */
 int wd_gmres_mixed(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_cycles, double tol, int *cycles_done,
                    double *host_resid);
 

@@ -56,6 +56,7 @@ struct wd_gmres_state {
     cudaGraphExec_t graph;
     const void *gx, *gb;  // what the captured cycle was built for
     int gm;
+    bool gmixed;          // the captured cycle is wd_gmres_mixed's
     double gtol;
     cudaStream_t gstream;
     long graph_launches;  // kernel launches inside one captured cycle
@@ -280,6 +281,8 @@ int ensure_workspace(wd_handle *h, int m, bool mixed) {
             g->m = m;
         }
         if (mixed && g->m32 < m) {
+            if (g->graph) cudaGraphExecDestroy(g->graph);
+            g->graph = nullptr;
             if (g->basis32) cudaFree(g->basis32);
             g->basis32 = nullptr;
             g->m32 = 0;
@@ -298,6 +301,7 @@ int ensure_workspace(wd_handle *h, int m, bool mixed) {
     g->sc = nullptr;
     g->graph = nullptr;
     g->gx = g->gb = nullptr;
+    g->gmixed = false;
     g->graph_launches = 0;
     g->last_m = g->last_kdim = 0;
     long long nbx = (h->V + kThreads * 8 - 1) / (kThreads * 8);  // ~8 elements per thread, at most ~8 blocks per SM
@@ -397,21 +401,26 @@ void wd::gmres_free(wd_handle *h) {
     h->gmres = nullptr;
 }
 
-extern "C" {
+namespace {
 
-int wd_gmres(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_cycles, double tol, int *cycles_done,
-             double *host_resid) {
-    WD_ENTER(h);
-    WD_PLAIN_ONLY(h, "wd_gmres");
+// The restart loop of wd_gmres (CV = double2) and wd_gmres_mixed (CV = float2): argument checks, work space, line 4 for
+// x_0, then cycles — the first one launch by launch (all caches warm), the second captured into a CUDA graph that the
+// later ones replay (WD_OPT_GMRES_GRAPH, non-default stream) — with one host synchronisation per cycle to read ||b - A x||.
+template <class CV>
+int gmres_driver(wd_handle *h, const char *name, void *dev_x, const void *dev_b, int m, int max_cycles, double tol, int *cycles_done,
+                 double *host_resid) {
+    constexpr bool MIXED = sizeof(CV) == sizeof(float2);
+    const std::string nm(name);
     if (!dev_x || !dev_b || m < 1 || m > kMaxM || max_cycles < 0 || !(tol > 0.0))
-        return fail(h, WD_EINVAL, "wd_gmres: null pointer, m outside 1..64, max_cycles < 0 or tol <= 0");
-    if (((size_t)dev_x | (size_t)dev_b) & 15) return fail(h, WD_EINVAL, "wd_gmres: spinor buffers must be 16-byte aligned");
-    if (dev_x == dev_b) return fail(h, WD_EINVAL, "wd_gmres: x overlaps b");
-    if (!h->has_gauge) return fail(h, WD_ESTATE, "wd_gmres: no gauge field loaded");
-    int rc = ensure_workspace(h, m, false);
+        return fail(h, WD_EINVAL, nm + ": null pointer, m outside 1..64, max_cycles < 0 or tol <= 0");
+    if (((size_t)dev_x | (size_t)dev_b) & 15) return fail(h, WD_EINVAL, nm + ": spinor buffers must be 16-byte aligned");
+    if (dev_x == dev_b) return fail(h, WD_EINVAL, nm + ": x overlaps b");
+    if (!h->has_gauge) return fail(h, WD_ESTATE, nm + ": no gauge field loaded");
+    if (MIXED && !h->f32) return fail(h, WD_ESTATE, nm + ": call wd_enable_f32 after loading the fields (single-precision copies of U and S)");
+    int rc = ensure_workspace(h, m, MIXED);
     if (rc) return rc;
     wd_gmres_state *g = h->gmres;
-    Cycle<double2> cyc{h, g, m, tol / 10.0};
+    Cycle<CV> cyc{h, g, m, tol / 10.0};
     double2 *x = (double2 *)dev_x;
     const double2 *b = (const double2 *)dev_b;
     struct { double beta, inv, lsq; int active, kdim, kdim_done; unsigned int ticket; } hs;
@@ -430,7 +439,7 @@ int wd_gmres(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_cycles
     int k = 0;
     const bool can_graph = (h->stream != nullptr) && h->gmres_graph;
     while (!(hs.beta < tol * r0) && k < max_cycles && hs.beta != 0.0) {
-        const bool have_graph = g->graph && g->gx == dev_x && g->gb == dev_b && g->gm == m && g->gtol == tol && g->gstream == h->stream;
+        const bool have_graph = g->graph && g->gx == dev_x && g->gb == dev_b && g->gm == m && g->gtol == tol && g->gstream == h->stream && g->gmixed == MIXED;
         if (have_graph) {
             WD_CUDA(h, cudaGraphLaunch(g->graph, h->stream));
             h->launches += g->graph_launches;
@@ -450,7 +459,7 @@ int wd_gmres(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_cycles
             const cudaError_t ie = cudaGraphInstantiate(&g->graph, graph, 0);
             cudaGraphDestroy(graph);
             WD_CUDA(h, ie);
-            g->gx = dev_x, g->gb = dev_b, g->gm = m, g->gtol = tol, g->gstream = h->stream;
+            g->gx = dev_x, g->gb = dev_b, g->gm = m, g->gtol = tol, g->gstream = h->stream, g->gmixed = MIXED;
             g->graph_launches = cyc.launches;
             WD_CUDA(h, cudaGraphLaunch(g->graph, h->stream));
             h->launches += g->graph_launches;
@@ -469,46 +478,22 @@ int wd_gmres(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_cycles
     return WD_OK;
 }
 
+}  // namespace
+
+extern "C" {
+
+int wd_gmres(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_cycles, double tol, int *cycles_done,
+             double *host_resid) {
+    WD_ENTER(h);
+    WD_PLAIN_ONLY(h, "wd_gmres");
+    return gmres_driver<double2>(h, "wd_gmres", dev_x, dev_b, m, max_cycles, tol, cycles_done, host_resid);
+}
+
 int wd_gmres_mixed(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_cycles, double tol, int *cycles_done,
                    double *host_resid) {
     WD_ENTER(h);
     WD_PLAIN_ONLY(h, "wd_gmres_mixed");
-    if (!dev_x || !dev_b || m < 1 || m > kMaxM || max_cycles < 0 || !(tol > 0.0))
-        return fail(h, WD_EINVAL, "wd_gmres_mixed: null pointer, m outside 1..64, max_cycles < 0 or tol <= 0");
-    if (((size_t)dev_x | (size_t)dev_b) & 15) return fail(h, WD_EINVAL, "wd_gmres_mixed: spinor buffers must be 16-byte aligned");
-    if (dev_x == dev_b) return fail(h, WD_EINVAL, "wd_gmres_mixed: x overlaps b");
-    if (!h->has_gauge) return fail(h, WD_ESTATE, "wd_gmres_mixed: no gauge field loaded");
-    if (!h->f32) return fail(h, WD_ESTATE, "wd_gmres_mixed: call wd_enable_f32 after loading the fields (single-precision copies of U and S)");
-    int rc = ensure_workspace(h, m, true);
-    if (rc) return rc;
-    wd_gmres_state *g = h->gmres;
-    Cycle<float2> cyc{h, g, m, tol / 10.0};
-    double2 *x = (double2 *)dev_x;
-    const double2 *b = (const double2 *)dev_b;
-    struct { double beta, inv, lsq; int active, kdim, kdim_done; unsigned int ticket; } hs;
-    auto read_scalars = [&]() -> int {
-        WD_CUDA(h, cudaMemcpyAsync(&hs, &g->sc->beta, sizeof(hs), cudaMemcpyDeviceToHost, h->stream));
-        WD_CUDA(h, cudaStreamSynchronize(h->stream));
-        return WD_OK;
-    };
-    if ((rc = cyc.residual(x, b))) return rc;
-    h->launches += cyc.launches;
-    if ((rc = read_scalars())) return rc;
-    const double r0 = hs.beta;
-    if (host_resid) host_resid[0] = r0;
-    int k = 0;
-    while (!(hs.beta < tol * r0) && k < max_cycles && hs.beta != 0.0) {
-        cyc.launches = 0;
-        if ((rc = cyc.body(x, b))) return rc;
-        h->launches += cyc.launches;
-        if ((rc = read_scalars())) return rc;
-        k++;
-        if (host_resid) host_resid[k] = hs.beta;
-    }
-    if (cycles_done) *cycles_done = k;
-    g->last_m = m;
-    g->last_kdim = (k > 0) ? hs.kdim_done : 0;
-    return WD_OK;
+    return gmres_driver<float2>(h, "wd_gmres_mixed", dev_x, dev_b, m, max_cycles, tol, cycles_done, host_resid);
 }
 
 int wd_gmres_last_hessenberg(wd_handle *h, double *host_H, int *kdim, double *lsq_resid) {

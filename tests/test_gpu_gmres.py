@@ -174,6 +174,18 @@ def test_mixed_precision_gmres_solves_the_fp64_system(torch):
         x = np.empty((1,) + b.shape)
         wd.wd_unpack_spinor(op.h, x, dx, 1)
         hist = hist[: cycles + 1]
+        # the same on a side stream, cycles 2.. replayed as one CUDA graph: bit for bit the launch-by-launch result
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            wd.wd_set_stream(op.h, st.cuda_stream)
+            wd.wd_pack_spinor(op.h, dx, np.ascontiguousarray(x0[None]), 1)
+            hist_g = np.full(max_cycles + 1, np.nan)
+            cycles_g = wd.wd_gmres_mixed(op.h, dx, db, m, max_cycles, tol, hist_g)
+            xg = np.empty_like(x)
+            wd.wd_unpack_spinor(op.h, xg, dx, 1)
+            wd.wd_synchronize(op.h)
+        wd.wd_set_stream(op.h, torch.cuda.current_stream().cuda_stream)
+        assert cycles_g == cycles and np.array_equal(hist_g[: cycles + 1], hist) and np.array_equal(xg, x)
         # the FP64 solver on the same handle afterwards: the two share scalars and must not disturb each other
         x64, hist64, cycles64, *_ = device_gmres(torch, op, b, x0, m, max_cycles, tol)
     assert info["cycles"] <= cycles <= info["cycles"] + 3 and cycles64 == info["cycles"]
