@@ -131,6 +131,27 @@ template <class CV> __device__ __forceinline__ double2 ldv(const CV *p, long lon
     return make_double2((double)v.x, (double)v.y);
 }
 template <class CV> __device__ __forceinline__ void stv(CV *p, long long i, double2 v) { p[i] = mk<CV>((R<CV>)v.x, (R<CV>)v.y); }
+// A thread moves 16 bytes per access: one double2, or two consecutive float2 (i even; the component base is a multiple of
+// 16 elements).  n = elements that exist (the last access of an odd-length component holds one).
+template <class CV> struct Epa { static constexpr int n = 16 / (int)sizeof(CV); };
+template <class CV> __device__ __forceinline__ void ldn(const CV *p, long long i, int n, double2 *x) {
+    if (Epa<CV>::n == 2) {
+        if (n == 2) {
+            const float4 v = *reinterpret_cast<const float4 *>(p + i);
+            x[0] = make_double2((double)v.x, (double)v.y);
+            x[1] = make_double2((double)v.z, (double)v.w);
+        } else {
+            x[0] = ldv(p, i);
+            x[1] = make_double2(0.0, 0.0);
+        }
+    } else {
+        x[0] = ldv(p, i);
+    }
+}
+template <class CV> __device__ __forceinline__ void stn(CV *p, long long i, int n, const double2 *x) {
+    if (Epa<CV>::n == 2 && n == 2) *reinterpret_cast<float4 *>(p + i) = make_float4((float)x[0].x, (float)x[0].y, (float)x[1].x, (float)x[1].y);
+    else stv(p, i, x[0]);
+}
 
 template <int OP, class CV>
 __global__ void __launch_bounds__(kThreads) k_fused(CV *__restrict__ w, const CV *__restrict__ vp,
@@ -141,25 +162,38 @@ __global__ void __launch_bounds__(kThreads) k_fused(CV *__restrict__ w, const CV
     double2 h = make_double2(0.0, 0.0);
     if (OP == OP_AXPY_DOT || OP == OP_AXPY_NORM) h = sc->H[h_in];
     double2 acc = make_double2(0.0, 0.0);
-    for (long long i = (long long)blockIdx.x * kThreads + threadIdx.x; i < V; i += (long long)gridDim.x * kThreads) {
-        double2 x = ldv(w, base + i);
+    constexpr int E = Epa<CV>::n;
+    const long long nacc = (V + E - 1) / E;
+    for (long long a = (long long)blockIdx.x * kThreads + threadIdx.x; a < nacc; a += (long long)gridDim.x * kThreads) {
+        const long long i = a * E;
+        const int n = (V - i < E) ? (int)(V - i) : E;
+        double2 x[E], p[E], q[E];
+        ldn(w, base + i, n, x);
         if (OP == OP_AXPY_DOT || OP == OP_AXPY_NORM) {
-            const double2 p = ldv(vp, base + i);
-            x.x = fma(-h.x, p.x, fma(h.y, p.y, x.x));
-            x.y = fma(-h.x, p.y, fma(-h.y, p.x, x.y));
-            stv(w, base + i, x);
-            if (sizeof(CV) == sizeof(float2)) x = ldv(w, base + i);  // the inner product sees the vector as stored
+            ldn(vp, base + i, n, p);
+#pragma unroll
+            for (int e = 0; e < E; e++) {
+                x[e].x = fma(-h.x, p[e].x, fma(h.y, p[e].y, x[e].x));
+                x[e].y = fma(-h.x, p[e].y, fma(-h.y, p[e].x, x[e].y));
+                if (sizeof(CV) == sizeof(float2)) x[e] = make_double2((double)(float)x[e].x, (double)(float)x[e].y);  // the inner product sees the vector as stored
+            }
+            stn(w, base + i, n, x);
         } else if (OP == OP_RESID_NORM) {
-            const double2 b = ldv(vp, base + i);
-            x = make_double2(b.x - x.x, b.y - x.y);
-            stv(w, base + i, x);
+            ldn(vp, base + i, n, p);
+#pragma unroll
+            for (int e = 0; e < E; e++) x[e] = make_double2(p[e].x - x[e].x, p[e].y - x[e].y);
+            stn(w, base + i, n, x);
         }
         if (OP == OP_DOT || OP == OP_AXPY_DOT) {  // conj(vn) * x
-            const double2 q = ldv(vn, base + i);
-            acc.x = fma(q.x, x.x, fma(q.y, x.y, acc.x));
-            acc.y = fma(q.x, x.y, fma(-q.y, x.x, acc.y));
+            ldn(vn, base + i, n, q);
+#pragma unroll
+            for (int e = 0; e < E; e++) {
+                acc.x = fma(q[e].x, x[e].x, fma(q[e].y, x[e].y, acc.x));
+                acc.y = fma(q[e].x, x[e].y, fma(-q[e].y, x[e].x, acc.y));
+            }
         } else {
-            acc.x = fma(x.x, x.x, fma(x.y, x.y, acc.x));
+#pragma unroll
+            for (int e = 0; e < E; e++) acc.x = fma(x[e].x, x[e].x, fma(x[e].y, x[e].y, acc.x));
         }
     }
     double2 total;
@@ -190,9 +224,17 @@ __global__ void __launch_bounds__(kThreads) k_scale(CD *__restrict__ dst, const 
     if (!always && !sc->active) return;
     const double s = sc->inv;
     const long long base = (long long)blockIdx.y * Vs;
-    for (long long i = (long long)blockIdx.x * kThreads + threadIdx.x; i < V; i += (long long)gridDim.x * kThreads) {
-        const double2 x = ldv(src, base + i);
-        stv(dst, base + i, make_double2(s * x.x, s * x.y));
+    constexpr int E = Epa<CD>::n;  // accesses sized by the destination
+    const long long nacc = (V + E - 1) / E;
+    for (long long a = (long long)blockIdx.x * kThreads + threadIdx.x; a < nacc; a += (long long)gridDim.x * kThreads) {
+        const long long i = a * E;
+        const int n = (V - i < E) ? (int)(V - i) : E;
+        double2 x[E];
+#pragma unroll
+        for (int e = 0; e < E; e++) x[e] = (e < n) ? ldv(src, base + i + e) : make_double2(0.0, 0.0);
+#pragma unroll
+        for (int e = 0; e < E; e++) x[e] = make_double2(s * x[e].x, s * x[e].y);
+        stn(dst, base + i, n, x);
     }
 }
 
@@ -250,14 +292,26 @@ __global__ void __launch_bounds__(kThreads) k_update(double2 *__restrict__ x, co
                                                      long long Vs, long long vec_stride, const Scalars *sc) {
     const int kd = sc->kdim;
     const long long base = (long long)blockIdx.y * Vs;
-    for (long long i = (long long)blockIdx.x * kThreads + threadIdx.x; i < V; i += (long long)gridDim.x * kThreads) {
-        double2 s = x[base + i];
+    constexpr int E = Epa<CV>::n;
+    const long long nacc = (V + E - 1) / E;
+    for (long long a = (long long)blockIdx.x * kThreads + threadIdx.x; a < nacc; a += (long long)gridDim.x * kThreads) {
+        const long long i = a * E;
+        const int n = (V - i < E) ? (int)(V - i) : E;
+        double2 s[E], v[E];
+#pragma unroll
+        for (int e = 0; e < E; e++) s[e] = (e < n) ? x[base + i + e] : make_double2(0.0, 0.0);
         for (int k = 0; k < kd; k++) {
-            const double2 yk = sc->y[k], v = ldv(basis, (long long)k * vec_stride + base + i);
-            s.x = fma(yk.x, v.x, fma(-yk.y, v.y, s.x));
-            s.y = fma(yk.x, v.y, fma(yk.y, v.x, s.y));
+            const double2 yk = sc->y[k];
+            ldn(basis, (long long)k * vec_stride + base + i, n, v);
+#pragma unroll
+            for (int e = 0; e < E; e++) {
+                s[e].x = fma(yk.x, v[e].x, fma(-yk.y, v[e].y, s[e].x));
+                s[e].y = fma(yk.x, v[e].y, fma(yk.y, v[e].x, s[e].y));
+            }
         }
-        x[base + i] = s;
+#pragma unroll
+        for (int e = 0; e < E; e++)
+            if (e < n) x[base + i + e] = s[e];
     }
 }
 
