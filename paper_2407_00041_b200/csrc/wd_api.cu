@@ -493,6 +493,10 @@ static int auto_kernel(const wd_handle *h, int nrhs) {
     if (nrhs > 1 && h->variant == 0 && 20 * nrhs >= 17 * 4 * ((nrhs + 3) / 4))
         for (int id = 0; id < kernel_count(); id++)
             if (!strcmp(kernel_info(id).name, "tmq_2x4x8") && geometry_fits(h, kernel_info(id))) return id;
+    // small lattices: a persistent TMA kernel costs ~25 us to start and drain whatever the volume; below 32 Ki sites the
+    // one-thread-per-site kernel wins for one or two right-hand sides (8^4: 13 us against 31 us; 8x8x16x32: 14.5 against
+    // 16.9 us; 16^4: 37 against 24.5 us, so not beyond)
+    if (h->V <= 32768 && nrhs <= 2) return 0;  // linear256
     const bool clover_fused = (h->csw != 0.0 || h->has_clover) && h->variant == 0;
     const char **pref = (nrhs > 1 && h->variant == 0) ? pref_multi : !clover_fused ? pref_hop : (h->gauge_rows == 2) ? pref_tworow : pref_clover;
     for (int i = 0; i < 6; i++)

@@ -127,7 +127,7 @@ def test_decomposed_bench_size_slab(torch, capsys):
 
 class _InProcessDist:
     """Stand-in for torch.distributed point-to-point between `world` ranks that are THREADS of this process sharing one
-    GPU: a send records an event on the sender's stream and leaves (tensor, event) in a mailbox; a receive blocks the
+    GPU: a send snapshots its buffer, records an event on the sender's stream and leaves (snapshot, event) in a mailbox; a receive blocks the
     receiving host thread until the message is there, makes its stream wait for the event and copies.  Only
     stream-ordered dependencies exist on the device (no kernel waits for another), so this is safe on one GPU."""
 
@@ -162,10 +162,14 @@ class _InProcessDist:
         works = []
         for op in ops:
             if op.fn == self.isend:
+                # a real send has read its buffer when its work has been waited for; here the work is a no-op, so the
+                # message is a snapshot taken in stream order (the sender may repack the buffer for its next application
+                # before the receiving thread gets to copy)
+                snap = op.tensor.clone()
                 ev = torch.cuda.Event()
                 ev.record(torch.cuda.current_stream())
                 with self.cv:
-                    self.box[(me, op.peer, op.tag)].append((op.tensor, ev))
+                    self.box[(me, op.peer, op.tag)].append((snap, ev))
                     self.cv.notify_all()
                 works.append(self._Work(lambda: None))
             else:

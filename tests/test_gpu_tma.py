@@ -165,7 +165,8 @@ def test_apply_host_pipelined_over_t_chunks(torch, dims, csw):
     psi = wdinputs.spinor(dims, 442, nrhs=nrhs)
     C = oracle.build_clover(dims, m0, csw, U) if csw else None
     ref = oracle.apply(dims, m0, U, C, psi)
-    with Op(torch, dims, m0, csw, U, C) as op:
+    # (lattices this small get the one-thread-per-site kernel automatically; the pipelined path needs a TMA kernel)
+    with Op(torch, dims, m0, csw, U, C, kernel=wd.kernel_id("tmw_2x4x16" if csw else "tmb_2x4x16")) as op:
         assert wd.wd_kernel_name(wd.wd_kernel_in_use(op.h)).startswith(("tma_", "tmb_", "tmw_"))
         out = np.empty_like(psi)
         wd.wd_apply_host(op.h, out, psi, nrhs)
