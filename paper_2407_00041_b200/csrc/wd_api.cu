@@ -476,9 +476,10 @@ static int auto_kernel(const wd_handle *h, int nrhs) {
     // Preference order.  One right-hand side with a clover term, fused: the warpgroup-split
     // kernel (64^4: 4.13 ms burst / 4.30 ms sustained against 4.15 / 4.35 ms of the first generation, which stays the
     // choice with two-row links).  The hopping term alone (csw = 0, or the unfused variant): the second generation on
-    // the 2x4x16 tile (pure Wilson 2.80 ms; 4x4x8 tile 2.88, tmw 3.06, tma 3.66 ms).  Several right-hand sides in one
-    // call: the second generation on the 4x4x8 tile with its four-slot ring (cfg 5: 25.8 ms; 2x4x16 with three slots
-    // 28.3, tmw 27.4, tma 28.5 ms).  linear256 always fits.
+    // the 2x4x16 tile (pure Wilson 2.75 ms; 4x4x8 tile 2.88, tmw 3.06, tma 3.66 ms).  Several right-hand sides in one
+    // call: the quad kernels of wd_tmq.cu (cfg 5: tmqb on the blocked layout 17.4 ms, tmq on the plain layout 20.8 ms when
+    // its units of four are well filled), else the second generation on the 4x4x8 tile with its four-slot ring (25.4 ms;
+    // 2x4x16 with three slots 28.3, tmw 27.4, tma 28.5 ms).  linear256 always fits, and wins on small lattices.
     static const char *pref_clover[] = {"tmw_2x4x16", "tma_2x4x16", "tmb_4x4x8", "tmb_2x8x8", "tile_1x4x4x16", "tile_2x4x4x4"};
     static const char *pref_tworow[] = {"tma_2x4x16", "tmw_2x4x16", "tmb_4x4x8", "tmb_2x8x8", "tile_1x4x4x16", "tile_2x4x4x4"};
     static const char *pref_hop[] = {"tmb_2x4x16", "tmb_4x4x8", "tmb_2x8x8", "tmw_2x4x16", "tile_1x4x4x16", "tile_2x4x4x4"};
