@@ -156,6 +156,44 @@ int wd_gmres_mixed(wd_handle *h, void *dev_x, const void *dev_b, int m, int max_
  * breakdown rule ended it); *lsq_resid (may be NULL) = min_y ||beta e_1 - H y||, the recurrence residual. */
 int wd_gmres_last_hessenberg(wd_handle *h, double *host_H, int *kdim, double *lsq_resid);
 
+/* ---- an entry point that allocates nothing ----
+ * WHO IT IS FOR.  Every other call of this library may reach cudaMalloc: wd_create and the wd_load_ / wd_enable_ calls
+ * always do, wd_gmres does for its Krylov basis and for the partial sums and counters of its reductions.  Some programs
+ * cannot afford that at the point where they need an inner product or a norm of device spinors: a solver written on top of
+ * PyTorch (or any framework whose caching allocator has already taken nearly all of the 180 GB), where a raw cudaMalloc
+ * from a library fails or carves memory out behind the allocator's back; an iteration loop between two operator
+ * applications, where cudaMalloc / cudaFree would stall every stream of the device because they synchronise it; a host
+ * program that forbids driver allocations after its own start-up phase.  For them:
+ *
+ * wd_inner_product_static: dev_result[r] = <a_r, b_r> = sum over the 12 components and the V sites of conj(a) * b, for
+ * r = 0 .. nrhs-1 — h_ij = v_i^H w of Algorithm 1 lines 10-11 and, with dev_a == dev_b, the squared norms of lines 5
+ * and 14.  No handle: dev_a, dev_b are DEVICE spinors of the current device in the PLAIN device layout
+ * (complex double [nrhs][12][Vs], of which the first V elements of every component are read; V = sites,
+ * Vs = wd_component_stride), dev_result is a DEVICE array of nrhs complex doubles; all three caller-owned and 16-byte
+ * aligned; cuda_stream as in wd_set_stream.  Asynchronous on that stream.  Same kernel structure and, for nrhs = 1, the
+ * same summation order as the reductions inside wd_gmres, so the result is deterministic.
+ *
+ * SCRATCH.  The per-block partial sums and the completion counters of the reduction sit in ONE fixed array of 65 792 bytes
+ * (4096 partial sums + 64 counters) that is part of the library image: every GPU on which libwd.so is loaded holds it from
+ * load to process exit, whether or not this function is ever called, and it never grows.  LIMIT: nrhs <= 64 per call (one
+ * counter per right-hand side); a larger nrhs is refused with WD_EINVAL and a text that says so — split the call.  V is
+ * not limited by the scratch (blocks loop over the sites).
+ *
+ * FIRST CALL ON A DEVICE.  The first call made with a given device current asks the CUDA runtime once for the address the
+ * array has on that device and keeps it (no allocation, but a runtime query that is not stream work): make that first call
+ * during set-up, before any stream capture is begun on that device; later calls only enqueue a 256-byte memset of the
+ * counters and one kernel.
+ *
+ * SHARING.  All calls on a device, from every stream and thread, use the same array, and it keeps what the previous call
+ * left in it.  The function clears the counters itself on every call; the partial sums need no clearing (each block writes
+ * its slot before any is read).  Two calls whose GPU work can overlap — different streams without an event between them,
+ * or two host threads — race on the array and return garbage: order them yourself.  Calls on one stream are safe.
+ *
+ * Errors: WD_EINVAL (null or misaligned pointer, V < 1, Vs < V, nrhs < 1, nrhs > 64), WD_ECUDA; text in
+ * wd_last_error(NULL).  Never WD_ENOMEM. */
+int wd_inner_product_static(const void *dev_a, const void *dev_b, long long V, long long Vs, int nrhs, void *dev_result,
+                            void *cuda_stream);
+
 /* ---- domain decomposition (Algorithm 3; local lattices, eqs. 2.1-2.4) ----
  * A handle for ONE hyper-rectangular sub-lattice of a global periodic lattice: local extents = global_dims / proc_grid
  * (int[4] each, order T,Z,Y,X; proc_coords = position of this sub-lattice in the grid).  In a direction with
@@ -269,7 +307,7 @@ int wd_kernel_for(const wd_handle *h, int nrhs);
 /* Number of kernel launches issued by this handle so far (all kernels of this library). */
 long wd_launch_count(const wd_handle *h);
 
-/* Text of the last error on this handle (h == NULL: of the last failed wd_create on this thread).
+/* Text of the last error on this handle (h == NULL: of the last failed wd_create or handle-free call on this thread).
  * Never NULL. */
 const char *wd_last_error(const wd_handle *h);
 

@@ -45,6 +45,7 @@ SIGNATURES = {
     "wd_gmres": (_i, [_vp, _vp, _vp, _i, _i, _d, ctypes.POINTER(_i), _vp]),
     "wd_gmres_mixed": (_i, [_vp, _vp, _vp, _i, _i, _d, ctypes.POINTER(_i), _vp]),
     "wd_gmres_last_hessenberg": (_i, [_vp, _vp, ctypes.POINTER(_i), ctypes.POINTER(_d)]),
+    "wd_inner_product_static": (_i, [_vp, _vp, ctypes.c_longlong, ctypes.c_longlong, _i, _vp, _vp]),
     "wd_spinor_bytes": (_sz, [_vp, _i]),
     "wd_component_stride": (ctypes.c_longlong, [_vp]),
     "wd_pack_spinor": (_i, [_vp, _vp, _vp, _i]),
@@ -205,6 +206,12 @@ def wd_gmres_last_hessenberg(h, host_H=None) -> tuple[int, float]:
     kd, lr = _i(0), _d(0.0)
     _check(h, lib().wd_gmres_last_hessenberg(h, _ptr(host_H), ctypes.byref(kd), ctypes.byref(lr)))
     return kd.value, lr.value
+
+
+def wd_inner_product_static(dev_a, dev_b, V: int, Vs: int, nrhs: int, dev_result, cuda_stream=None) -> None:
+    """dev_result[r] = <a_r, b_r> without any allocation inside the library (include/wd.h: for callers that cannot
+    call cudaMalloc).  dev_result: device array of nrhs complex doubles; at most 64 right-hand sides per call."""
+    _check(None, lib().wd_inner_product_static(_ptr(dev_a), _ptr(dev_b), V, Vs, nrhs, _ptr(dev_result), _ptr(cuda_stream)))
 
 
 def wd_spinor_bytes(h, nrhs: int = 1) -> int:

@@ -21,7 +21,9 @@
 #include <cmath>
 #include <cstddef>
 #include <cstring>
+#include <mutex>
 #include <new>
+#include <string>
 #include <vector>
 
 #include "wd_handle.h"
@@ -566,3 +568,93 @@ int wd_gmres_last_hessenberg(wd_handle *h, double *host_H, int *kdim, double *ls
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// wd_inner_product_static — the inner product of lines 10-11 / the norm of lines 5, 14 of Algorithm 1
+// for callers that must not allocate (include/wd.h has the contract).  It is k_fused<OP_DOT> with the same grid-wide
+// reduction (grid_reduce above: one partial per block, the last block adds them in a fixed order), but the per-block
+// partials and the completion counters — which wd_gmres keeps in cudaMalloc'ed memory behind its Scalars — live in a
+// fixed array inside the library image.  Nothing below calls cudaMalloc / cudaFree or anything that allocates.
+namespace {
+
+constexpr int kStaticSlots = 4096;    // per-block partial sums (16 B each), shared by the right-hand sides of a call
+constexpr int kStaticMaxRhs = 64;     // one completion counter per right-hand side
+constexpr int kStaticTicketSlots = kStaticMaxRhs * (int)sizeof(unsigned int) / (int)sizeof(double2);  // 16 double2 = 64 counters
+constexpr int kStaticMaxDevices = 64;
+
+// 64 KiB + 256 B per GPU that loads libwd.so, for the life of the process.  [0, kStaticSlots): partials;
+// the last 256 bytes: the counters.  Shared by every call on the device; holds whatever the last call left.
+static __device__ __align__(256) double2 g_static_scratch[kStaticSlots + kStaticTicketSlots];
+
+// g_static_scratch as a host expression is only a shadow the runtime uses to look the symbol up; its DEVICE address, which
+// differs from GPU to GPU, is asked for once per device (with that device current) and kept here.
+std::mutex g_static_mutex;
+double2 *g_static_addr[kStaticMaxDevices];
+int g_static_nsm[kStaticMaxDevices];
+
+// result[r] = sum over the 12 components and V sites of conj(a) * b, right-hand side r = blockIdx.z
+__global__ void __launch_bounds__(kThreads) k_dot_static(const double2 *__restrict__ a, const double2 *__restrict__ b, long long V,
+                                                         long long Vs, double2 *scratch, double2 *__restrict__ result) {
+    const long long base = ((long long)blockIdx.z * 12 + blockIdx.y) * Vs;
+    double2 acc = make_double2(0.0, 0.0);
+    for (long long i = (long long)blockIdx.x * kThreads + threadIdx.x; i < V; i += (long long)gridDim.x * kThreads) {
+        const double2 q = a[base + i], x = b[base + i];
+        acc.x = fma(q.x, x.x, fma(q.y, x.y, acc.x));
+        acc.y = fma(q.x, x.y, fma(-q.y, x.x, acc.y));
+    }
+    const unsigned int nblk = gridDim.x * gridDim.y;
+    unsigned int *tickets = reinterpret_cast<unsigned int *>(scratch + kStaticSlots);
+    double2 total;
+    if (grid_reduce(acc, scratch + (size_t)blockIdx.z * nblk, tickets + blockIdx.z, &total)) result[blockIdx.z] = total;
+}
+
+int static_fail(int code, const std::string &msg) { return fail(nullptr, code, "wd_inner_product_static: " + msg); }
+
+}  // namespace
+
+extern "C" int wd_inner_product_static(const void *dev_a, const void *dev_b, long long V, long long Vs, int nrhs, void *dev_result,
+                                       void *cuda_stream) {
+    // argument checks first: they need no GPU
+    if (!dev_a || !dev_b || !dev_result) return static_fail(WD_EINVAL, "null pointer");
+    if (V < 1 || Vs < V || V >= (1LL << 40)) return static_fail(WD_EINVAL, "need 1 <= V <= Vs and V < 2^40");
+    if (nrhs < 1) return static_fail(WD_EINVAL, "nrhs < 1");
+    if (nrhs > kStaticMaxRhs)
+        return static_fail(WD_EINVAL, "nrhs = " + std::to_string(nrhs) + " is beyond the maximum of " + std::to_string(kStaticMaxRhs) +
+                                          " right-hand sides per call that the fixed scratch array (" +
+                                          std::to_string(sizeof(double2) * (kStaticSlots + kStaticTicketSlots)) +
+                                          " bytes, never grown) has counters and partial-sum slots for; split the call");
+    if (((size_t)dev_a | (size_t)dev_b | (size_t)dev_result) & 15) return static_fail(WD_EINVAL, "pointers must be 16-byte aligned");
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    int dev = -1;
+    WD_CUDA(nullptr, cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return static_fail(WD_EINVAL, "device ordinal beyond " + std::to_string(kStaticMaxDevices - 1));
+    double2 *scratch;
+    int nsm;
+    {  // first call on this device: look the array's device address up (the set-up step the header documents)
+        std::lock_guard<std::mutex> lock(g_static_mutex);
+        if (!g_static_addr[dev]) {
+            double2 *p = nullptr;
+            WD_CUDA(nullptr, cudaGetSymbolAddress((void **)&p, g_static_scratch));
+            int n = 0;
+            WD_CUDA(nullptr, cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev));
+            if (!p || n < 1) return static_fail(WD_ECUDA, "no device address for the scratch array");
+            g_static_nsm[dev] = n;
+            g_static_addr[dev] = p;
+        }
+        scratch = g_static_addr[dev];
+        nsm = g_static_nsm[dev];
+    }
+    // blocks per component: as wd_gmres (about 8 elements per thread, at most ~8 blocks per SM over the 12 components), and no
+    // more than the partial-sum slots allow; nrhs <= 64 leaves at least 5
+    long long nbx = (V + kThreads * 8 - 1) / (kThreads * 8);
+    const long long cap = (long long)nsm * 8 / 12 + 1, fit = kStaticSlots / (12LL * nrhs);
+    if (nbx > cap) nbx = cap;
+    if (nbx > fit) nbx = fit;
+    if (nbx < 1) nbx = 1;
+    // the counters must start at zero; a call that failed half-way may have left them otherwise
+    WD_CUDA(nullptr, cudaMemsetAsync(scratch + kStaticSlots, 0, sizeof(double2) * kStaticTicketSlots, stream));
+    k_dot_static<<<dim3((unsigned)nbx, 12, (unsigned)nrhs), kThreads, 0, stream>>>((const double2 *)dev_a, (const double2 *)dev_b, V, Vs,
+                                                                                  scratch, (double2 *)dev_result);
+    WD_CUDA(nullptr, cudaGetLastError());
+    return WD_OK;
+}
