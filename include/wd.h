@@ -68,7 +68,9 @@ enum {
     WD_OPT_ZGROUP = 4,    /* number of Z-tiles per rasterisation group in tiled geometries; 0 = automatic         */
     WD_OPT_DEVICE_PACK = 5,/* 1 = wd_load_* / wd_pack_* transpose on the device instead of on the host (default 0) */
     WD_OPT_HOST_PIPELINE = 6,/* wd_apply_host: 1 = overlap upload, compute and download over T chunks (default), 0 = serial */
-    WD_OPT_GMRES_GRAPH = 7,/* wd_gmres: 1 = replay restart cycles as one CUDA graph (default; needs a non-default stream), 0 = launch by launch */
+    WD_OPT_GMRES_GRAPH = 7,/* wd_gmres: 1 = replay restart cycles as one CUDA graph (default; needs a non-default stream), 0 = launch by launch.
+                              A captured cycle is reused only for the same x, b, m, tol and stream AND an unchanged handle: any
+                              wd_set_option, wd_load_gauge, wd_load_clover, wd_build_clover or wd_enable_f32 makes the next solve capture anew */
     WD_OPT_GAUGE_ROWS = 8  /* 3 = links stored as 9 complex numbers (default).  2 = two-row storage for SU(3) links: the
                               fused TMA kernel of one right-hand side reads rows 0, 1 (384 instead of 576 B per site) and
                               rebuilds row 2 = conj(row 0 x row 1) in registers.  EXACT ONLY FOR SU(3) LINKS: with 2 the
@@ -231,8 +233,9 @@ int wd_dd_exterior(wd_handle *h, void *dev_out, int nrhs, int mu, const void *de
                    const void *dev_recv_from_minus);
 
 /* ---- FP32 variant (the paper's PRECISION templating) ----
- * wd_enable_f32: makes single-precision copies of the loaded links and of S on the device (call again after the FP64
- * fields change).  A single-precision device spinor is the device layout with 8-byte elements: wd_spinor_bytes_f32
+ * wd_enable_f32: makes single-precision copies of the loaded links and of S on the device.  The copies go stale when the
+ * FP64 fields change (wd_load_gauge, wd_load_clover, wd_build_clover): wd_apply_f32 and wd_gmres_mixed then return
+ * WD_ESTATE until wd_enable_f32 is called again.  A single-precision device spinor is the device layout with 8-byte elements: wd_spinor_bytes_f32
  * bytes, 8-byte aligned; it is produced from / turned into an FP64 device spinor by wd_convert_spinor (to_f32 = 1:
  * dst float <- src double; 0: dst double <- src float; both DEVICE pointers).  wd_apply_f32: out = D in with every load,
  * store and arithmetic operation in FP32 (one fused pass per right-hand side); the error against the FP64 operator is

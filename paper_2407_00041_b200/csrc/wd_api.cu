@@ -126,6 +126,7 @@ int wd_create(wd_handle **out, int T, int Z, int Y, int X, double m0, double csw
     h->s_up = h->s_dn = nullptr;
     h->pipe_ready = false;
     h->launches = 0;
+    h->config_epoch = h->fields_epoch = 0;
     h->gmres = nullptr;
     h->dd = nullptr;
     h->f32 = nullptr;
@@ -247,6 +248,7 @@ static int store_chunked(wd_handle *h, double2 *host, const double2 *dev, int nc
 int wd_load_gauge(wd_handle *h, const double *host_U) {
     WD_ENTER(h);
     if (!host_U) return fail(h, WD_EINVAL, "wd_load_gauge: null pointer");
+    h->config_epoch++, h->fields_epoch++;
     if (h->clover_built) {  // S was built from the links that are being replaced: it must be rebuilt (or loaded)
         h->has_clover = h->clover_built = false;
     }
@@ -276,6 +278,7 @@ static int ensure_clover_storage(wd_handle *h) {
 int wd_load_clover(wd_handle *h, const double *host_C) {
     WD_ENTER(h);
     if (!host_C) return fail(h, WD_EINVAL, "wd_load_clover: null pointer");
+    h->config_epoch++, h->fields_epoch++;
     int rc = ensure_clover_storage(h);
     if (rc) return rc;
     if (h->device_pack) {
@@ -301,6 +304,7 @@ int wd_build_clover(wd_handle *h) {
     if (!h->has_gauge) return fail(h, WD_ESTATE, "wd_build_clover: no gauge field loaded");
     if (dd_open_mask(h))
         return fail(h, WD_ESTATE, "wd_build_clover: plaquettes cross the seams of a decomposed handle; load S with wd_load_clover");
+    h->config_epoch++, h->fields_epoch++;
     int rc = ensure_clover_storage(h);
     if (rc) return rc;
     WD_CUDA(h, launch_build_clover(h->dS, h->dU, h->n, h->V, h->Vs, h->m0 + 4.0, h->csw, h->stream));
@@ -523,6 +527,7 @@ long wd_launch_count(const wd_handle *h) { return h ? h->launches : 0; }
 
 int wd_set_option(wd_handle *h, int option, long value) {
     if (!h) return WD_EINVAL;
+    h->config_epoch++;  // a captured GMRES cycle has the kernel choice, variant, chunking and link storage baked in
     switch (option) {
     case WD_OPT_VARIANT:
         if (value != 0 && value != 1) return fail(h, WD_EINVAL, "WD_OPT_VARIANT: 0 (fused) or 1 (unfused)");

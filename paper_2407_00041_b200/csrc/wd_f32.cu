@@ -15,6 +15,7 @@ using namespace wd;
 struct wd_f32_state {
     float2 *dU, *dS;
     bool has_clover;
+    long fields_epoch;  // h->fields_epoch when the copies were made
 };
 
 namespace {
@@ -35,6 +36,8 @@ template <class D, class S> cudaError_t convert(D *dst, const S *src, long long 
 }
 
 }  // namespace
+
+bool wd::f32_current(const wd_handle *h) { return h->f32 && h->f32->dU && h->f32->fields_epoch == h->fields_epoch; }
 
 void wd::f32_free(wd_handle *h) {
     if (!h->f32) return;
@@ -57,6 +60,8 @@ int wd_enable_f32(wd_handle *h) {
         h->f32->has_clover = false;
     }
     wd_f32_state *f = h->f32;
+    h->config_epoch++;
+    f->fields_epoch = -1;  // not current until both conversions are enqueued
     if (!f->dU) WD_CUDA(h, cudaMalloc((void **)&f->dU, (size_t)h->Vs * kGaugeComps * sizeof(float2)));
     WD_CUDA(h, convert(f->dU, h->dU, h->Vs * kGaugeComps, h->nsm, h->stream));
     h->launches++;
@@ -66,6 +71,7 @@ int wd_enable_f32(wd_handle *h) {
         WD_CUDA(h, convert(f->dS, h->dS, h->Vs * kCloverSlots, h->nsm, h->stream));
         h->launches++;
     }
+    f->fields_epoch = h->fields_epoch;
     return WD_OK;
 }
 
@@ -94,6 +100,8 @@ int wd_apply_f32(wd_handle *h, void *dev_out, const void *dev_in, int nrhs) {
     const char *o = (const char *)dev_out, *i = (const char *)dev_in;
     if (o < i + bytes && i < o + bytes) return fail(h, WD_EINVAL, "wd_apply_f32: out overlaps in");
     if (!h->f32 || !h->f32->dU) return fail(h, WD_ESTATE, "wd_apply_f32: call wd_enable_f32 after loading the fields");
+    if (!f32_current(h))
+        return fail(h, WD_ESTATE, "wd_apply_f32: the FP64 links or S changed after wd_enable_f32; call wd_enable_f32 again (the FP32 copies are stale)");
     if (h->csw != 0.0 && !h->f32->has_clover) return fail(h, WD_ESTATE, "wd_apply_f32: no FP32 self-coupling field (wd_enable_f32)");
     const int self = h->f32->has_clover ? SELF_CLOVER : SELF_MASS;
     // geometry: the TMA kernel (the FP64 skeleton on 8-byte elements) where its 2x4x16 tile divides the lattice, else

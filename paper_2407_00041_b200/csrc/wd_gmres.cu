@@ -58,6 +58,7 @@ struct wd_gmres_state {
     cudaGraphExec_t graph;
     const void *gx, *gb;  // what the captured cycle was built for
     int gm;
+    long gepoch;          // h->config_epoch at capture: options, fields and FP32 copies the cycle has baked in
     bool gmixed;          // the captured cycle is wd_gmres_mixed's
     double gtol;
     cudaStream_t gstream;
@@ -357,6 +358,7 @@ int ensure_workspace(wd_handle *h, int m, bool mixed) {
     g->sc = nullptr;
     g->graph = nullptr;
     g->gx = g->gb = nullptr;
+    g->gepoch = -1;
     g->gmixed = false;
     g->graph_launches = 0;
     g->last_m = g->last_kdim = 0;
@@ -365,11 +367,17 @@ int ensure_workspace(wd_handle *h, int m, bool mixed) {
     if (nbx > cap) nbx = cap;
     if (nbx < 1) nbx = 1;
     g->nbx = (int)nbx;
-    h->gmres = g;
-    // the scalars, followed by the per-block partial sums and room for a copy of H
+    // the scalars, followed by the per-block partial sums and room for a copy of H; the state is published only once
+    // they exist (a handle whose state had no scalars would hand the kernels a null pointer on the next call)
     const size_t extra = (size_t)g->nbx * 12 * sizeof(double2) + (size_t)(kMaxM + 1) * kMaxM * sizeof(double2);
-    WD_CUDA(h, cudaMalloc((void **)&g->sc, sizeof(Scalars) + extra));
-    WD_CUDA(h, cudaMemsetAsync(g->sc, 0, sizeof(Scalars) + extra, h->stream));
+    cudaError_t e = cudaMalloc((void **)&g->sc, sizeof(Scalars) + extra);
+    if (e == cudaSuccess) e = cudaMemsetAsync(g->sc, 0, sizeof(Scalars) + extra, h->stream);
+    if (e != cudaSuccess) {
+        if (g->sc) cudaFree(g->sc);
+        delete g;
+        WD_CUDA(h, e);
+    }
+    h->gmres = g;
     return ensure_workspace(h, m, mixed);
 }
 
@@ -473,6 +481,7 @@ int gmres_driver(wd_handle *h, const char *name, void *dev_x, const void *dev_b,
     if (dev_x == dev_b) return fail(h, WD_EINVAL, nm + ": x overlaps b");
     if (!h->has_gauge) return fail(h, WD_ESTATE, nm + ": no gauge field loaded");
     if (MIXED && !h->f32) return fail(h, WD_ESTATE, nm + ": call wd_enable_f32 after loading the fields (single-precision copies of U and S)");
+    if (MIXED && !f32_current(h)) return fail(h, WD_ESTATE, nm + ": the FP64 links or S changed after wd_enable_f32; call wd_enable_f32 again");
     int rc = ensure_workspace(h, m, MIXED);
     if (rc) return rc;
     wd_gmres_state *g = h->gmres;
@@ -495,7 +504,7 @@ int gmres_driver(wd_handle *h, const char *name, void *dev_x, const void *dev_b,
     int k = 0;
     const bool can_graph = (h->stream != nullptr) && h->gmres_graph;
     while (!(hs.beta < tol * r0) && k < max_cycles && hs.beta != 0.0) {
-        const bool have_graph = g->graph && g->gx == dev_x && g->gb == dev_b && g->gm == m && g->gtol == tol && g->gstream == h->stream && g->gmixed == MIXED;
+        const bool have_graph = can_graph && g->graph && g->gepoch == h->config_epoch && g->gx == dev_x && g->gb == dev_b && g->gm == m && g->gtol == tol && g->gstream == h->stream && g->gmixed == MIXED;
         if (have_graph) {
             WD_CUDA(h, cudaGraphLaunch(g->graph, h->stream));
             h->launches += g->graph_launches;
@@ -516,6 +525,7 @@ int gmres_driver(wd_handle *h, const char *name, void *dev_x, const void *dev_b,
             cudaGraphDestroy(graph);
             WD_CUDA(h, ie);
             g->gx = dev_x, g->gb = dev_b, g->gm = m, g->gtol = tol, g->gstream = h->stream, g->gmixed = MIXED;
+            g->gepoch = h->config_epoch;
             g->graph_launches = cyc.launches;
             WD_CUDA(h, cudaGraphLaunch(g->graph, h->stream));
             h->launches += g->graph_launches;

@@ -43,6 +43,9 @@ struct wd_handle {
     cudaEvent_t ev_up[kMaxPipeChunks], ev_cmp[kMaxPipeChunks], ev_misc[2];
     bool pipe_ready;
     long launches;
+    // config_epoch: bumped by everything that changes what a captured GMRES cycle has baked in (options, fields, the FP32
+    // copies); fields_epoch: bumped when the FP64 links or S change — the FP32 copies remember the value they were made from
+    long config_epoch, fields_epoch;
     std::string err;
     wd_gmres_state *gmres;  // workspace of wd_gmres (Krylov basis, Hessenberg matrix, CUDA graph), or null
     wd_dd_state *dd;        // sub-lattice state of a domain-decomposed operator (wd_create_local), or null
@@ -89,6 +92,7 @@ int launch_op(wd_handle *h, const KernelInfo &k, const KParams &p, int self);
 void gmres_free(wd_handle *h);  // wd_gmres.cu
 void dd_free(wd_handle *h);     // wd_dd.cu
 void f32_free(wd_handle *h);    // wd_f32.cu
+bool f32_current(const wd_handle *h);  // wd_f32.cu: FP32 copies exist and were made from the present FP64 fields
 int dd_open_mask(const wd_handle *h);  // bit mu: direction mu does not wrap on this handle (wd_create_local)
 
 }  // namespace wd

@@ -109,7 +109,9 @@ struct MapCache {
         int nrhs;
         TmaMaps maps;
     };
-    static constexpr int kEntries = 48;  // a GMRES(m) cycle applies the operator to m + 2 different vectors
+    static constexpr int kEntries = 80;  // a GMRES(m) cycle applies the operator to m + 2 <= 66 different vectors, in cyclic
+                                         // order (round-robin eviction of fewer entries would miss on every one); the rest
+                                         // is for the caller's own buffers
     Entry e[kEntries];
     int used = 0, next = 0;
     const TmaMaps *find(int tag, const void *psi, const void *U, const void *S, int nrhs) const {

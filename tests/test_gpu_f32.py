@@ -83,3 +83,32 @@ def test_convert_is_ieee_rounding_and_open_boundaries_work_in_fp32(torch):
         back = np.empty_like(psi)
         wd.wd_unpack_spinor(op.h, back, b64, 1)
         assert np.array_equal(back, r32(psi))
+
+
+def test_fp32_copies_go_stale_when_the_fp64_fields_change(torch):
+    """wd_enable_f32 copies the links and S as they are; after wd_load_gauge / wd_load_clover / wd_build_clover the copies
+    describe the OLD operator, so wd_apply_f32 and wd_gmres_mixed refuse (WD_ESTATE) until wd_enable_f32 is called again."""
+    dims, m0, csw = (4, 4, 8, 16), -0.2, 1.0
+    U1, U2 = wdinputs.gauge_exp(dims, 921, 0.5), wdinputs.gauge_exp(dims, 922, 0.5)
+    psi = wdinputs.spinor(dims, 923)
+    with Op(torch, dims, m0, csw, U1, build_clover=True) as op:
+        wd.wd_enable_f32(op.h)
+        out1 = apply_f32(torch, op, psi, 1)
+        wd.wd_load_gauge(op.h, U2)
+        wd.wd_build_clover(op.h)
+        n32 = wd.wd_spinor_bytes_f32(op.h, 1) // 4
+        a, b = torch.zeros(n32, dtype=torch.float32, device="cuda"), torch.zeros(n32, dtype=torch.float32, device="cuda")
+        with pytest.raises(wd.WDError) as e:
+            wd.wd_apply_f32(op.h, a, b, 1)
+        assert e.value.code == wd.WD_ESTATE and "stale" in str(e.value)
+        x, y = op.dev_spinor(), op.dev_spinor()
+        x.zero_()
+        wd.wd_pack_spinor(op.h, y, psi, 1)
+        with pytest.raises(wd.WDError) as e:
+            wd.wd_gmres_mixed(op.h, x, y, 4, 2, 1e-6)
+        assert e.value.code == wd.WD_ESTATE
+        wd.wd_enable_f32(op.h)
+        out2 = apply_f32(torch, op, psi, 1)
+        C2 = oracle.build_clover(dims, m0, csw, U2)
+        assert rel_l2(out2, oracle.apply(dims, m0, r32(U2), r32(C2), r32(psi))) <= TOL32
+        assert rel_l2(out1, out2) > 1e-2  # it really is another operator

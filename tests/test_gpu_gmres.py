@@ -196,3 +196,48 @@ def test_mixed_precision_gmres_solves_the_fp64_system(torch):
     assert abs(hist[0] - info["resid"][0]) <= 1e-12 * hist[0]
     assert rel_l2(x[0], f(xo)) <= 1e-7     # both residuals are 1e-10 ||r_0||: the solutions differ by cond(D) times that
     assert rel_l2(x64, f(xo)) <= TOL_X
+
+
+def test_captured_cycle_is_not_replayed_after_the_operator_or_an_option_changed(torch):
+    """A captured restart cycle has the kernel choice, the self-coupling mode and the field pointers baked in.  With the
+    SAME x, b, m, tol and stream: (1) a first wd_load_clover on a csw = 0 handle turns the mass term into S(x) — the next
+    solve must solve the NEW system (checked with the oracle's operator), not replay the old cycle; (2) WD_OPT_GMRES_GRAPH
+    = 0 must really run launch by launch (same bits, and no graph is kept for the next call to fall back on)."""
+    cfg = wdinputs.CONFIGS[2]
+    dims, m0, m, tol, max_cycles = cfg["dims"], 0.0, 6, 1e-9, 60
+    U = wdinputs.config_gauge(cfg)
+    C = oracle.build_clover(dims, m0, cfg["csw"], U)
+    b = wdinputs.spinor(dims, cfg["spinor_seed"])[0]
+    with Op(torch, dims, m0, 0.0, U) as op:
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            wd.wd_set_stream(op.h, st.cuda_stream)
+            db, dx = op.dev_spinor(), op.dev_spinor()
+            wd.wd_pack_spinor(op.h, db, np.ascontiguousarray(b[None]), 1)
+
+            def solve():
+                dx.zero_()
+                hist = np.full(max_cycles + 1, np.nan)
+                cycles = wd.wd_gmres(op.h, dx, db, m, max_cycles, tol, hist)
+                x = np.empty((1,) + b.shape)
+                wd.wd_unpack_spinor(op.h, x, dx, 1)
+                return x[0], hist[: cycles + 1], cycles
+
+            x_w, hist_w, cyc_w = solve()  # pure Wilson; cycles 2.. are a graph keyed on (dx, db, m, tol, stream)
+            assert cyc_w >= 3 and hist_w[-1] < tol * hist_w[0]
+            rw = c(b) - wilson_operator(dims, m0, U, None)(c(x_w))
+            assert np.linalg.norm(rw.ravel()) <= 1.01 * tol * hist_w[0]
+
+            wd.wd_load_clover(op.h, C)  # allocates S: the operator is now Wilson-clover
+            x_c, hist_c, cyc_c = solve()
+            assert cyc_c >= 3 and hist_c[-1] < tol * hist_c[0]
+            rc = c(b) - wilson_operator(dims, m0, U, C)(c(x_c))
+            assert np.linalg.norm(rc.ravel()) <= 1.01 * tol * hist_c[0]
+            xo, info = gmres(wilson_operator(dims, m0, U, C), c(b), m=m, tol=tol, max_cycles=max_cycles)
+            assert cyc_c == info["cycles"] and rel_l2(x_c, f(xo)) <= TOL_X
+
+            wd.wd_set_option(op.h, wd.WD_OPT_GMRES_GRAPH, 0)  # same key, graph switched off
+            x_e, hist_e, cyc_e = solve()
+            assert cyc_e == cyc_c and np.array_equal(x_e, x_c) and np.array_equal(hist_e, hist_c)
+            wd.wd_synchronize(op.h)
+        wd.wd_set_stream(op.h, torch.cuda.current_stream().cuda_stream)
