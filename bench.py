@@ -9,9 +9,14 @@ of the configured lattice (default: BASELINE.json configs[3], 64^4, m0=-0.4, csw
 links, S built on the device).  Inputs rotate over three fields and outputs over two, 25.8 GB are
 touched per step (>> L2), so no L2 flush is needed between timed iterations.
 
-The path does not shard (BASELINE.json: "Everything runs on one GPU"): with --gpus N > 1 every rank
-runs an independent replica on its own GPU ("replicas only", DESIGN.md), no data-path collective;
+BASELINE.json's headline path is single-GPU.  With --gpus N > 1 the default (--parallel dd) is STRONG scaling of the
+domain-decomposed operator of SURVEY.md section 8(f)1 (the same global lattice cut over N ranks, half-spinor faces
+exchanged over NCCL; run_dd below); --parallel replicas runs N independent copies with no data-path collective.
 value = units of all ranks / max-over-ranks device time.
+
+The default line also carries two sub-records measured in the same process: "sustained" (8 s of back-to-back
+applications after the timed region, the figure of the LAST second with its clocks: the steady state of the power cap)
+and "cfg5" (BASELINE.json configs[4], 48^3 x 96 with 12 right-hand sides, blocked layout, run after cfg 4's buffers are freed).
 
 Prints ONE JSON line on rank 0.  `--impl reference` times the CPU oracle (oracle/, as it stands)
 on the host cores on a bounded sample of the same workload.
@@ -62,6 +67,11 @@ def parse_args():
                          "(strong scaling, default); replicas = N independent copies (weak)")
     ap.add_argument("--gmres", type=int, default=0, metavar="M",
                     help="also run restarted GMRES(M) on the device (wd_gmres) and report its timing")
+    ap.add_argument("--sustain-seconds", type=float, default=8.0,
+                    help="back-to-back applications after the timed region; the last second is reported as 'sustained' (0 = skip)")
+    ap.add_argument("--no-cfg5", action="store_true", help="skip the cfg 5 (12 right-hand sides) sub-record of the default line")
+    ap.add_argument("--print-source-hash", type=str, default="", metavar="KERNEL",
+                    help="print the hash of the sources kernel KERNEL is built from (goes into profiles/roofline_traffic.json) and exit")
     ap.add_argument("--graph", action="store_true",
                     help="also time the K steps captured as ONE CUDA graph (cfg 3: 100 back-to-back applies)")
     return ap.parse_args()
@@ -88,18 +98,40 @@ def peak_hbm():
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
+KERNEL_SOURCES = {  # the files a kernel family is compiled from (paper_2407_00041_b200/csrc/)
+    "tmw": ["wd_tmw.cu"], "tma": ["wd_tma.cu"], "tmb": ["wd_tmb.cu"], "tmq": ["wd_tmq.cu"], "tmqb": ["wd_tmq.cu"],
+    "_tma_shared": ["wd_tma_common.cuh", "wd_tma_plan.cuh", "wd_tma.cuh", "wd_smem_ops.cuh", "wd_math.cuh", "wd_internal.h"],
+    "_ldg": ["wd_kernels.cu", "wd_ldg_kernels.cuh", "wd_math.cuh", "wd_internal.h"],
+}
+
+
+def kernel_source_hash(kernel_name):
+    """sha256 (16 hex digits) of the sources the named kernel geometry is built from: a capture in
+    profiles/roofline_traffic.json is only quoted for the build it was taken from."""
+    import hashlib
+
+    fam = kernel_name.split("_")[0].split("/")[0]
+    files = KERNEL_SOURCES[fam] + KERNEL_SOURCES["_tma_shared"] if fam in KERNEL_SOURCES else KERNEL_SOURCES["_ldg"]
+    hsh = hashlib.sha256()
+    for f in files:
+        hsh.update(open(os.path.join(ROOT, "paper_2407_00041_b200", "csrc", f), "rb").read())
+    return hsh.hexdigest()[:16]
+
+
 def ncu_traffic(name):
     """(dram bytes per launch of the dominant kernel, where that number comes from): a CONSTANT read from the
-    committed ncu capture table profiles/roofline_traffic.json (ncu cannot run inside a timed bench), or (None, None)."""
+    committed ncu capture table profiles/roofline_traffic.json (ncu cannot run inside a timed bench) — quoted only if the
+    kernel's sources still hash to what the entry recorded at capture time; otherwise (None, why)."""
     p = os.path.join(ROOT, "profiles", "roofline_traffic.json")
     if os.path.exists(p):
         try:
-            tab = json.load(open(p))
-            ent = tab.get(name)
+            ent = json.load(open(p)).get(name)
             if isinstance(ent, dict):
+                now = kernel_source_hash(name)
+                if ent.get("source_hash") != now:
+                    return None, (f"profiles/roofline_traffic.json has a capture for {name}, but of another build "
+                                  f"(source hash {ent.get('source_hash')}, now {now}): not quoted")
                 return ent.get("bytes"), "profiles/roofline_traffic.json: " + ent.get("source", "?")
-            if ent is not None:
-                return ent, "profiles/roofline_traffic.json: " + str(tab.get("_source", "?"))
         except Exception:
             pass
     return None, None
@@ -306,18 +338,17 @@ def run_dd(args, torch, dist, world, rank, local):
     clover = cfg["csw"] != 0.0
     flop = FLOP_WILSON + (FLOP_CLOVER if clover else 0)
     d = Decomposition(dims, default_grid(world, dims))
-    # ---- setup (untimed).  Every rank draws the global fields from the counter-based generators and keeps its part.
-    U = wdinputs.config_gauge(cfg)
-    Ul = d.extract(U, rank)
-    Cl = wdd.local_clover(d, rank, cfg["m0"], cfg["csw"], d.extract(U, rank, halo=1)) if clover else None
-    del U
+    # ---- setup (untimed).  The generators are counter-based: every rank draws only ITS sites of the global fields (and the
+    # one-site halo of links its clover term needs), never the global field (9.7 GB per rank at 64^4 otherwise).
+    Ul = wdinputs.config_gauge_sites(cfg, d.global_sites(rank))
+    Cl = wdd.local_clover(d, rank, cfg["m0"], cfg["csw"], wdinputs.config_gauge_sites(cfg, d.global_sites(rank, halo=1))) if clover else None
     lo = wdd.LocalOperator(torch, d, rank, cfg["m0"], cfg["csw"], Ul, Cl)
     del Ul, Cl
     op = wdd.DistributedOperator(torch, dist, lo)
     ins = [lo.spinor(nrhs) for _ in range(3)]
     outs = [lo.spinor(nrhs) for _ in range(2)]
     for k in range(3):
-        psi = np.stack([d.extract(wdinputs.spinor(dims, cfg["spinor_seed"] + 100 * k + r)[0], rank) for r in range(nrhs)])
+        psi = wdinputs.spinor_sites(cfg["spinor_seed"] + 100 * k, d.global_sites(rank), nrhs)
         wd.wd_pack_spinor(lo.h, ins[k], psi, nrhs)
     del psi
     torch.cuda.synchronize()
@@ -370,6 +401,111 @@ def run_dd(args, torch, dist, world, rank, local):
     dist.destroy_process_group()
     if rank == 0:
         print(json.dumps(line), flush=True)
+
+
+def sustained_record(torch, step, stream, local, seconds, ms_guess, alg_bytes_step, flop_step, peak):
+    """Back-to-back applications for >= `seconds` (two batches of ~0.1 s always in flight, so the GPU never idles); the
+    figure reported is that of the LAST second, with the SM clock, power and throttle reasons sampled during that second:
+    the steady state under the board's power cap, which a 20-step burst at full clock does not show."""
+    batch = max(5, int(0.1 / (ms_guess * 1e-3)))
+    counter = [0]
+
+    def enqueue():
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(batch):
+            step(counter[0])
+            counter[0] += 1
+        e1.record(stream)
+        return e0, e1
+
+    def run_for(sec):
+        times, t0 = [], time.time()
+        pending = enqueue()
+        while True:
+            nxt = enqueue() if time.time() - t0 < sec else None
+            pending[1].synchronize()
+            times.append(pending[0].elapsed_time(pending[1]))
+            if nxt is None:
+                return times
+            pending = nxt
+
+    by_second = []  # ms per step of every whole second before the last one: shows the drift towards the steady state
+    soak = []
+    for _ in range(max(int(round(seconds)) - 1, 1)):
+        sec = run_for(1.0)
+        by_second.append(round(sum(sec) / (len(sec) * batch), 4))
+        soak += sec
+    smp = ClockSampler(local)
+    smp.start()
+    last = run_for(1.0)
+    smp.stop_flag = True
+    smp.join()
+    ms = sum(last) / (len(last) * batch)
+    by_second.append(round(ms, 4))
+    gbs = alg_bytes_step / (ms * 1e-3) / 1e9
+    return {"seconds": seconds, "ms_per_step": ms, "steps_total": (len(soak) + len(last)) * batch,
+            "steps_in_last_second": len(last) * batch, "first_batch_ms_per_step": soak[0] / batch, "ms_per_step_by_second": by_second,
+            "value": flop_step / (ms * 1e-3) / 1e9, "unit": "GFLOP/s", "achieved_gbs": gbs, "frac": gbs / peak,
+            "frac_of_8000_spec": gbs / 8000.0, "clocks": smp.summary(),
+            "what": "ms per step, algorithmic GB/s and clocks of the last second of the run"}
+
+
+def cfg5_record(torch, wd, wdinputs, local, steps, warmup, peak):
+    """BASELINE.json configs[4] (48^3 x 96, Wilson-clover, 12 right-hand sides, blocked multi-RHS layout) as a sub-record of
+    the default line: same timing rules as the main record (device events on the launching stream, inputs resident and
+    far larger than L2, clocks sampled during the timed region)."""
+    cfg = dict(wdinputs.CONFIGS[5])
+    dims, nrhs = cfg["dims"], cfg["nrhs"]
+    V = wdinputs.volume(dims)
+    h = wd.wd_create(*dims, cfg["m0"], cfg["csw"])
+    try:
+        stream = torch.cuda.current_stream()
+        wd.wd_set_stream(h, stream.cuda_stream)
+        wd.wd_set_option(h, wd.WD_OPT_DEVICE_PACK, 1)
+        wd.wd_set_option(h, wd.WD_OPT_RHS_BLOCK, 4)
+        U = wdinputs.config_gauge(cfg)
+        wd.wd_load_gauge(h, U)
+        del U
+        wd.wd_build_clover(h)
+        n64 = wd.wd_spinor_bytes(h, nrhs) // 8
+        unit64 = wd.wd_spinor_bytes(h, 4) // 8
+        ins = [torch.empty(n64, dtype=torch.float64, device="cuda") for _ in range(2)]
+        outs = [torch.empty(n64, dtype=torch.float64, device="cuda") for _ in range(2)]
+        for u in range(nrhs // 4):  # a unit of four right-hand sides at a time (8 GB of host memory, not 24)
+            part = wdinputs.spinor(dims, cfg["spinor_seed"] + u, nrhs=4)
+            wd.wd_pack_spinor(h, ins[0][u * unit64:], part, 4)
+            del part
+        wd.wd_apply(h, ins[1], ins[0], nrhs)
+        ins[1].mul_(1.0 / 8.0)
+        torch.cuda.synchronize()
+        kname = wd.wd_kernel_name(wd.wd_kernel_for(h, nrhs))
+        for k in range(warmup):
+            wd.wd_apply(h, outs[k % 2], ins[k % 2], nrhs)
+        torch.cuda.synchronize()
+        smp = ClockSampler(local)
+        smp.start()
+        l0 = wd.wd_launch_count(h)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for k in range(steps):
+            wd.wd_apply(h, outs[k % 2], ins[k % 2], nrhs)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        launches = wd.wd_launch_count(h) - l0
+        smp.stop_flag = True
+        smp.join()
+        ms = e0.elapsed_time(e1) / steps
+        alg = V * (576 + 576 + 384 * nrhs)
+        gbs = alg / (ms * 1e-3) / 1e9
+        traffic, traffic_src = ncu_traffic(kname + f"/clover/x{nrhs}@" + "x".join(map(str, dims)))
+        return {"workload": cfg["name"], "lattice": list(dims), "nrhs": nrhs, "kernel": kname, "rhs_layout": "blocked [unit][12][Vs][4]",
+                "steps": steps, "warmup": warmup, "ms_per_step": ms, "value": V * nrhs * (FLOP_WILSON + FLOP_CLOVER) / (ms * 1e-3) / 1e9,
+                "unit": "GFLOP/s", "site_rhs_per_s": V * nrhs / (ms * 1e-3), "algorithmic_bytes_per_launch": alg, "achieved_gbs": gbs,
+                "frac": gbs / peak, "hbm_roof_ms": alg / (peak * 1e9) * 1e3, "traffic": traffic, "traffic_source": traffic_src,
+                "gpu_launches": launches, "clocks": smp.summary()}
+    finally:
+        wd.wd_destroy(h)
 
 
 def run_ours(args):
@@ -498,7 +634,10 @@ def run_ours(args):
 
     line = {
         "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+        # --parallel dd (the default): the N > 1 lines cut this same lattice over N ranks, so the N = 1 point of that curve is
+        # a strong-scaling point; replicas: per-GPU work fixed
+        "scaling": "strong" if args.parallel == "dd" else "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "sites_per_s": site_rhs_per_s, "hbm_gbs_algorithmic": site_rhs_per_s * alg_bytes_site_rhs / 1e9,
         "config": {"workload": cfg["name"], "lattice": list(dims), "m0": cfg["m0"], "csw": cfg["csw"],
@@ -510,6 +649,10 @@ def run_ours(args):
         "roofline": roofline, "gpu_launches": launches, "clocks": sampler.summary(),
     }
 
+    # ---- the steady state of the power cap: seconds of back-to-back applications, the last second reported
+    if args.sustain_seconds > 0 and rank == 0 and world == 1:
+        line["sustained"] = sustained_record(torch, step, stream, local, args.sustain_seconds, ms_per_step, alg_bytes_step,
+                                             V * nrhs * flop, peak)
     # ---- end to end through the C-ABI with HOST buffers (pinned), copies inside the timed region
     if args.rhs_block != 1:  # the host-to-host path, the FP32 variant and GMRES below use the plain device layout
         wd.wd_set_option(h, wd.WD_OPT_RHS_BLOCK, 1)
@@ -645,6 +788,13 @@ def run_ours(args):
     wd.wd_destroy(h)
     del ins, outs
     torch.cuda.empty_cache()
+    # ---- cfg 5 (12 right-hand sides) in the same line, now that cfg 4's buffers are gone
+    if rank == 0 and world == 1 and args.config == 4 and not args.dims and not args.nrhs and not args.no_cfg5:
+        try:
+            line["cfg5"] = cfg5_record(torch, wd, wdinputs, local, max(5, min(args.steps, 20)), max(3, min(args.warmup, 5)), peak)
+        except Exception as exc:  # a sub-record never costs the main line
+            line["cfg5"] = {"error": repr(exc)}
+        torch.cuda.empty_cache()
 
     # ---- ceilings measured on this GPU in this run (bench-only library, include/wd_bench.h): streaming read-only /
     # copy / 7 reads per write (the operator's mix), and the FP64 FMA roof that co-limits a multi-RHS application
@@ -686,7 +836,9 @@ def run_ours(args):
 
 if __name__ == "__main__":
     a = parse_args()
-    if a.impl == "reference":
+    if a.print_source_hash:
+        print(kernel_source_hash(a.print_source_hash))
+    elif a.impl == "reference":
         run_reference(a)
     else:
         run_ours(a)

@@ -130,3 +130,22 @@ def test_face_exchange_over_gloo_world2(tmp_path, gdims, grid):
     for k in (0, 1):
         res = json.loads((tmp_path / ("rank%d.json" % k)).read_text())
         assert res["ok"] and res["n"] == 1
+
+
+def test_site_list_generators_draw_a_rank_part_without_the_global_field():
+    """bench.py --gpus N: every rank draws only its own sites (and the link halo of its clover term).  The site-list
+    generators must give, bit for bit, the rows of the global field the full generators give."""
+    import wdinputs
+
+    dims = (4, 6, 2, 8)
+    d = Decomposition(dims, (2, 3, 1, 1))
+    for cfg in (dict(gauge=("haar", 77)), dict(gauge=("exp", 78, 0.4))):
+        U = wdinputs.config_gauge(cfg, dims)
+        for rank in (0, 4):
+            for halo in (0, 1):
+                sites = d.global_sites(rank, halo)
+                assert np.array_equal(wdinputs.config_gauge_sites(cfg, sites), U[sites])
+                assert np.array_equal(wdinputs.config_gauge_sites(cfg, sites), d.extract(U, rank, halo))
+    psi = wdinputs.spinor(dims, 79, nrhs=3)
+    sites = d.global_sites(5)
+    assert np.array_equal(wdinputs.spinor_sites(79, sites, 3), psi[:, sites])

@@ -44,8 +44,11 @@ def _load():
         lib.wdin_su3_exp.argtypes = [dp, u64, u64, f64]
         lib.wdin_su3_unit.argtypes = [dp, u64]
         lib.wdin_selfcoupling_random.argtypes = [dp, u64, u64, f64, f64]
+        lib.wdin_gaussian_sites.argtypes = [dp, dp, u64, u64, u64]
+        lib.wdin_su3_haar_sites.argtypes = [dp, dp, u64, u64]
+        lib.wdin_su3_exp_sites.argtypes = [dp, dp, u64, u64, f64]
         for f in (lib.wdin_gaussian, lib.wdin_su3_haar, lib.wdin_su3_exp, lib.wdin_su3_unit,
-                  lib.wdin_selfcoupling_random):
+                  lib.wdin_selfcoupling_random, lib.wdin_gaussian_sites, lib.wdin_su3_haar_sites, lib.wdin_su3_exp_sites):
             f.restype = None
         _lib = lib
     return _lib
@@ -69,6 +72,30 @@ def spinor(dims, seed: int, nrhs: int = 1) -> np.ndarray:
     for r in range(nrhs):
         _load().wdin_gaussian(out[r].ctypes.data, V * 24, seed + r)
     return out
+
+
+def spinor_sites(seed: int, sites, nrhs: int = 1) -> np.ndarray:
+    """The rows spinor(dims, seed, nrhs)[:, sites] without generating the rest: [nrhs][len(sites)][12][2].  `sites`: global
+    canonical site indices (int64), e.g. Decomposition.global_sites(rank)."""
+    sites = np.ascontiguousarray(sites, dtype=np.int64)
+    out = np.empty((nrhs, len(sites), 12, 2), dtype=np.float64)
+    for r in range(nrhs):
+        _load().wdin_gaussian_sites(out[r].ctypes.data, sites.ctypes.data, len(sites), 24, seed + r)
+    return out
+
+
+def config_gauge_sites(cfg: dict, sites) -> np.ndarray:
+    """The rows config_gauge(cfg)[sites] without generating the rest: [len(sites)][4][3][3][2]."""
+    sites = np.ascontiguousarray(sites, dtype=np.int64)
+    U = np.empty((len(sites), 4, 3, 3, 2), dtype=np.float64)
+    g = cfg["gauge"]
+    if g[0] == "haar":
+        _load().wdin_su3_haar_sites(U.ctypes.data, sites.ctypes.data, len(sites), g[1])
+    elif g[0] == "exp":
+        _load().wdin_su3_exp_sites(U.ctypes.data, sites.ctypes.data, len(sites), g[1], g[2])
+    else:
+        raise ValueError(g)
+    return U
 
 
 def gauge_haar(dims, seed: int) -> np.ndarray:

@@ -51,6 +51,15 @@ static inline double gauss(uint64_t seed, uint64_t n) {
     return (n & 1) ? g1 : g0;
 }
 
+/* `per_site` (even) consecutive normals for each listed site: out[k][0..per_site) = normals per_site*sites[k] .. of the stream */
+void wdin_gaussian_sites(double *out, const int64_t *sites, uint64_t nsites, uint64_t per_site, uint64_t seed) {
+    const uint64_t pp = per_site / 2;
+#pragma omp parallel for schedule(static)
+    for (int64_t k = 0; k < (int64_t)nsites; k++)
+        for (uint64_t q = 0; q < pp; q++)
+            gauss_pair(seed, pp * (uint64_t)sites[k] + q, out + per_site * k + 2 * q, out + per_site * k + 2 * q + 1);
+}
+
 void wdin_gaussian(double *out, uint64_t n, uint64_t seed) {
 #pragma omp parallel for schedule(static)
     for (int64_t p = 0; p < (int64_t)((n + 1) / 2); p++) {
@@ -77,11 +86,10 @@ static cplx det3(cplx m[3][3]) {
 
 /* Haar SU(3): columns of a complex Gaussian matrix orthonormalised by modified Gram-Schmidt
  * (= QR with positive R diagonal, Haar on U(3)), then multiplied by exp(-i arg(det)/3). */
-void wdin_su3_haar(double *U, uint64_t nlinks, uint64_t seed) {
-#pragma omp parallel for schedule(static)
-    for (int64_t l = 0; l < (int64_t)nlinks; l++) {
+static void haar_link(double *o, uint64_t seed, uint64_t l) {
+    {
         cplx g[3][3];
-        gaussian_3x3(g, seed, (uint64_t)l);
+        gaussian_3x3(g, seed, l);
         for (int c = 0; c < 3; c++) {
             for (int p = 0; p < c; p++) {
                 cplx dot = 0;
@@ -96,13 +104,25 @@ void wdin_su3_haar(double *U, uint64_t nlinks, uint64_t seed) {
         cplx d = det3(g);
         double th = atan2(cimag(d), creal(d)) / 3.0;
         cplx ph = cos(th) - I * sin(th);
-        double *o = U + 18 * l;
         for (int k = 0; k < 9; k++) {
             cplx v = g[k / 3][k % 3] * ph;
             o[2 * k] = creal(v);
             o[2 * k + 1] = cimag(v);
         }
     }
+}
+
+void wdin_su3_haar(double *U, uint64_t nlinks, uint64_t seed) {
+#pragma omp parallel for schedule(static)
+    for (int64_t l = 0; l < (int64_t)nlinks; l++) haar_link(U + 18 * l, seed, (uint64_t)l);
+}
+
+/* The same values for a LIST of sites of a gauge field (links 4*site .. 4*site+3 of the stream): U[k] receives the four
+ * links of site sites[k], so a rank of a decomposed lattice draws its own part without generating the global field. */
+void wdin_su3_haar_sites(double *U, const int64_t *sites, uint64_t nsites, uint64_t seed) {
+#pragma omp parallel for schedule(static)
+    for (int64_t k = 0; k < (int64_t)nsites; k++)
+        for (int mu = 0; mu < 4; mu++) haar_link(U + 18 * (4 * k + mu), seed, 4 * (uint64_t)sites[k] + mu);
 }
 
 static void matmul3(cplx c[3][3], cplx a[3][3], cplx b[3][3]) {
@@ -119,11 +139,10 @@ static void matmul3(cplx c[3][3], cplx a[3][3], cplx b[3][3]) {
 
 /* U = exp(i*eps*H), H = (G+G^H)/2 - tr/3 with G complex Gaussian: scaling and squaring around a
  * degree-20 Taylor polynomial (argument norm scaled below 1/4). */
-void wdin_su3_exp(double *U, uint64_t nlinks, uint64_t seed, double eps) {
-#pragma omp parallel for schedule(static)
-    for (int64_t l = 0; l < (int64_t)nlinks; l++) {
+static void exp_link(double *o, uint64_t seed, uint64_t l, double eps) {
+    {
         cplx g[3][3], a[3][3];
-        gaussian_3x3(g, seed, (uint64_t)l);
+        gaussian_3x3(g, seed, l);
         cplx tr = 0;
         for (int i = 0; i < 3; i++) tr += creal(g[i][i]);
         double nrm = 0;
@@ -151,12 +170,22 @@ void wdin_su3_exp(double *U, uint64_t nlinks, uint64_t seed, double eps) {
                 }
         }
         for (int q = 0; q < s; q++) matmul3(e, e, e);
-        double *o = U + 18 * l;
         for (int k = 0; k < 9; k++) {
             o[2 * k] = creal(e[k / 3][k % 3]);
             o[2 * k + 1] = cimag(e[k / 3][k % 3]);
         }
     }
+}
+
+void wdin_su3_exp(double *U, uint64_t nlinks, uint64_t seed, double eps) {
+#pragma omp parallel for schedule(static)
+    for (int64_t l = 0; l < (int64_t)nlinks; l++) exp_link(U + 18 * l, seed, (uint64_t)l, eps);
+}
+
+void wdin_su3_exp_sites(double *U, const int64_t *sites, uint64_t nsites, uint64_t seed, double eps) {
+#pragma omp parallel for schedule(static)
+    for (int64_t k = 0; k < (int64_t)nsites; k++)
+        for (int mu = 0; mu < 4; mu++) exp_link(U + 18 * (4 * k + mu), seed, 4 * (uint64_t)sites[k] + mu, eps);
 }
 
 void wdin_su3_unit(double *U, uint64_t nlinks) {
