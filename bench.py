@@ -564,10 +564,20 @@ def run_ours(args):
         alg_bytes_site_rhs = (gauge_b + self_b) / nrhs + 384
         alg_bytes_step = V * (gauge_b + self_b + 384 * nrhs)
     U = wdinputs.config_gauge(cfg)
-    wd.wd_load_gauge(h, U)
+    t_setup = time.time()
+    wd.wd_load_gauge(h, U)  # synchronous: H2D copy of the canonical array + transpose on the device (WD_OPT_DEVICE_PACK)
+    setup = {"load_gauge_ms": (time.time() - t_setup) * 1e3, "gauge_bytes": V * 576}
     del U
     if clover:
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0.record(stream)
         wd.wd_build_clover(h)
+        c1.record(stream)
+        torch.cuda.synchronize()
+        cms = c0.elapsed_time(c1)
+        setup.update({"build_clover_ms": cms, "build_clover_tflops": V * 60 * 198 / (cms * 1e-3) / 1e12,
+                      "build_clover_gbs": V * 1152 / (cms * 1e-3) / 1e9,
+                      "build_clover_what": "k_build_clover, first call: 60 3x3 complex products per site (FP64-bound), reads U, writes S"})
     n64 = wd.wd_spinor_bytes(h, nrhs) // 8
     ins = [torch.empty(n64, dtype=torch.float64, device="cuda") for _ in range(3)]
     outs = [torch.empty(n64, dtype=torch.float64, device="cuda") for _ in range(2)]
@@ -646,7 +656,7 @@ def run_ours(args):
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": f"inputs larger than L2 ({alg_bytes_step / 1e9:.2f} GB touched per step); "
                          "3 inputs / 2 outputs rotate"},
-        "roofline": roofline, "gpu_launches": launches, "clocks": sampler.summary(),
+        "roofline": roofline, "gpu_launches": launches, "clocks": sampler.summary(), "setup": setup,
     }
 
     # ---- the steady state of the power cap: seconds of back-to-back applications, the last second reported

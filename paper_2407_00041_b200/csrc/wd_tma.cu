@@ -4,7 +4,7 @@
 // out(x) = S(x) psi(x) - 1/2 sum_mu [ (1-gamma_mu) U_mu(x) psi(x+mu) + (1+gamma_mu) U_mu(x-mu)^H psi(x-mu) ]
 // (eq. 1.13), steps a1-a7 of SURVEY.md §8(a) in one pass.
 //
-// Why this shape (profiles/r1a_*.md): the one-thread-per-site LDG kernels are latency-bound — the
+// Why this shape (round-1 ncu captures of the LDG kernels; summary in DESIGN.md section 5): the one-thread-per-site LDG kernels are latency-bound — the
 // bytes in flight per SM are (resident warps) x (registers a thread can spare), and with 140-180
 // registers per thread only 8-11 warps fit.  Here the bytes in flight are decoupled from registers:
 //   * a persistent CTA (one per SM) owns a BZ x BY x BX tile of sites and marches it along T;
