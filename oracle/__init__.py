@@ -35,7 +35,6 @@ def _load():
         i, d, p = ctypes.c_int, ctypes.c_double, ctypes.c_void_p
         lib.wdref_apply.argtypes = [i, i, i, i, d, p, p, p, p, i]
         lib.wdref_build_clover.argtypes = [i, i, i, i, d, d, p, p]
-        lib.wdref_apply_sites.argtypes = [i, i, i, i, d, d, p, p, p, ctypes.c_int64, p]
         lib.wdref_build_clover_full.argtypes = [i, i, i, i, d, d, p, p]
         lib.wdref_dense.argtypes = [i, i, i, i, d, d, p, p]
         lib.wdref_gamma.argtypes = [i, p]
@@ -71,21 +70,6 @@ def apply(dims, m0, U, C, psi) -> np.ndarray:
     if rc != 0:
         raise RuntimeError(f"wdref_apply failed: {rc}")
     return out[0] if squeeze else out
-
-
-def apply_sites(dims, m0, csw, U, psi, sites) -> np.ndarray:
-    """(D psi)(x) for x in sites only ([nsites][12][2]); S built from U when csw != 0."""
-    T, Z, Y, X = dims
-    V = T * Z * Y * X
-    U, psi = _f64(U), _f64(psi)
-    assert U.size == V * 72 and psi.size == V * 24
-    sites = np.ascontiguousarray(sites, dtype=np.int64)
-    out = np.empty((sites.size, 12, 2), dtype=np.float64)
-    rc = _load().wdref_apply_sites(T, Z, Y, X, float(m0), float(csw), U.ctypes.data, psi.ctypes.data,
-                                   sites.ctypes.data, sites.size, out.ctypes.data)
-    if rc != 0:
-        raise RuntimeError(f"wdref_apply_sites failed: {rc}")
-    return out
 
 
 def build_clover(dims, m0, csw, U) -> np.ndarray:

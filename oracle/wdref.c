@@ -301,34 +301,6 @@ int wdref_build_clover(int T, int Z, int Y, int X, double m0, double csw, const 
     return 0;
 }
 
-/* (D psi)(x) at the listed sites only, from U, psi, m0, csw alone: S(x) is built from U by
- * eq. 2.5 when csw != 0.  For parity checks at lattice sizes where a whole-lattice oracle pass
- * would take too long; same per-site arithmetic as wdref_apply + wdref_build_clover. */
-int wdref_apply_sites(int T, int Z, int Y, int X, double m0, double csw, const double *U,
-                      const double *in, const int64_t *sites, int64_t nsites,
-                      double *out /* [nsites][12][2] */) {
-    if (T < 1 || Z < 1 || Y < 1 || X < 1 || !U || !out || !in || !sites || nsites < 0) return -1;
-    dims_t d = {{T, Z, Y, X}};
-    const int64_t V = (int64_t)T * Z * Y * X;
-    cplx gam[4][4][4];
-    for (int mu = 0; mu < 4; mu++) gamma_c(mu, gam[mu]);
-    for (int64_t k = 0; k < nsites; k++)
-        if (sites[k] < 0 || sites[k] >= V) return -2;
-#pragma omp parallel for schedule(dynamic, 16)
-    for (int64_t k = 0; k < nsites; k++) {
-        cplx acc[12], S[12][12];
-        if (csw != 0.0) { /* same S as wdref_build_clover -> wdref_apply: through the 42 entries */
-            cplx c42[42];
-            selfcoupling_full(&d, m0, csw, U, sites[k], gam, S);
-            pack_selfcoupling(S, c42);
-            expand_selfcoupling(c42, S);
-        }
-        apply_site(&d, m0, U, (csw != 0.0) ? S : NULL, (const cplx *)in, sites[k], gam, acc);
-        for (int i = 0; i < 12; i++) ((cplx *)out)[k * 12 + i] = acc[i];
-    }
-    return 0;
-}
-
 /* ---- dense assembly of eq. 1.13 from Kronecker products (tiny lattices only) ------------ */
 static void kron_4x3(cplx A[4][4], m3 B, cplx K[12][12]) {
     for (int s = 0; s < 4; s++)

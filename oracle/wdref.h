@@ -22,11 +22,6 @@ extern "C" {
 int wdref_apply(int T, int Z, int Y, int X, double m0, const double *U, const double *C,
                 double *out, const double *in, int nrhs);
 
-/* out[k] = (D in)(sites[k]) for the listed sites only; S(x) is built from U (eq. 2.5) when
- * csw != 0.  in: one spinor [V][12][2]; out: [nsites][12][2]. */
-int wdref_apply_sites(int T, int Z, int Y, int X, double m0, double csw, const double *U,
-                      const double *in, const int64_t *sites, int64_t nsites, double *out);
-
 /* C = the 42 stored entries of S(x), eq. 2.5 with Q of eq. 1.12. */
 int wdref_build_clover(int T, int Z, int Y, int X, double m0, double csw, const double *U,
                        double *C);

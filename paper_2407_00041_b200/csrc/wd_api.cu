@@ -484,10 +484,10 @@ static int auto_kernel(const wd_handle *h, int nrhs) {
     // call: the quad kernels of wd_tmq.cu (cfg 5: tmqb on the blocked layout 17.4 ms, tmq on the plain layout 20.8 ms when
     // its units of four are well filled), else the second generation on the 4x4x8 tile with its four-slot ring (25.4 ms;
     // 2x4x16 with three slots 28.3, tmw 27.4, tma 28.5 ms).  linear256 always fits, and wins on small lattices.
-    static const char *pref_clover[] = {"tmw_2x4x16", "tma_2x4x16", "tmb_4x4x8", "tmb_2x8x8"};
-    static const char *pref_tworow[] = {"tma_2x4x16", "tmw_2x4x16", "tmb_4x4x8", "tmb_2x8x8"};
-    static const char *pref_hop[] = {"tmb_2x4x16", "tmb_4x4x8", "tmb_2x8x8", "tmw_2x4x16"};
-    static const char *pref_multi[] = {"tmb_4x4x8", "tmb_2x8x8", "tmb_2x4x16", "tmw_2x4x16"};
+    static const char *pref_clover[] = {"tmw_2x4x16", "tma_2x4x16", "tmb_4x4x8"};
+    static const char *pref_tworow[] = {"tma_2x4x16", "tmw_2x4x16", "tmb_4x4x8"};
+    static const char *pref_hop[] = {"tmb_2x4x16", "tmb_4x4x8", "tmw_2x4x16"};
+    static const char *pref_multi[] = {"tmb_4x4x8", "tmb_2x4x16", "tmw_2x4x16"};
     if (h->rhs_block > 1) {  // blocked multi-RHS layout: the kernels written for it
         for (int id = 0; id < kernel_count(); id++)
             if (kernel_info(id).rhs_block == h->rhs_block && geometry_fits(h, kernel_info(id))) return id;
@@ -506,7 +506,7 @@ static int auto_kernel(const wd_handle *h, int nrhs) {
     const char **pref = (nrhs > 1 && h->variant == 0) ? pref_multi : !clover_fused ? pref_hop : (h->gauge_rows == 2) ? pref_tworow : pref_clover;
     // (the tiled one-thread-per-site kernels are never chosen: linear256 beats them wherever no TMA tile divides the
     // lattice — 20^4: 88 against 113 us, 36^4: 0.80 against 1.04 ms — they stay selectable with WD_OPT_KERNEL)
-    for (int i = 0; i < 4; i++)
+    for (int i = 0; i < 3; i++)
         for (int id = 0; id < kernel_count(); id++)
             if (!strcmp(kernel_info(id).name, pref[i]) && geometry_fits(h, kernel_info(id))) return id;
     return 0;

@@ -81,7 +81,6 @@ cudaError_t launch_tma_2x4x16(const KParams &p, int self, cudaStream_t st);
 cudaError_t launch_tmq_2x4x8(const KParams &p, int self, cudaStream_t st);   // four right-hand sides per work item
 cudaError_t launch_tmqb_2x4x8(const KParams &p, int self, cudaStream_t st);  // the same on the blocked multi-RHS layout
 cudaError_t launch_tmb_4x4x8(const KParams &p, int self, cudaStream_t st);
-cudaError_t launch_tmb_2x8x8(const KParams &p, int self, cudaStream_t st);
 cudaError_t launch_tmb_2x4x16(const KParams &p, int self, cudaStream_t st);  // three ring slots
 // first generation with two compute warpgroups per tile (wd_tmw.cu)
 cudaError_t launch_tmw_2x4x16(const KParams &p, int self, cudaStream_t st);

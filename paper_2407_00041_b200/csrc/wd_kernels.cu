@@ -63,14 +63,13 @@ cudaError_t launch_selfcoupling(const KParams &p, int self, cudaStream_t st) {
 }
 
 // ---- registry -------------------------------------------------------------------------------
-// linear: any lattice.  tile_*: LDG kernels for lattices no TMA tile divides (cfg 1: 4^4).  tma/tmb: the TMA kernels.
+// linear256: any lattice (the automatic choice where no TMA tile divides it, and for small lattices).  tile_1x4x4x16: the
+// tiled one-thread-per-site kernel, used by the FP32 variant and selectable.  tma / tmb / tmw / tmq / tmqb: the TMA kernels.
 static const KernelInfo kKernels[] = {
     {"linear256", 0, 0, 0, 0, 256, false, 1, launch_linear<256>},
     {"tile_1x4x4x16", 1, 4, 4, 16, 256, false, 1, launch_tiled<1, 4, 4, 16>},
-    {"tile_2x4x4x4", 2, 4, 4, 4, 128, false, 1, launch_tiled<2, 4, 4, 4>},
     {"tma_2x4x16", 1, 2, 4, 16, 160, true, 1, launch_tma_2x4x16},
     {"tmb_4x4x8", 1, 4, 4, 8, 160, true, 1, launch_tmb_4x4x8},
-    {"tmb_2x8x8", 1, 2, 8, 8, 160, true, 1, launch_tmb_2x8x8},
     {"tmb_2x4x16", 1, 2, 4, 16, 160, true, 1, launch_tmb_2x4x16},
     {"tmw_2x4x16", 1, 2, 4, 16, 384, true, 1, launch_tmw_2x4x16},
     {"tmq_2x4x8", 1, 2, 4, 8, 384, true, 1, launch_tmq_2x4x8},

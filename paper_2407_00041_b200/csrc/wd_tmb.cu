@@ -434,6 +434,5 @@ template <int BZ, int BY, int BX, int KR = 4> static cudaError_t launch_tma(cons
 
 // Tiles of 128 sites whose shared-memory plan fits 227 KB (2x4x16 is 816 B too large)
 cudaError_t launch_tmb_4x4x8(const KParams &p, int self, cudaStream_t st) { return tmb::launch_tma<4, 4, 8>(p, self, st); }
-cudaError_t launch_tmb_2x8x8(const KParams &p, int self, cudaStream_t st) { return tmb::launch_tma<2, 8, 8>(p, self, st); }
 cudaError_t launch_tmb_2x4x16(const KParams &p, int self, cudaStream_t st) { return tmb::launch_tma<2, 4, 16, 3>(p, self, st); }
 }  // namespace wd

@@ -44,7 +44,7 @@ def test_decomposed_operator_matches_oracle_on_the_global_lattice(torch, gdims, 
         em.close()
 
 
-@pytest.mark.parametrize("kernel", ["tmw_2x4x16", "tma_2x4x16", "tmb_4x4x8", "tmb_2x8x8", "tmq_2x4x8", "tile_1x4x4x16", "linear256"])
+@pytest.mark.parametrize("kernel", ["tmw_2x4x16", "tma_2x4x16", "tmb_4x4x8", "tmq_2x4x8", "tile_1x4x4x16", "linear256"])
 def test_every_kernel_family_supports_open_boundaries(torch, kernel):
     gdims, grid, m0, csw = (8, 8, 16, 32), (2, 2, 1, 2), -0.4, 1.0
     U = wdinputs.gauge_exp(gdims, 811, 0.5)

@@ -146,7 +146,7 @@ def test_tiled_rasterisation_parameters(torch, tchunk, zgroup):
     psi = wdinputs.spinor(dims, 312)
     C = oracle.build_clover(dims, m0, 1.0, U)
     ref = oracle.apply(dims, m0, U, C, psi)
-    for name in ("tile_1x4x4x16", "tile_2x4x4x4"):
+    for name in ("tile_1x4x4x16",):
         if tchunk == 1 and name.startswith("tile_2"):
             continue
         with Op(torch, dims, m0, 1.0, U, C, kernel=wd.kernel_id(name), tchunk=tchunk, zgroup=zgroup) as op:

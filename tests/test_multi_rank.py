@@ -1,7 +1,7 @@
-"""N > 1 path on CPU (gloo, world_size 2).  The operator does not shard (BASELINE.json: one GPU, no halo
-exchange), so bench.py --gpus N runs N independent replicas; the only cross-rank logic is the
-aggregation of the timing — max over ranks of the device time, sum over ranks of the work — and the
-rule that only rank 0 runs / prints the reference arm."""
+"""N > 1 plumbing of bench.py on CPU (gloo, world_size 2): the aggregation of the timing — max over ranks of the device
+time, sum over ranks of the work — which both --parallel modes use (dd: the decomposed operator, strong scaling, the
+default; replicas: N independent copies), and the rule that only rank 0 runs / prints the reference arm.  The exchange
+of the decomposed operator itself is covered by tests/test_decomposition.py (gloo) and tests/test_gpu_dd.py."""
 import json
 import os
 import subprocess

@@ -286,14 +286,3 @@ def test_inputs_are_what_the_recipe_says():
     g = wdinputs.gaussian(200000, 7)
     assert abs(g.mean()) < 0.01 and abs(g.std() - 1) < 0.01
     assert np.array_equal(wdinputs.spinor(dims, 5, nrhs=2)[1], wdinputs.spinor(dims, 6)[0])
-
-
-def test_apply_sites_equals_whole_lattice_apply():
-    dims, m0, csw = (4, 6, 4, 4), -0.4, 1.0
-    U = wdinputs.gauge_haar(dims, 101)
-    psi = wdinputs.spinor(dims, 102)[0]
-    sites = np.array([0, 1, 17, 100, 383, 200, 5], dtype=np.int64)
-    full = oracle.apply(dims, m0, U, oracle.build_clover(dims, m0, csw, U), psi)
-    assert np.array_equal(oracle.apply_sites(dims, m0, csw, U, psi, sites), full[sites])
-    full_w = oracle.apply(dims, m0, U, None, psi)
-    assert np.array_equal(oracle.apply_sites(dims, m0, 0.0, U, psi, sites), full_w[sites])
