@@ -571,13 +571,18 @@ def run_ours(args):
     if clover:
         c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         c0.record(stream)
+        wd.wd_build_clover(h)  # the first launch of a kernel also pays for loading its code
+        c1.record(stream)
+        torch.cuda.synchronize()
+        first_ms = c0.elapsed_time(c1)
+        c0.record(stream)
         wd.wd_build_clover(h)
         c1.record(stream)
         torch.cuda.synchronize()
         cms = c0.elapsed_time(c1)
-        setup.update({"build_clover_ms": cms, "build_clover_tflops": V * 60 * 198 / (cms * 1e-3) / 1e12,
+        setup.update({"build_clover_ms": cms, "build_clover_first_call_ms": first_ms, "build_clover_tflops": V * 60 * 198 / (cms * 1e-3) / 1e12,
                       "build_clover_gbs": V * 1152 / (cms * 1e-3) / 1e9,
-                      "build_clover_what": "k_build_clover, first call: 60 3x3 complex products per site (FP64-bound), reads U, writes S"})
+                      "build_clover_what": "k_build_clover, second call: 60 3x3 complex products per site (FP64-bound), reads U, writes S"})
     n64 = wd.wd_spinor_bytes(h, nrhs) // 8
     ins = [torch.empty(n64, dtype=torch.float64, device="cuda") for _ in range(3)]
     outs = [torch.empty(n64, dtype=torch.float64, device="cuda") for _ in range(2)]
